@@ -1,0 +1,158 @@
+"""ctypes wrapper around oracle/fof_oracle.c — the CPU oracle.
+
+TEST INFRASTRUCTURE, NOT PRODUCT: only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this package.  It imports nothing from
+paper_2510_26851_b200 and shares no code with the CUDA path.
+
+Every function cites the passage of the paper it follows in oracle/fof_oracle.c.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "fof_oracle.c")
+_LIB = os.path.join(_HERE, "libfof_oracle.so")
+# -ffp-contract=off: the float32 link predicate must not be contracted into FMAs.
+CFLAGS = ["-O2", "-std=c99", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC"]
+
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (building the checker is not using it)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.check_call(["gcc", *CFLAGS, "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        f32p = ctypes.POINTER(ctypes.c_float)
+        i32p = ctypes.POINTER(ctypes.c_int32)
+        f64p = ctypes.POINTER(ctypes.c_double)
+        u64p = ctypes.POINTER(ctypes.c_uint64)
+        lib.oracle_wrap1.restype = ctypes.c_float
+        lib.oracle_wrap1.argtypes = [ctypes.c_float, ctypes.c_float]
+        lib.oracle_wrap.restype = ctypes.c_int
+        lib.oracle_wrap.argtypes = [f32p, ctypes.c_int64, ctypes.c_float, f32p]
+        lib.oracle_link.restype = ctypes.c_int
+        lib.oracle_link.argtypes = [f32p, f32p, ctypes.c_float, ctypes.c_float]
+        for fn in (lib.oracle_labels_brute, lib.oracle_labels_cells):
+            fn.restype = ctypes.c_int
+            fn.argtypes = [f32p, ctypes.c_int64, ctypes.c_float, ctypes.c_float, i32p, u64p]
+        lib.oracle_groups.restype = ctypes.c_int64
+        lib.oracle_groups.argtypes = [f32p, f32p, i32p, ctypes.c_int64, ctypes.c_float, ctypes.c_int32,
+                                      ctypes.c_int64, i32p, i32p, f64p, f64p, i32p]
+        lib.oracle_pref.restype = ctypes.c_int
+        lib.oracle_pref.argtypes = [f32p, ctypes.c_int64, ctypes.c_float, ctypes.c_float, u64p]
+        lib.oracle_linking_length.restype = ctypes.c_float
+        lib.oracle_linking_length.argtypes = [ctypes.c_float, ctypes.c_float, ctypes.c_int64]
+        _lib = lib
+    return _lib
+
+
+def _f(x) -> float:
+    """round once to float32 (what the C side receives), as a Python float for ctypes."""
+    return float(np.float32(x))
+
+
+class OracleError(RuntimeError):
+    pass
+
+
+def _f32(a):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    return a, a.ctypes.data_as(ctypes.POINTER(ctypes.c_float))
+
+
+def _pos(pos):
+    pos = np.ascontiguousarray(pos, dtype=np.float32).reshape(-1, 3)
+    return pos, pos.ctypes.data_as(ctypes.POINTER(ctypes.c_float))
+
+
+def _check(rc):
+    if rc < 0:
+        raise OracleError({-1: "bad argument", -2: "non-finite position", -3: "out of memory"}.get(int(rc), str(rc)))
+    return rc
+
+
+def wrap1(x: float, L: float) -> float:
+    return float(_load().oracle_wrap1(_f(x), _f(L)))
+
+
+def wrap(pos, L: float) -> np.ndarray:
+    pos, p = _pos(pos)
+    out = np.empty_like(pos)
+    _check(_load().oracle_wrap(p, pos.shape[0], _f(L), out.ctypes.data_as(ctypes.POINTER(ctypes.c_float))))
+    return out
+
+
+def link(wi, wj, L: float, b: float) -> bool:
+    wi, pi = _f32(wi)
+    wj, pj = _f32(wj)
+    return bool(_load().oracle_link(pi, pj, _f(L), _f(b)))
+
+
+def _labels(fn, pos, L, b):
+    pos, p = _pos(pos)
+    N = pos.shape[0]
+    labels = np.empty(N, dtype=np.int32)
+    E = ctypes.c_uint64(0)
+    _check(fn(p, N, _f(L), _f(b), labels.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)),
+              ctypes.byref(E)))
+    return labels, int(E.value)
+
+
+def labels_brute(pos, L: float, b: float):
+    """(labels int32 [N], E) by all-pairs + min-label sweeps. O(N^2): tiny inputs only."""
+    return _labels(_load().oracle_labels_brute, pos, L, b)
+
+
+def labels_cells(pos, L: float, b: float):
+    """(labels int32 [N], E) by cell list + sequential union-find."""
+    return _labels(_load().oracle_labels_cells, pos, L, b)
+
+
+def groups(pos, labels, L: float, N_min: int, mass=None):
+    """dict(K, group_label, group_size, group_mass f64, group_com f64 [K,3], particle_group)."""
+    pos, p = _pos(pos)
+    N = pos.shape[0]
+    labels = np.ascontiguousarray(labels, dtype=np.int32)
+    cap = max(1, N // max(1, int(N_min)))
+    gl = np.empty(cap, np.int32)
+    gs = np.empty(cap, np.int32)
+    gm = np.empty(cap, np.float64)
+    gc = np.empty((cap, 3), np.float64)
+    pg = np.empty(N, np.int32)
+    mp = None
+    if mass is not None:
+        mass, mp = _f32(mass)
+    i32p = ctypes.POINTER(ctypes.c_int32)
+    f64p = ctypes.POINTER(ctypes.c_double)
+    K = _check(_load().oracle_groups(p, mp, labels.ctypes.data_as(i32p), N, _f(L), int(N_min), cap,
+                                     gl.ctypes.data_as(i32p), gs.ctypes.data_as(i32p), gm.ctypes.data_as(f64p),
+                                     gc.ctypes.data_as(f64p), pg.ctypes.data_as(i32p)))
+    K = int(K)
+    return dict(K=K, group_label=gl[:K].copy(), group_size=gs[:K].copy(), group_mass=gm[:K].copy(),
+                group_com=gc[:K].copy(), particle_group=pg)
+
+
+def pref(pos, L: float, b: float) -> int:
+    """P_ref: candidate pairs on the tightest grid n_ref = floor(L/b) (metric denominator)."""
+    pos, p = _pos(pos)
+    P = ctypes.c_uint64(0)
+    _check(_load().oracle_pref(p, pos.shape[0], _f(L), _f(b), ctypes.byref(P)))
+    return int(P.value)
+
+
+def linking_length(b_frac: float, L: float, N: int) -> float:
+    return float(_load().oracle_linking_length(_f(b_frac), _f(L), int(N)))
