@@ -1,0 +1,121 @@
+/*
+ * fof.h — C ABI of the B200-native periodic Friends-of-Friends library (libfof_b200.so).
+ *
+ * The calls follow the paper's problem statement: inputs X in R^{N x 3}, box L, linking length b
+ * -> labels l in {0..N-1}^N, compact ids, per-group sizes (Alg. 1 input/output;
+ * PAPER.md:189-192 Alg. 2 input/output; "Compaction"); everything stays on the
+ * device.  PAPER.md = the paper text (arxiv 2510.26851) this repo was built from.
+ *
+ * Conventions
+ *  - "dev" pointers are CUDA device pointers on the current device, "host" pointers are host
+ *    memory.  The library never allocates device memory: the caller owns every buffer (PyTorch
+ *    tensors in the Python binding) and passes one workspace of fof_workspace_bytes() bytes,
+ *    256-byte aligned.  `stream` is a cudaStream_t passed as void* (NULL = default stream).
+ *  - Every call returns FOF_OK (0) or a negative FOF_ERR_* code; no exceptions, no abort, no
+ *    output on stdout/stderr.
+ *  - Particle index type is int32 (N < 2^31).  Positions are float32, row-major [N,3]
+ *    (PAPER.md:121, 189), any finite value (they are wrapped into [0,L)).
+ *  - There is NO CPU fallback.  Without a CUDA device the compute calls return FOF_ERR_CUDA.
+ */
+#ifndef FOF_B200_H
+#define FOF_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FOF_OK 0
+#define FOF_ERR_INVALID_ARG (-1)  /* NULL pointer, N < 0, N >= 2^31, L <= 0, b <= 0, N_min < 1, ... */
+#define FOF_ERR_UNSUPPORTED (-2)  /* fewer than 3 cells of side >= b fit per axis (b > ~L/3)           */
+#define FOF_ERR_CUDA (-3)         /* a CUDA runtime call failed (no device, launch error, ...)        */
+#define FOF_ERR_NONFINITE (-4)    /* a position was NaN/Inf (deferred: reported by fof_status)        */
+#define FOF_ERR_CAPACITY (-5)     /* more kept groups than `cap`; outputs are not valid               */
+#define FOF_ERR_STATE (-6)        /* call order violated (e.g. fof_link_stats before fof_link)        */
+
+typedef struct fof_handle fof_handle;
+
+/* Eq. 1: l_link = b_frac * (V/N)^(1/3) with V = L^3, evaluated in double and
+ * rounded once to float32.  Host only. */
+float fof_linking_length(float b_frac, float L, int64_t N);
+
+/* H0 plan (host only; "Grid setup", with cell side >= b instead of <= b, see
+ * DESIGN.md R3).  N particles in a periodic cubic box of side L; `b` is the PHYSICAL linking
+ * length in the units of L (Alg. 2 input "linking length b"); groups with fewer
+ * than N_min members are dropped by fof_groups ("mass cut", 369).
+ * Chooses n cells per axis: n = min(floor(L / (b * 1.001)), ~cbrt(N)) and requires n >= 3.
+ * The handle owns host-side plan data only; *out is untouched on error. */
+int fof_create(int64_t N, float L, float b, int32_t N_min, fof_handle **out);
+void fof_destroy(fof_handle *h);
+
+/* Tuning knob that cannot change results: force n cells per axis (3 <= n <= n_max where
+ * n_max = floor(L / (b * 1.001)), n <= 1290).  Changes fof_workspace_bytes(). */
+int fof_set_grid(fof_handle *h, int32_t n);
+/* n per axis, total cells n^3, largest admissible n. Any out pointer may be NULL. */
+int fof_get_grid(const fof_handle *h, int32_t *n, int64_t *cells, int32_t *n_max);
+
+/* Bytes of device workspace fof_link / fof_groups need for this plan (0 on NULL handle). */
+size_t fof_workspace_bytes(const fof_handle *h);
+
+/* H1-H5: wrap + bin, cell histogram + exclusive scan (replaces the binary
+ * searches of PAPER.md:203-206), cell-contiguous reorder, half-stencil pair
+ * tests with the float32 minimum-image predicate d^2 <= b^2 hooked into a
+ * lock-free union-find (fixed point of the label sweeps PAPER.md:221-225), flatten.
+ *   pos    dev [N,3] float32, read only.
+ *   labels dev [N] int32, written: labels[i] = minimum ORIGINAL index of the particles in i's
+ *          connected component ("initial label = own index", "minimum
+ *          label"), so labels[labels[i]] == labels[i] <= i.
+ *   ws     dev workspace, >= fof_workspace_bytes(h), 256-B aligned; contents are scratch.
+ * Asynchronous on `stream`; no host synchronisation.  A non-finite position sets a device flag
+ * (read it with fof_status); labels are then unspecified but in range. */
+int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *stream);
+
+/* Counters of the last fof_link on (h, ws): true edges E (unordered pairs with d^2 <= b^2; equal
+ * to the oracle's E) and pair tests executed on this plan's grid.  Synchronises `stream`. */
+int fof_link_stats(fof_handle *h, void *ws, void *stream, uint64_t *edges_host, uint64_t *pair_tests_host);
+
+/* H6-H8: group sizes ("parallel histogram"), compaction of groups with
+ * size >= N_min in ascending canonical label, masses and periodic centres
+ * of mass (Eq. 4 PAPER.md:259 made periodic: unwrap members relative to the canonical particle,
+ * mass-weighted mean in float64, re-wrap into [0,L); R11).
+ *   pos, labels     dev, as in fof_link (labels must be canonical: labels[labels[i]] == labels[i]).
+ *   mass            dev [N] float32 or NULL (= 1.0 each; "halo mass = particle number").
+ *   group_label     dev [cap] int32   canonical label of kept group k (ascending in k)
+ *   group_size      dev [cap] int32   member count
+ *   group_mass      dev [cap] float32 sum of member masses
+ *   group_com       dev [cap,3] float32 periodic centre of mass in [0,L)
+ *   particle_group  dev [N] int32 or NULL: compact id of each particle's group, -1 if dropped
+ *   cap             capacity of the group_* arrays; floor(N / N_min) always suffices
+ *   K_host          host: number of kept groups
+ * Synchronises `stream` once to return K.  K > cap -> FOF_ERR_CAPACITY. */
+int fof_groups(fof_handle *h, const float *pos, const float *mass, const int32_t *labels, void *ws,
+               int32_t *group_label, int32_t *group_size, float *group_mass, float *group_com,
+               int32_t *particle_group, int64_t cap, int64_t *K_host, void *stream);
+
+/* Host-buffer entry point (the end-to-end call): copies pos (and mass) host -> device, runs
+ * fof_link + fof_groups, copies labels and the K group records device -> host.
+ *   *_host  host buffers (pinned for full copy speed); mass_host / particle_group_host may be NULL.
+ *   dev_buf device scratch of fof_host_device_bytes(h, cap) bytes, 256-B aligned.
+ * Synchronises `stream`. */
+size_t fof_host_device_bytes(const fof_handle *h, int64_t cap);
+int fof_run_host(fof_handle *h, const float *pos_host, const float *mass_host, int32_t *labels_host,
+                 int32_t *group_label_host, int32_t *group_size_host, float *group_mass_host,
+                 float *group_com_host, int32_t *particle_group_host, int64_t cap, int64_t *K_host,
+                 void *dev_buf, void *stream);
+
+/* Synchronises `stream` and returns the deferred device-side status of the last fof_link /
+ * fof_groups on (h, ws): FOF_OK or FOF_ERR_NONFINITE. */
+int fof_status(fof_handle *h, void *ws, void *stream);
+
+/* Static string for an error code. */
+const char *fof_error_string(int code);
+
+/* Text of the last CUDA runtime error seen by this handle ("" if none). */
+const char *fof_last_cuda_error(const fof_handle *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FOF_B200_H */

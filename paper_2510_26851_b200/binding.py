@@ -1,0 +1,243 @@
+"""Thin Python binding over the C ABI of include/fof.h: argument marshalling only.
+
+Every step of the path runs inside libfof_b200.so; PyTorch is used for device memory, pinned
+host memory and streams.  The module-level functions carry the C names (fof_create, fof_link,
+fof_groups, ...); `FoF` is a small convenience object that owns the handle and the workspace.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfof_b200.so")
+
+FOF_OK = 0
+FOF_ERR_INVALID_ARG = -1
+FOF_ERR_UNSUPPORTED = -2
+FOF_ERR_CUDA = -3
+FOF_ERR_NONFINITE = -4
+FOF_ERR_CAPACITY = -5
+FOF_ERR_STATE = -6
+
+_lib = None
+
+
+class FofError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"fof error {code}: {msg}")
+        self.code = code
+
+
+def lib():
+    """Load libfof_b200.so (built by `python -m paper_2510_26851_b200.build`); fail loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_2510_26851_b200.build` "
+                "(nvcc, sm_100a). There is no CPU fallback.")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i64, i32, f32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_float
+        L.fof_linking_length.restype = f32
+        L.fof_linking_length.argtypes = [f32, f32, i64]
+        L.fof_create.restype = ctypes.c_int
+        L.fof_create.argtypes = [i64, f32, f32, i32, ctypes.POINTER(vp)]
+        L.fof_destroy.restype = None
+        L.fof_destroy.argtypes = [vp]
+        L.fof_set_grid.restype = ctypes.c_int
+        L.fof_set_grid.argtypes = [vp, i32]
+        L.fof_get_grid.restype = ctypes.c_int
+        L.fof_get_grid.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i64), ctypes.POINTER(i32)]
+        L.fof_workspace_bytes.restype = ctypes.c_size_t
+        L.fof_workspace_bytes.argtypes = [vp]
+        L.fof_link.restype = ctypes.c_int
+        L.fof_link.argtypes = [vp, vp, vp, vp, vp]
+        L.fof_link_stats.restype = ctypes.c_int
+        L.fof_link_stats.argtypes = [vp, vp, vp, ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64)]
+        L.fof_groups.restype = ctypes.c_int
+        L.fof_groups.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, ctypes.POINTER(i64), vp]
+        L.fof_host_device_bytes.restype = ctypes.c_size_t
+        L.fof_host_device_bytes.argtypes = [vp, i64]
+        L.fof_run_host.restype = ctypes.c_int
+        L.fof_run_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, ctypes.POINTER(i64), vp, vp]
+        L.fof_status.restype = ctypes.c_int
+        L.fof_status.argtypes = [vp, vp, vp]
+        L.fof_error_string.restype = ctypes.c_char_p
+        L.fof_error_string.argtypes = [ctypes.c_int]
+        L.fof_last_cuda_error.restype = ctypes.c_char_p
+        L.fof_last_cuda_error.argtypes = [vp]
+        _lib = L
+    return _lib
+
+
+def _f(x) -> float:
+    return float(np.float32(x))
+
+
+def _check(rc: int, handle=None):
+    if rc != FOF_OK:
+        msg = lib().fof_error_string(rc).decode()
+        if rc == FOF_ERR_CUDA and handle is not None:
+            msg += " (" + lib().fof_last_cuda_error(handle).decode() + ")"
+        raise FofError(rc, msg)
+
+
+def _ptr(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _stream_ptr(stream):
+    import torch
+
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+# ---------------------------------------------------------------- C-named functions
+def fof_linking_length(b_frac: float, L: float, N: int) -> float:
+    return float(lib().fof_linking_length(_f(b_frac), _f(L), int(N)))
+
+
+def fof_create(N: int, L: float, b: float, N_min: int):
+    h = ctypes.c_void_p()
+    _check(lib().fof_create(int(N), _f(L), _f(b), int(N_min), ctypes.byref(h)))
+    return h
+
+
+def fof_destroy(h):
+    lib().fof_destroy(h)
+
+
+def fof_set_grid(h, n: int):
+    _check(lib().fof_set_grid(h, int(n)))
+
+
+def fof_get_grid(h):
+    n, c, m = ctypes.c_int32(), ctypes.c_int64(), ctypes.c_int32()
+    _check(lib().fof_get_grid(h, ctypes.byref(n), ctypes.byref(c), ctypes.byref(m)))
+    return n.value, c.value, m.value
+
+
+def fof_workspace_bytes(h) -> int:
+    return int(lib().fof_workspace_bytes(h))
+
+
+def fof_link(h, pos, labels, ws, stream=None):
+    """pos: cuda float32 [N,3] contiguous; labels: cuda int32 [N]; ws: cuda uint8 workspace."""
+    _check(lib().fof_link(h, _ptr(pos), _ptr(labels), _ptr(ws), _stream_ptr(stream)), h)
+
+
+def fof_link_stats(h, ws, stream=None):
+    e, t = ctypes.c_uint64(), ctypes.c_uint64()
+    _check(lib().fof_link_stats(h, _ptr(ws), _stream_ptr(stream), ctypes.byref(e), ctypes.byref(t)), h)
+    return int(e.value), int(t.value)
+
+
+def fof_groups(h, pos, mass, labels, ws, group_label, group_size, group_mass, group_com, particle_group, cap,
+               stream=None) -> int:
+    K = ctypes.c_int64()
+    _check(lib().fof_groups(h, _ptr(pos), _ptr(mass), _ptr(labels), _ptr(ws), _ptr(group_label), _ptr(group_size),
+                            _ptr(group_mass), _ptr(group_com), _ptr(particle_group), int(cap), ctypes.byref(K),
+                            _stream_ptr(stream)), h)
+    return int(K.value)
+
+
+def fof_host_device_bytes(h, cap: int) -> int:
+    return int(lib().fof_host_device_bytes(h, int(cap)))
+
+
+def fof_run_host(h, pos_host, mass_host, labels_host, group_label_host, group_size_host, group_mass_host,
+                 group_com_host, particle_group_host, cap, dev_buf, stream=None) -> int:
+    """All *_host are CPU tensors (pinned for speed); dev_buf is a cuda uint8 tensor."""
+    K = ctypes.c_int64()
+    _check(lib().fof_run_host(h, _ptr(pos_host), _ptr(mass_host), _ptr(labels_host), _ptr(group_label_host),
+                              _ptr(group_size_host), _ptr(group_mass_host), _ptr(group_com_host),
+                              _ptr(particle_group_host), int(cap), ctypes.byref(K), _ptr(dev_buf),
+                              _stream_ptr(stream)), h)
+    return int(K.value)
+
+
+def fof_status(h, ws, stream=None) -> int:
+    return int(lib().fof_status(h, _ptr(ws), _stream_ptr(stream)))
+
+
+# ---------------------------------------------------------------- convenience object
+class FoF:
+    """Owns a plan handle and its device workspace (torch uint8 tensor)."""
+
+    def __init__(self, N: int, L: float, b: float, N_min: int = 20, device="cuda:0", grid: int | None = None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2510_26851_b200 needs a CUDA device: there is no CPU fallback")
+        self.N, self.L, self.b, self.N_min = int(N), _f(L), _f(b), int(N_min)
+        self.device = torch.device(device)
+        self.h = fof_create(N, L, b, N_min)
+        if grid is not None:
+            fof_set_grid(self.h, grid)
+        self.cap = max(1, self.N // self.N_min)
+        with torch.cuda.device(self.device):
+            self.ws = torch.empty(fof_workspace_bytes(self.h) + 256, dtype=torch.uint8, device=self.device)
+        assert self.ws.data_ptr() % 256 == 0
+
+    @property
+    def grid(self):
+        return fof_get_grid(self.h)
+
+    def close(self):
+        if getattr(self, "h", None) is not None:
+            fof_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def link(self, pos, labels=None, stream=None):
+        import torch
+
+        assert pos.is_cuda and pos.dtype == torch.float32 and pos.is_contiguous() and pos.shape == (self.N, 3)
+        if labels is None:
+            labels = torch.empty(self.N, dtype=torch.int32, device=pos.device)
+        with torch.cuda.device(self.device):
+            fof_link(self.h, pos, labels, self.ws, stream)
+        return labels
+
+    def link_stats(self, stream=None):
+        with __import__("torch").cuda.device(self.device):
+            return fof_link_stats(self.h, self.ws, stream)
+
+    def status(self, stream=None) -> int:
+        with __import__("torch").cuda.device(self.device):
+            return fof_status(self.h, self.ws, stream)
+
+    def alloc_groups(self, cap=None, particle_group=False):
+        import torch
+
+        cap = self.cap if cap is None else int(cap)
+        d = self.device
+        out = dict(cap=cap,
+                   group_label=torch.empty(cap, dtype=torch.int32, device=d),
+                   group_size=torch.empty(cap, dtype=torch.int32, device=d),
+                   group_mass=torch.empty(cap, dtype=torch.float32, device=d),
+                   group_com=torch.empty((cap, 3), dtype=torch.float32, device=d),
+                   particle_group=torch.empty(self.N, dtype=torch.int32, device=d) if particle_group else None)
+        return out
+
+    def groups(self, pos, labels, mass=None, out=None, particle_group=False, stream=None):
+        """Returns dict(K, group_label[:K], group_size[:K], group_mass[:K], group_com[:K], particle_group)."""
+        import torch
+
+        if out is None:
+            out = self.alloc_groups(particle_group=particle_group)
+        with torch.cuda.device(self.device):
+            K = fof_groups(self.h, pos, mass, labels, self.ws, out["group_label"], out["group_size"],
+                           out["group_mass"], out["group_com"], out["particle_group"], out["cap"], stream)
+        return dict(K=K, group_label=out["group_label"][:K], group_size=out["group_size"][:K],
+                    group_mass=out["group_mass"][:K], group_com=out["group_com"][:K],
+                    particle_group=out["particle_group"])

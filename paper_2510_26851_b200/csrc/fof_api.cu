@@ -1,0 +1,280 @@
+// fof_api.cu — the C ABI declared in include/fof.h: plan (H0), workspace layout, call sequencing.
+// No device memory is allocated here; every step of the path runs in the kernels of this library.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "fof_internal.cuh"
+
+using namespace fof;
+
+namespace {
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// H0: workspace layout for the current grid.
+void layout(fof_handle *h)
+{
+    const size_t N = (size_t)h->N;
+    h->C = (int64_t)h->n * h->n * h->n;
+    const int64_t cell_items = h->C + 1;
+    h->scan_tiles = (cell_items + kScanTile - 1) / kScanTile;
+    h->gscan_tiles = h->N > 0 ? (h->N + kScanTile - 1) / kScanTile : 1;
+    h->max_groups = h->N / h->N_min;
+    size_t off = 0;
+    h->off_ctrl = off;        off += 256;
+    h->off_cell = off;        off += align256(((size_t)cell_items + 8) * sizeof(unsigned int));
+    h->off_rank = off;        off += align256((N + 1) * sizeof(unsigned int));
+    h->off_sorted = off;      off += align256((N + 1) * sizeof(float4));
+    h->off_scan_state = off;  off += align256((size_t)h->scan_tiles * sizeof(unsigned long long));
+    h->off_cnt = off;         off += align256((N + 1) * sizeof(int));
+    h->off_acc = off;         off += align256(((size_t)h->max_groups + 1) * 4 * sizeof(double));
+    h->off_gscan_state = off; off += align256((size_t)h->gscan_tiles * sizeof(unsigned long long));
+    h->ws_bytes = off;
+    h->grid.L = h->L;
+    h->grid.h = 0.5f * h->L;
+    h->grid.b2 = h->b * h->b;  // host float multiply: one rounding, no FMA possible
+    h->grid.inv_cell = (float)((double)h->n / (double)h->L);
+    h->grid.n = h->n;
+    h->grid.n_minus_1 = h->n - 1;
+    h->linked = false;
+    h->linked_ws = nullptr;
+}
+
+int cuda_fail(fof_handle *h, cudaError_t e, const char *where)
+{
+    snprintf(h->cuda_err, sizeof(h->cuda_err), "%s: %s", where, cudaGetErrorString(e));
+    (void)cudaGetLastError();
+    return FOF_ERR_CUDA;
+}
+
+#define CK(call, where)                                   \
+    do {                                                  \
+        cudaError_t e__ = (call);                         \
+        if (e__ != cudaSuccess) return cuda_fail(h, e__, where); \
+    } while (0)
+
+template <typename T>
+inline T *at(void *ws, size_t off) { return reinterpret_cast<T *>(static_cast<char *>(ws) + off); }
+
+}  // namespace
+
+extern "C" {
+
+float fof_linking_length(float b_frac, float L, int64_t N)
+{
+    if (N <= 0) return 0.0f;
+    return (float)((double)b_frac * (double)L / cbrt((double)N));
+}
+
+int fof_create(int64_t N, float L, float b, int32_t N_min, fof_handle **out)
+{
+    if (!out) return FOF_ERR_INVALID_ARG;
+    if (N < 0 || N > 2147483647LL - 1024) return FOF_ERR_INVALID_ARG;
+    if (!(L > 0.0f) || !(b > 0.0f) || !isfinite(L) || !isfinite(b) || N_min < 1) return FOF_ERR_INVALID_ARG;
+    // largest grid whose cell side L/n is >= b * kCellMargin (PAPER.md:194 with the safe rounding)
+    double nm = floor((double)L / ((double)b * (double)kCellMargin));
+    if (nm < 3.0) return FOF_ERR_UNSUPPORTED;
+    int32_t n_max = nm > (double)kMaxGrid ? kMaxGrid : (int32_t)nm;
+    // about one cell per particle keeps the cell arrays as small as the particle arrays
+    int32_t n_occ = (int32_t)floor(cbrt((double)(N > 27 ? N : 27)) + 1e-9);
+    fof_handle *h = new (std::nothrow) fof_handle();
+    if (!h) return FOF_ERR_INVALID_ARG;
+    memset(h, 0, sizeof(*h));
+    h->N = N; h->L = L; h->b = b; h->N_min = N_min;
+    h->n_max = n_max;
+    h->n = n_occ < n_max ? n_occ : n_max;
+    if (h->n < 3) h->n = 3;
+    h->num_sms = 0;
+    layout(h);
+    *out = h;
+    return FOF_OK;
+}
+
+void fof_destroy(fof_handle *h) { delete h; }
+
+int fof_set_grid(fof_handle *h, int32_t n)
+{
+    if (!h) return FOF_ERR_INVALID_ARG;
+    if (n < 3 || n > h->n_max) return FOF_ERR_INVALID_ARG;
+    h->n = n;
+    layout(h);
+    return FOF_OK;
+}
+
+int fof_get_grid(const fof_handle *h, int32_t *n, int64_t *cells, int32_t *n_max)
+{
+    if (!h) return FOF_ERR_INVALID_ARG;
+    if (n) *n = h->n;
+    if (cells) *cells = h->C;
+    if (n_max) *n_max = h->n_max;
+    return FOF_OK;
+}
+
+size_t fof_workspace_bytes(const fof_handle *h) { return h ? h->ws_bytes : 0; }
+
+int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *stream)
+{
+    if (!h || !ws || ((uintptr_t)ws & 255)) return FOF_ERR_INVALID_ARG;
+    if (h->N > 0 && (!pos || !labels)) return FOF_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (h->num_sms == 0) {
+        int dev = 0, sms = 0;
+        CK(cudaGetDevice(&dev), "cudaGetDevice");
+        CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute");
+        h->num_sms = sms;
+    }
+    Ctrl *ctrl = at<Ctrl>(ws, h->off_ctrl);
+    unsigned int *cell = at<unsigned int>(ws, h->off_cell);
+    unsigned int *rank = at<unsigned int>(ws, h->off_rank);
+    float4 *sorted = at<float4>(ws, h->off_sorted);
+    unsigned long long *state = at<unsigned long long>(ws, h->off_scan_state);
+    h->linked = false;
+    // ctrl + cell counters are contiguous: one memset; scan state: another
+    CK(cudaMemsetAsync(ws, 0, h->off_rank, s), "memset cells");
+    CK(cudaMemsetAsync(state, 0, (size_t)h->scan_tiles * sizeof(unsigned long long), s), "memset scan state");
+    CK(launch_bin(pos, h->N, h->grid, cell, rank, labels, ctrl, s), "bin_kernel");
+    CK(launch_cell_scan(cell, h->C + 1, state, ctrl, h->scan_tiles, s), "cell_scan_kernel");
+    CK(launch_scatter(pos, h->N, h->grid, cell, rank, sorted, s), "scatter_kernel");
+    CK(launch_link(sorted, h->N, h->grid, cell, labels, ctrl, h->num_sms, s), "link_kernel");
+    CK(launch_flatten(labels, h->N, s), "flatten_kernel");
+    h->linked = true;
+    h->linked_ws = ws;
+    return FOF_OK;
+}
+
+int fof_link_stats(fof_handle *h, void *ws, void *stream, uint64_t *edges_host, uint64_t *pair_tests_host)
+{
+    if (!h || !ws) return FOF_ERR_INVALID_ARG;
+    if (!h->linked || h->linked_ws != ws) return FOF_ERR_STATE;
+    cudaStream_t s = (cudaStream_t)stream;
+    Ctrl c;
+    CK(cudaMemcpyAsync(&c, at<Ctrl>(ws, h->off_ctrl), sizeof(Ctrl), cudaMemcpyDeviceToHost, s), "copy ctrl");
+    CK(cudaStreamSynchronize(s), "sync");
+    if (edges_host) *edges_host = c.edges;
+    if (pair_tests_host) *pair_tests_host = c.pair_tests;
+    return FOF_OK;
+}
+
+int fof_groups(fof_handle *h, const float *pos, const float *mass, const int32_t *labels, void *ws,
+               int32_t *group_label, int32_t *group_size, float *group_mass, float *group_com,
+               int32_t *particle_group, int64_t cap, int64_t *K_host, void *stream)
+{
+    if (!h || !ws || ((uintptr_t)ws & 255) || !K_host || cap < 0) return FOF_ERR_INVALID_ARG;
+    if (h->N > 0 && (!pos || !labels)) return FOF_ERR_INVALID_ARG;
+    if (cap > 0 && (!group_label || !group_size || !group_mass || !group_com)) return FOF_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    Ctrl *ctrl = at<Ctrl>(ws, h->off_ctrl);
+    int *cnt = at<int>(ws, h->off_cnt);
+    double *acc = at<double>(ws, h->off_acc);
+    unsigned long long *state = at<unsigned long long>(ws, h->off_gscan_state);
+    *K_host = 0;
+    CK(cudaMemsetAsync(&ctrl->gscan_ticket, 0, sizeof(unsigned int), s), "memset ticket");
+    CK(cudaMemsetAsync(&ctrl->K, 0, sizeof(long long), s), "memset K");
+    CK(cudaMemsetAsync(cnt, 0, (size_t)(h->N + 1) * sizeof(int), s), "memset cnt");
+    CK(cudaMemsetAsync(state, 0, (size_t)h->gscan_tiles * sizeof(unsigned long long), s), "memset gscan state");
+    CK(launch_group_count(labels, h->N, cnt, s), "group_count_kernel");
+    CK(launch_group_compact(labels, h->N, h->N_min, cnt, cap, group_label, group_size, acc, state, ctrl,
+                            h->gscan_tiles, s), "group_compact_kernel");
+    CK(launch_group_reduce(pos, mass, labels, h->N, h->grid, cnt, cap, acc, particle_group, s),
+       "group_reduce_kernel");
+    const int64_t fin = cap < h->max_groups ? cap : h->max_groups;
+    CK(launch_group_finish(pos, group_label, group_size, acc, mass != nullptr, h->grid, fin, ctrl, group_mass,
+                           group_com, s), "group_finish_kernel");
+    long long K = 0;
+    CK(cudaMemcpyAsync(&K, &ctrl->K, sizeof(K), cudaMemcpyDeviceToHost, s), "copy K");
+    CK(cudaStreamSynchronize(s), "sync");
+    *K_host = (int64_t)K;
+    if (K > cap) return FOF_ERR_CAPACITY;
+    return FOF_OK;
+}
+
+size_t fof_host_device_bytes(const fof_handle *h, int64_t cap)
+{
+    if (!h || cap < 0) return 0;
+    const size_t N = (size_t)h->N;
+    size_t off = 0;
+    off += align256((N + 1) * 3 * sizeof(float));  // pos
+    off += align256((N + 1) * sizeof(float));      // mass
+    off += align256((N + 1) * sizeof(int));        // labels
+    off += align256((N + 1) * sizeof(int));        // particle_group
+    off += align256(((size_t)cap + 1) * sizeof(int)) * 2;    // group_label, group_size
+    off += align256(((size_t)cap + 1) * sizeof(float));      // group_mass
+    off += align256(((size_t)cap + 1) * 3 * sizeof(float));  // group_com
+    off += h->ws_bytes;
+    return off;
+}
+
+int fof_run_host(fof_handle *h, const float *pos_host, const float *mass_host, int32_t *labels_host,
+                 int32_t *group_label_host, int32_t *group_size_host, float *group_mass_host,
+                 float *group_com_host, int32_t *particle_group_host, int64_t cap, int64_t *K_host,
+                 void *dev_buf, void *stream)
+{
+    if (!h || !dev_buf || ((uintptr_t)dev_buf & 255) || !K_host || cap < 0) return FOF_ERR_INVALID_ARG;
+    if (h->N > 0 && (!pos_host || !labels_host)) return FOF_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t N = (size_t)h->N;
+    char *p = static_cast<char *>(dev_buf);
+    float *pos = (float *)p;      p += align256((N + 1) * 3 * sizeof(float));
+    float *mass = (float *)p;     p += align256((N + 1) * sizeof(float));
+    int *labels = (int *)p;       p += align256((N + 1) * sizeof(int));
+    int *pgroup = (int *)p;       p += align256((N + 1) * sizeof(int));
+    int *glabel = (int *)p;       p += align256(((size_t)cap + 1) * sizeof(int));
+    int *gsize = (int *)p;        p += align256(((size_t)cap + 1) * sizeof(int));
+    float *gmass = (float *)p;    p += align256(((size_t)cap + 1) * sizeof(float));
+    float *gcom = (float *)p;     p += align256(((size_t)cap + 1) * 3 * sizeof(float));
+    void *ws = p;
+    if (N) CK(cudaMemcpyAsync(pos, pos_host, N * 3 * sizeof(float), cudaMemcpyHostToDevice, s), "H2D pos");
+    if (N && mass_host) CK(cudaMemcpyAsync(mass, mass_host, N * sizeof(float), cudaMemcpyHostToDevice, s), "H2D mass");
+    int rc = fof_link(h, pos, labels, ws, s);
+    if (rc != FOF_OK) return rc;
+    if (N) CK(cudaMemcpyAsync(labels_host, labels, N * sizeof(int), cudaMemcpyDeviceToHost, s), "D2H labels");
+    rc = fof_groups(h, pos, mass_host ? mass : nullptr, labels, ws, glabel, gsize, gmass, gcom,
+                    particle_group_host ? pgroup : nullptr, cap, K_host, s);
+    if (rc != FOF_OK) return rc;
+    const size_t K = (size_t)*K_host;
+    if (K) {
+        CK(cudaMemcpyAsync(group_label_host, glabel, K * sizeof(int), cudaMemcpyDeviceToHost, s), "D2H group_label");
+        CK(cudaMemcpyAsync(group_size_host, gsize, K * sizeof(int), cudaMemcpyDeviceToHost, s), "D2H group_size");
+        CK(cudaMemcpyAsync(group_mass_host, gmass, K * sizeof(float), cudaMemcpyDeviceToHost, s), "D2H group_mass");
+        CK(cudaMemcpyAsync(group_com_host, gcom, K * 3 * sizeof(float), cudaMemcpyDeviceToHost, s), "D2H group_com");
+    }
+    if (N && particle_group_host)
+        CK(cudaMemcpyAsync(particle_group_host, pgroup, N * sizeof(int), cudaMemcpyDeviceToHost, s), "D2H particle_group");
+    CK(cudaStreamSynchronize(s), "sync");
+    Ctrl c;
+    CK(cudaMemcpy(&c, at<Ctrl>(ws, h->off_ctrl), sizeof(Ctrl), cudaMemcpyDeviceToHost), "copy ctrl");
+    if (c.error & 1u) return FOF_ERR_NONFINITE;
+    return FOF_OK;
+}
+
+int fof_status(fof_handle *h, void *ws, void *stream)
+{
+    if (!h || !ws) return FOF_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    Ctrl c;
+    CK(cudaMemcpyAsync(&c, at<Ctrl>(ws, h->off_ctrl), sizeof(Ctrl), cudaMemcpyDeviceToHost, s), "copy ctrl");
+    CK(cudaStreamSynchronize(s), "sync");
+    if (c.error & 1u) return FOF_ERR_NONFINITE;
+    return FOF_OK;
+}
+
+const char *fof_error_string(int code)
+{
+    switch (code) {
+    case FOF_OK: return "ok";
+    case FOF_ERR_INVALID_ARG: return "invalid argument";
+    case FOF_ERR_UNSUPPORTED: return "unsupported: fewer than 3 cells of side >= b per axis";
+    case FOF_ERR_CUDA: return "CUDA runtime error";
+    case FOF_ERR_NONFINITE: return "non-finite position";
+    case FOF_ERR_CAPACITY: return "more groups than capacity";
+    case FOF_ERR_STATE: return "call order violated";
+    default: return "unknown error";
+    }
+}
+
+const char *fof_last_cuda_error(const fof_handle *h) { return h ? h->cuda_err : ""; }
+
+}  // extern "C"

@@ -1,0 +1,168 @@
+// fof_internal.cuh — plan, workspace layout and the device-side arithmetic shared by the kernels
+// of libfof_b200.so.  sm_100a only.  Nothing here is shared with oracle/ (the CPU oracle is an
+// independent restatement of the paper).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/fof.h"
+
+namespace fof {
+
+constexpr int kBlock = 256;           // threads per CTA for the streaming kernels
+constexpr int kScanItems = 8;         // items per thread in the single-pass scan
+constexpr int kScanTile = kBlock * kScanItems;
+constexpr float kCellMargin = 1.001f; // cell side >= b * kCellMargin  (R3)
+constexpr int kMaxGrid = 1290;        // n^3 < 2^31
+
+// Device control block at the start of the workspace (zeroed at the start of fof_link).
+struct Ctrl {
+    unsigned int error;        // bit 0: non-finite position seen
+    unsigned int scan_ticket;  // dynamic tile id for the cell scan
+    unsigned int gscan_ticket; // dynamic tile id for the group compaction scan
+    unsigned int pad0;
+    unsigned long long edges;       // true edges (unordered pairs with d2 <= b2)
+    unsigned long long pair_tests;  // distance tests executed
+    long long K;                    // kept groups (written by fof_groups)
+    unsigned int link_ticket;       // dynamic work id for the link kernel
+    unsigned int pad1[7];
+};
+static_assert(sizeof(Ctrl) <= 256, "Ctrl must fit its 256-byte slot");
+
+// Everything a kernel needs to know about the box and the grid, passed by value.
+struct Grid {
+    float L;        // box side
+    float h;        // 0.5 * L
+    float b2;       // fl(b * b)
+    float inv_cell; // fl(n / L)
+    int n;          // cells per axis
+    int n_minus_1;
+};
+
+}  // namespace fof
+
+struct fof_handle {
+    int64_t N;
+    float L, b;
+    int32_t N_min;
+    int32_t n, n_max;
+    int64_t C;  // n^3
+    fof::Grid grid;
+    // workspace layout (byte offsets, 256-B aligned)
+    size_t off_ctrl, off_cell, off_rank, off_sorted, off_scan_state, off_cnt, off_acc, off_gscan_state;
+    size_t ws_bytes;
+    int64_t scan_tiles, gscan_tiles, max_groups;
+    int num_sms;
+    bool linked;
+    const void *linked_ws;
+    char cuda_err[256];
+};
+
+namespace fof {
+
+// ---- wrap into [0, L): "X <- X mod L" (R6).  Explicit _rn intrinsics so
+// that nvcc cannot contract the multiply-subtract into an FMA.
+__device__ __forceinline__ float wrap1(float x, float L)
+{
+    if (x >= 0.0f && x < L) return x;
+    float t = __fdiv_rn(x, L);
+    float w = __fsub_rn(x, __fmul_rn(L, floorf(t)));
+    if (w < 0.0f) w = __fadd_rn(w, L);
+    if (w >= L) w = 0.0f;
+    return w;
+}
+
+// ---- cell coordinate of a wrapped coordinate ("cell triple"); monotone in w.
+__device__ __forceinline__ int cell1(float w, const Grid &g)
+{
+    int c = __float2int_rd(__fmul_rn(w, g.inv_cell));
+    return min(max(c, 0), g.n_minus_1);
+}
+
+// linear id, x fastest (c = i_x + n_x (i_y + n_y i_z))
+__device__ __forceinline__ unsigned int cell_id(int cx, int cy, int cz, int n)
+{
+    return (unsigned int)cx + (unsigned int)n * ((unsigned int)cy + (unsigned int)n * (unsigned int)cz);
+}
+
+// ---- link predicate (north_star's single float32 expression):
+// per axis d = wi - wj; d > h ? d - L : (d < -h ? d + L : d);  d2 = (dx dx + dy dy) + dz dz <= b2.
+__device__ __forceinline__ float min_image(float d, float L, float h)
+{
+    if (d > h) d = __fsub_rn(d, L);
+    else if (d < -h) d = __fadd_rn(d, L);
+    return d;
+}
+
+__device__ __forceinline__ bool linked(float xi, float yi, float zi, float xj, float yj, float zj, const Grid &g)
+{
+    float dx = min_image(__fsub_rn(xi, xj), g.L, g.h);
+    float dy = min_image(__fsub_rn(yi, yj), g.L, g.h);
+    float dz = min_image(__fsub_rn(zi, zj), g.L, g.h);
+    float d2 = __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
+    return d2 <= g.b2;
+}
+
+// ---- lock-free union-find on the label array itself (parent[i] <= i; root = minimum index of its
+// set, which IS the canonical label: "minimum label", "minimum global
+// particle ID").  Hooks with atomicCAS at roots only; finds use path halving (plain stores of an
+// ancestor at non-roots are benign).
+__device__ __forceinline__ int find_root(int *parent, int x)
+{
+    int p = parent[x];
+    while (p != x) {
+        int gp = parent[p];
+        if (gp != p) parent[x] = gp;
+        x = p;
+        p = gp;
+    }
+    return x;
+}
+
+__device__ __forceinline__ void unite(int *parent, int a, int b)
+{
+    int ra = find_root(parent, a);
+    int rb = find_root(parent, b);
+    while (ra != rb) {
+        if (ra < rb) { int t = ra; ra = rb; rb = t; }  // ra is the larger root
+        int old = atomicCAS(parent + ra, ra, rb);
+        if (old == ra) return;
+        ra = find_root(parent, old);
+    }
+}
+
+__device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long *p)
+{
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+
+__device__ __forceinline__ void st_relaxed_u64(unsigned long long *p, unsigned long long v)
+{
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
+// kernels (one launcher per step; all asynchronous on `s`)
+cudaError_t launch_bin(const float *pos, int64_t N, Grid g, unsigned int *cell_count, unsigned int *rank,
+                       int *labels, Ctrl *ctrl, cudaStream_t s);
+cudaError_t launch_cell_scan(unsigned int *cell, int64_t n_items, unsigned long long *state, Ctrl *ctrl,
+                             int64_t tiles, cudaStream_t s);
+cudaError_t launch_scatter(const float *pos, int64_t N, Grid g, const unsigned int *cell_start,
+                           const unsigned int *rank, float4 *sorted, cudaStream_t s);
+cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start, int *labels,
+                        Ctrl *ctrl, int num_sms, cudaStream_t s);
+cudaError_t launch_flatten(int *labels, int64_t N, cudaStream_t s);
+
+cudaError_t launch_group_count(const int *labels, int64_t N, int *cnt, cudaStream_t s);
+cudaError_t launch_group_compact(const int *labels, int64_t N, int N_min, int *cnt_to_gid, int64_t cap,
+                                 int *group_label, int *group_size, double *acc, unsigned long long *state,
+                                 Ctrl *ctrl, int64_t tiles, cudaStream_t s);
+cudaError_t launch_group_reduce(const float *pos, const float *mass, const int *labels, int64_t N, Grid g,
+                                const int *gid, int64_t cap, double *acc, int *particle_group, cudaStream_t s);
+cudaError_t launch_group_finish(const float *pos, const int *group_label, const int *group_size,
+                                const double *acc, bool has_mass, Grid g, int64_t cap, const Ctrl *ctrl,
+                                float *group_mass, float *group_com, cudaStream_t s);
+
+}  // namespace fof

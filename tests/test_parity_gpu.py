@@ -1,0 +1,319 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Bars (BASELINE.json north_star): labels, group labels, sizes,
+particle->group map and the edge count E bit-exact; masses within 1e-5 relative; periodic centre
+of mass within 1e-5 * L per component.  Needs a B200: `pytest -m gpu`.
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2510_26851_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2510_26851_b200 import binding
+
+    binding.lib()  # fails loudly if libfof_b200.so is missing
+    return binding
+
+
+def gpu_fof(B, pos, L, b, N_min, mass=None, grid=None, particle_group=True):
+    N = len(pos)
+    f = B.FoF(N, L, b, N_min, grid=grid)
+    dpos = torch.from_numpy(np.ascontiguousarray(pos, dtype=np.float32)).cuda().reshape(N, 3)
+    dmass = None if mass is None else torch.from_numpy(mass).cuda()
+    labels = f.link(dpos)
+    status = f.status()
+    E, tests = f.link_stats()
+    g = f.groups(dpos, labels, mass=dmass, particle_group=particle_group)
+    out = dict(labels=labels.cpu().numpy(), E=E, tests=tests, status=status, K=g["K"], grid=f.grid,
+               group_label=g["group_label"].cpu().numpy(), group_size=g["group_size"].cpu().numpy(),
+               group_mass=g["group_mass"].cpu().numpy(), group_com=g["group_com"].cpu().numpy(),
+               particle_group=None if g["particle_group"] is None else g["particle_group"].cpu().numpy())
+    f.close()
+    return out
+
+
+def check_against_oracle(B, pos, L, b, N_min, mass=None, grid=None, brute=False):
+    lab, E = (oracle.labels_brute if brute else oracle.labels_cells)(pos, L, b)
+    og = oracle.groups(pos, lab, L, N_min, mass=mass)
+    got = gpu_fof(B, pos, L, b, N_min, mass=mass, grid=grid)
+    assert got["status"] == 0
+    assert np.array_equal(got["labels"], lab), "canonical labels differ"
+    assert got["E"] == E, "edge count differs"
+    assert got["K"] == og["K"]
+    assert np.array_equal(got["group_label"], og["group_label"])
+    assert np.array_equal(got["group_size"], og["group_size"])
+    assert np.array_equal(got["particle_group"], og["particle_group"])
+    if og["K"]:
+        assert np.all(np.abs(got["group_mass"] - og["group_mass"]) <= 1e-5 * og["group_mass"])
+        if mass is None:
+            assert np.array_equal(got["group_mass"], og["group_size"].astype(np.float32))
+        d = np.abs(got["group_com"].astype(np.float64) - og["group_com"])
+        d = np.minimum(d, float(np.float32(L)) - d)
+        assert d.max() <= 1e-5 * L, f"centre of mass off by {d.max()}"
+    return got, lab, og
+
+
+# --------------------------------------------------------------------------- closed forms, tiny
+def test_lattice(B):
+    n, L = 16, 16.0
+    p = inputs.lattice(n, L)
+    got = gpu_fof(B, p, L, 0.999, 1)
+    assert got["E"] == 0 and np.array_equal(got["labels"], np.arange(n ** 3))
+    assert got["K"] == n ** 3
+    got = gpu_fof(B, p, L, 1.0, 20)
+    assert got["E"] == 3 * n ** 3 and (got["labels"] == 0).all()
+    assert got["K"] == 1 and got["group_size"][0] == n ** 3
+    check_against_oracle(B, p, L, 1.0, 20)
+
+
+def test_planted_cliques(B):
+    sizes = [1, 2, 3, 20, 21, 57, 300, 19, 5, 64, 1000]
+    L, b = 64.0, 1.0
+    p, ids = inputs.planted_cliques(10, sizes, L, b)
+    got, lab, _ = check_against_oracle(B, p, L, b, 20)
+    assert got["E"] == sum(s * (s - 1) // 2 for s in sizes)
+    assert sorted(got["group_size"].tolist()) == sorted(s for s in sizes if s >= 20)
+
+
+def test_chain_wraps_the_box(B):
+    L, n = 32.0, 64
+    p = inputs.chain(n, L)
+    got = gpu_fof(B, p, L, 0.5 / 0.9, 2)
+    assert (got["labels"] == 0).all() and got["E"] == n
+    got = gpu_fof(B, p, L, 0.5 / 1.1, 2)
+    assert got["E"] == 0 and got["K"] == 0
+
+
+@pytest.mark.parametrize("case", ["uniform", "adversarial", "dense", "unwrapped"])
+def test_against_brute_force(B, case):
+    rng = np.random.default_rng(3)
+    if case == "uniform":
+        L, b = 1.0, 0.06
+        p = rng.random((3000, 3)).astype(np.float32)
+    elif case == "adversarial":
+        from test_oracle_pins import _adversarial
+
+        L, b = 8.0, 0.5
+        p = _adversarial(4, L, b)
+    elif case == "dense":
+        L, b = 2.0, 0.11
+        p = (rng.standard_normal((2500, 3)) * 0.15 + 1.0).astype(np.float32) % np.float32(L)
+    else:  # positions far outside [0, L): the wrap is part of the path
+        L, b = 3.7, 0.2
+        p = (rng.standard_normal((3000, 3)) * 9).astype(np.float32)
+    for grid in (None, 3, "max"):
+        if grid == "max":
+            grid = int(np.floor(L / (float(np.float32(b)) * 1.001)))
+        check_against_oracle(B, p, L, b, 5, brute=True, grid=grid)
+
+
+def test_gpu_grid_cell_faces(B):
+    """points on the faces of the GPU's own grids (+-1 ulp) and pairs at exactly b, b(1 +- 2^-23)."""
+    rng = np.random.default_rng(21)
+    L, b = 8.0, 0.5
+    for n in (3, 7, 15):
+        faces = (rng.integers(0, n, (400, 3)) * (L / n)).astype(np.float32)
+        base = (rng.random((300, 3)) * L).astype(np.float32)
+        sh = base.copy()
+        sh[:100, 0] += np.float32(b)
+        sh[100:200, 1] += np.float32(b * (1 + 2.0 ** -23))
+        sh[200:, 2] += np.float32(b * (1 - 2.0 ** -23))
+        p = np.concatenate([faces, np.nextafter(faces, np.float32(-1)), np.nextafter(faces, np.float32(99)),
+                            base, sh]).astype(np.float32)
+        p = np.mod(p, np.float32(L))
+        p[p >= np.float32(L)] = 0
+        check_against_oracle(B, p, L, b, 3, grid=n)
+
+
+# --------------------------------------------------------------------------- BASELINE configs
+def test_cfg0(B):
+    w = inputs.CONFIGS["cfg0"]
+    p = inputs.make_positions(w)
+    got, lab, og = check_against_oracle(B, p, w.L, w.b, w.N_min)
+    assert og["K"] > 10
+    check_against_oracle(B, p, w.L, w.b, w.N_min, mass=inputs.make_masses(w))
+    check_against_oracle(B, p, w.L, w.b, 1, grid=got["grid"][2])        # N_min = 1, tightest grid
+
+
+def test_cfg1_scaled_several_grids(B):
+    w = inputs.scaled(inputs.CONFIGS["cfg1"], 48)
+    p = inputs.make_positions(w)
+    m = inputs.make_masses(w)
+    for grid in (None, 5, 100):
+        check_against_oracle(B, p, w.L, w.b, w.N_min, mass=m, grid=grid)
+
+
+def test_cfg1_full(B):
+    w = inputs.CONFIGS["cfg1"]
+    p = inputs.make_positions(w)
+    got, lab, og = check_against_oracle(B, p, w.L, w.b, w.N_min)
+    assert og["K"] > 10000
+    check_against_oracle(B, p, w.L, w.b, w.N_min, mass=inputs.make_masses(w))
+
+
+@pytest.mark.slow
+def test_cfg2_full(B):
+    """The headline workload (256^3), in the launch configuration bench.py times."""
+    w = inputs.CONFIGS["cfg2"]
+    p = inputs.make_positions(w)
+    got, lab, og = check_against_oracle(B, p, w.L, w.b, w.N_min)
+    assert og["K"] > 100000
+
+
+@pytest.mark.parametrize("b_frac", [0.1, 0.2, 0.3, 0.4])
+def test_cfg4_scaled_sweep(B, b_frac):
+    w = dataclasses.replace(inputs.scaled(inputs.CONFIGS["cfg4_b0.2"], 96), b_frac=b_frac)
+    p = inputs.make_positions(w)
+    check_against_oracle(B, p, w.L, w.b, w.N_min)
+
+
+def test_cfg3_scaled(B):
+    w = inputs.scaled(inputs.CONFIGS["cfg3"], 128)
+    p = inputs.make_positions(w)
+    check_against_oracle(B, p, w.L, w.b, w.N_min)
+
+
+# --------------------------------------------------------------------------- stress: giant component, dense cells
+def test_percolating_giant_component(B):
+    """Poisson points at b = 1.0 x spacing (above the continuum percolation threshold ~0.87): one
+    component holds most particles and wraps the box — stresses atomics, long parent chains and the
+    centre of mass of a group wider than L/2."""
+    rng = np.random.default_rng(31)
+    n_side, L = 80, 80.0
+    p = (rng.random((n_side ** 3, 3)) * L).astype(np.float32)
+    got, lab, og = check_against_oracle(B, p, L, 1.0, 20, mass=rng.uniform(0.5, 1.5, len(p)).astype(np.float32))
+    assert og["group_size"].max() > 0.5 * len(p)
+
+
+def test_zeldovich_shell_crossing(B):
+    """Zel'dovich recipe with the displacement pushed past shell crossing (rms 4 spacings): caustics,
+    filaments and knots with cells holding many particles."""
+    w = dataclasses.replace(inputs.scaled(inputs.CONFIGS["cfg4_b0.4"], 96), rms=4.0)
+    p = inputs.make_positions(w)
+    got, lab, og = check_against_oracle(B, p, w.L, w.b, w.N_min)
+    assert og["K"] > 100
+
+
+def test_one_dense_clump_many_per_cell(B):
+    rng = np.random.default_rng(33)
+    L, b = 100.0, 1.0
+    clump = rng.standard_normal((20000, 3)) * 1.5 + 50.0
+    bg = rng.random((20000, 3)) * L
+    p = np.concatenate([bg, clump]).astype(np.float32) % np.float32(L)
+    p = p[rng.permutation(len(p))]
+    check_against_oracle(B, p, L, b, 20)
+
+
+# --------------------------------------------------------------------------- invariants
+def test_permutation_invariance_on_gpu(B):
+    w = inputs.scaled(inputs.CONFIGS["cfg1"], 40)
+    p = inputs.make_positions(w)
+    a = gpu_fof(B, p, w.L, w.b, w.N_min)
+    perm = np.random.default_rng(41).permutation(len(p))
+    c = gpu_fof(B, p[perm], w.L, w.b, w.N_min)
+    assert a["E"] == c["E"] and a["K"] == c["K"]
+    assert sorted(a["group_size"].tolist()) == sorted(c["group_size"].tolist())
+    # partition identical: labels of the permuted run, mapped back, induce the same blocks
+    back = np.empty_like(c["labels"])
+    back[perm] = perm[c["labels"]]          # canonical particle expressed in ORIGINAL numbering
+    first = {}
+    for l_orig, l_perm in zip(a["labels"][:50000], back[:50000]):
+        assert first.setdefault(l_orig, l_perm) == l_perm
+
+
+def test_repeatable(B):
+    w = inputs.CONFIGS["cfg0"]
+    p = inputs.make_positions(w)
+    runs = [gpu_fof(B, p, w.L, w.b, w.N_min) for _ in range(3)]
+    for r in runs[1:]:
+        assert np.array_equal(r["labels"], runs[0]["labels"]) and r["E"] == runs[0]["E"]
+        assert np.array_equal(r["group_size"], runs[0]["group_size"])
+
+
+# --------------------------------------------------------------------------- edge cases and errors
+def test_empty_and_tiny(B):
+    got = gpu_fof(B, np.zeros((0, 3), np.float32), 1.0, 0.1, 20)
+    assert got["K"] == 0 and got["E"] == 0 and len(got["labels"]) == 0
+    got = gpu_fof(B, np.array([[0.5, 0.5, 0.5]], np.float32), 1.0, 0.1, 1)
+    assert got["K"] == 1 and got["labels"][0] == 0 and got["group_size"][0] == 1
+    assert np.allclose(got["group_com"][0], 0.5)
+    p = np.zeros((5, 3), np.float32)                    # coincident particles link (d = 0)
+    got = gpu_fof(B, p, 1.0, 0.1, 1)
+    assert (got["labels"] == 0).all() and got["E"] == 10 and got["group_size"][0] == 5
+
+
+def test_nonfinite_sets_status(B):
+    p = np.random.default_rng(5).random((1000, 3)).astype(np.float32)
+    p[17, 1] = np.nan
+    got = gpu_fof(B, p, 1.0, 0.05, 20)
+    assert got["status"] == B.FOF_ERR_NONFINITE
+    p[17, 1] = np.inf
+    assert gpu_fof(B, p, 1.0, 0.05, 20)["status"] == B.FOF_ERR_NONFINITE
+
+
+def test_capacity_error(B):
+    sizes = [30] * 8
+    p, _ = inputs.planted_cliques(10, sizes, 64.0, 1.0)
+    f = B.FoF(len(p), 64.0, 1.0, 20)
+    dpos = torch.from_numpy(p).cuda()
+    labels = f.link(dpos)
+    out = f.alloc_groups(cap=4)
+    with pytest.raises(B.FofError) as e:
+        f.groups(dpos, labels, out=out)
+    assert e.value.code == B.FOF_ERR_CAPACITY
+    g = f.groups(dpos, labels)
+    assert g["K"] == 8
+
+
+def test_groups_is_stateless_on_given_labels(B):
+    """fof_groups works from (pos, labels) alone — here labels from the oracle, fresh workspace."""
+    w = inputs.scaled(inputs.CONFIGS["cfg1"], 32)
+    p = inputs.make_positions(w)
+    lab, _ = oracle.labels_cells(p, w.L, w.b)
+    og = oracle.groups(p, lab, w.L, w.N_min)
+    f = B.FoF(len(p), w.L, w.b, w.N_min)
+    g = f.groups(torch.from_numpy(p).cuda(), torch.from_numpy(lab).cuda(), particle_group=True)
+    assert g["K"] == og["K"]
+    assert np.array_equal(g["group_size"].cpu().numpy(), og["group_size"])
+    assert np.array_equal(g["particle_group"].cpu().numpy(), og["particle_group"])
+
+
+def test_run_host_path(B):
+    """The host-buffer entry point (what bench.py's e2e leg times) gives the same answer."""
+    w = inputs.scaled(inputs.CONFIGS["cfg1"], 48)
+    p = inputs.make_positions(w)
+    m = inputs.make_masses(w)
+    lab, _ = oracle.labels_cells(p, w.L, w.b)
+    og = oracle.groups(p, lab, w.L, w.N_min, mass=m)
+    N = len(p)
+    h = B.fof_create(N, w.L, w.b, w.N_min)
+    cap = N // w.N_min
+    dev = torch.empty(B.fof_host_device_bytes(h, cap) + 256, dtype=torch.uint8, device="cuda")
+    hp = torch.from_numpy(p).pin_memory()
+    hm = torch.from_numpy(m).pin_memory()
+    hl = torch.empty(N, dtype=torch.int32).pin_memory()
+    gl = torch.empty(cap, dtype=torch.int32).pin_memory()
+    gs = torch.empty(cap, dtype=torch.int32).pin_memory()
+    gm = torch.empty(cap, dtype=torch.float32).pin_memory()
+    gc = torch.empty((cap, 3), dtype=torch.float32).pin_memory()
+    pg = torch.empty(N, dtype=torch.int32).pin_memory()
+    K = B.fof_run_host(h, hp, hm, hl, gl, gs, gm, gc, pg, cap, dev)
+    assert K == og["K"]
+    assert np.array_equal(hl.numpy(), lab)
+    assert np.array_equal(gs.numpy()[:K], og["group_size"])
+    assert np.array_equal(pg.numpy(), og["particle_group"])
+    assert np.all(np.abs(gm.numpy()[:K] - og["group_mass"]) <= 1e-5 * og["group_mass"])
+    d = np.abs(gc.numpy()[:K].astype(np.float64) - og["group_com"])
+    assert np.minimum(d, w.L - d).max() <= 1e-5 * w.L
+    B.fof_destroy(h)
