@@ -1,0 +1,338 @@
+#!/usr/bin/env python
+"""bench.py — periodic FoF throughput on B200 (BASELINE.json metric: linked particles/s, pair
+tests/s, achieved HBM GB/s vs peak).
+
+A "step" is one pass of the whole hot path (fof_link + fof_groups: H0-H8 of DESIGN.md §1) over
+one synthetic particle set.  Default workload: BASELINE.json configs[2] (256^3 clustered
+particles, the configuration north_star's 40 %-of-roofline target is quoted on).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2] [--impl ours|reference]
+
+N > 1 (under torchrun): the path does not shard in this build ("replicas only"):
+every rank runs an independent particle set (seed + rank); value = all ranks' particles / max time.
+`--impl reference` times the CPU oracle (oracle/, as it stands) on rank 0 only.
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2510_26851_b200 import inputs  # noqa: E402
+
+METRIC = "fof_linked_particles_per_s"
+UNIT = "particles/s"
+
+# Algorithmic bytes per particle of each profiled stage (the compulsory streams of
+# SURVEY.md §8d split per kernel).  Cell arrays, neighbour re-reads and scan state are
+# implementation cost and are deliberately NOT counted.
+ALG_BYTES_PER_PARTICLE = {
+    "link.clear": 0,
+    "link.bin": 12 + 4,            # read pos, write parent (labels[i] = i)
+    "link.cell_scan": 0,
+    "link.scatter": 12 + 16,       # read pos, write sorted (x, y, z, idx)
+    "link.pairs": 16 + 4,          # read sorted once, update parent
+    "link.flatten": 4 + 4,         # read parent, write label
+    "groups.clear": 0,
+    "groups.count": 4 + 4,         # read labels, size RMW
+    "groups.compact": 4 + 4,       # read sizes, write id map
+    "groups.reduce": 12 + 4 + 4 + 4,  # read pos, mass, labels, id
+    "groups.finish": 0,
+}
+
+
+def peaks():
+    """(hbm GB/s, source)"""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (measured copy, burst)"
+    except Exception:
+        return 6650.0, "fallback 6.65 TB/s (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.p, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.p = None
+        return self
+
+    def _read(self):
+        for line in self.p.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.p is not None:
+            time.sleep(0.15)
+            self.p.terminate()
+            try:
+                self.p.wait(timeout=2)
+            except Exception:
+                self.p.kill()
+            self.t.join(timeout=2)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def workload_for_rank(name: str, rank: int) -> inputs.Workload:
+    import dataclasses
+
+    w = inputs.CONFIGS[name]
+    return dataclasses.replace(w, seed=w.seed + 1000 * rank) if rank else w
+
+
+def time_oracle(pos, w, mass=None):
+    """One pass of the oracle (cell list + union-find + groups), wall clock, single thread."""
+    import oracle
+
+    t0 = time.perf_counter()
+    lab, E = oracle.labels_cells(pos, w.L, w.b)
+    og = oracle.groups(pos, lab, w.L, w.N_min, mass=mass)
+    return time.perf_counter() - t0, lab, E, og
+
+
+# ------------------------------------------------------------------------------------------------
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands, on the host cores, rank 0 only."""
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    w = inputs.CONFIGS[args.workload]
+    budget_s = 150.0
+    # bounded sample: the full workload if K+W passes fit the budget, else the same recipe at a
+    # smaller particle count (same density, same b, same halo population per particle)
+    probe = inputs.scaled(w, min(w.n_side, 64))
+    t_probe, *_ = time_oracle(inputs.make_positions(probe), probe)
+    per_particle = t_probe / probe.N
+    n_side = w.n_side
+    while n_side > 32 and per_particle * n_side ** 3 * (args.steps + args.warmup) > budget_s:
+        n_side //= 2
+    ws = w if n_side == w.n_side else inputs.scaled(w, n_side)
+    pos = inputs.make_positions(ws)
+    for _ in range(args.warmup):
+        time_oracle(pos, ws)
+    t = 0.0
+    for _ in range(args.steps):
+        t += time_oracle(pos, ws)[0]
+    value = ws.N * args.steps / t
+    sample = (f"{ws.name}: N={ws.N} of the workload's {w.N} particles per step"
+              + ("" if ws is w else " (same recipe, density, b and halo population per particle; smaller box)"))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": args.workload, "N": w.N, "L": w.L, "b": w.b, "N_min": w.N_min, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2510_26851_b200 import binding as B
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    B.lib()  # fail loudly if libfof_b200.so is missing
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    w = workload_for_rank(args.workload, rank)
+    pos_np = inputs.make_positions(w)
+    N = w.N
+    hpos = torch.from_numpy(pos_np).pin_memory()
+    dpos = hpos.to(dev, non_blocking=True)
+    f = B.FoF(N, w.L, w.b, w.N_min, device=dev, grid=args.grid)
+    out = f.alloc_groups()
+    labels = torch.empty(N, dtype=torch.int32, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        f.link(dpos, labels)
+        return f.groups(dpos, labels, out=out)["K"]
+
+    for _ in range(max(args.warmup, 3)):
+        K_groups = step()
+    torch.cuda.synchronize()
+
+    # ---- timed region: device-resident inputs; K steps bracketed by barrier + synchronize
+    B.fof_profile_enable(f.h, args.steps)
+    launches0 = B.fof_launch_count(f.h)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    torch.cuda.synchronize()
+    with ClockSampler(local_rank) as clk:
+        e0.record(stream)
+        for _ in range(args.steps):
+            step()
+        e1.record(stream)
+        torch.cuda.synchronize()
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    launches = B.fof_launch_count(f.h) - launches0
+    stages = B.fof_profile_read(f.h)
+    B.fof_profile_enable(f.h, 0)
+    E, pair_tests = f.link_stats()
+    t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_step = float(t.item()) / args.steps
+    value = world * N / (ms_step * 1e-3)
+
+    # ---- end to end: host buffers through the C ABI (fof_run_host), copies inside the timed region
+    cap = out["cap"]
+    h2 = B.fof_create(N, w.L, w.b, w.N_min)
+    if args.grid:
+        B.fof_set_grid(h2, args.grid)
+    dev_buf = torch.empty(B.fof_host_device_bytes(h2, cap) + 256, dtype=torch.uint8, device=dev)
+    pin = lambda *s, dt=torch.int32: torch.empty(*s, dtype=dt).pin_memory()  # noqa: E731
+    hl, gl, gs = pin(N), pin(cap), pin(cap)
+    gm, gc = pin(cap, dt=torch.float32), pin((cap, 3), dt=torch.float32)
+    e2e_steps = max(3, min(args.steps, 10))
+    for _ in range(2):
+        Kh = B.fof_run_host(h2, hpos, None, hl, gl, gs, gm, gc, None, cap, dev_buf)
+    barrier()
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(e2e_steps):
+        Kh = B.fof_run_host(h2, hpos, None, hl, gl, gs, gm, gc, None, cap, dev_buf)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    barrier()
+    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_ms = float(t.item()) / e2e_steps
+    B.fof_destroy(h2)
+    assert Kh == K_groups, (Kh, K_groups)
+    assert torch.equal(hl.to(dev), labels), "host-path labels differ from device-path labels"
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (live CUDA-event times from inside the timed region)
+    peak, peak_src = peaks()
+    top = max(stages, key=lambda k: stages[k])
+    alg = ALG_BYTES_PER_PARTICLE.get(top, 0) * N
+    achieved = alg / (stages[top] * 1e-3) / 1e9 if stages[top] > 0 else 0.0
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")  # written by hand from the ncu --set full capture
+    if os.path.exists(tpath):
+        try:
+            with open(tpath) as fh:
+                traffic = json.load(fh).get(args.workload, {}).get(top)
+        except Exception:
+            traffic = None
+    total_alg = sum(ALG_BYTES_PER_PARTICLE.get(k, 0) for k in stages) * N
+    roofline = {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                "alg_bytes_per_launch": alg, "kernel_ms": stages[top],
+                "path": {"alg_bytes_per_step": total_alg, "achieved": total_alg / (ms_step * 1e-3) / 1e9,
+                         "frac": total_alg / (ms_step * 1e-3) / 1e9 / peak,
+                         "frac_of_8000_nominal": total_alg / (ms_step * 1e-3) / 1e9 / 8000.0}}
+
+    # ---- the oracle timed beside it on the host cores (a reported baseline, not the target)
+    cpu = None
+    parity = None
+    if world == 1 and not args.no_cpu:
+        t_cpu, lab, E_ref, og = time_oracle(pos_np, w)
+        cpu = {"value": N / t_cpu, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"full workload {w.name} (N={N}), 1 pass, {t_cpu:.2f} s, host has {os.cpu_count()} cores"}
+        parity = bool(np.array_equal(labels.cpu().numpy(), lab) and E == E_ref and K_groups == og["K"]
+                      and np.array_equal(out["group_size"][:K_groups].cpu().numpy(), og["group_size"]))
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": w.name, "N": N, "L": w.L, "b": w.b, "N_min": w.N_min, "grid_n": f.grid[0],
+                   "cells": f.grid[1], "groups_kept": K_groups, "true_edges": E, "pair_tests": pair_tests,
+                   "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "l2": "inputs + workspace per step exceed the 126 MB L2 (pos 12N + sorted 16N + labels 4N ...)"
+                         if N * 32 > 126e6 else "working set fits L2 (small workload)"},
+        "pair_tests_per_s": pair_tests / (stages["link.pairs"] * 1e-3) if stages.get("link.pairs") else None,
+        "stage_ms": {k: round(v, 5) for k, v in stages.items()},
+        "roofline": roofline, "cpu_baseline": cpu, "parity_vs_oracle_in_this_run": parity,
+        "e2e": {"value": world * N / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
+                "h2d_bytes_per_step": int(hpos.numel() * 4),
+                "d2h_bytes_per_step": int(N * 4 + Kh * (4 + 4 + 4 + 12) + 8)},
+        "gpu_launches": int(launches), "clocks": clk.summary(),
+    }
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2", choices=sorted(inputs.CONFIGS))
+    ap.add_argument("--grid", type=int, default=None, help="force n cells per axis (tuning knob)")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

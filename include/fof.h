@@ -109,6 +109,21 @@ int fof_run_host(fof_handle *h, const float *pos_host, const float *mass_host, i
  * fof_groups on (h, ws): FOF_OK or FOF_ERR_NONFINITE. */
 int fof_status(fof_handle *h, void *ws, void *stream);
 
+/* Measurement aids (they never change results).
+ * fof_profile_enable(h, slots): slots > 0 makes fof_link / fof_groups record a CUDA event on
+ * `stream` before and after every stage (one kernel launch or one memset group each), into one of
+ * `slots` event sets used round-robin, one set per fof_link call (and the fof_groups calls that
+ * follow it); slots = 0 switches profiling off.  fof_profile_read synchronises the recorded events
+ * and returns, for each stage k < fof_profile_count(h), the MEAN device time in milliseconds over
+ * the sets recorded since the previous read (0 for a stage that did not run), then forgets them.
+ * fof_profile_name(h, k) is a static string ("link.bin", "groups.reduce", ...).
+ * fof_launch_count: kernels this handle has launched so far (memsets and copies not counted). */
+int fof_profile_enable(fof_handle *h, int slots);
+int fof_profile_count(const fof_handle *h);
+const char *fof_profile_name(const fof_handle *h, int k);
+int fof_profile_read(fof_handle *h, float *ms, int cap);
+uint64_t fof_launch_count(const fof_handle *h);
+
 /* Static string for an error code. */
 const char *fof_error_string(int code);
 

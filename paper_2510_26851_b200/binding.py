@@ -65,6 +65,16 @@ def lib():
         L.fof_run_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, ctypes.POINTER(i64), vp, vp]
         L.fof_status.restype = ctypes.c_int
         L.fof_status.argtypes = [vp, vp, vp]
+        L.fof_profile_enable.restype = ctypes.c_int
+        L.fof_profile_enable.argtypes = [vp, ctypes.c_int]
+        L.fof_profile_count.restype = ctypes.c_int
+        L.fof_profile_count.argtypes = [vp]
+        L.fof_profile_name.restype = ctypes.c_char_p
+        L.fof_profile_name.argtypes = [vp, ctypes.c_int]
+        L.fof_profile_read.restype = ctypes.c_int
+        L.fof_profile_read.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.c_int]
+        L.fof_launch_count.restype = ctypes.c_uint64
+        L.fof_launch_count.argtypes = [vp]
         L.fof_error_string.restype = ctypes.c_char_p
         L.fof_error_string.argtypes = [ctypes.c_int]
         L.fof_last_cuda_error.restype = ctypes.c_char_p
@@ -162,6 +172,27 @@ def fof_run_host(h, pos_host, mass_host, labels_host, group_label_host, group_si
 
 def fof_status(h, ws, stream=None) -> int:
     return int(lib().fof_status(h, _ptr(ws), _stream_ptr(stream)))
+
+
+def fof_profile_enable(h, slots: int):
+    _check(lib().fof_profile_enable(h, int(slots)), h)
+
+
+def fof_profile_names(h):
+    n = lib().fof_profile_count(h)
+    return [lib().fof_profile_name(h, k).decode() for k in range(n)]
+
+
+def fof_profile_read(h):
+    """{stage name: mean device milliseconds} over the steps recorded since the last read."""
+    n = lib().fof_profile_count(h)
+    buf = (ctypes.c_float * n)()
+    _check(lib().fof_profile_read(h, buf, n), h)
+    return {lib().fof_profile_name(h, k).decode(): float(buf[k]) for k in range(n)}
+
+
+def fof_launch_count(h) -> int:
+    return int(lib().fof_launch_count(h))
 
 
 # ---------------------------------------------------------------- convenience object

@@ -56,6 +56,27 @@ int cuda_fail(fof_handle *h, cudaError_t e, const char *where)
         if (e__ != cudaSuccess) return cuda_fail(h, e__, where); \
     } while (0)
 
+// Profiled stages, in execution order (fof_profile_name).
+enum Stage { kLinkClear = 0, kLinkBin, kLinkScan, kLinkScatter, kLinkPairs, kLinkFlatten,
+             kGroupsClear, kGroupsCount, kGroupsCompact, kGroupsReduce, kGroupsFinish, kNumStages };
+const char *const kStageName[kNumStages] = {
+    "link.clear", "link.bin", "link.cell_scan", "link.scatter", "link.pairs", "link.flatten",
+    "groups.clear", "groups.count", "groups.compact", "groups.reduce", "groups.finish"};
+static_assert(kNumStages <= kMaxStages, "raise kMaxStages");
+
+struct StageTimer {  // records the two events of a stage around its launches
+    fof_handle *h; cudaStream_t s; int k;
+    StageTimer(fof_handle *h_, cudaStream_t s_, int k_, int kernels) : h(h_), s(s_), k(k_)
+    {
+        h->launches += (unsigned long long)kernels;
+        if (h->prof_slots) {
+            cudaEventRecord(h->ev[(h->prof_cur * kMaxStages + k) * 2], s);
+            h->ev_valid[h->prof_cur * kMaxStages + k] = true;
+        }
+    }
+    ~StageTimer() { if (h->prof_slots) cudaEventRecord(h->ev[(h->prof_cur * kMaxStages + k) * 2 + 1], s); }
+};
+
 template <typename T>
 inline T *at(void *ws, size_t off) { return reinterpret_cast<T *>(static_cast<char *>(ws) + off); }
 
@@ -93,7 +114,62 @@ int fof_create(int64_t N, float L, float b, int32_t N_min, fof_handle **out)
     return FOF_OK;
 }
 
-void fof_destroy(fof_handle *h) { delete h; }
+void fof_destroy(fof_handle *h)
+{
+    if (!h) return;
+    fof_profile_enable(h, 0);
+    delete h;
+}
+
+int fof_profile_enable(fof_handle *h, int slots)
+{
+    if (!h || slots < 0 || slots > 1024) return FOF_ERR_INVALID_ARG;
+    if (h->prof_slots) {
+        const int n = h->prof_slots * kMaxStages * 2;
+        h->prof_slots = 0;
+        for (int k = 0; k < n; ++k) (void)cudaEventDestroy(h->ev[k]);
+        delete[] h->ev; delete[] h->ev_valid;
+        h->ev = nullptr; h->ev_valid = nullptr;
+    }
+    if (slots) {
+        const int n = slots * kMaxStages * 2;
+        h->ev = new (std::nothrow) cudaEvent_t[n];
+        h->ev_valid = new (std::nothrow) bool[slots * kMaxStages]();
+        if (!h->ev || !h->ev_valid) return FOF_ERR_INVALID_ARG;
+        for (int k = 0; k < n; ++k) CK(cudaEventCreate(&h->ev[k]), "cudaEventCreate");
+        h->prof_cur = slots - 1;
+        h->prof_slots = slots;
+    }
+    return FOF_OK;
+}
+
+int fof_profile_count(const fof_handle *) { return kNumStages; }
+
+const char *fof_profile_name(const fof_handle *, int k) { return (k >= 0 && k < kNumStages) ? kStageName[k] : ""; }
+
+int fof_profile_read(fof_handle *h, float *ms, int cap)
+{
+    if (!h || !ms || cap < 0) return FOF_ERR_INVALID_ARG;
+    if (!h->prof_slots) return FOF_ERR_STATE;
+    for (int k = 0; k < kNumStages && k < cap; ++k) {
+        double sum = 0.0;
+        int cnt = 0;
+        for (int sl = 0; sl < h->prof_slots; ++sl) {
+            const int e = sl * kMaxStages + k;
+            if (!h->ev_valid[e]) continue;
+            float t = 0.0f;
+            CK(cudaEventSynchronize(h->ev[2 * e + 1]), "cudaEventSynchronize");
+            CK(cudaEventElapsedTime(&t, h->ev[2 * e], h->ev[2 * e + 1]), "cudaEventElapsedTime");
+            sum += t;
+            ++cnt;
+            h->ev_valid[e] = false;
+        }
+        ms[k] = cnt ? (float)(sum / cnt) : 0.0f;
+    }
+    return FOF_OK;
+}
+
+uint64_t fof_launch_count(const fof_handle *h) { return h ? h->launches : 0; }
 
 int fof_set_grid(fof_handle *h, int32_t n)
 {
@@ -133,13 +209,21 @@ int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *s
     unsigned long long *state = at<unsigned long long>(ws, h->off_scan_state);
     h->linked = false;
     // ctrl + cell counters are contiguous: one memset; scan state: another
-    CK(cudaMemsetAsync(ws, 0, h->off_rank, s), "memset cells");
-    CK(cudaMemsetAsync(state, 0, (size_t)h->scan_tiles * sizeof(unsigned long long), s), "memset scan state");
-    CK(launch_bin(pos, h->N, h->grid, cell, rank, labels, ctrl, s), "bin_kernel");
-    CK(launch_cell_scan(cell, h->C + 1, state, ctrl, h->scan_tiles, s), "cell_scan_kernel");
-    CK(launch_scatter(pos, h->N, h->grid, cell, rank, sorted, s), "scatter_kernel");
-    CK(launch_link(sorted, h->N, h->grid, cell, labels, ctrl, h->num_sms, s), "link_kernel");
-    CK(launch_flatten(labels, h->N, s), "flatten_kernel");
+    const int has = h->N > 0;
+    if (h->prof_slots) {
+        h->prof_cur = (h->prof_cur + 1) % h->prof_slots;
+        for (int k = 0; k < kNumStages; ++k) h->ev_valid[h->prof_cur * kMaxStages + k] = false;
+    }
+    {
+        StageTimer t(h, s, kLinkClear, 0);
+        CK(cudaMemsetAsync(ws, 0, h->off_rank, s), "memset cells");
+        CK(cudaMemsetAsync(state, 0, (size_t)h->scan_tiles * sizeof(unsigned long long), s), "memset scan state");
+    }
+    { StageTimer t(h, s, kLinkBin, has); CK(launch_bin(pos, h->N, h->grid, cell, rank, labels, ctrl, s), "bin_kernel"); }
+    { StageTimer t(h, s, kLinkScan, 1); CK(launch_cell_scan(cell, h->C + 1, state, ctrl, h->scan_tiles, s), "cell_scan_kernel"); }
+    { StageTimer t(h, s, kLinkScatter, has); CK(launch_scatter(pos, h->N, h->grid, cell, rank, sorted, s), "scatter_kernel"); }
+    { StageTimer t(h, s, kLinkPairs, has); CK(launch_link(sorted, h->N, h->grid, cell, labels, ctrl, h->num_sms, s), "link_kernel"); }
+    { StageTimer t(h, s, kLinkFlatten, has); CK(launch_flatten(labels, h->N, s), "flatten_kernel"); }
     h->linked = true;
     h->linked_ws = ws;
     return FOF_OK;
@@ -171,18 +255,33 @@ int fof_groups(fof_handle *h, const float *pos, const float *mass, const int32_t
     double *acc = at<double>(ws, h->off_acc);
     unsigned long long *state = at<unsigned long long>(ws, h->off_gscan_state);
     *K_host = 0;
-    CK(cudaMemsetAsync(&ctrl->gscan_ticket, 0, sizeof(unsigned int), s), "memset ticket");
-    CK(cudaMemsetAsync(&ctrl->K, 0, sizeof(long long), s), "memset K");
-    CK(cudaMemsetAsync(cnt, 0, (size_t)(h->N + 1) * sizeof(int), s), "memset cnt");
-    CK(cudaMemsetAsync(state, 0, (size_t)h->gscan_tiles * sizeof(unsigned long long), s), "memset gscan state");
-    CK(launch_group_count(labels, h->N, cnt, s), "group_count_kernel");
-    CK(launch_group_compact(labels, h->N, h->N_min, cnt, cap, group_label, group_size, acc, state, ctrl,
-                            h->gscan_tiles, s), "group_compact_kernel");
-    CK(launch_group_reduce(pos, mass, labels, h->N, h->grid, cnt, cap, acc, particle_group, s),
-       "group_reduce_kernel");
+    const int has = h->N > 0;
+    if (h->prof_slots)
+        for (int k = kGroupsClear; k <= kGroupsFinish; ++k) h->ev_valid[h->prof_cur * kMaxStages + k] = false;
+    {
+        StageTimer t(h, s, kGroupsClear, 0);
+        CK(cudaMemsetAsync(&ctrl->gscan_ticket, 0, sizeof(unsigned int), s), "memset ticket");
+        CK(cudaMemsetAsync(&ctrl->K, 0, sizeof(long long), s), "memset K");
+        CK(cudaMemsetAsync(cnt, 0, (size_t)(h->N + 1) * sizeof(int), s), "memset cnt");
+        CK(cudaMemsetAsync(state, 0, (size_t)h->gscan_tiles * sizeof(unsigned long long), s), "memset gscan state");
+    }
+    { StageTimer t(h, s, kGroupsCount, has); CK(launch_group_count(labels, h->N, cnt, s), "group_count_kernel"); }
+    {
+        StageTimer t(h, s, kGroupsCompact, has);
+        CK(launch_group_compact(labels, h->N, h->N_min, cnt, cap, group_label, group_size, acc, state, ctrl,
+                                h->gscan_tiles, s), "group_compact_kernel");
+    }
+    {
+        StageTimer t(h, s, kGroupsReduce, has);
+        CK(launch_group_reduce(pos, mass, labels, h->N, h->grid, cnt, cap, acc, particle_group, s),
+           "group_reduce_kernel");
+    }
     const int64_t fin = cap < h->max_groups ? cap : h->max_groups;
-    CK(launch_group_finish(pos, group_label, group_size, acc, mass != nullptr, h->grid, fin, ctrl, group_mass,
-                           group_com, s), "group_finish_kernel");
+    {
+        StageTimer t(h, s, kGroupsFinish, fin > 0);
+        CK(launch_group_finish(pos, group_label, group_size, acc, mass != nullptr, h->grid, fin, ctrl, group_mass,
+                               group_com, s), "group_finish_kernel");
+    }
     long long K = 0;
     CK(cudaMemcpyAsync(&K, &ctrl->K, sizeof(K), cudaMemcpyDeviceToHost, s), "copy K");
     CK(cudaStreamSynchronize(s), "sync");

@@ -15,6 +15,7 @@ constexpr int kScanItems = 8;         // items per thread in the single-pass sca
 constexpr int kScanTile = kBlock * kScanItems;
 constexpr float kCellMargin = 1.001f; // cell side >= b * kCellMargin  (R3)
 constexpr int kMaxGrid = 1290;        // n^3 < 2^31
+constexpr int kMaxStages = 24;        // profiled stages (fof_profile_*)
 
 // Device control block at the start of the workspace (zeroed at the start of fof_link).
 struct Ctrl {
@@ -57,6 +58,12 @@ struct fof_handle {
     bool linked;
     const void *linked_ws;
     char cuda_err[256];
+    // measurement aids
+    int prof_slots;        // 0 = profiling off; else event sets used round-robin, one per fof_link call
+    int prof_cur;          // slot of the current (last) fof_link
+    cudaEvent_t *ev;       // [slot][2k] before, [slot][2k+1] after stage k
+    bool *ev_valid;        // [slot][k]
+    unsigned long long launches;
 };
 
 namespace fof {
