@@ -225,7 +225,7 @@ def run_ours(args):
     launches = B.fof_launch_count(f.h) - launches0
     stages = B.fof_profile_read(f.h)
     B.fof_profile_enable(f.h, 0)
-    E, pair_tests = f.link_stats()
+    E, pair_tests, grid_pairs = f.link_stats()
     t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -301,11 +301,12 @@ def run_ours(args):
         "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": w.name, "N": N, "L": w.L, "b": w.b, "N_min": w.N_min, "grid_n": f.grid[0],
-                   "cells": f.grid[1], "groups_kept": K_groups, "true_edges": E, "pair_tests": pair_tests,
+                   "cells": f.grid[1], "groups_kept": K_groups, "true_edges": E, "pair_tests": pair_tests, "grid_pairs": grid_pairs,
                    "parallelism": "replicas only" if world > 1 else "1 GPU",
                    "l2": "inputs + workspace per step exceed the 126 MB L2 (pos 12N + sorted 16N + labels 4N ...)"
                          if N * 32 > 126e6 else "working set fits L2 (small workload)"},
         "pair_tests_per_s": pair_tests / (stages["link.pairs"] * 1e-3) if stages.get("link.pairs") else None,
+        "grid_pairs_per_s": grid_pairs / (stages["link.pairs"] * 1e-3) if stages.get("link.pairs") else None,
         "stage_ms": {k: round(v, 5) for k, v in stages.items()},
         "roofline": roofline, "cpu_baseline": cpu, "parity_vs_oracle_in_this_run": parity,
         "e2e": {"value": world * N / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,

@@ -73,8 +73,11 @@ size_t fof_workspace_bytes(const fof_handle *h);
 int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *stream);
 
 /* Counters of the last fof_link on (h, ws): true edges E (unordered pairs with d^2 <= b^2; equal
- * to the oracle's E) and pair tests executed on this plan's grid.  Synchronises `stream`. */
-int fof_link_stats(fof_handle *h, void *ws, void *stream, uint64_t *edges_host, uint64_t *pair_tests_host);
+ * to the oracle's E), distance tests executed (after the geometric reach filter), and the
+ * candidate pairs the unfiltered half stencil implies on this plan's grid (P_exec of DESIGN.md §7).
+ * Any out pointer may be NULL.  Synchronises `stream`. */
+int fof_link_stats(fof_handle *h, void *ws, void *stream, uint64_t *edges_host, uint64_t *pair_tests_host,
+                   uint64_t *grid_pairs_host);
 
 /* H6-H8: group sizes ("parallel histogram"), compaction of groups with
  * size >= N_min in ascending canonical label, masses and periodic centres

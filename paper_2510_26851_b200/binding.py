@@ -56,7 +56,8 @@ def lib():
         L.fof_link.restype = ctypes.c_int
         L.fof_link.argtypes = [vp, vp, vp, vp, vp]
         L.fof_link_stats.restype = ctypes.c_int
-        L.fof_link_stats.argtypes = [vp, vp, vp, ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64)]
+        L.fof_link_stats.argtypes = [vp, vp, vp, ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64),
+                                     ctypes.POINTER(ctypes.c_uint64)]
         L.fof_groups.restype = ctypes.c_int
         L.fof_groups.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, ctypes.POINTER(i64), vp]
         L.fof_host_device_bytes.restype = ctypes.c_size_t
@@ -141,9 +142,11 @@ def fof_link(h, pos, labels, ws, stream=None):
 
 
 def fof_link_stats(h, ws, stream=None):
-    e, t = ctypes.c_uint64(), ctypes.c_uint64()
-    _check(lib().fof_link_stats(h, _ptr(ws), _stream_ptr(stream), ctypes.byref(e), ctypes.byref(t)), h)
-    return int(e.value), int(t.value)
+    """(true edges E, distance tests executed, candidate pairs of the unfiltered stencil on this grid)"""
+    e, t, gp = ctypes.c_uint64(), ctypes.c_uint64(), ctypes.c_uint64()
+    _check(lib().fof_link_stats(h, _ptr(ws), _stream_ptr(stream), ctypes.byref(e), ctypes.byref(t),
+                                ctypes.byref(gp)), h)
+    return int(e.value), int(t.value), int(gp.value)
 
 
 def fof_groups(h, pos, mass, labels, ws, group_label, group_size, group_mass, group_com, particle_group, cap,

@@ -26,8 +26,9 @@ struct Ctrl {
     unsigned long long edges;       // true edges (unordered pairs with d2 <= b2)
     unsigned long long pair_tests;  // distance tests executed
     long long K;                    // kept groups (written by fof_groups)
-    unsigned int link_ticket;       // dynamic work id for the link kernel
-    unsigned int pad1[7];
+    unsigned long long grid_pairs;  // candidate pairs of the unfiltered half stencil on this grid
+    unsigned int overflow_tiles;    // link tiles whose staged particles exceeded the shared-memory capacity
+    unsigned int pad1[5];
 };
 static_assert(sizeof(Ctrl) <= 256, "Ctrl must fit its 256-byte slot");
 
@@ -39,6 +40,19 @@ struct Grid {
     float inv_cell; // fl(n / L)
     int n;          // cells per axis
     int n_minus_1;
+    float reach;    // b in cell units + slack: how close to a cell face a particle must be to have
+                    // a partner in the cell behind it (kernels_link.cu candidate_ranges)
+};
+
+// H4 tiling: a CTA owns Sx x Sy x Sz home cells and stages them plus their half-stencil shell
+// ((Sx+2) x (Sy+2) x (Sz+1) cells) in shared memory.
+constexpr int kLinkBlock = 256;
+constexpr int kMaxHomeRows = 64;  // Sy * Sz
+struct Tile {
+    int Sx, Sy, Sz;   // home cells per tile and axis
+    int tx, ty, tz;   // tiles per axis
+    int cap;          // staged-particle capacity of one CTA
+    int ncell_max;    // (Sx+2)(Sy+2)(Sz+1)
 };
 
 }  // namespace fof
@@ -51,6 +65,11 @@ struct fof_handle {
     int64_t C;  // n^3
     fof::Grid grid;
     // workspace layout (byte offsets, 256-B aligned)
+    fof::Tile tile;
+    size_t tile_smem;   // dynamic shared memory of the link kernel
+    int link_w;         // lanes per home particle in the link kernel (4, 8, 16 or 32)
+    int64_t ntiles;
+    size_t off_tileflag;
     size_t off_ctrl, off_cell, off_rank, off_sorted, off_scan_state, off_cnt, off_acc, off_gscan_state;
     size_t ws_bytes;
     int64_t scan_tiles, gscan_tiles, max_groups;
@@ -158,8 +177,10 @@ cudaError_t launch_cell_scan(unsigned int *cell, int64_t n_items, unsigned long 
                              int64_t tiles, cudaStream_t s);
 cudaError_t launch_scatter(const float *pos, int64_t N, Grid g, const unsigned int *cell_start,
                            const unsigned int *rank, float4 *sorted, cudaStream_t s);
-cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start, int *labels,
-                        Ctrl *ctrl, int num_sms, cudaStream_t s);
+cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, Tile tp, size_t smem, int w, int64_t ntiles,
+                        const unsigned int *cell_start, int *labels, unsigned char *tile_flags, Ctrl *ctrl,
+                        int num_sms, cudaStream_t s);
+cudaError_t launch_grid_pairs(const unsigned int *cell_start, Grid g, Ctrl *ctrl, int num_sms, cudaStream_t s);
 cudaError_t launch_flatten(int *labels, int64_t N, cudaStream_t s);
 
 cudaError_t launch_group_count(const int *labels, int64_t N, int *cnt, cudaStream_t s);

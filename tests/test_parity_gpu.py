@@ -33,9 +33,9 @@ def gpu_fof(B, pos, L, b, N_min, mass=None, grid=None, particle_group=True):
     dmass = None if mass is None else torch.from_numpy(mass).cuda()
     labels = f.link(dpos)
     status = f.status()
-    E, tests = f.link_stats()
+    E, tests, grid_pairs = f.link_stats()
     g = f.groups(dpos, labels, mass=dmass, particle_group=particle_group)
-    out = dict(labels=labels.cpu().numpy(), E=E, tests=tests, status=status, K=g["K"], grid=f.grid,
+    out = dict(labels=labels.cpu().numpy(), E=E, tests=tests, grid_pairs=grid_pairs, status=status, K=g["K"], grid=f.grid,
                group_label=g["group_label"].cpu().numpy(), group_size=g["group_size"].cpu().numpy(),
                group_mass=g["group_mass"].cpu().numpy(), group_com=g["group_com"].cpu().numpy(),
                particle_group=None if g["particle_group"] is None else g["particle_group"].cpu().numpy())
