@@ -39,11 +39,12 @@ UNIT = "particles/s"
 # implementation cost and are deliberately NOT counted.
 ALG_BYTES_PER_PARTICLE = {
     "link.clear": 0,
-    "link.bin": 12 + 4,            # read pos, write parent (labels[i] = i)
+    "link.bin": 12,                # read pos (histogram)
     "link.cell_scan": 0,
     "link.scatter": 12 + 16,       # read pos, write sorted (x, y, z, idx)
-    "link.pairs": 16 + 4,          # read sorted once, update parent
-    "link.flatten": 4 + 4,         # read parent, write label
+    "link.pairs": 16 + 4,          # read sorted once, write parent
+    "link.flatten": 4 + 4 + 4 + 4, # flatten parent read + write; read idx, min-per-root RMW
+    "link.labels": 4 + 4,          # gather the root's minimum, write labels (original order)
     "groups.clear": 0,
     "groups.count": 4 + 4,         # read labels, size RMW
     "groups.compact": 4 + 4,       # read sizes, write id map

@@ -15,68 +15,22 @@ namespace {
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-// H0: link-kernel tiling for the current grid.  A tile of Sx x Sy x Sz home cells stages
-// (Sx+2)(Sy+2)(Sz+1) cells; the mean staged particle count is kept below cap / 2.2 so that
-// clustered tiles still fit.  Sx + 2 = 32 makes the row loops lane-exact.  Tuning knobs that cannot
-// change results: FOF_TILE="sx,sy,sz", FOF_TILE_SMEM_KB, FOF_LINK_W (lanes per home particle).
-void plan_tiles(fof_handle *h)
-{
-    const int n = h->n;
-    size_t smem = 72 * 1024;
-    if (const char *e = getenv("FOF_TILE_SMEM_KB")) { int kb = atoi(e); if (kb >= 16 && kb <= 200) smem = (size_t)kb * 1024; }
-    h->link_w = 8;
-    if (const char *e = getenv("FOF_LINK_W")) { int w = atoi(e); if (w == 4 || w == 8 || w == 16 || w == 32) h->link_w = w; }
-    const double rho = (double)h->N / (double)h->C;
-    auto cap_for = [&](int sx, int sy, int sz) {
-        const long ncell = (long)(sx + 2) * (sy + 2) * (sz + 1);
-        (void)ncell;
-        const long bytes = (long)smem - 2048;  // static shared memory of the kernel (row table, counters)
-        return bytes > 0 ? (int)((bytes / 22) & ~7L) : 0;
-    };
-    int Sx = n >= 32 ? 30 : n, Sy = 1, Sz = 1;
-    bool found = false;
-    for (; Sx >= 1 && !found; Sx = Sx > 1 ? Sx / 2 : 0) {
-        for (int s = 8; s >= 1; --s) {
-            const int sy = s < n ? s : n;
-            const long ncell = (long)(Sx + 2) * (sy + 2) * (sy + 1);
-            const int cap = cap_for(Sx, sy, sy);
-            if (cap >= 64 && rho * (double)ncell <= (double)cap / 2.2) { Sy = Sz = sy; found = true; break; }
-        }
-        if (found) break;
-    }
-    if (!found) { Sx = 1; Sy = Sz = 1; }
-    if (const char *e = getenv("FOF_TILE")) {
-        int a = 0, b = 0, c = 0;
-        if (sscanf(e, "%d,%d,%d", &a, &b, &c) == 3 && a >= 1 && b >= 1 && c >= 1 && b * c <= kMaxHomeRows &&
-            cap_for(a, b, c) >= 64) {
-            Sx = a < n ? a : n; Sy = b < n ? b : n; Sz = c < n ? c : n;
-        }
-    }
-    Tile &t = h->tile;
-    t.Sx = Sx; t.Sy = Sy; t.Sz = Sz;
-    t.tx = (n + Sx - 1) / Sx; t.ty = (n + Sy - 1) / Sy; t.tz = (n + Sz - 1) / Sz;
-    t.ncell_max = (Sx + 2) * (Sy + 2) * (Sz + 1);
-    t.cap = cap_for(Sx, Sy, Sz);
-    if (t.cap > 65528) t.cap = 65528;  // staged slots are queued as uint16
-    h->tile_smem = (size_t)t.cap * 22;
-    h->ntiles = (int64_t)t.tx * t.ty * t.tz;
-}
-
 // H0: workspace layout for the current grid.
 void layout(fof_handle *h)
 {
     const size_t N = (size_t)h->N;
     h->C = (int64_t)h->n * h->n * h->n;
-    plan_tiles(h);
     const int64_t cell_items = h->C + 1;
     h->scan_tiles = (cell_items + kScanTile - 1) / kScanTile;
     h->gscan_tiles = h->N > 0 ? (h->N + kScanTile - 1) / kScanTile : 1;
     h->max_groups = h->N / h->N_min;
     size_t off = 0;
     h->off_ctrl = off;        off += 256;
-    h->off_tileflag = off;    off += align256((size_t)h->ntiles);
     h->off_cell = off;        off += align256(((size_t)cell_items + 8) * sizeof(unsigned int));
+    h->off_rel = off;         off += align256((N + 1) * sizeof(unsigned int));  // cleared with ctrl + cells
     h->off_rank = off;        off += align256((N + 1) * sizeof(unsigned int));
+    h->off_idx = off;         off += align256((N + 1) * sizeof(int));
+    h->off_minidx = off;      off += align256((N + 1) * sizeof(int));
     h->off_sorted = off;      off += align256((N + 1) * sizeof(float4));
     h->off_scan_state = off;  off += align256((size_t)h->scan_tiles * sizeof(unsigned long long));
     h->off_cnt = off;         off += align256((N + 1) * sizeof(int));
@@ -111,10 +65,10 @@ int cuda_fail(fof_handle *h, cudaError_t e, const char *where)
     } while (0)
 
 // Profiled stages, in execution order (fof_profile_name).
-enum Stage { kLinkClear = 0, kLinkBin, kLinkScan, kLinkScatter, kLinkPairs, kLinkFlatten,
+enum Stage { kLinkClear = 0, kLinkBin, kLinkScan, kLinkScatter, kLinkPairs, kLinkFlatten, kLinkLabels,
              kGroupsClear, kGroupsCount, kGroupsCompact, kGroupsReduce, kGroupsFinish, kNumStages };
 const char *const kStageName[kNumStages] = {
-    "link.clear", "link.bin", "link.cell_scan", "link.scatter", "link.pairs", "link.flatten",
+    "link.clear", "link.bin", "link.cell_scan", "link.scatter", "link.pairs", "link.flatten", "link.labels",
     "groups.clear", "groups.count", "groups.compact", "groups.reduce", "groups.finish"};
 static_assert(kNumStages <= kMaxStages, "raise kMaxStages");
 
@@ -262,7 +216,7 @@ int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *s
     float4 *sorted = at<float4>(ws, h->off_sorted);
     unsigned long long *state = at<unsigned long long>(ws, h->off_scan_state);
     h->linked = false;
-    // ctrl + cell counters are contiguous: one memset; scan state: another
+    // ctrl + cell counters + rel (union-find forest: all roots) are contiguous: one memset; scan state: another
     const int has = h->N > 0;
     if (h->prof_slots) {
         h->prof_cur = (h->prof_cur + 1) % h->prof_slots;
@@ -273,15 +227,17 @@ int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *s
         CK(cudaMemsetAsync(ws, 0, h->off_rank, s), "memset cells");
         CK(cudaMemsetAsync(state, 0, (size_t)h->scan_tiles * sizeof(unsigned long long), s), "memset scan state");
     }
-    { StageTimer t(h, s, kLinkBin, has); CK(launch_bin(pos, h->N, h->grid, cell, rank, labels, ctrl, s), "bin_kernel"); }
+    { StageTimer t(h, s, kLinkBin, has); CK(launch_bin(pos, h->N, h->grid, cell, rank, ctrl, s), "bin_kernel"); }
     { StageTimer t(h, s, kLinkScan, 1); CK(launch_cell_scan(cell, h->C + 1, state, ctrl, h->scan_tiles, s), "cell_scan_kernel"); }
     { StageTimer t(h, s, kLinkScatter, has); CK(launch_scatter(pos, h->N, h->grid, cell, rank, sorted, s), "scatter_kernel"); }
+    unsigned int *rel = at<unsigned int>(ws, h->off_rel);
+    int *idx_s = at<int>(ws, h->off_idx), *minidx = at<int>(ws, h->off_minidx);
     {
-        StageTimer t(h, s, kLinkPairs, 2 * has);
-        CK(launch_link(sorted, h->N, h->grid, h->tile, h->tile_smem, h->link_w, h->ntiles, cell, labels,
-                       at<unsigned char>(ws, h->off_tileflag), ctrl, h->num_sms, s), "link kernels");
+        StageTimer t(h, s, kLinkPairs, has);
+        CK(launch_link(sorted, h->N, h->grid, cell, rel, idx_s, minidx, ctrl, h->num_sms, s), "link_kernel");
     }
-    { StageTimer t(h, s, kLinkFlatten, has); CK(launch_flatten(labels, h->N, s), "flatten_kernel"); }
+    { StageTimer t(h, s, kLinkFlatten, has); CK(launch_flatten_min(rel, idx_s, minidx, h->N, s), "flatten_min_kernel"); }
+    { StageTimer t(h, s, kLinkLabels, has); CK(launch_write_labels(rel, idx_s, minidx, labels, h->N, s), "write_labels_kernel"); }
     h->linked = true;
     h->linked_ws = ws;
     return FOF_OK;

@@ -27,8 +27,7 @@ struct Ctrl {
     unsigned long long pair_tests;  // distance tests executed
     long long K;                    // kept groups (written by fof_groups)
     unsigned long long grid_pairs;  // candidate pairs of the unfiltered half stencil on this grid
-    unsigned int overflow_tiles;    // link tiles whose staged particles exceeded the shared-memory capacity
-    unsigned int pad1[5];
+    unsigned int pad1[6];
 };
 static_assert(sizeof(Ctrl) <= 256, "Ctrl must fit its 256-byte slot");
 
@@ -44,16 +43,7 @@ struct Grid {
                     // a partner in the cell behind it (kernels_link.cu candidate_ranges)
 };
 
-// H4 tiling: a CTA owns Sx x Sy x Sz home cells and stages them plus their half-stencil shell
-// ((Sx+2) x (Sy+2) x (Sz+1) cells) in shared memory.
-constexpr int kLinkBlock = 256;
-constexpr int kMaxHomeRows = 64;  // Sy * Sz
-struct Tile {
-    int Sx, Sy, Sz;   // home cells per tile and axis
-    int tx, ty, tz;   // tiles per axis
-    int cap;          // staged-particle capacity of one CTA
-    int ncell_max;    // (Sx+2)(Sy+2)(Sz+1)
-};
+constexpr int kLinkBlock = 256;     // threads per CTA of the link kernel
 
 }  // namespace fof
 
@@ -65,12 +55,8 @@ struct fof_handle {
     int64_t C;  // n^3
     fof::Grid grid;
     // workspace layout (byte offsets, 256-B aligned)
-    fof::Tile tile;
-    size_t tile_smem;   // dynamic shared memory of the link kernel
-    int link_w;         // lanes per home particle in the link kernel (4, 8, 16 or 32)
-    int64_t ntiles;
-    size_t off_tileflag;
     size_t off_ctrl, off_cell, off_rank, off_sorted, off_scan_state, off_cnt, off_acc, off_gscan_state;
+    size_t off_rel, off_idx, off_minidx;  // union-find (cell-sorted space), original index, min original index
     size_t ws_bytes;
     int64_t scan_tiles, gscan_tiles, max_groups;
     int num_sms;
@@ -130,34 +116,6 @@ __device__ __forceinline__ bool linked(float xi, float yi, float zi, float xj, f
     return d2 <= g.b2;
 }
 
-// ---- lock-free union-find on the label array itself (parent[i] <= i; root = minimum index of its
-// set, which IS the canonical label: "minimum label", "minimum global
-// particle ID").  Hooks with atomicCAS at roots only; finds use path halving (plain stores of an
-// ancestor at non-roots are benign).
-__device__ __forceinline__ int find_root(int *parent, int x)
-{
-    int p = parent[x];
-    while (p != x) {
-        int gp = parent[p];
-        if (gp != p) parent[x] = gp;
-        x = p;
-        p = gp;
-    }
-    return x;
-}
-
-__device__ __forceinline__ void unite(int *parent, int a, int b)
-{
-    int ra = find_root(parent, a);
-    int rb = find_root(parent, b);
-    while (ra != rb) {
-        if (ra < rb) { int t = ra; ra = rb; rb = t; }  // ra is the larger root
-        int old = atomicCAS(parent + ra, ra, rb);
-        if (old == ra) return;
-        ra = find_root(parent, old);
-    }
-}
-
 __device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long *p)
 {
     unsigned long long v;
@@ -172,16 +130,17 @@ __device__ __forceinline__ void st_relaxed_u64(unsigned long long *p, unsigned l
 
 // kernels (one launcher per step; all asynchronous on `s`)
 cudaError_t launch_bin(const float *pos, int64_t N, Grid g, unsigned int *cell_count, unsigned int *rank,
-                       int *labels, Ctrl *ctrl, cudaStream_t s);
+                       Ctrl *ctrl, cudaStream_t s);
 cudaError_t launch_cell_scan(unsigned int *cell, int64_t n_items, unsigned long long *state, Ctrl *ctrl,
                              int64_t tiles, cudaStream_t s);
 cudaError_t launch_scatter(const float *pos, int64_t N, Grid g, const unsigned int *cell_start,
                            const unsigned int *rank, float4 *sorted, cudaStream_t s);
-cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, Tile tp, size_t smem, int w, int64_t ntiles,
-                        const unsigned int *cell_start, int *labels, unsigned char *tile_flags, Ctrl *ctrl,
-                        int num_sms, cudaStream_t s);
+cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start, unsigned int *rel,
+                        int *idx_s, int *minidx, Ctrl *ctrl, int num_sms, cudaStream_t s);
 cudaError_t launch_grid_pairs(const unsigned int *cell_start, Grid g, Ctrl *ctrl, int num_sms, cudaStream_t s);
-cudaError_t launch_flatten(int *labels, int64_t N, cudaStream_t s);
+cudaError_t launch_flatten_min(unsigned int *rel, const int *idx_s, int *minidx, int64_t N, cudaStream_t s);
+cudaError_t launch_write_labels(const unsigned int *rel, const int *idx_s, const int *minidx, int *labels, int64_t N,
+                                cudaStream_t s);
 
 cudaError_t launch_group_count(const int *labels, int64_t N, int *cnt, cudaStream_t s);
 cudaError_t launch_group_compact(const int *labels, int64_t N, int N_min, int *cnt_to_gid, int64_t cap,

@@ -7,13 +7,11 @@ namespace fof {
 
 // ---------------------------------------------------------------------------------------------
 // H1 + first half of H2: one thread per particle.  Reads pos once; the atomicAdd on the cell
-// counter returns the particle's rank inside its cell, which makes H3 atomic-free.  Also
-// initialises the union-find (labels[i] = i, "initial label = own index").
+// counter returns the particle's rank inside its cell, which makes H3 atomic-free.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kBlock) bin_kernel(const float *__restrict__ pos, int64_t N, Grid g,
                                                      unsigned int *__restrict__ cell_count,
-                                                     unsigned int *__restrict__ rank, int *__restrict__ labels,
-                                                     Ctrl *ctrl)
+                                                     unsigned int *__restrict__ rank, Ctrl *ctrl)
 {
     int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x;
     if (i >= N) return;
@@ -27,7 +25,6 @@ __global__ void __launch_bounds__(kBlock) bin_kernel(const float *__restrict__ p
     z = wrap1(z, g.L);
     unsigned int c = cell_id(cell1(x, g), cell1(y, g), cell1(z, g), g.n);
     rank[i] = atomicAdd(cell_count + c, 1u);
-    labels[i] = (int)i;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -147,9 +144,9 @@ __global__ void __launch_bounds__(kBlock) scatter_kernel(const float *__restrict
 static inline unsigned int blocks_for(int64_t n, int per_block) { return (unsigned int)((n + per_block - 1) / per_block); }
 
 cudaError_t launch_bin(const float *pos, int64_t N, Grid g, unsigned int *cell_count, unsigned int *rank,
-                       int *labels, Ctrl *ctrl, cudaStream_t s)
+                       Ctrl *ctrl, cudaStream_t s)
 {
-    if (N > 0) bin_kernel<<<blocks_for(N, kBlock), kBlock, 0, s>>>(pos, N, g, cell_count, rank, labels, ctrl);
+    if (N > 0) bin_kernel<<<blocks_for(N, kBlock), kBlock, 0, s>>>(pos, N, g, cell_count, rank, ctrl);
     return cudaGetLastError();
 }
 
