@@ -102,63 +102,98 @@ __device__ __forceinline__ void row_range(const unsigned int *__restrict__ cs, c
     end = (int)__ldg(cs + rb + b);
 }
 
+// ---- warp-level work distribution.  The candidate ranges of the 32 home particles of a warp are
+// cut into chunks of at most kChunk candidates, queued in shared memory, and handed out to the
+// lanes round-robin, so that a lane sitting in a dense cell does not hold 31 idle lanes hostage.
+constexpr int kChunk = 8;                 // candidates per chunk
+constexpr int kQueue = 256;               // chunks per warp and window
+constexpr int kWarpsPerCta = kLinkBlock / 32;
+
 template <bool WRAP>
-__device__ __forceinline__ void link_particle(const float4 *__restrict__ sorted, const unsigned int *__restrict__ cs,
-                                              unsigned int *rel, int si, const float4 &me, const Home &h,
-                                              const Grid &g, unsigned int &edges, unsigned int &tests)
+__device__ __forceinline__ void warp_link(const float4 *__restrict__ sorted, const unsigned int *__restrict__ cs,
+                                          unsigned int *rel, int si, bool valid, const float4 &me, const Home &h,
+                                          const Grid &g, int2 *q, unsigned int &edges, unsigned int &tests)
 {
+    constexpr int NR = WRAP ? 10 : 5;
     const int n = g.n;
-    int root = si - (int)rel[si];
-    int beg[5], end[5];
-    // home row: the rest of my cell, plus the +x cell
-    {
-        const int rb = n * (h.cy + n * h.cz);
+    const int lane = threadIdx.x & 31;
+    int beg[NR], len[NR];
+#pragma unroll
+    for (int k = 0; k < NR; ++k) beg[k] = len[k] = 0;
+    if (valid) {
+        int yp = h.cy + 1, ym = h.cy - 1, zp = h.cz + 1;
+        if (WRAP) {
+            if (yp == n) yp = 0;
+            if (ym < 0) ym = n - 1;
+            if (zp == n) zp = 0;
+        }
+        int e;
+        // home row: the rest of my cell, plus the +x cell
         beg[0] = si + 1;
-        end[0] = (int)__ldg(cs + rb + min(h.cx + 1 + (h.xh ? 1 : 0), n));
-    }
+        len[0] = (int)__ldg(cs + n * (h.cy + n * h.cz) + min(h.cx + 1 + (h.xh ? 1 : 0), n)) - beg[0];
+        if (h.yh) { row_range<WRAP>(cs, h, yp, h.cz, n, true, beg[1], e); len[1] = e - beg[1]; }
+        if (h.zh) {
+            row_range<WRAP>(cs, h, h.cy, zp, n, true, beg[2], e); len[2] = e - beg[2];
+            if (h.yl) { row_range<WRAP>(cs, h, ym, zp, n, true, beg[3], e); len[3] = e - beg[3]; }
+            if (h.yh) { row_range<WRAP>(cs, h, yp, zp, n, true, beg[4], e); len[4] = e - beg[4]; }
+        }
+        if (WRAP) {
+            // cells behind the periodic x faces: cell 0 of a row when cx = n-1 reaches up, cell n-1
+            // when cx = 0 reaches down (never for the home row's lower side: half stencil)
+            const bool up = h.xh && h.cx == n - 1, dn = h.xl && h.cx == 0;
+            if (up || dn) {
+                const int ys[5] = {h.cy, yp, h.cy, ym, yp};
+                const int zs[5] = {h.cz, h.cz, zp, zp, zp};
+                const bool on[5] = {true, h.yh, h.zh, h.zh && h.yl, h.zh && h.yh};
 #pragma unroll
-    for (int k = 1; k < 5; ++k) beg[k] = end[k] = 0;
-    int yp = h.cy + 1, ym = h.cy - 1, zp = h.cz + 1;
-    if (WRAP) {
-        if (yp == n) yp = 0;
-        if (ym < 0) ym = n - 1;
-        if (zp == n) zp = 0;
-    }
-    if (h.yh) row_range<WRAP>(cs, h, yp, h.cz, n, true, beg[1], end[1]);
-    if (h.zh) {
-        row_range<WRAP>(cs, h, h.cy, zp, n, true, beg[2], end[2]);
-        if (h.yl) row_range<WRAP>(cs, h, ym, zp, n, true, beg[3], end[3]);
-        if (h.yh) row_range<WRAP>(cs, h, yp, zp, n, true, beg[4], end[4]);
-    }
-#pragma unroll
-    for (int k = 0; k < 5; ++k) {
-        tests += (unsigned int)(end[k] - beg[k]);
-        test_range<WRAP>(sorted, rel, beg[k], end[k], me, si, root, g, edges);
-    }
-    if (WRAP) {
-        // cells behind the periodic x faces: cell 0 of a row when cx = n-1 reaches up, cell n-1 when
-        // cx = 0 reaches down (never for the home row's lower side: half stencil)
-        const bool up = h.xh && h.cx == n - 1, dn = h.xl && h.cx == 0;
-        if (up || dn) {
-            const int ys[5] = {h.cy, yp, h.cy, ym, yp};
-            const int zs[5] = {h.cz, h.cz, zp, zp, zp};
-            const bool on[5] = {true, h.yh, h.zh, h.zh && h.yl, h.zh && h.yh};
-#pragma unroll
-            for (int k = 0; k < 5; ++k) {
-                if (!on[k]) continue;
-                const int rb = n * (ys[k] + n * zs[k]);
-                if (up) {
-                    const int b0 = (int)__ldg(cs + rb), e0 = (int)__ldg(cs + rb + 1);
-                    tests += (unsigned int)(e0 - b0);
-                    test_range<true>(sorted, rel, b0, e0, me, si, root, g, edges);
-                }
-                if (dn && k > 0) {
-                    const int b0 = (int)__ldg(cs + rb + n - 1), e0 = (int)__ldg(cs + rb + n);
-                    tests += (unsigned int)(e0 - b0);
-                    test_range<true>(sorted, rel, b0, e0, me, si, root, g, edges);
+                for (int k = 0; k < 5; ++k) {
+                    if (!on[k] || (!up && k == 0)) continue;
+                    // up and dn exclude each other unless n == 1 row cell... (n >= 3: cx cannot be both)
+                    const int c = n * (ys[k] + n * zs[k]) + (up ? 0 : n - 1);
+                    beg[5 + k] = (int)__ldg(cs + c);
+                    len[5 + k] = (int)__ldg(cs + c + 1) - beg[5 + k];
                 }
             }
         }
+    }
+    int nch = 0;
+#pragma unroll
+    for (int k = 0; k < NR; ++k) nch += (len[k] + kChunk - 1) / kChunk;
+    int incl = nch;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+    }
+    const int total = __shfl_sync(0xffffffffu, incl, 31);
+    const int excl = incl - nch;
+    for (int base = 0; base < total; base += kQueue) {
+        int pos = excl - base;
+#pragma unroll
+        for (int k = 0; k < NR; ++k)
+            for (int o = 0; o < len[k]; o += kChunk, ++pos)
+                if (pos >= 0 && pos < kQueue) q[pos] = make_int2(beg[k] + o, (min(kChunk, len[k] - o) << 8) | lane);
+        __syncwarp();
+        const int cnt = min(kQueue, total - base);
+        for (int j0 = 0; j0 < cnt; j0 += 32) {
+            const int j = j0 + lane;
+            const bool has = j < cnt;
+            const int2 c = has ? q[j] : make_int2(0, lane);
+            const int owner = c.y & 31;
+            float4 o4;
+            o4.x = __shfl_sync(0xffffffffu, me.x, owner);
+            o4.y = __shfl_sync(0xffffffffu, me.y, owner);
+            o4.z = __shfl_sync(0xffffffffu, me.z, owner);
+            o4.w = 0.0f;
+            const int osi = __shfl_sync(0xffffffffu, si, owner);
+            if (has) {
+                const int cb = c.x, ce = c.x + (c.y >> 8);
+                tests += (unsigned int)(ce - cb);
+                int root = osi - (int)rel[osi];
+                test_range<WRAP>(sorted, rel, cb, ce, o4, osi, root, g, edges);
+            }
+        }
+        __syncwarp();
     }
 }
 
@@ -169,6 +204,8 @@ __global__ void __launch_bounds__(kLinkBlock) link_kernel(const float4 *__restri
                                                           int *__restrict__ minidx, Ctrl *ctrl)
 {
     __shared__ unsigned int s_edges, s_tests;
+    __shared__ int2 s_queue[kWarpsPerCta][kQueue];
+    int2 *q = s_queue[threadIdx.x >> 5];
     if (threadIdx.x == 0) { s_edges = 0; s_tests = 0; }
     __syncthreads();
     unsigned int edges = 0, tests = 0;
@@ -198,11 +235,8 @@ __global__ void __launch_bounds__(kLinkBlock) link_kernel(const float4 *__restri
             needwrap = n < 6 || (h.xl && h.cx == 0) || (h.xh && h.cx == n - 1) || (h.yl && h.cy == 0) ||
                        (h.yh && h.cy == n - 1) || (h.zh && h.cz == n - 1);
         }
-        if (__any_sync(0xffffffffu, needwrap)) {
-            if (valid) link_particle<true>(sorted, cell_start, rel, si, me, h, g, edges, tests);
-        } else {
-            if (valid) link_particle<false>(sorted, cell_start, rel, si, me, h, g, edges, tests);
-        }
+        if (__any_sync(0xffffffffu, needwrap)) warp_link<true>(sorted, cell_start, rel, si, valid, me, h, g, q, edges, tests);
+        else warp_link<false>(sorted, cell_start, rel, si, valid, me, h, g, q, edges, tests);
     }
     for (int o = 16; o > 0; o >>= 1) {
         edges += __shfl_xor_sync(0xffffffffu, edges, o);
