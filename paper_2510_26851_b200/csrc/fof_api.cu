@@ -31,6 +31,7 @@ void layout(fof_handle *h)
     h->off_rank = off;        off += align256((N + 1) * sizeof(unsigned int));
     h->off_idx = off;         off += align256((N + 1) * sizeof(int));
     h->off_minidx = off;      off += align256((N + 1) * sizeof(int));
+    h->off_dense = off;       off += align256((N / kDenseCell + 2) * sizeof(unsigned int));
     h->off_sorted = off;      off += align256((N + 1) * sizeof(float4));
     h->off_scan_state = off;  off += align256((size_t)h->scan_tiles * sizeof(unsigned long long));
     h->off_cnt = off;         off += align256((N + 1) * sizeof(int));
@@ -228,13 +229,14 @@ int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *s
         CK(cudaMemsetAsync(state, 0, (size_t)h->scan_tiles * sizeof(unsigned long long), s), "memset scan state");
     }
     { StageTimer t(h, s, kLinkBin, has); CK(launch_bin(pos, h->N, h->grid, cell, rank, ctrl, s), "bin_kernel"); }
-    { StageTimer t(h, s, kLinkScan, 1); CK(launch_cell_scan(cell, h->C + 1, state, ctrl, h->scan_tiles, s), "cell_scan_kernel"); }
+    { StageTimer t(h, s, kLinkScan, 1); CK(launch_cell_scan(cell, h->C + 1, state, ctrl, at<unsigned int>(ws, h->off_dense), h->scan_tiles, s), "cell_scan_kernel"); }
     { StageTimer t(h, s, kLinkScatter, has); CK(launch_scatter(pos, h->N, h->grid, cell, rank, sorted, s), "scatter_kernel"); }
     unsigned int *rel = at<unsigned int>(ws, h->off_rel);
     int *idx_s = at<int>(ws, h->off_idx), *minidx = at<int>(ws, h->off_minidx);
     {
-        StageTimer t(h, s, kLinkPairs, has);
-        CK(launch_link(sorted, h->N, h->grid, cell, rel, idx_s, minidx, ctrl, h->num_sms, s), "link_kernel");
+        StageTimer t(h, s, kLinkPairs, 2 * has);
+        CK(launch_link(sorted, h->N, h->grid, cell, at<unsigned int>(ws, h->off_dense), rel, idx_s, minidx, ctrl,
+                       h->num_sms, s), "link kernels");
     }
     { StageTimer t(h, s, kLinkFlatten, has); CK(launch_flatten_min(rel, idx_s, minidx, h->N, s), "flatten_min_kernel"); }
     { StageTimer t(h, s, kLinkLabels, has); CK(launch_write_labels(rel, idx_s, minidx, labels, h->N, s), "write_labels_kernel"); }

@@ -27,7 +27,8 @@ struct Ctrl {
     unsigned long long pair_tests;  // distance tests executed
     long long K;                    // kept groups (written by fof_groups)
     unsigned long long grid_pairs;  // candidate pairs of the unfiltered half stencil on this grid
-    unsigned int pad1[6];
+    unsigned int ndense;            // entries of the dense-cell list (written by the cell scan)
+    unsigned int pad1[5];
 };
 static_assert(sizeof(Ctrl) <= 256, "Ctrl must fit its 256-byte slot");
 
@@ -43,7 +44,9 @@ struct Grid {
                     // a partner in the cell behind it (kernels_link.cu candidate_ranges)
 };
 
-constexpr int kLinkBlock = 256;     // threads per CTA of the link kernel
+constexpr int kLinkBlock = 256;     // threads per CTA of the link kernels
+constexpr int kDenseCell = 8;       // cells with kDenseCell..kDenseMax particles: own pairs go to link_dense_kernel
+constexpr int kDenseMax = 256;
 
 }  // namespace fof
 
@@ -56,7 +59,7 @@ struct fof_handle {
     fof::Grid grid;
     // workspace layout (byte offsets, 256-B aligned)
     size_t off_ctrl, off_cell, off_rank, off_sorted, off_scan_state, off_cnt, off_acc, off_gscan_state;
-    size_t off_rel, off_idx, off_minidx;  // union-find (cell-sorted space), original index, min original index
+    size_t off_rel, off_idx, off_minidx, off_dense;  // union-find (cell-sorted space), original index, min original index
     size_t ws_bytes;
     int64_t scan_tiles, gscan_tiles, max_groups;
     int num_sms;
@@ -132,11 +135,12 @@ __device__ __forceinline__ void st_relaxed_u64(unsigned long long *p, unsigned l
 cudaError_t launch_bin(const float *pos, int64_t N, Grid g, unsigned int *cell_count, unsigned int *rank,
                        Ctrl *ctrl, cudaStream_t s);
 cudaError_t launch_cell_scan(unsigned int *cell, int64_t n_items, unsigned long long *state, Ctrl *ctrl,
-                             int64_t tiles, cudaStream_t s);
+                             unsigned int *dense_list, int64_t tiles, cudaStream_t s);
 cudaError_t launch_scatter(const float *pos, int64_t N, Grid g, const unsigned int *cell_start,
                            const unsigned int *rank, float4 *sorted, cudaStream_t s);
-cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start, unsigned int *rel,
-                        int *idx_s, int *minidx, Ctrl *ctrl, int num_sms, cudaStream_t s);
+cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
+                        const unsigned int *dense_list, unsigned int *rel, int *idx_s, int *minidx, Ctrl *ctrl,
+                        int num_sms, cudaStream_t s);
 cudaError_t launch_grid_pairs(const unsigned int *cell_start, Grid g, Ctrl *ctrl, int num_sms, cudaStream_t s);
 cudaError_t launch_flatten_min(unsigned int *rel, const int *idx_s, int *minidx, int64_t N, cudaStream_t s);
 cudaError_t launch_write_labels(const unsigned int *rel, const int *idx_s, const int *minidx, int *labels, int64_t N,

@@ -70,14 +70,28 @@ template <bool WRAP>
 __device__ __forceinline__ void test_range(const float4 *__restrict__ sorted, unsigned int *rel, int beg, int end,
                                            const float4 &me, int si, int &root, const Grid &g, unsigned int &edges)
 {
-    for (int t = beg; t < end; ++t) {
-        const float4 pj = __ldg(sorted + t);
-        if (linked_t<WRAP>(me, pj, g)) {
-            ++edges;
-            if (t - (int)rel[t] != root) {  // not yet known to be in one set
-                root = unite_rel(rel, si, t);
-                if (si != root) rel[si] = (unsigned int)(si - root);
-                if (t != root) rel[t] = (unsigned int)(t - root);
+    // four candidates per trip: all loads (positions and parent offsets) are issued before the first
+    // test, so one memory latency covers four tests.  A parent offset read early may be stale after
+    // a union in the same trip; that only costs a redundant find.
+    for (int t = beg; t < end; t += 4) {
+        float4 pj[4];
+        unsigned int rj[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int tt = min(t + u, end - 1);
+            pj[u] = __ldg(sorted + tt);
+            rj[u] = rel[tt];
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int tt = t + u;
+            if (tt < end && linked_t<WRAP>(me, pj[u], g)) {
+                ++edges;
+                if (tt - (int)rj[u] != root) {  // not yet known to be in one set
+                    root = unite_rel(rel, si, tt);
+                    if (si != root) rel[si] = (unsigned int)(si - root);
+                    if (tt != root) rel[tt] = (unsigned int)(tt - root);
+                }
             }
         }
     }
@@ -129,8 +143,14 @@ __device__ __forceinline__ void warp_link(const float4 *__restrict__ sorted, con
         }
         int e;
         // home row: the rest of my cell, plus the +x cell
-        beg[0] = si + 1;
-        len[0] = (int)__ldg(cs + n * (h.cy + n * h.cz) + min(h.cx + 1 + (h.xh ? 1 : 0), n)) - beg[0];
+        // (the pairs inside a DENSE home cell belong to link_dense_kernel)
+        {
+            const unsigned int *row = cs + n * (h.cy + n * h.cz) + h.cx;
+            const int c0 = (int)__ldg(row), c1 = (int)__ldg(row + 1);
+            const int e0 = (h.xh && h.cx + 1 < n) ? (int)__ldg(row + 2) : c1;
+            beg[0] = (c1 - c0 >= kDenseCell && c1 - c0 <= kDenseMax) ? c1 : si + 1;
+            len[0] = e0 - beg[0];
+        }
         if (h.yh) { row_range<WRAP>(cs, h, yp, h.cz, n, true, beg[1], e); len[1] = e - beg[1]; }
         if (h.zh) {
             row_range<WRAP>(cs, h, h.cy, zp, n, true, beg[2], e); len[2] = e - beg[2];
@@ -203,11 +223,8 @@ __global__ void __launch_bounds__(kLinkBlock) link_kernel(const float4 *__restri
                                                           unsigned int *rel, int *__restrict__ idx_s,
                                                           int *__restrict__ minidx, Ctrl *ctrl)
 {
-    __shared__ unsigned int s_edges, s_tests;
     __shared__ int2 s_queue[kWarpsPerCta][kQueue];
     int2 *q = s_queue[threadIdx.x >> 5];
-    if (threadIdx.x == 0) { s_edges = 0; s_tests = 0; }
-    __syncthreads();
     unsigned int edges = 0, tests = 0;
     const int n = g.n;
     const float lo = g.reach, hi = 1.0f - g.reach;
@@ -242,11 +259,100 @@ __global__ void __launch_bounds__(kLinkBlock) link_kernel(const float4 *__restri
         edges += __shfl_xor_sync(0xffffffffu, edges, o);
         tests += __shfl_xor_sync(0xffffffffu, tests, o);
     }
-    if ((threadIdx.x & 31) == 0) { atomicAdd(&s_edges, edges); atomicAdd(&s_tests, tests); }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        if (s_edges) atomicAdd(&ctrl->edges, (unsigned long long)s_edges);
-        if (s_tests) atomicAdd(&ctrl->pair_tests, (unsigned long long)s_tests);
+    if ((threadIdx.x & 31) == 0) {  // one pair of global atomics per warp: no CTA barrier at the end
+        if (edges) atomicAdd(&ctrl->edges, (unsigned long long)edges);
+        if (tests) atomicAdd(&ctrl->pair_tests, (unsigned long long)tests);
+    }
+}
+
+// H4 (dense cells): all pairs inside one cell that holds kDenseCell..kDenseMax particles, one warp
+// per cell, run BEFORE link_kernel (every parent entry of the cell is still a root and no other
+// warp touches it).  The cell is cut into blocks of 32 particles.  For a tile (block I, block J <= I)
+// lane i builds the adjacency bitmask of its particle against the 32 particles of J with
+// warp-uniform loads (one transaction per candidate, 32 tests per trip).  Diagonal tile: the
+// components of the 32-node graph are closed by squaring the reachability masks through shuffles,
+// and written as parent offsets with plain stores -- no atomics.  Off-diagonal tile: the masks are
+// reduced to (component of I, component of J) pairs and only those are united.
+// Pairs inside one cell never wrap (cell side <= L/3 < L/2).
+__global__ void __launch_bounds__(kLinkBlock) link_dense_kernel(const float4 *__restrict__ sorted, Grid g,
+                                                                const unsigned int *__restrict__ cell_start,
+                                                                const unsigned int *__restrict__ dense_list,
+                                                                unsigned int *rel, Ctrl *ctrl)
+{
+    __shared__ unsigned char s_lab_all[kWarpsPerCta][kDenseMax];
+    __shared__ float4 s_pj_all[kWarpsPerCta][32];
+    unsigned char *s_lab = s_lab_all[threadIdx.x >> 5];
+    float4 *s_pj = s_pj_all[threadIdx.x >> 5];
+    const int lane = threadIdx.x & 31;
+    const unsigned int nd = ctrl->ndense;
+    const unsigned int nwarps = gridDim.x * kWarpsPerCta;
+    const float inf = __int_as_float(0x7f800000);
+    unsigned int edges = 0, tests = 0;
+    for (unsigned int ci = blockIdx.x * kWarpsPerCta + (threadIdx.x >> 5); ci < nd; ci += nwarps) {
+        const unsigned int c = __ldg(dense_list + ci);
+        const int b0 = (int)__ldg(cell_start + c), e0 = (int)__ldg(cell_start + c + 1);
+        for (int ib = b0; ib < e0; ib += 32) {
+            const int i = ib + lane;
+            const bool valid = i < e0;
+            // a lane without a particle sits at +inf: d2 = inf fails the test on both sides of a tile
+            float4 me = make_float4(inf, inf, inf, 0.0f);
+            if (valid) me = __ldg(sorted + i);
+            int lab = lane;  // lane of the smallest member of my component inside block I
+            for (int jb = ib; jb >= b0; jb -= 32) {  // diagonal tile first, then the earlier blocks
+                // block J staged in shared memory: the tile loop reads it with broadcast LDS.128
+                __syncwarp();
+                s_pj[lane] = (jb == ib) ? me : __ldg(sorted + jb + lane);  // earlier blocks are full
+                __syncwarp();
+                const int cnt = min(32, e0 - jb);
+                unsigned int adj = 0;
+#pragma unroll 1
+                for (int j0 = 0; j0 < cnt; j0 += 8) {
+#pragma unroll
+                    for (int u = 0; u < 8; ++u)
+                        if (linked_t<false>(me, s_pj[j0 + u], g)) adj |= 1u << (j0 + u);
+                }
+                if (jb == ib) {
+                    adj &= ~(1u << lane);
+                    edges += (unsigned int)__popc(adj & ((1u << lane) - 1u));
+                    if (valid) tests += (unsigned int)lane;
+                    // components of the 32-node graph: breadth-first from the lowest unlabelled lane; one
+                    // REDUX (warp OR of the visited lanes' adjacency) per BFS level
+                    const unsigned int self = 1u << lane;
+                    unsigned int todo = 0xffffffffu;
+                    while (todo) {
+                        const int r = __ffs((int)todo) - 1;
+                        unsigned int vis = 1u << r;
+                        while (true) {
+                            const unsigned int nxt = vis | __reduce_or_sync(0xffffffffu, (vis & self) ? adj : 0u);
+                            if (nxt == vis) break;
+                            vis = nxt;
+                        }
+                        if (vis & self) lab = r;
+                        todo &= ~vis;
+                    }
+                    if (valid && lab != lane) rel[i] = (unsigned int)(lane - lab);
+                    s_lab[i - b0] = (unsigned char)lab;
+                } else {
+                    edges += (unsigned int)__popc(adj);
+                    if (valid) tests += 32u;
+                    unsigned int reps = 0;
+                    for (unsigned int m = adj; m; m &= m - 1u) reps |= 1u << s_lab[jb - b0 + __ffs((int)m) - 1];
+                    const unsigned int peers = __match_any_sync(0xffffffffu, lab);
+                    reps = __reduce_or_sync(peers, reps);
+                    if (lane == lab)
+                        for (unsigned int m = reps; m; m &= m - 1u) unite_rel(rel, i, jb + __ffs((int)m) - 1);
+                }
+            }
+        }
+        __syncwarp();
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        edges += __shfl_xor_sync(0xffffffffu, edges, o);
+        tests += __shfl_xor_sync(0xffffffffu, tests, o);
+    }
+    if (lane == 0) {
+        if (edges) atomicAdd(&ctrl->edges, (unsigned long long)edges);
+        if (tests) atomicAdd(&ctrl->pair_tests, (unsigned long long)tests);
     }
 }
 
@@ -319,11 +425,13 @@ cudaError_t launch_grid_pairs(const unsigned int *cell_start, Grid g, Ctrl *ctrl
 
 static inline unsigned int blocks_for(int64_t n, int per_block) { return (unsigned int)((n + per_block - 1) / per_block); }
 
-cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start, unsigned int *rel,
-                        int *idx_s, int *minidx, Ctrl *ctrl, int num_sms, cudaStream_t s)
+cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
+                        const unsigned int *dense_list, unsigned int *rel, int *idx_s, int *minidx, Ctrl *ctrl,
+                        int num_sms, cudaStream_t s)
 {
     if (N <= 0) return cudaSuccess;
     const unsigned int grid = (unsigned int)min((int64_t)blocks_for(N, kLinkBlock), (int64_t)num_sms * 32);
+    link_dense_kernel<<<(unsigned int)num_sms * 8, kLinkBlock, 0, s>>>(sorted, g, cell_start, dense_list, rel, ctrl);
     link_kernel<<<grid, kLinkBlock, 0, s>>>(sorted, N, g, cell_start, rel, idx_s, minidx, ctrl);
     return cudaGetLastError();
 }

@@ -59,7 +59,8 @@ __device__ __forceinline__ unsigned int lookback(unsigned long long *state, unsi
 }
 
 __global__ void __launch_bounds__(kBlock) cell_scan_kernel(unsigned int *data, int64_t n_items,
-                                                           unsigned long long *state, Ctrl *ctrl)
+                                                           unsigned long long *state, Ctrl *ctrl,
+                                                           unsigned int *__restrict__ dense_list)
 {
     __shared__ unsigned int s_tile, s_prefix;
     __shared__ unsigned int s_warp[kBlock / 32];
@@ -77,6 +78,30 @@ __global__ void __launch_bounds__(kBlock) cell_scan_kernel(unsigned int *data, i
     } else {
 #pragma unroll
         for (int k = 0; k < kScanItems; ++k) v[k] = (base + k < n_items) ? data[base + k] : 0u;
+    }
+    // cells holding kDenseCell..kDenseMax particles are listed for link_dense_kernel (order is
+    // irrelevant); one atomic per warp that has any
+    {
+        unsigned int nd = 0;
+#pragma unroll
+        for (int k = 0; k < kScanItems; ++k)
+            nd += (v[k] >= (unsigned int)kDenseCell && v[k] <= (unsigned int)kDenseMax) ? 1u : 0u;
+        if (__any_sync(0xffffffffu, nd != 0u)) {
+            unsigned int incl_d = nd;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const unsigned int t = __shfl_up_sync(0xffffffffu, incl_d, o);
+                if (lane >= o) incl_d += t;
+            }
+            unsigned int wbase = 0;
+            if (lane == 31) wbase = atomicAdd(&ctrl->ndense, incl_d);
+            wbase = __shfl_sync(0xffffffffu, wbase, 31);
+            unsigned int dst = wbase + incl_d - nd;
+#pragma unroll
+            for (int k = 0; k < kScanItems; ++k)
+                if (v[k] >= (unsigned int)kDenseCell && v[k] <= (unsigned int)kDenseMax)
+                    dense_list[dst++] = (unsigned int)(base + k);
+        }
     }
     unsigned int sum = 0;
 #pragma unroll
@@ -151,9 +176,9 @@ cudaError_t launch_bin(const float *pos, int64_t N, Grid g, unsigned int *cell_c
 }
 
 cudaError_t launch_cell_scan(unsigned int *cell, int64_t n_items, unsigned long long *state, Ctrl *ctrl,
-                             int64_t tiles, cudaStream_t s)
+                             unsigned int *dense_list, int64_t tiles, cudaStream_t s)
 {
-    cell_scan_kernel<<<(unsigned int)tiles, kBlock, 0, s>>>(cell, n_items, state, ctrl);
+    cell_scan_kernel<<<(unsigned int)tiles, kBlock, 0, s>>>(cell, n_items, state, ctrl, dense_list);
     return cudaGetLastError();
 }
 
