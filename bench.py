@@ -39,9 +39,10 @@ UNIT = "particles/s"
 # implementation cost and are deliberately NOT counted.
 ALG_BYTES_PER_PARTICLE = {
     "link.clear": 0,
-    "link.bin": 12,                # read pos (histogram)
-    "link.cell_scan": 0,
-    "link.scatter": 12 + 16,       # read pos, write sorted (x, y, z, idx)
+    "link.hist": 12,               # read pos (histogram)
+    "link.offsets": 0,
+    "link.partition": 12,          # read pos (reorder); the bin-contiguous intermediate is not counted
+    "link.cell_sort": 16,          # write sorted (x, y, z, idx)
     "link.pairs": 16 + 4,          # read sorted once, write parent
     "link.flatten": 4 + 4 + 4 + 4, # flatten parent read + write; read idx, min-per-root RMW
     "link.labels": 4 + 4,          # gather the root's minimum, write labels (original order)

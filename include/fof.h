@@ -51,7 +51,7 @@ int fof_create(int64_t N, float L, float b, int32_t N_min, fof_handle **out);
 void fof_destroy(fof_handle *h);
 
 /* Tuning knob that cannot change results: force n cells per axis (3 <= n <= n_max where
- * n_max = floor(L / (b * 1.001)), n <= 1290).  Changes fof_workspace_bytes(). */
+ * n_max = floor(L / (b * 1.001)), n <= 1024).  Changes fof_workspace_bytes(). */
 int fof_set_grid(fof_handle *h, int32_t n);
 /* n per axis, total cells n^3, largest admissible n. Any out pointer may be NULL. */
 int fof_get_grid(const fof_handle *h, int32_t *n, int64_t *cells, int32_t *n_max);

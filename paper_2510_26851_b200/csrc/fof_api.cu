@@ -21,19 +21,22 @@ void layout(fof_handle *h)
     const size_t N = (size_t)h->N;
     h->C = (int64_t)h->n * h->n * h->n;
     const int64_t cell_items = h->C + 1;
-    h->scan_tiles = (cell_items + kScanTile - 1) / kScanTile;
+    h->sort.shift = kMinShift;
+    while (((h->C + ((int64_t)1 << h->sort.shift) - 1) >> h->sort.shift) > kMaxBins) ++h->sort.shift;
+    h->sort.bins = (int)((h->C + ((int64_t)1 << h->sort.shift) - 1) >> h->sort.shift);
     h->gscan_tiles = h->N > 0 ? (h->N + kScanTile - 1) / kScanTile : 1;
     h->max_groups = h->N / h->N_min;
     size_t off = 0;
     h->off_ctrl = off;        off += 256;
     h->off_cell = off;        off += align256(((size_t)cell_items + 8) * sizeof(unsigned int));
-    h->off_rel = off;         off += align256((N + 1) * sizeof(unsigned int));  // cleared with ctrl + cells
-    h->off_rank = off;        off += align256((N + 1) * sizeof(unsigned int));
+    h->off_rel = off;         off += align256((N + 1) * sizeof(unsigned int));
+    h->off_cta_hist = off;    off += align256((size_t)kMaxPartCtas * h->sort.bins * sizeof(unsigned int));
+    h->off_bin_base = off;    off += align256(((size_t)h->sort.bins + 2) * sizeof(unsigned int));
+    h->off_part = off;        off += align256((N + 1) * sizeof(float4));
     h->off_idx = off;         off += align256((N + 1) * sizeof(int));
     h->off_minidx = off;      off += align256((N + 1) * sizeof(int));
     h->off_dense = off;       off += align256((N / kDenseCell + 2) * sizeof(unsigned int));
     h->off_sorted = off;      off += align256((N + 1) * sizeof(float4));
-    h->off_scan_state = off;  off += align256((size_t)h->scan_tiles * sizeof(unsigned long long));
     h->off_cnt = off;         off += align256((N + 1) * sizeof(int));
     h->off_acc = off;         off += align256(((size_t)h->max_groups + 1) * 4 * sizeof(double));
     h->off_gscan_state = off; off += align256((size_t)h->gscan_tiles * sizeof(unsigned long long));
@@ -66,10 +69,10 @@ int cuda_fail(fof_handle *h, cudaError_t e, const char *where)
     } while (0)
 
 // Profiled stages, in execution order (fof_profile_name).
-enum Stage { kLinkClear = 0, kLinkBin, kLinkScan, kLinkScatter, kLinkPairs, kLinkFlatten, kLinkLabels,
+enum Stage { kLinkClear = 0, kLinkHist, kLinkOffsets, kLinkPartition, kLinkCellSort, kLinkPairs, kLinkFlatten, kLinkLabels,
              kGroupsClear, kGroupsCount, kGroupsCompact, kGroupsReduce, kGroupsFinish, kNumStages };
 const char *const kStageName[kNumStages] = {
-    "link.clear", "link.bin", "link.cell_scan", "link.scatter", "link.pairs", "link.flatten", "link.labels",
+    "link.clear", "link.hist", "link.offsets", "link.partition", "link.cell_sort", "link.pairs", "link.flatten", "link.labels",
     "groups.clear", "groups.count", "groups.compact", "groups.reduce", "groups.finish"};
 static_assert(kNumStages <= kMaxStages, "raise kMaxStages");
 
@@ -85,6 +88,25 @@ struct StageTimer {  // records the two events of a stage around its launches
     }
     ~StageTimer() { if (h->prof_slots) cudaEventRecord(h->ev[(h->prof_cur * kMaxStages + k) * 2 + 1], s); }
 };
+
+}  // namespace
+
+namespace fof {
+void StageHook::begin(int k, int kernels)
+{
+    h->launches += (unsigned long long)kernels;
+    if (h->prof_slots) {
+        cudaEventRecord(h->ev[(h->prof_cur * kMaxStages + base + k) * 2], s);
+        h->ev_valid[h->prof_cur * kMaxStages + base + k] = true;
+    }
+}
+void StageHook::end(int k)
+{
+    if (h->prof_slots) cudaEventRecord(h->ev[(h->prof_cur * kMaxStages + base + k) * 2 + 1], s);
+}
+}  // namespace fof
+
+namespace {
 
 template <typename T>
 inline T *at(void *ws, size_t off) { return reinterpret_cast<T *>(static_cast<char *>(ws) + off); }
@@ -211,32 +233,35 @@ int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *s
         CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute");
         h->num_sms = sms;
     }
+    {   // level-1 partition: 2 CTAs of 1024 threads per SM while two bin tables fit the shared memory
+        const int per_sm = (size_t)h->sort.bins * sizeof(unsigned int) <= 100 * 1024 ? 2 : 1;
+        h->part_ctas = h->num_sms * per_sm < kMaxPartCtas ? h->num_sms * per_sm : kMaxPartCtas;
+    }
     Ctrl *ctrl = at<Ctrl>(ws, h->off_ctrl);
     unsigned int *cell = at<unsigned int>(ws, h->off_cell);
-    unsigned int *rank = at<unsigned int>(ws, h->off_rank);
     float4 *sorted = at<float4>(ws, h->off_sorted);
-    unsigned long long *state = at<unsigned long long>(ws, h->off_scan_state);
+    unsigned int *rel = at<unsigned int>(ws, h->off_rel);
+    int *idx_s = at<int>(ws, h->off_idx), *minidx = at<int>(ws, h->off_minidx);
+    unsigned int *dense = at<unsigned int>(ws, h->off_dense);
     h->linked = false;
-    // ctrl + cell counters + rel (union-find forest: all roots) are contiguous: one memset; scan state: another
     const int has = h->N > 0;
     if (h->prof_slots) {
         h->prof_cur = (h->prof_cur + 1) % h->prof_slots;
         for (int k = 0; k < kNumStages; ++k) h->ev_valid[h->prof_cur * kMaxStages + k] = false;
     }
-    {
+    {   // only the control block needs clearing: every other array is fully written by the sort
         StageTimer t(h, s, kLinkClear, 0);
-        CK(cudaMemsetAsync(ws, 0, h->off_rank, s), "memset cells");
-        CK(cudaMemsetAsync(state, 0, (size_t)h->scan_tiles * sizeof(unsigned long long), s), "memset scan state");
+        CK(cudaMemsetAsync(ctrl, 0, 256, s), "memset ctrl");
     }
-    { StageTimer t(h, s, kLinkBin, has); CK(launch_bin(pos, h->N, h->grid, cell, rank, ctrl, s), "bin_kernel"); }
-    { StageTimer t(h, s, kLinkScan, 1); CK(launch_cell_scan(cell, h->C + 1, state, ctrl, at<unsigned int>(ws, h->off_dense), h->scan_tiles, s), "cell_scan_kernel"); }
-    { StageTimer t(h, s, kLinkScatter, has); CK(launch_scatter(pos, h->N, h->grid, cell, rank, sorted, s), "scatter_kernel"); }
-    unsigned int *rel = at<unsigned int>(ws, h->off_rel);
-    int *idx_s = at<int>(ws, h->off_idx), *minidx = at<int>(ws, h->off_minidx);
+    {
+        StageHook hook{h, s, kLinkHist};
+        CK(launch_sort(pos, h->N, h->grid, h->sort, h->part_ctas, at<unsigned int>(ws, h->off_cta_hist),
+                       at<unsigned int>(ws, h->off_bin_base), at<float4>(ws, h->off_part), cell, sorted, rel, idx_s,
+                       minidx, dense, ctrl, hook, s), "sort kernels");
+    }
     {
         StageTimer t(h, s, kLinkPairs, 2 * has);
-        CK(launch_link(sorted, h->N, h->grid, cell, at<unsigned int>(ws, h->off_dense), rel, idx_s, minidx, ctrl,
-                       h->num_sms, s), "link kernels");
+        CK(launch_link(sorted, h->N, h->grid, cell, dense, rel, ctrl, h->num_sms, s), "link kernels");
     }
     { StageTimer t(h, s, kLinkFlatten, has); CK(launch_flatten_min(rel, idx_s, minidx, h->N, s), "flatten_min_kernel"); }
     { StageTimer t(h, s, kLinkLabels, has); CK(launch_write_labels(rel, idx_s, minidx, labels, h->N, s), "write_labels_kernel"); }

@@ -14,20 +14,25 @@ constexpr int kBlock = 256;           // threads per CTA for the streaming kerne
 constexpr int kScanItems = 8;         // items per thread in the single-pass scan
 constexpr int kScanTile = kBlock * kScanItems;
 constexpr float kCellMargin = 1.001f; // cell side >= b * kCellMargin  (R3)
-constexpr int kMaxGrid = 1290;        // n^3 < 2^31
+constexpr int kMaxGrid = 1024;        // n^3 <= 2^30: at most kMaxBins bins of 2^15 cells
+constexpr int kPartThreads = 1024;    // threads per CTA of the level-1 partition kernels
+constexpr int kCellSortThreads = 512; // threads per CTA of the level-2 cell sort
+constexpr int kMinShift = 12;         // a bin is 2^shift consecutive cell ids, shift in [12, 15]
+constexpr int kMaxBins = 32768;       // level-1 bins (one shared-memory counter each)
+constexpr int kMaxPartCtas = 512;     // CTAs of the level-1 kernels (2 per SM)
 constexpr int kMaxStages = 24;        // profiled stages (fof_profile_*)
 
 // Device control block at the start of the workspace (zeroed at the start of fof_link).
 struct Ctrl {
     unsigned int error;        // bit 0: non-finite position seen
-    unsigned int scan_ticket;  // dynamic tile id for the cell scan
+    unsigned int scan_ticket;  // blocks of part_offsets_kernel that have finished
     unsigned int gscan_ticket; // dynamic tile id for the group compaction scan
     unsigned int pad0;
     unsigned long long edges;       // true edges (unordered pairs with d2 <= b2)
     unsigned long long pair_tests;  // distance tests executed
     long long K;                    // kept groups (written by fof_groups)
     unsigned long long grid_pairs;  // candidate pairs of the unfiltered half stencil on this grid
-    unsigned int ndense;            // entries of the dense-cell list (written by the cell scan)
+    unsigned int ndense;            // entries of the dense-cell list (written by cell_sort_kernel)
     unsigned int pad1[5];
 };
 static_assert(sizeof(Ctrl) <= 256, "Ctrl must fit its 256-byte slot");
@@ -50,6 +55,13 @@ constexpr int kDenseMax = 256;
 
 }  // namespace fof
 
+namespace fof {
+struct SortPlan {
+    int shift;  // cells per bin = 2^shift
+    int bins;   // ceil(C / 2^shift) <= kMaxBins
+};
+}  // namespace fof
+
 struct fof_handle {
     int64_t N;
     float L, b;
@@ -58,11 +70,12 @@ struct fof_handle {
     int64_t C;  // n^3
     fof::Grid grid;
     // workspace layout (byte offsets, 256-B aligned)
-    size_t off_ctrl, off_cell, off_rank, off_sorted, off_scan_state, off_cnt, off_acc, off_gscan_state;
+    fof::SortPlan sort;
+    size_t off_ctrl, off_cell, off_part, off_cta_hist, off_bin_base, off_sorted, off_cnt, off_acc, off_gscan_state;
     size_t off_rel, off_idx, off_minidx, off_dense;  // union-find (cell-sorted space), original index, min original index
     size_t ws_bytes;
-    int64_t scan_tiles, gscan_tiles, max_groups;
-    int num_sms;
+    int64_t gscan_tiles, max_groups;
+    int num_sms, part_ctas;
     bool linked;
     const void *linked_ws;
     char cuda_err[256];
@@ -131,16 +144,22 @@ __device__ __forceinline__ void st_relaxed_u64(unsigned long long *p, unsigned l
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
+// Brackets one profiled stage (fof_profile_*) around the launches of a multi-kernel launcher.
+struct StageHook {
+    fof_handle *h;
+    cudaStream_t s;
+    int base;  // stage id of the launcher's first kernel
+    void begin(int k, int kernels);
+    void end(int k);
+};
+
 // kernels (one launcher per step; all asynchronous on `s`)
-cudaError_t launch_bin(const float *pos, int64_t N, Grid g, unsigned int *cell_count, unsigned int *rank,
-                       Ctrl *ctrl, cudaStream_t s);
-cudaError_t launch_cell_scan(unsigned int *cell, int64_t n_items, unsigned long long *state, Ctrl *ctrl,
-                             unsigned int *dense_list, int64_t tiles, cudaStream_t s);
-cudaError_t launch_scatter(const float *pos, int64_t N, Grid g, const unsigned int *cell_start,
-                           const unsigned int *rank, float4 *sorted, cudaStream_t s);
+cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp, int ctas, unsigned int *cta_hist,
+                        unsigned int *bin_base, float4 *part, unsigned int *cell_start, float4 *sorted,
+                        unsigned int *rel, int *idx_s, int *minidx, unsigned int *dense_list, Ctrl *ctrl,
+                        StageHook &hook, cudaStream_t s);
 cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
-                        const unsigned int *dense_list, unsigned int *rel, int *idx_s, int *minidx, Ctrl *ctrl,
-                        int num_sms, cudaStream_t s);
+                        const unsigned int *dense_list, unsigned int *rel, Ctrl *ctrl, int num_sms, cudaStream_t s);
 cudaError_t launch_grid_pairs(const unsigned int *cell_start, Grid g, Ctrl *ctrl, int num_sms, cudaStream_t s);
 cudaError_t launch_flatten_min(unsigned int *rel, const int *idx_s, int *minidx, int64_t N, cudaStream_t s);
 cudaError_t launch_write_labels(const unsigned int *rel, const int *idx_s, const int *minidx, int *labels, int64_t N,

@@ -220,8 +220,7 @@ __device__ __forceinline__ void warp_link(const float4 *__restrict__ sorted, con
 // H4.  Persistent grid: each CTA walks chunks of kLinkBlock consecutive cell-sorted particles.
 __global__ void __launch_bounds__(kLinkBlock) link_kernel(const float4 *__restrict__ sorted, int64_t N, Grid g,
                                                           const unsigned int *__restrict__ cell_start,
-                                                          unsigned int *rel, int *__restrict__ idx_s,
-                                                          int *__restrict__ minidx, Ctrl *ctrl)
+                                                          unsigned int *rel, Ctrl *ctrl)
 {
     __shared__ int2 s_queue[kWarpsPerCta][kQueue];
     int2 *q = s_queue[threadIdx.x >> 5];
@@ -237,9 +236,6 @@ __global__ void __launch_bounds__(kLinkBlock) link_kernel(const float4 *__restri
         bool needwrap = false;
         if (valid) {
             me = __ldg(sorted + si);
-            const int oi = __float_as_int(me.w);
-            idx_s[si] = oi;
-            minidx[si] = oi;
             const float ux = __fmul_rn(me.x, g.inv_cell), uy = __fmul_rn(me.y, g.inv_cell),
                         uz = __fmul_rn(me.z, g.inv_cell);
             h.cx = min(__float2int_rd(ux), g.n_minus_1);
@@ -426,13 +422,12 @@ cudaError_t launch_grid_pairs(const unsigned int *cell_start, Grid g, Ctrl *ctrl
 static inline unsigned int blocks_for(int64_t n, int per_block) { return (unsigned int)((n + per_block - 1) / per_block); }
 
 cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
-                        const unsigned int *dense_list, unsigned int *rel, int *idx_s, int *minidx, Ctrl *ctrl,
-                        int num_sms, cudaStream_t s)
+                        const unsigned int *dense_list, unsigned int *rel, Ctrl *ctrl, int num_sms, cudaStream_t s)
 {
     if (N <= 0) return cudaSuccess;
     const unsigned int grid = (unsigned int)min((int64_t)blocks_for(N, kLinkBlock), (int64_t)num_sms * 32);
     link_dense_kernel<<<(unsigned int)num_sms * 8, kLinkBlock, 0, s>>>(sorted, g, cell_start, dense_list, rel, ctrl);
-    link_kernel<<<grid, kLinkBlock, 0, s>>>(sorted, N, g, cell_start, rel, idx_s, minidx, ctrl);
+    link_kernel<<<grid, kLinkBlock, 0, s>>>(sorted, N, g, cell_start, rel, ctrl);
     return cudaGetLastError();
 }
 

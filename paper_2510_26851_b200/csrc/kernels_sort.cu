@@ -1,191 +1,336 @@
 // kernels_sort.cu — H1 wrap + bin, H2 cell histogram + exclusive scan, H3 cell-contiguous reorder.
 // PAPER.md:193-199 (Alg. 2: wrap, grid setup, cell indexing, sort by cell); the exclusive scan of
 // the cell histogram replaces the per-particle lower/upper_bound searches of PAPER.md:203-206.
+//
+// Design: a two-level counting sort that never issues a global atomic per
+// particle and never writes a lone 16-byte record to a random DRAM address.
+//   level 1  the cell ids are cut into `bins` runs of 2^shift consecutive cells (~4096 particles
+//            each).  part_hist_kernel: every CTA histograms its contiguous chunk of the input over
+//            the bins in shared memory; part_offsets_kernel turns the [CTA][bin] counts into
+//            write cursors (bin-major, CTA-minor exclusive scan); part_scatter_kernel re-reads the
+//            chunk and writes (x, y, z, bitcast idx) records bin-contiguously.  The open write
+//            streams (CTAs x bins x 32 B) fit the L2, so DRAM sees merged lines.
+//   level 2  cell_sort_kernel: one CTA per bin histograms the bin's particles over its 2^shift
+//            cells in shared memory, scans, writes cell_start[] coalesced, and moves every record
+//            to its final place (inside the bin's window of `sorted`, L2 resident).  It also
+//            initialises the union-find forest, the original-index arrays of H5 and the list of
+//            dense cells of H4.
 #include "fof_internal.cuh"
 
 namespace fof {
 
-// ---------------------------------------------------------------------------------------------
-// H1 + first half of H2: one thread per particle.  Reads pos once; the atomicAdd on the cell
-// counter returns the particle's rank inside its cell, which makes H3 atomic-free.
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kBlock) bin_kernel(const float *__restrict__ pos, int64_t N, Grid g,
-                                                     unsigned int *__restrict__ cell_count,
-                                                     unsigned int *__restrict__ rank, Ctrl *ctrl)
+// wrapped position (non-finite -> 0 and `bad`) and linear cell id of one particle
+__device__ __forceinline__ unsigned int wrap_cell(float &x, float &y, float &z, const Grid &g, bool &bad)
 {
-    int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x;
-    if (i >= N) return;
-    float x = pos[3 * i + 0], y = pos[3 * i + 1], z = pos[3 * i + 2];
-    if (!(isfinite(x) && isfinite(y) && isfinite(z))) {
-        atomicOr(&ctrl->error, 1u);
-        x = y = z = 0.0f;
-    }
+    if (!(isfinite(x) && isfinite(y) && isfinite(z))) { bad = true; x = y = z = 0.0f; }
     x = wrap1(x, g.L);
     y = wrap1(y, g.L);
     z = wrap1(z, g.L);
-    unsigned int c = cell_id(cell1(x, g), cell1(y, g), cell1(z, g), g.n);
-    rank[i] = atomicAdd(cell_count + c, 1u);
+    return cell_id(cell1(x, g), cell1(y, g), cell1(z, g), g.n);
 }
 
-// ---------------------------------------------------------------------------------------------
-// H2: single-pass exclusive scan (decoupled look-back) over the cell counters, in place.
-// state[tile] = (flag << 32) | value, flag 1 = tile aggregate, 2 = inclusive prefix; one 64-bit
-// word so that flag and value are published together.  Tiles are handed out by an atomic ticket,
-// so a tile only ever waits on tiles that already started.
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ unsigned int lookback(unsigned long long *state, unsigned int tile, unsigned int aggregate,
-                                                 int lane)
+// Walks the particles [i0, i1) of one CTA four at a time: thread t takes the quads t, t + T, ...
+// With VEC (pos 16-byte aligned, i0 a multiple of 4) a quad is three 128-bit loads, all issued
+// before the first use, so every thread keeps 48 bytes in flight; f(x, y, z, i) is called per particle.
+template <bool VEC, typename F>
+__device__ __forceinline__ void for_each_particle(const float *__restrict__ pos, int64_t i0, int64_t i1, F f)
 {
-    // executed by one full warp; returns the exclusive prefix of `tile` (valid in every lane)
-    unsigned int exclusive = 0;
-    int64_t idx = (int64_t)tile - 1;
-    while (true) {
-        int64_t j = idx - lane;
-        unsigned long long v = (2ull << 32);  // tiles before 0: prefix 0
-        if (j >= 0) {
-            do { v = ld_relaxed_u64(state + j); } while ((v >> 32) == 0);
+    for (int64_t i = i0 + 4 * (int64_t)threadIdx.x; i < i1; i += 4 * (int64_t)kPartThreads) {
+        if (VEC && i + 4 <= i1) {
+            const float4 *q = reinterpret_cast<const float4 *>(pos + 3 * i);
+            const float4 a = __ldg(q), b = __ldg(q + 1), c = __ldg(q + 2);
+            f(a.x, a.y, a.z, i);
+            f(a.w, b.x, b.y, i + 1);
+            f(b.z, b.w, c.x, i + 2);
+            f(c.y, c.z, c.w, i + 3);
+        } else {
+            const int m = (int)min((int64_t)4, i1 - i);
+            float v[12];
+#pragma unroll
+            for (int k = 0; k < 12; ++k) v[k] = (k < 3 * m) ? __ldg(pos + 3 * i + k) : 0.0f;
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (k < m) f(v[3 * k], v[3 * k + 1], v[3 * k + 2], i + k);
         }
-        unsigned int flag = (unsigned int)(v >> 32), val = (unsigned int)v;
-        unsigned int full = __ballot_sync(0xffffffffu, flag == 2);
-        int stop = full ? __ffs(full) - 1 : 31;           // nearest predecessor with a full prefix
-        unsigned int part = (lane <= stop) ? val : 0;
-        for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
-        exclusive += part;
-        if (full) break;
-        idx -= 32;
     }
-    if (lane == 0) st_relaxed_u64(state + tile, (2ull << 32) | (unsigned long long)(exclusive + aggregate));
-    return exclusive;
 }
 
-__global__ void __launch_bounds__(kBlock) cell_scan_kernel(unsigned int *data, int64_t n_items,
-                                                           unsigned long long *state, Ctrl *ctrl,
-                                                           unsigned int *__restrict__ dense_list)
+// ---------------------------------------------------------------------------------------------
+// H1 + H2 (level 1): per-CTA histogram of its chunk over the bins.
+// ---------------------------------------------------------------------------------------------
+template <bool VEC>
+__global__ void __launch_bounds__(kPartThreads) part_hist_kernel(const float *__restrict__ pos, int64_t N, Grid g,
+                                                                 int shift, int bins, int64_t chunk,
+                                                                 unsigned int *__restrict__ cta_hist, Ctrl *ctrl)
 {
-    __shared__ unsigned int s_tile, s_prefix;
-    __shared__ unsigned int s_warp[kBlock / 32];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_tile = atomicAdd(&ctrl->scan_ticket, 1u);
+    extern __shared__ unsigned int s_bin[];
+    for (int b = threadIdx.x; b < bins; b += kPartThreads) s_bin[b] = 0u;
     __syncthreads();
-    const unsigned int tile = s_tile;
-    const int64_t base = (int64_t)tile * kScanTile + (int64_t)tid * kScanItems;
+    const int64_t i0 = (int64_t)blockIdx.x * chunk;
+    const int64_t i1 = min(N, i0 + chunk);
+    bool any_bad = false;
+    for_each_particle<VEC>(pos, i0, i1, [&](float x, float y, float z, int64_t) {
+        const unsigned int c = wrap_cell(x, y, z, g, any_bad);
+        atomicAdd(&s_bin[c >> shift], 1u);
+    });
+    if (any_bad) atomicOr(&ctrl->error, 1u);
+    __syncthreads();
+    unsigned int *dst = cta_hist + (int64_t)blockIdx.x * bins;
+    for (int b = threadIdx.x; b < bins; b += kPartThreads) dst[b] = s_bin[b];
+}
 
-    unsigned int v[kScanItems];
-    if (base + kScanItems <= n_items) {
-        const uint4 a = *reinterpret_cast<const uint4 *>(data + base);
-        const uint4 b = *reinterpret_cast<const uint4 *>(data + base + 4);
-        v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
-    } else {
+// ---------------------------------------------------------------------------------------------
+// cta_hist[k][b] <- sum over k' < k of cta_hist[k'][b] (in place), bin_base[b] <- sum over b' < b
+// of the bin totals, bin_base[bins] = N.  Block = 32 bins x 8 groups of CTAs; the last block to
+// finish scans the bin totals.
+// ---------------------------------------------------------------------------------------------
+constexpr int kOffGroups = 8;
+
+__global__ void __launch_bounds__(32 * kOffGroups) part_offsets_kernel(unsigned int *cta_hist, int ctas, int bins,
+                                                                       unsigned int *bin_base, Ctrl *ctrl)
+{
+    __shared__ unsigned int s_part[kOffGroups][33];
+    __shared__ unsigned int s_last;
+    __shared__ unsigned int s_warp[32 * kOffGroups / 32];
+    const int bx = threadIdx.x & 31, gy = threadIdx.x >> 5;
+    const int b = blockIdx.x * 32 + bx;
+    const int per = (ctas + kOffGroups - 1) / kOffGroups;
+    const int k0 = gy * per, k1 = min(ctas, k0 + per);
+    unsigned int sum = 0;
+    if (b < bins)
+        for (int k = k0; k < k1; ++k) sum += cta_hist[(int64_t)k * bins + b];
+    s_part[gy][bx] = sum;
+    __syncthreads();
+    unsigned int run = 0, total = 0;
 #pragma unroll
-        for (int k = 0; k < kScanItems; ++k) v[k] = (base + k < n_items) ? data[base + k] : 0u;
+    for (int q = 0; q < kOffGroups; ++q) {
+        const unsigned int t = s_part[q][bx];
+        if (q < gy) run += t;
+        total += t;
     }
-    // cells holding kDenseCell..kDenseMax particles are listed for link_dense_kernel (order is
-    // irrelevant); one atomic per warp that has any
-    {
-        unsigned int nd = 0;
+    if (b < bins) {
+        for (int k = k0; k < k1; ++k) {
+            unsigned int *p = cta_hist + (int64_t)k * bins + b;
+            const unsigned int t = *p;
+            *p = run;
+            run += t;
+        }
+        if (gy == 0) bin_base[b + 1] = total;  // totals, shifted by one; scanned below
+    }
+    // last block done: inclusive scan of bin_base[1..bins] in place, bin_base[0] = 0
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(&ctrl->scan_ticket, 1u) == gridDim.x - 1) ? 1u : 0u;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    constexpr int T = 32 * kOffGroups;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    unsigned int carry = 0;
+    for (int base = 0; base < bins; base += T) {
+        const int j = base + threadIdx.x;
+        const unsigned int v = (j < bins) ? ((volatile unsigned int *)bin_base)[j + 1] : 0u;
+        unsigned int incl = v;
 #pragma unroll
-        for (int k = 0; k < kScanItems; ++k)
-            nd += (v[k] >= (unsigned int)kDenseCell && v[k] <= (unsigned int)kDenseMax) ? 1u : 0u;
-        if (__any_sync(0xffffffffu, nd != 0u)) {
-            unsigned int incl_d = nd;
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned int t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        if (lane == 31) s_warp[warp] = incl;
+        __syncthreads();
+        unsigned int off = carry, tot = 0;
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const unsigned int t = __shfl_up_sync(0xffffffffu, incl_d, o);
-                if (lane >= o) incl_d += t;
-            }
-            unsigned int wbase = 0;
-            if (lane == 31) wbase = atomicAdd(&ctrl->ndense, incl_d);
-            wbase = __shfl_sync(0xffffffffu, wbase, 31);
-            unsigned int dst = wbase + incl_d - nd;
+        for (int w = 0; w < T / 32; ++w) {
+            const unsigned int t = s_warp[w];
+            if (w < warp) off += t;
+            tot += t;
+        }
+        if (j < bins) bin_base[j + 1] = off + incl;
+        carry += tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) bin_base[0] = 0u;
+}
+
+// ---------------------------------------------------------------------------------------------
+// H3 (level 1): bin-contiguous records.  Same chunk -> CTA map as part_hist_kernel, so the
+// shared-memory cursors (cta_hist + bin_base) hand out exactly the slots that were counted.
+// ---------------------------------------------------------------------------------------------
+template <bool VEC>
+__global__ void __launch_bounds__(kPartThreads) part_scatter_kernel(const float *__restrict__ pos, int64_t N, Grid g,
+                                                                    int shift, int bins, int64_t chunk,
+                                                                    const unsigned int *__restrict__ cta_hist,
+                                                                    const unsigned int *__restrict__ bin_base,
+                                                                    float4 *__restrict__ part)
+{
+    extern __shared__ unsigned int s_bin[];
+    const unsigned int *src = cta_hist + (int64_t)blockIdx.x * bins;
+    for (int b = threadIdx.x; b < bins; b += kPartThreads) s_bin[b] = src[b] + bin_base[b];
+    __syncthreads();
+    const int64_t i0 = (int64_t)blockIdx.x * chunk;
+    const int64_t i1 = min(N, i0 + chunk);
+    bool bad = false;
+    for_each_particle<VEC>(pos, i0, i1, [&](float x, float y, float z, int64_t i) {
+        const unsigned int c = wrap_cell(x, y, z, g, bad);
+        const unsigned int dst = atomicAdd(&s_bin[c >> shift], 1u);
+        part[dst] = make_float4(x, y, z, __int_as_float((int)i));
+    });
+}
+
+// ---------------------------------------------------------------------------------------------
+// H2 + H3 (level 2): one CTA per bin.  Shared memory: one counter per cell of the bin.
+//   1. histogram of the bin's records over its cells (shared-memory atomics);
+//   2. exclusive scan -> cell_start[] (coalesced), list of dense cells for link_dense_kernel;
+//   3. records re-read (L2) and moved to their final slot; rel = 0 (every particle a root),
+//      idx_s = minidx = original index (inputs of H5).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned int cell_of(const float4 &v, const Grid &g)
+{
+    return cell_id(cell1(v.x, g), cell1(v.y, g), cell1(v.z, g), g.n);
+}
+
+__global__ void __launch_bounds__(kCellSortThreads) cell_sort_kernel(
+    const float4 *__restrict__ part, const unsigned int *__restrict__ bin_base, Grid g, int shift, int64_t C,
+    unsigned int *__restrict__ cell_start, float4 *sorted, unsigned int *__restrict__ rel,
+    int *__restrict__ idx_s, int *__restrict__ minidx, unsigned int *__restrict__ dense_list, Ctrl *ctrl)
+{
+    extern __shared__ unsigned int s_cell[];  // [2^shift]
+    __shared__ unsigned long long s_warp[kCellSortThreads / 32];
+    __shared__ unsigned int s_dbase;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int cpb = 1 << shift;
+    const int64_t cell0 = (int64_t)blockIdx.x << shift;
+    const int ncell = (int)min((int64_t)cpb, C - cell0);
+    const unsigned int p0 = bin_base[blockIdx.x], p1 = bin_base[blockIdx.x + 1];
+
+    for (int c = tid; c < cpb; c += kCellSortThreads) s_cell[c] = 0u;
+    __syncthreads();
+    // four records in flight per thread
+    for (unsigned int p = p0 + tid; p < p1; p += 4 * kCellSortThreads) {
+        float4 v[4];
 #pragma unroll
-            for (int k = 0; k < kScanItems; ++k)
-                if (v[k] >= (unsigned int)kDenseCell && v[k] <= (unsigned int)kDenseMax)
-                    dense_list[dst++] = (unsigned int)(base + k);
+        for (int u = 0; u < 4; ++u) v[u] = __ldg(part + min(p + u * kCellSortThreads, p1 - 1));
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (p + u * kCellSortThreads < p1) atomicAdd(&s_cell[cell_of(v[u], g) - (unsigned int)cell0], 1u);
+    }
+    __syncthreads();
+
+    // thread t owns cells [t * per, (t + 1) * per); (count, dense cells) packed in one 64-bit scan
+    const int per = cpb / kCellSortThreads;  // 8 .. 64, multiple of 4
+    const int c_lo = tid * per;
+    unsigned long long mine = 0;
+    for (int k = 0; k < per; k += 4) {
+        const uint4 v = *reinterpret_cast<const uint4 *>(s_cell + c_lo + k);
+        const unsigned int a[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            mine += a[u];
+            if (a[u] >= (unsigned int)kDenseCell && a[u] <= (unsigned int)kDenseMax) mine += 1ull << 32;
         }
     }
-    unsigned int sum = 0;
-#pragma unroll
-    for (int k = 0; k < kScanItems; ++k) { unsigned int t = v[k]; v[k] = sum; sum += t; }  // thread-exclusive
-    unsigned int incl = sum;
+    unsigned long long incl = mine;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-        unsigned int t = __shfl_up_sync(0xffffffffu, incl, o);
+        const unsigned long long t = __shfl_up_sync(0xffffffffu, incl, o);
         if (lane >= o) incl += t;
     }
     if (lane == 31) s_warp[warp] = incl;
     __syncthreads();
-    unsigned int warp_off = 0, total = 0;
+    unsigned long long woff = 0, total = 0;
 #pragma unroll
-    for (int w = 0; w < kBlock / 32; ++w) {
-        unsigned int t = s_warp[w];
-        if (w < warp) warp_off += t;
+    for (int w = 0; w < kCellSortThreads / 32; ++w) {
+        const unsigned long long t = s_warp[w];
+        if (w < warp) woff += t;
         total += t;
     }
-    if (warp == 0) {
-        if (tile == 0) {
-            if (lane == 0) { st_relaxed_u64(state, (2ull << 32) | total); s_prefix = 0; }
-        } else {
-            if (lane == 0) st_relaxed_u64(state + tile, (1ull << 32) | total);
-            unsigned int ex = lookback(state, tile, total, lane);
-            if (lane == 0) s_prefix = ex;
-        }
+    if (tid == 0) {
+        const unsigned int nd = (unsigned int)(total >> 32);
+        s_dbase = nd ? atomicAdd(&ctrl->ndense, nd) : 0u;
     }
     __syncthreads();
-    const unsigned int off = s_prefix + warp_off + (incl - sum);
-    if (base + kScanItems <= n_items) {
-        uint4 a = make_uint4(v[0] + off, v[1] + off, v[2] + off, v[3] + off);
-        uint4 b = make_uint4(v[4] + off, v[5] + off, v[6] + off, v[7] + off);
-        *reinterpret_cast<uint4 *>(data + base) = a;
-        *reinterpret_cast<uint4 *>(data + base + 4) = b;
-    } else {
+    const unsigned long long excl = woff + incl - mine;
+    unsigned int run = p0 + (unsigned int)excl;
+    unsigned int drun = s_dbase + (unsigned int)(excl >> 32);
+    for (int k = 0; k < per; k += 4) {
+        uint4 v = *reinterpret_cast<const uint4 *>(s_cell + c_lo + k);
+        unsigned int a[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
-        for (int k = 0; k < kScanItems; ++k)
-            if (base + k < n_items) data[base + k] = v[k] + off;
+        for (int u = 0; u < 4; ++u) {
+            const unsigned int cnt = a[u];
+            a[u] = run;
+            if (cnt >= (unsigned int)kDenseCell && cnt <= (unsigned int)kDenseMax)
+                dense_list[drun++] = (unsigned int)(cell0 + c_lo + k + u);
+            run += cnt;
+        }
+        v = make_uint4(a[0], a[1], a[2], a[3]);
+        *reinterpret_cast<uint4 *>(s_cell + c_lo + k) = v;  // now the write cursor of each cell
+        if (c_lo + k + 3 < ncell) *reinterpret_cast<uint4 *>(cell_start + cell0 + c_lo + k) = v;
+        else {
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (c_lo + k + u < ncell) cell_start[cell0 + c_lo + k + u] = a[u];
+        }
+    }
+    if (cell0 + ncell == C && tid == 0) cell_start[C] = p1;
+    __syncthreads();
+
+    for (unsigned int p = p0 + tid; p < p1; p += 4 * kCellSortThreads) {
+        float4 v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = __ldg(part + min(p + u * kCellSortThreads, p1 - 1));
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (p + u * kCellSortThreads < p1)
+                sorted[atomicAdd(&s_cell[cell_of(v[u], g) - (unsigned int)cell0], 1u)] = v[u];
+    }
+    __syncthreads();
+    // the per-particle arrays of H4 / H5, written coalesced from the records this CTA just placed
+    for (unsigned int p = p0 + tid; p < p1; p += kCellSortThreads) {
+        const int oi = __float_as_int(__ldcg(&sorted[p].w));
+        rel[p] = 0u;
+        idx_s[p] = oi;
+        minidx[p] = oi;
     }
 }
 
-// ---------------------------------------------------------------------------------------------
-// H3: reorder particles cell-contiguously; sorted[j] = (wx, wy, wz, bitcast(original index)).
-// dst = cell_start[cell] + rank: no atomics, the cell id is recomputed from pos (bit-identical
-// to H1 because it is the same code on the same input).
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kBlock) scatter_kernel(const float *__restrict__ pos, int64_t N, Grid g,
-                                                         const unsigned int *__restrict__ cell_start,
-                                                         const unsigned int *__restrict__ rank,
-                                                         float4 *__restrict__ sorted)
+static inline cudaError_t set_smem(const void *fn, size_t bytes)
 {
-    int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x;
-    if (i >= N) return;
-    float x = pos[3 * i + 0], y = pos[3 * i + 1], z = pos[3 * i + 2];
-    if (!(isfinite(x) && isfinite(y) && isfinite(z))) x = y = z = 0.0f;
-    x = wrap1(x, g.L);
-    y = wrap1(y, g.L);
-    z = wrap1(z, g.L);
-    unsigned int c = cell_id(cell1(x, g), cell1(y, g), cell1(z, g), g.n);
-    unsigned int dst = cell_start[c] + rank[i];
-    sorted[dst] = make_float4(x, y, z, __int_as_float((int)i));
+    if (bytes <= 48 * 1024) return cudaSuccess;
+    return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
-static inline unsigned int blocks_for(int64_t n, int per_block) { return (unsigned int)((n + per_block - 1) / per_block); }
-
-cudaError_t launch_bin(const float *pos, int64_t N, Grid g, unsigned int *cell_count, unsigned int *rank,
-                       Ctrl *ctrl, cudaStream_t s)
+cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp, int ctas, unsigned int *cta_hist,
+                        unsigned int *bin_base, float4 *part, unsigned int *cell_start, float4 *sorted,
+                        unsigned int *rel, int *idx_s, int *minidx, unsigned int *dense_list, Ctrl *ctrl,
+                        StageHook &hook, cudaStream_t s)
 {
-    if (N > 0) bin_kernel<<<blocks_for(N, kBlock), kBlock, 0, s>>>(pos, N, g, cell_count, rank, ctrl);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_cell_scan(unsigned int *cell, int64_t n_items, unsigned long long *state, Ctrl *ctrl,
-                             unsigned int *dense_list, int64_t tiles, cudaStream_t s)
-{
-    cell_scan_kernel<<<(unsigned int)tiles, kBlock, 0, s>>>(cell, n_items, state, ctrl, dense_list);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_scatter(const float *pos, int64_t N, Grid g, const unsigned int *cell_start,
-                           const unsigned int *rank, float4 *sorted, cudaStream_t s)
-{
-    if (N > 0) scatter_kernel<<<blocks_for(N, kBlock), kBlock, 0, s>>>(pos, N, g, cell_start, rank, sorted);
+    if (N <= 0) return cudaSuccess;
+    const size_t smem_bins = (size_t)sp.bins * sizeof(unsigned int);
+    const size_t smem_cells = ((size_t)1 << sp.shift) * sizeof(unsigned int);
+    cudaError_t e;
+    const bool vec = ((uintptr_t)pos & 15) == 0;
+    auto hist = vec ? part_hist_kernel<true> : part_hist_kernel<false>;
+    auto scat = vec ? part_scatter_kernel<true> : part_scatter_kernel<false>;
+    if ((e = set_smem((const void *)hist, smem_bins)) != cudaSuccess) return e;
+    if ((e = set_smem((const void *)scat, smem_bins)) != cudaSuccess) return e;
+    if ((e = set_smem((const void *)cell_sort_kernel, smem_cells)) != cudaSuccess) return e;
+    const int64_t chunk = ((N + ctas - 1) / ctas + 3) & ~(int64_t)3;  // a multiple of 4: quads stay aligned
+    const int64_t C = (int64_t)g.n * g.n * g.n;
+    hook.begin(0, 1);
+    hist<<<ctas, kPartThreads, smem_bins, s>>>(pos, N, g, sp.shift, sp.bins, chunk, cta_hist, ctrl);
+    hook.end(0);
+    hook.begin(1, 1);
+    part_offsets_kernel<<<(sp.bins + 31) / 32, 32 * kOffGroups, 0, s>>>(cta_hist, ctas, sp.bins, bin_base, ctrl);
+    hook.end(1);
+    hook.begin(2, 1);
+    scat<<<ctas, kPartThreads, smem_bins, s>>>(pos, N, g, sp.shift, sp.bins, chunk, cta_hist, bin_base,
+                                                             part);
+    hook.end(2);
+    hook.begin(3, 1);
+    cell_sort_kernel<<<sp.bins, kCellSortThreads, smem_cells, s>>>(part, bin_base, g, sp.shift, C, cell_start, sorted,
+                                                                  rel, idx_s, minidx, dense_list, ctrl);
+    hook.end(3);
     return cudaGetLastError();
 }
 
