@@ -19,7 +19,7 @@ constexpr int kPartThreads = 1024;    // threads per CTA of the level-1 partitio
 constexpr int kCellSortThreads = 512; // threads per CTA of the level-2 cell sort
 constexpr int kMinShift = 12;         // a bin is 2^shift consecutive cell ids, shift in [12, 15]
 constexpr int kMaxBins = 32768;       // level-1 bins (one shared-memory counter each)
-constexpr int kMaxPartCtas = 512;     // CTAs of the level-1 kernels (2 per SM)
+constexpr int kMaxPartCtas = 512;     // CTAs of the level-1 kernels (one per SM)
 constexpr int kMaxStages = 24;        // profiled stages (fof_profile_*)
 
 // Device control block at the start of the workspace (zeroed at the start of fof_link).
