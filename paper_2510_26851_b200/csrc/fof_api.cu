@@ -35,7 +35,7 @@ void layout(fof_handle *h)
     h->off_part = off;        off += align256((N + 1) * sizeof(float4));
     h->off_idx = off;         off += align256((N + 1) * sizeof(int));
     h->off_minidx = off;      off += align256((N + 1) * sizeof(int));
-    h->off_dense = off;       off += align256((N / kDenseCell + 2) * sizeof(unsigned int));
+    h->off_dense = off;       off += align256((N / kDenseCell + N / 32 + 2) * sizeof(unsigned long long));
     h->off_sorted = off;      off += align256((N + 1) * sizeof(float4));
     h->off_cnt = off;         off += align256((N + 1) * sizeof(int));
     h->off_acc = off;         off += align256(((size_t)h->max_groups + 1) * 4 * sizeof(double));
@@ -240,7 +240,7 @@ int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *s
     float4 *sorted = at<float4>(ws, h->off_sorted);
     unsigned int *rel = at<unsigned int>(ws, h->off_rel);
     int *idx_s = at<int>(ws, h->off_idx), *minidx = at<int>(ws, h->off_minidx);
-    unsigned int *dense = at<unsigned int>(ws, h->off_dense);
+    unsigned long long *dense = at<unsigned long long>(ws, h->off_dense);
     h->linked = false;
     const int has = h->N > 0;
     if (h->prof_slots) {

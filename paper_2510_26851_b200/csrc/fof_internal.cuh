@@ -32,7 +32,7 @@ struct Ctrl {
     unsigned long long pair_tests;  // distance tests executed
     long long K;                    // kept groups (written by fof_groups)
     unsigned long long grid_pairs;  // candidate pairs of the unfiltered half stencil on this grid
-    unsigned int ndense;            // entries of the dense-cell list (written by cell_sort_kernel)
+    unsigned int ndense;            // work items (dense cell, tile) listed by cell_sort_kernel
     unsigned int pad1[5];
 };
 static_assert(sizeof(Ctrl) <= 256, "Ctrl must fit its 256-byte slot");
@@ -50,8 +50,17 @@ struct Grid {
 };
 
 constexpr int kLinkBlock = 256;     // threads per CTA of the link kernels
-constexpr int kDenseCell = 8;       // cells with kDenseCell..kDenseMax particles: own pairs go to link_dense_kernel
-constexpr int kDenseMax = 256;
+constexpr int kDenseCell = 8;       // cells with >= kDenseCell particles are DENSE: every pair that involves one of
+                                    // their particles belongs to link_tiles_kernel, all others to link_sparse_kernel
+
+// A dense cell of m particles is cut into dense_tiles(m) tiles of dense_tile_size(m) <= 32
+// consecutive particles (balanced: 43 -> 22 + 21, not 32 + 11); one work item per tile.
+__host__ __device__ __forceinline__ unsigned int dense_tiles(unsigned int m) { return (m + 31u) >> 5; }
+__host__ __device__ __forceinline__ unsigned int dense_tile_size(unsigned int m)
+{
+    const unsigned int T = dense_tiles(m);
+    return T <= 16u ? (m + T - 1u) / T : 32u;
+}
 
 }  // namespace fof
 
@@ -156,10 +165,11 @@ struct StageHook {
 // kernels (one launcher per step; all asynchronous on `s`)
 cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp, int ctas, unsigned int *cta_hist,
                         unsigned int *bin_base, float4 *part, unsigned int *cell_start, float4 *sorted,
-                        unsigned int *rel, int *idx_s, int *minidx, unsigned int *dense_list, Ctrl *ctrl,
+                        unsigned int *rel, int *idx_s, int *minidx, unsigned long long *dense_list, Ctrl *ctrl,
                         StageHook &hook, cudaStream_t s);
 cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
-                        const unsigned int *dense_list, unsigned int *rel, Ctrl *ctrl, int num_sms, cudaStream_t s);
+                        const unsigned long long *dense_list, unsigned int *rel, Ctrl *ctrl, int num_sms,
+                        cudaStream_t s);
 cudaError_t launch_grid_pairs(const unsigned int *cell_start, Grid g, Ctrl *ctrl, int num_sms, cudaStream_t s);
 cudaError_t launch_flatten_min(unsigned int *rel, const int *idx_s, int *minidx, int64_t N, cudaStream_t s);
 cudaError_t launch_write_labels(const unsigned int *rel, const int *idx_s, const int *minidx, int *labels, int64_t N,

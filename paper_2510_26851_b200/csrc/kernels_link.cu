@@ -6,12 +6,23 @@
 // set, the converged min-label of PAPER.md:91.
 //
 // Design.  The union-find runs in CELL-SORTED index space: a component is a
-// spatially compact object, so its parent entries sit in a few cache lines and the "already in
-// one set?" check of an edge is a coalesced / L1-resident load instead of a random access into
-// a 4N-byte array.  One thread owns one cell-sorted particle and walks its (at most five)
-// candidate ranges: the rest of its own cell (+ the +x cell), and the rows (dy,dz) = (+1,0),
-// (-1,+1), (0,+1), (+1,+1), each a contiguous run of up to three cells of the sorted array.
-// A geometric reach filter drops every neighbour cell that is farther than b from the particle.
+// spatially compact object, so its parent entries sit in a few cache lines.  Every unordered
+// pair of particles in the same or in adjacent cells is tested exactly once, by one of two kernels:
+//   link_tiles_kernel   pairs with at least one particle in a DENSE cell (>= kDenseCell particles).
+//                       One warp per (dense cell, tile of <= 32 of its particles): the tile sits in
+//                       registers, one particle per lane; the candidates (the tile itself, the
+//                       earlier tiles of the cell, and the particles of the 26 neighbour cells that
+//                       lie within b of the cell) are staged 32 at a time in shared memory and
+//                       broadcast, so one trip of 11 instructions tests 32 pairs.  The adjacency
+//                       comes out as ballot bitmasks; components of the tile are closed in registers
+//                       and only one hook per (component, adjacent candidate) reaches the union-find.
+//                       A pair of two dense cells belongs to the one that sees the other in its
+//                       forward half stencil.
+//   link_sparse_kernel  pairs of two sparse cells.  One thread per particle collects its candidate
+//                       ranges (own cell after itself + the 13 forward cells, reach-filtered);
+//                       the ranges of a warp are flattened into one list of candidate slots that
+//                       the 32 lanes walk together, so a lane with many candidates does not hold
+//                       the others hostage.
 // The canonical label (minimum ORIGINAL index of the component) is produced by two streaming
 // passes: flatten + atomicMin of the original index at the root, then a scatter of that minimum
 // to labels[original index].
@@ -35,11 +46,11 @@ __device__ __forceinline__ bool linked_t(const float4 &a, const float4 &b, const
     return d2 <= g.b2;
 }
 
-// ---- union-find on `rel`: rel[s] = s - parent(s) >= 0 (a root has rel 0, so the forest is
-// initialised by a memset; the root of a set is its smallest cell-sorted index).  Hooks are
-// atomicCAS(rel + root, 0, distance) and can only succeed on a true root; every plain load may
-// return a stale value, which is always the offset to SOME ancestor (links only ever move up), so
-// staleness costs hops, never correctness.  Plain path-halving stores at non-roots are benign.
+// ---- union-find on `rel`: rel[s] = s - parent(s) >= 0 (a root has rel 0; the root of a set is
+// its smallest cell-sorted index).  Hooks are atomicCAS(rel + root, 0, distance) and can only
+// succeed on a true root; every plain load may return a stale value, which is always the offset
+// to SOME ancestor (links only ever move up), so staleness costs hops, never correctness.  Plain
+// path-halving stores at non-roots are benign.
 __device__ __forceinline__ int find_rel(unsigned int *rel, int x)
 {
     unsigned int d = rel[x];
@@ -65,166 +76,342 @@ __device__ __forceinline__ int unite_rel(unsigned int *rel, int a, int b)
     return ra;
 }
 
-// One candidate range of one home particle.  `root` caches the home particle's current root.
-template <bool WRAP>
-__device__ __forceinline__ void test_range(const float4 *__restrict__ sorted, unsigned int *rel, int beg, int end,
-                                           const float4 &me, int si, int &root, const Grid &g, unsigned int &edges)
-{
-    // four candidates per trip: all loads (positions and parent offsets) are issued before the first
-    // test, so one memory latency covers four tests.  A parent offset read early may be stale after
-    // a union in the same trip; that only costs a redundant find.
-    for (int t = beg; t < end; t += 4) {
-        float4 pj[4];
-        unsigned int rj[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const int tt = min(t + u, end - 1);
-            pj[u] = __ldg(sorted + tt);
-            rj[u] = rel[tt];
-        }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const int tt = t + u;
-            if (tt < end && linked_t<WRAP>(me, pj[u], g)) {
-                ++edges;
-                if (tt - (int)rj[u] != root) {  // not yet known to be in one set
-                    root = unite_rel(rel, si, tt);
-                    if (si != root) rel[si] = (unsigned int)(si - root);
-                    if (tt != root) rel[tt] = (unsigned int)(tt - root);
-                }
-            }
-        }
-    }
-}
-
-// Everything thread `si` needs to know about its candidates.
-struct Home {
-    int cx, cy, cz;
-    bool xl, xh, yl, yh, zh;  // within `reach` of the low / high face of its cell
-};
-
-// Row (y', z') of the grid, cells [cx - xl, cx + 1 + xh) clipped to the row: one run of `sorted`.
-// The cells reached through the periodic x faces are handled by wrapped_pieces().
-template <bool WRAP>
-__device__ __forceinline__ void row_range(const unsigned int *__restrict__ cs, const Home &h, int yy, int zz, int n,
-                                          bool with_lower, int &beg, int &end)
-{
-    const int rb = n * (yy + n * zz);
-    const int a = max(h.cx - (with_lower && h.xl ? 1 : 0), 0);
-    const int b = min(h.cx + 1 + (h.xh ? 1 : 0), n);
-    beg = (int)__ldg(cs + rb + a);
-    end = (int)__ldg(cs + rb + b);
-}
-
-// ---- warp-level work distribution.  The candidate ranges of the 32 home particles of a warp are
-// cut into chunks of at most kChunk candidates, queued in shared memory, and handed out to the
-// lanes round-robin, so that a lane sitting in a dense cell does not hold 31 idle lanes hostage.
-constexpr int kChunk = 8;                 // candidates per chunk
-constexpr int kQueue = 256;               // chunks per warp and window
 constexpr int kWarpsPerCta = kLinkBlock / 32;
+constexpr unsigned int kFull = 0xffffffffu;
 
-template <bool WRAP>
-__device__ __forceinline__ void warp_link(const float4 *__restrict__ sorted, const unsigned int *__restrict__ cs,
-                                          unsigned int *rel, int si, bool valid, const float4 &me, const Home &h,
-                                          const Grid &g, int2 *q, unsigned int &edges, unsigned int &tests)
+__device__ __forceinline__ unsigned int lanemask_lt()
 {
-    constexpr int NR = WRAP ? 10 : 5;
-    const int n = g.n;
-    const int lane = threadIdx.x & 31;
-    int beg[NR], len[NR];
-#pragma unroll
-    for (int k = 0; k < NR; ++k) beg[k] = len[k] = 0;
-    if (valid) {
-        int yp = h.cy + 1, ym = h.cy - 1, zp = h.cz + 1;
-        if (WRAP) {
-            if (yp == n) yp = 0;
-            if (ym < 0) ym = n - 1;
-            if (zp == n) zp = 0;
-        }
-        int e;
-        // home row: the rest of my cell, plus the +x cell
-        // (the pairs inside a DENSE home cell belong to link_dense_kernel)
-        {
-            const unsigned int *row = cs + n * (h.cy + n * h.cz) + h.cx;
-            const int c0 = (int)__ldg(row), c1 = (int)__ldg(row + 1);
-            const int e0 = (h.xh && h.cx + 1 < n) ? (int)__ldg(row + 2) : c1;
-            beg[0] = (c1 - c0 >= kDenseCell && c1 - c0 <= kDenseMax) ? c1 : si + 1;
-            len[0] = e0 - beg[0];
-        }
-        if (h.yh) { row_range<WRAP>(cs, h, yp, h.cz, n, true, beg[1], e); len[1] = e - beg[1]; }
-        if (h.zh) {
-            row_range<WRAP>(cs, h, h.cy, zp, n, true, beg[2], e); len[2] = e - beg[2];
-            if (h.yl) { row_range<WRAP>(cs, h, ym, zp, n, true, beg[3], e); len[3] = e - beg[3]; }
-            if (h.yh) { row_range<WRAP>(cs, h, yp, zp, n, true, beg[4], e); len[4] = e - beg[4]; }
-        }
-        if (WRAP) {
-            // cells behind the periodic x faces: cell 0 of a row when cx = n-1 reaches up, cell n-1
-            // when cx = 0 reaches down (never for the home row's lower side: half stencil)
-            const bool up = h.xh && h.cx == n - 1, dn = h.xl && h.cx == 0;
-            if (up || dn) {
-                const int ys[5] = {h.cy, yp, h.cy, ym, yp};
-                const int zs[5] = {h.cz, h.cz, zp, zp, zp};
-                const bool on[5] = {true, h.yh, h.zh, h.zh && h.yl, h.zh && h.yh};
-#pragma unroll
-                for (int k = 0; k < 5; ++k) {
-                    if (!on[k] || (!up && k == 0)) continue;
-                    // up and dn exclude each other unless n == 1 row cell... (n >= 3: cx cannot be both)
-                    const int c = n * (ys[k] + n * zs[k]) + (up ? 0 : n - 1);
-                    beg[5 + k] = (int)__ldg(cs + c);
-                    len[5 + k] = (int)__ldg(cs + c + 1) - beg[5 + k];
-                }
-            }
-        }
+    unsigned int m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+
+// =============================================================================================
+// link_tiles_kernel: pairs that involve a dense cell.
+// =============================================================================================
+
+// Tile I (one particle per lane, `me`; idle lanes sit at +inf) against a batch of `cnt` <= 32
+// candidates staged in shared memory.  Returns, in lane k, the mask of tile lanes linked to
+// candidate k; `nedges` (warp-uniform) counts the set bits of all masks.
+template <bool WRAP>
+__device__ __forceinline__ unsigned int batch_adjacency(const float4 &me, const float4 *s_pj, int cnt, const Grid &g,
+                                                        int lane, unsigned int &nedges)
+{
+    unsigned int adjT = 0;
+#pragma unroll 4
+    for (int k = 0; k < cnt; ++k) {
+        const unsigned int bal = __ballot_sync(kFull, linked_t<WRAP>(me, s_pj[k], g));
+        if (lane == k) adjT = bal;
+        nedges += (unsigned int)__popc(bal);
     }
-    int nch = 0;
-#pragma unroll
-    for (int k = 0; k < NR; ++k) nch += (len[k] + kChunk - 1) / kChunk;
-    int incl = nch;
+    return adjT;
+}
+
+// Hooks of one batch: candidate k (cell-sorted index in s_pj[k].w) joins every component of the
+// tile it is linked to.  `grp` = lanes of my tile component, `leader` = I am its lowest lane.
+__device__ __forceinline__ void batch_unions(unsigned int adjT, const float4 *s_pj, int cnt, unsigned int *rel, int ib,
+                                             unsigned int grp, bool leader, int lane)
+{
+    const unsigned int active = __reduce_or_sync(kFull, adjT);  // tile lanes with any link into the batch
+    if (!active) return;
+    unsigned int lead = __ballot_sync(kFull, leader && (grp & active));
+    const int j = (lane < cnt) ? __float_as_int(s_pj[lane].w) : 0;
+    while (lead) {
+        const int gl = __ffs((int)lead) - 1;
+        lead &= lead - 1u;
+        const unsigned int members = __shfl_sync(kFull, grp, gl);
+        if (adjT & members) unite_rel(rel, j, ib + gl);
+    }
+}
+
+// Neighbour cells of a dense cell: candidates from the 26 cells around (cx, cy, cz), filtered to
+// those within `reach` of the cell, compacted into batches of 32.
+template <bool WRAP>
+__device__ __forceinline__ void tile_neighbours(const float4 *__restrict__ sorted,
+                                                const unsigned int *__restrict__ cs, unsigned int *rel, float4 *s_pj,
+                                                const float4 &me, int ib, int cntI, unsigned int grp, bool leader,
+                                                int cx, int cy, int cz, const Grid &g, int lane,
+                                                unsigned int &nedges, unsigned int &ntests)
+{
+    const int n = g.n;
+    // lane q < 27 looks up neighbour cell q = (dx + 1) + 3 (dy + 1) + 9 (dz + 1); q > 13 is the forward half
+    int nx = 0, ny = 0, nz = 0, beg = 0, len = 0;
+    if (lane < 27 && lane != 13) {
+        nx = cx + lane % 3 - 1;
+        ny = cy + (lane / 3) % 3 - 1;
+        nz = cz + lane / 9 - 1;
+        if (WRAP) {
+            nx = nx < 0 ? n - 1 : (nx >= n ? 0 : nx);
+            ny = ny < 0 ? n - 1 : (ny >= n ? 0 : ny);
+            nz = nz < 0 ? n - 1 : (nz >= n ? 0 : nz);
+        }
+        const unsigned int c = cell_id(nx, ny, nz, n);
+        beg = (int)__ldg(cs + c);
+        len = (int)__ldg(cs + c + 1) - beg;
+        // a dense neighbour in my backward half owns our pairs itself
+        if (len >= kDenseCell && lane < 13) len = 0;
+    }
+    int incl = len;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-        const int v = __shfl_up_sync(0xffffffffu, incl, o);
+        const int v = __shfl_up_sync(kFull, incl, o);
         if (lane >= o) incl += v;
     }
-    const int total = __shfl_sync(0xffffffffu, incl, 31);
-    const int excl = incl - nch;
-    for (int base = 0; base < total; base += kQueue) {
-        int pos = excl - base;
+    const int total = __shfl_sync(kFull, incl, 31);
+    const int excl = incl - len;
+    const float lo = g.reach, hi = 1.0f - g.reach;
+    int nc = 0;  // candidates waiting in s_pj (warp-uniform)
+    for (int base = 0; base < total; base += 32) {
+        const int p = base + lane;
+        const bool has = p < total;
+        // owner q of slot p: the first lane whose inclusive prefix exceeds p
+        int q = 0;
 #pragma unroll
-        for (int k = 0; k < NR; ++k)
-            for (int o = 0; o < len[k]; o += kChunk, ++pos)
-                if (pos >= 0 && pos < kQueue) q[pos] = make_int2(beg[k] + o, (min(kChunk, len[k] - o) << 8) | lane);
+        for (int st = 16; st > 0; st >>= 1) {
+            const int v = __shfl_sync(kFull, incl, q + st - 1);
+            if (v <= p) q += st;
+        }
+        q = min(q, 31);
+        const int j = __shfl_sync(kFull, beg, q) + (p - __shfl_sync(kFull, excl, q));
+        const int qx = __shfl_sync(kFull, nx, q), qy = __shfl_sync(kFull, ny, q), qz = __shfl_sync(kFull, nz, q);
+        bool pass = false;
+        float4 pj = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (has) {
+            pj = __ldg(sorted + j);
+            // position of the candidate inside ITS cell; it can reach my cell only from within
+            // `reach` of the face(s) it shares with it (the same margins as the sparse kernel's flags)
+            const float fx = __fmul_rn(pj.x, g.inv_cell) - (float)qx;
+            const float fy = __fmul_rn(pj.y, g.inv_cell) - (float)qy;
+            const float fz = __fmul_rn(pj.z, g.inv_cell) - (float)qz;
+            const int dx = q % 3 - 1, dy = (q / 3) % 3 - 1, dz = q / 9 - 1;
+            pass = (dx == 0 || (dx < 0 ? fx > hi : fx < lo)) && (dy == 0 || (dy < 0 ? fy > hi : fy < lo)) &&
+                   (dz == 0 || (dz < 0 ? fz > hi : fz < lo));
+            pj.w = __int_as_float(j);
+        }
+        const unsigned int bal = __ballot_sync(kFull, pass);
+        if (pass) s_pj[nc + __popc(bal & lanemask_lt())] = pj;
+        nc += __popc(bal);
         __syncwarp();
-        const int cnt = min(kQueue, total - base);
-        for (int j0 = 0; j0 < cnt; j0 += 32) {
-            const int j = j0 + lane;
-            const bool has = j < cnt;
-            const int2 c = has ? q[j] : make_int2(0, lane);
-            const int owner = c.y & 31;
-            float4 o4;
-            o4.x = __shfl_sync(0xffffffffu, me.x, owner);
-            o4.y = __shfl_sync(0xffffffffu, me.y, owner);
-            o4.z = __shfl_sync(0xffffffffu, me.z, owner);
-            o4.w = 0.0f;
-            const int osi = __shfl_sync(0xffffffffu, si, owner);
-            if (has) {
-                const int cb = c.x, ce = c.x + (c.y >> 8);
-                tests += (unsigned int)(ce - cb);
-                int root = osi - (int)rel[osi];
-                test_range<WRAP>(sorted, rel, cb, ce, o4, osi, root, g, edges);
+        if (nc >= 32) {
+            const unsigned int adjT = batch_adjacency<WRAP>(me, s_pj, 32, g, lane, nedges);
+            ntests += 32u * (unsigned int)cntI;
+            batch_unions(adjT, s_pj, 32, rel, ib, grp, leader, lane);
+            const float4 keep = s_pj[32 + lane];
+            __syncwarp();
+            s_pj[lane] = keep;
+            nc -= 32;
+            __syncwarp();
+        }
+    }
+    if (nc) {
+        const unsigned int adjT = batch_adjacency<WRAP>(me, s_pj, nc, g, lane, nedges);
+        ntests += (unsigned int)(nc * cntI);
+        batch_unions(adjT, s_pj, nc, rel, ib, grp, leader, lane);
+    }
+    __syncwarp();
+}
+
+__global__ void __launch_bounds__(kLinkBlock) link_tiles_kernel(const float4 *__restrict__ sorted, Grid g,
+                                                                const unsigned int *__restrict__ cell_start,
+                                                                const unsigned long long *__restrict__ items,
+                                                                unsigned int *rel, Ctrl *ctrl)
+{
+    __shared__ float4 s_pj_all[kWarpsPerCta][64];
+    float4 *s_pj = s_pj_all[threadIdx.x >> 5];
+    const int lane = threadIdx.x & 31;
+    const unsigned int nitems = ctrl->ndense;
+    const unsigned int nwarps = gridDim.x * kWarpsPerCta;
+    const float inf = __int_as_float(0x7f800000);
+    const int n = g.n;
+    unsigned int nedges = 0, ntests = 0;  // warp-uniform
+    for (unsigned int it = blockIdx.x * kWarpsPerCta + (threadIdx.x >> 5); it < nitems; it += nwarps) {
+        const unsigned long long item = __ldg(items + it);
+        const unsigned int c = (unsigned int)(item >> 32);
+        const int t = (int)(unsigned int)item;
+        const int b0 = (int)__ldg(cell_start + c), e0 = (int)__ldg(cell_start + c + 1);
+        const int ts = (int)dense_tile_size((unsigned int)(e0 - b0));
+        const int ib = b0 + t * ts;
+        const int cntI = min(ts, e0 - ib);
+        // a lane without a particle sits at +inf: d2 = inf (or NaN) fails every test
+        float4 me = make_float4(inf, inf, inf, 0.0f);
+        if (lane < cntI) me = __ldg(sorted + ib + lane);
+        me.w = __int_as_float(ib + lane);
+
+        // ---- the tile against itself (pairs inside one cell never wrap: cell side <= L/3)
+        __syncwarp();
+        s_pj[lane] = me;
+        __syncwarp();
+        unsigned int e_diag = 0;
+        unsigned int adj = batch_adjacency<false>(me, s_pj, cntI, g, lane, e_diag) & ~(1u << lane);
+        // every real particle is linked to itself (d2 = 0) and every pair shows up twice; a lane at
+        // +inf gives inf - inf = NaN and is linked to nothing
+        nedges += (e_diag - (unsigned int)cntI) >> 1;
+        ntests += (unsigned int)(cntI * (cntI - 1) / 2);
+        int lab = lane;  // lowest lane of my component inside the tile
+        if (__any_sync(kFull, adj != 0u)) {
+            // breadth-first from the lowest unlabelled lane; one warp OR-reduction per level
+            const unsigned int self = 1u << lane;
+            unsigned int todo = cntI >= 32 ? kFull : ((1u << cntI) - 1u);
+            while (todo) {
+                const int r = __ffs((int)todo) - 1;
+                unsigned int vis = 1u << r;
+                while (true) {
+                    const unsigned int nxt = vis | __reduce_or_sync(kFull, (vis & self) ? adj : 0u);
+                    if (nxt == vis) break;
+                    vis = nxt;
+                }
+                if (vis & self) lab = r;
+                todo &= ~vis;
             }
+            if (lab != lane) unite_rel(rel, ib + lane, ib + lab);
+        }
+        const unsigned int grp = __match_any_sync(kFull, lab);
+        const bool leader = lab == lane;
+
+        // ---- the earlier tiles of my cell (all full: ts particles)
+        for (int jt = 0; jt < t; ++jt) {
+            const int jb = b0 + jt * ts;
+            __syncwarp();
+            if (lane < ts) {
+                float4 pj = __ldg(sorted + jb + lane);
+                pj.w = __int_as_float(jb + lane);
+                s_pj[lane] = pj;
+            }
+            __syncwarp();
+            const unsigned int adjT = batch_adjacency<false>(me, s_pj, ts, g, lane, nedges);
+            ntests += (unsigned int)(ts * cntI);
+            batch_unions(adjT, s_pj, ts, rel, ib, grp, leader, lane);
         }
         __syncwarp();
+
+        // ---- the 26 neighbour cells
+        const int cx = (int)(c % (unsigned int)n), cy = (int)((c / (unsigned int)n) % (unsigned int)n),
+                  cz = (int)(c / ((unsigned int)n * (unsigned int)n));
+        const bool wrap = n < 6 || cx == 0 || cx == n - 1 || cy == 0 || cy == n - 1 || cz == 0 || cz == n - 1;
+        if (wrap) tile_neighbours<true>(sorted, cell_start, rel, s_pj, me, ib, cntI, grp, leader, cx, cy, cz, g, lane, nedges, ntests);
+        else tile_neighbours<false>(sorted, cell_start, rel, s_pj, me, ib, cntI, grp, leader, cx, cy, cz, g, lane, nedges, ntests);
+    }
+    if (lane == 0) {
+        if (nedges) atomicAdd(&ctrl->edges, (unsigned long long)nedges);
+        if (ntests) atomicAdd(&ctrl->pair_tests, (unsigned long long)ntests);
     }
 }
 
-// H4.  Persistent grid: each CTA walks chunks of kLinkBlock consecutive cell-sorted particles.
-__global__ void __launch_bounds__(kLinkBlock) link_kernel(const float4 *__restrict__ sorted, int64_t N, Grid g,
-                                                          const unsigned int *__restrict__ cell_start,
-                                                          unsigned int *rel, Ctrl *ctrl)
+// =============================================================================================
+// link_sparse_kernel: pairs of two sparse cells.
+// =============================================================================================
+constexpr int kStencil = 14;                        // own cell + 13 forward cells
+constexpr int kMaxRanges = 32 * kStencil;           // candidate ranges of one warp
+constexpr int kMaxSlots = kMaxRanges * (kDenseCell - 1);  // a sparse cell holds < kDenseCell particles
+constexpr int kBitmapWords = (kMaxSlots + 31) / 32;
+
+// Stencil order: q = 0 own cell, 1 the +x cell, then the rows (dy, dz) = (+1, 0), (-1, +1), (0, +1),
+// (+1, +1) with dx = -1, 0, +1 each.
+struct SparseSmem {
+    int2 range[kMaxRanges];            // (first candidate, first slot << 5 | owner lane)
+    unsigned int bitmap[kBitmapWords]; // bit p set: a range starts at slot p
+};
+
+template <bool WRAP>
+__device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, const unsigned int *__restrict__ cs,
+                                            unsigned int *rel, int si, bool valid, const float4 &me, int cx, int cy,
+                                            int cz, float fx, float fy, float fz, const Grid &g, SparseSmem &sm,
+                                            int lane, unsigned int &nedges, unsigned int &ntests)
 {
-    __shared__ int2 s_queue[kWarpsPerCta][kQueue];
-    int2 *q = s_queue[threadIdx.x >> 5];
-    unsigned int edges = 0, tests = 0;
+    const int n = g.n;
+    const float lo = g.reach, hi = 1.0f - g.reach;
+    const bool xl = fx < lo, xh = fx > hi, yl = fy < lo, yh = fy > hi, zh = fz > hi;
+    int beg[kStencil], len[kStencil];
+    bool live = valid;
+#pragma unroll
+    for (int q = 0; q < kStencil; ++q) {
+        const int dx = q == 0 ? 0 : (q == 1 ? 1 : (q - 2) % 3 - 1);
+        const int dy = q < 2 ? 0 : (q < 5 ? 1 : (q < 8 ? -1 : (q < 11 ? 0 : 1)));
+        const int dz = q < 5 ? 0 : 1;
+        // the cell can hold a partner only if I am within `reach` of every face between us
+        const bool want = live && (dx == 0 || (dx < 0 ? xl : xh)) && (dy == 0 || (dy < 0 ? yl : yh)) && (dz == 0 || zh);
+        beg[q] = 0;
+        len[q] = 0;
+        if (want) {
+            int ax = cx + dx, ay = cy + dy, az = cz + dz;
+            if (WRAP) {
+                ax = ax < 0 ? n - 1 : (ax >= n ? 0 : ax);
+                ay = ay < 0 ? n - 1 : (ay >= n ? 0 : ay);
+                az = az >= n ? 0 : az;
+            }
+            const unsigned int c = cell_id(ax, ay, az, n);
+            const int b = (int)__ldg(cs + c), e = (int)__ldg(cs + c + 1);
+            if (e - b < kDenseCell) {  // pairs with a dense cell belong to link_tiles_kernel
+                beg[q] = q == 0 ? si + 1 : b;
+                len[q] = e - beg[q];
+            } else if (q == 0) {
+                live = false;  // my own cell is dense: nothing to do here
+            }
+        }
+    }
+    // flatten: one packed warp scan gives every lane its first slot (low 16 bits) and range id (high)
+    unsigned int mine = 0;
+#pragma unroll
+    for (int q = 0; q < kStencil; ++q) mine += (unsigned int)len[q] + (len[q] > 0 ? 0x10000u : 0u);
+    unsigned int incl = mine;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned int v = __shfl_up_sync(kFull, incl, o);
+        if (lane >= o) incl += v;
+    }
+    const unsigned int all = __shfl_sync(kFull, incl, 31);
+    const int total = (int)(all & 0xffffu);
+    if (total == 0) return;
+    const int words = (total + 31) >> 5;
+    for (int w = lane; w < words; w += 32) sm.bitmap[w] = 0u;
+    __syncwarp();
+    {
+        int slot = (int)((incl - mine) & 0xffffu), rid = (int)((incl - mine) >> 16);
+#pragma unroll
+        for (int q = 0; q < kStencil; ++q)
+            if (len[q] > 0) {
+                sm.range[rid++] = make_int2(beg[q], (slot << 5) | lane);
+                atomicOr(&sm.bitmap[slot >> 5], 1u << (slot & 31));
+                slot += len[q];
+            }
+    }
+    __syncwarp();
+    if (lane == 0) ntests += (unsigned int)total;
+    const unsigned int le = lanemask_lt() | (1u << lane);
+    int before = 0;  // ranges that start in earlier words
+    for (int w = 0; w < words; ++w) {
+        const unsigned int bits = sm.bitmap[w];
+        const int p = (w << 5) + lane;
+        const int2 r = sm.range[before + __popc(bits & le) - 1];  // p >= 0 has a range: slot 0 starts one
+        before += __popc(bits);
+        const int owner = r.y & 31;
+        float4 o4;
+        o4.x = __shfl_sync(kFull, me.x, owner);
+        o4.y = __shfl_sync(kFull, me.y, owner);
+        o4.z = __shfl_sync(kFull, me.z, owner);
+        o4.w = 0.0f;
+        const int osi = __shfl_sync(kFull, si, owner);
+        if (p < total) {
+            const int j = r.x + (p - (r.y >> 5));
+            const float4 pj = __ldg(sorted + j);
+            if (linked_t<WRAP>(o4, pj, g)) {
+                ++nedges;
+                unite_rel(rel, osi, j);
+            }
+        }
+    }
+    __syncwarp();
+}
+
+// Persistent grid: each warp walks chunks of 32 consecutive cell-sorted particles.
+__global__ void __launch_bounds__(kLinkBlock) link_sparse_kernel(const float4 *__restrict__ sorted, int64_t N, Grid g,
+                                                                 const unsigned int *__restrict__ cell_start,
+                                                                 unsigned int *rel, Ctrl *ctrl)
+{
+    __shared__ SparseSmem s_all[kWarpsPerCta];
+    SparseSmem &sm = s_all[threadIdx.x >> 5];
+    const int lane = threadIdx.x & 31;
+    unsigned int nedges = 0, ntests = 0;  // per lane
     const int n = g.n;
     const float lo = g.reach, hi = 1.0f - g.reach;
     for (int64_t base = (int64_t)blockIdx.x * kLinkBlock; base < N; base += (int64_t)gridDim.x * kLinkBlock) {
@@ -232,123 +419,34 @@ __global__ void __launch_bounds__(kLinkBlock) link_kernel(const float4 *__restri
         const bool valid = s64 < N;
         const int si = (int)s64;
         float4 me = make_float4(0.f, 0.f, 0.f, 0.f);
-        Home h;
+        int cx = 0, cy = 0, cz = 0;
+        float fx = 0.5f, fy = 0.5f, fz = 0.5f;
         bool needwrap = false;
         if (valid) {
             me = __ldg(sorted + si);
             const float ux = __fmul_rn(me.x, g.inv_cell), uy = __fmul_rn(me.y, g.inv_cell),
                         uz = __fmul_rn(me.z, g.inv_cell);
-            h.cx = min(__float2int_rd(ux), g.n_minus_1);
-            h.cy = min(__float2int_rd(uy), g.n_minus_1);
-            h.cz = min(__float2int_rd(uz), g.n_minus_1);
-            const float fx = ux - (float)h.cx, fy = uy - (float)h.cy, fz = uz - (float)h.cz;
-            h.xl = fx < lo; h.xh = fx > hi;
-            h.yl = fy < lo; h.yh = fy > hi;
-            h.zh = fz > hi;
-            needwrap = n < 6 || (h.xl && h.cx == 0) || (h.xh && h.cx == n - 1) || (h.yl && h.cy == 0) ||
-                       (h.yh && h.cy == n - 1) || (h.zh && h.cz == n - 1);
+            cx = min(__float2int_rd(ux), g.n_minus_1);
+            cy = min(__float2int_rd(uy), g.n_minus_1);
+            cz = min(__float2int_rd(uz), g.n_minus_1);
+            fx = ux - (float)cx;
+            fy = uy - (float)cy;
+            fz = uz - (float)cz;
+            needwrap = n < 6 || (fx < lo && cx == 0) || (fx > hi && cx == n - 1) || (fy < lo && cy == 0) ||
+                       (fy > hi && cy == n - 1) || (fz > hi && cz == n - 1);
         }
-        if (__any_sync(0xffffffffu, needwrap)) warp_link<true>(sorted, cell_start, rel, si, valid, me, h, g, q, edges, tests);
-        else warp_link<false>(sorted, cell_start, rel, si, valid, me, h, g, q, edges, tests);
+        if (__any_sync(kFull, needwrap))
+            sparse_warp<true>(sorted, cell_start, rel, si, valid, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
+        else
+            sparse_warp<false>(sorted, cell_start, rel, si, valid, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
     }
     for (int o = 16; o > 0; o >>= 1) {
-        edges += __shfl_xor_sync(0xffffffffu, edges, o);
-        tests += __shfl_xor_sync(0xffffffffu, tests, o);
+        nedges += __shfl_xor_sync(kFull, nedges, o);
+        ntests += __shfl_xor_sync(kFull, ntests, o);
     }
-    if ((threadIdx.x & 31) == 0) {  // one pair of global atomics per warp: no CTA barrier at the end
-        if (edges) atomicAdd(&ctrl->edges, (unsigned long long)edges);
-        if (tests) atomicAdd(&ctrl->pair_tests, (unsigned long long)tests);
-    }
-}
-
-// H4 (dense cells): all pairs inside one cell that holds kDenseCell..kDenseMax particles, one warp
-// per cell, run BEFORE link_kernel (every parent entry of the cell is still a root and no other
-// warp touches it).  The cell is cut into blocks of 32 particles.  For a tile (block I, block J <= I)
-// lane i builds the adjacency bitmask of its particle against the 32 particles of J with
-// warp-uniform loads (one transaction per candidate, 32 tests per trip).  Diagonal tile: the
-// components of the 32-node graph are closed by squaring the reachability masks through shuffles,
-// and written as parent offsets with plain stores -- no atomics.  Off-diagonal tile: the masks are
-// reduced to (component of I, component of J) pairs and only those are united.
-// Pairs inside one cell never wrap (cell side <= L/3 < L/2).
-__global__ void __launch_bounds__(kLinkBlock) link_dense_kernel(const float4 *__restrict__ sorted, Grid g,
-                                                                const unsigned int *__restrict__ cell_start,
-                                                                const unsigned int *__restrict__ dense_list,
-                                                                unsigned int *rel, Ctrl *ctrl)
-{
-    __shared__ unsigned char s_lab_all[kWarpsPerCta][kDenseMax];
-    __shared__ float4 s_pj_all[kWarpsPerCta][32];
-    unsigned char *s_lab = s_lab_all[threadIdx.x >> 5];
-    float4 *s_pj = s_pj_all[threadIdx.x >> 5];
-    const int lane = threadIdx.x & 31;
-    const unsigned int nd = ctrl->ndense;
-    const unsigned int nwarps = gridDim.x * kWarpsPerCta;
-    const float inf = __int_as_float(0x7f800000);
-    unsigned int edges = 0, tests = 0;
-    for (unsigned int ci = blockIdx.x * kWarpsPerCta + (threadIdx.x >> 5); ci < nd; ci += nwarps) {
-        const unsigned int c = __ldg(dense_list + ci);
-        const int b0 = (int)__ldg(cell_start + c), e0 = (int)__ldg(cell_start + c + 1);
-        for (int ib = b0; ib < e0; ib += 32) {
-            const int i = ib + lane;
-            const bool valid = i < e0;
-            // a lane without a particle sits at +inf: d2 = inf fails the test on both sides of a tile
-            float4 me = make_float4(inf, inf, inf, 0.0f);
-            if (valid) me = __ldg(sorted + i);
-            int lab = lane;  // lane of the smallest member of my component inside block I
-            for (int jb = ib; jb >= b0; jb -= 32) {  // diagonal tile first, then the earlier blocks
-                // block J staged in shared memory: the tile loop reads it with broadcast LDS.128
-                __syncwarp();
-                s_pj[lane] = (jb == ib) ? me : __ldg(sorted + jb + lane);  // earlier blocks are full
-                __syncwarp();
-                const int cnt = min(32, e0 - jb);
-                unsigned int adj = 0;
-#pragma unroll 1
-                for (int j0 = 0; j0 < cnt; j0 += 8) {
-#pragma unroll
-                    for (int u = 0; u < 8; ++u)
-                        if (linked_t<false>(me, s_pj[j0 + u], g)) adj |= 1u << (j0 + u);
-                }
-                if (jb == ib) {
-                    adj &= ~(1u << lane);
-                    edges += (unsigned int)__popc(adj & ((1u << lane) - 1u));
-                    if (valid) tests += (unsigned int)lane;
-                    // components of the 32-node graph: breadth-first from the lowest unlabelled lane; one
-                    // REDUX (warp OR of the visited lanes' adjacency) per BFS level
-                    const unsigned int self = 1u << lane;
-                    unsigned int todo = 0xffffffffu;
-                    while (todo) {
-                        const int r = __ffs((int)todo) - 1;
-                        unsigned int vis = 1u << r;
-                        while (true) {
-                            const unsigned int nxt = vis | __reduce_or_sync(0xffffffffu, (vis & self) ? adj : 0u);
-                            if (nxt == vis) break;
-                            vis = nxt;
-                        }
-                        if (vis & self) lab = r;
-                        todo &= ~vis;
-                    }
-                    if (valid && lab != lane) rel[i] = (unsigned int)(lane - lab);
-                    s_lab[i - b0] = (unsigned char)lab;
-                } else {
-                    edges += (unsigned int)__popc(adj);
-                    if (valid) tests += 32u;
-                    unsigned int reps = 0;
-                    for (unsigned int m = adj; m; m &= m - 1u) reps |= 1u << s_lab[jb - b0 + __ffs((int)m) - 1];
-                    const unsigned int peers = __match_any_sync(0xffffffffu, lab);
-                    reps = __reduce_or_sync(peers, reps);
-                    if (lane == lab)
-                        for (unsigned int m = reps; m; m &= m - 1u) unite_rel(rel, i, jb + __ffs((int)m) - 1);
-                }
-            }
-        }
-        __syncwarp();
-    }
-    for (int o = 16; o > 0; o >>= 1) {
-        edges += __shfl_xor_sync(0xffffffffu, edges, o);
-        tests += __shfl_xor_sync(0xffffffffu, tests, o);
-    }
-    if (lane == 0) {
-        if (edges) atomicAdd(&ctrl->edges, (unsigned long long)edges);
-        if (tests) atomicAdd(&ctrl->pair_tests, (unsigned long long)tests);
+    if (lane == 0) {  // one pair of global atomics per warp: no CTA barrier at the end
+        if (nedges) atomicAdd(&ctrl->edges, (unsigned long long)nedges);
+        if (ntests) atomicAdd(&ctrl->pair_tests, (unsigned long long)ntests);
     }
 }
 
@@ -422,12 +520,13 @@ cudaError_t launch_grid_pairs(const unsigned int *cell_start, Grid g, Ctrl *ctrl
 static inline unsigned int blocks_for(int64_t n, int per_block) { return (unsigned int)((n + per_block - 1) / per_block); }
 
 cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
-                        const unsigned int *dense_list, unsigned int *rel, Ctrl *ctrl, int num_sms, cudaStream_t s)
+                        const unsigned long long *dense_list, unsigned int *rel, Ctrl *ctrl, int num_sms,
+                        cudaStream_t s)
 {
     if (N <= 0) return cudaSuccess;
     const unsigned int grid = (unsigned int)min((int64_t)blocks_for(N, kLinkBlock), (int64_t)num_sms * 32);
-    link_dense_kernel<<<(unsigned int)num_sms * 8, kLinkBlock, 0, s>>>(sorted, g, cell_start, dense_list, rel, ctrl);
-    link_kernel<<<grid, kLinkBlock, 0, s>>>(sorted, N, g, cell_start, rel, ctrl);
+    link_tiles_kernel<<<(unsigned int)num_sms * 8, kLinkBlock, 0, s>>>(sorted, g, cell_start, dense_list, rel, ctrl);
+    link_sparse_kernel<<<grid, kLinkBlock, 0, s>>>(sorted, N, g, cell_start, rel, ctrl);
     return cudaGetLastError();
 }
 

@@ -180,7 +180,7 @@ __global__ void __launch_bounds__(kPartThreads) part_scatter_kernel(const float 
 // ---------------------------------------------------------------------------------------------
 // H2 + H3 (level 2): one CTA per bin.  Shared memory: one counter per cell of the bin.
 //   1. histogram of the bin's records over its cells (shared-memory atomics);
-//   2. exclusive scan -> cell_start[] (coalesced), list of dense cells for link_dense_kernel;
+//   2. exclusive scan -> cell_start[] (coalesced), work items of link_tiles_kernel (dense cells);
 //   3. records re-read (L2) and moved to their final slot; rel = 0 (every particle a root),
 //      idx_s = minidx = original index (inputs of H5).
 // ---------------------------------------------------------------------------------------------
@@ -192,7 +192,7 @@ __device__ __forceinline__ unsigned int cell_of(const float4 &v, const Grid &g)
 __global__ void __launch_bounds__(kCellSortThreads) cell_sort_kernel(
     const float4 *__restrict__ part, const unsigned int *__restrict__ bin_base, Grid g, int shift, int64_t C,
     unsigned int *__restrict__ cell_start, float4 *sorted, unsigned int *__restrict__ rel,
-    int *__restrict__ idx_s, int *__restrict__ minidx, unsigned int *__restrict__ dense_list, Ctrl *ctrl)
+    int *__restrict__ idx_s, int *__restrict__ minidx, unsigned long long *__restrict__ dense_list, Ctrl *ctrl)
 {
     extern __shared__ unsigned int s_cell[];  // [2^shift]
     __shared__ unsigned long long s_warp[kCellSortThreads / 32];
@@ -226,7 +226,7 @@ __global__ void __launch_bounds__(kCellSortThreads) cell_sort_kernel(
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             mine += a[u];
-            if (a[u] >= (unsigned int)kDenseCell && a[u] <= (unsigned int)kDenseMax) mine += 1ull << 32;
+            if (a[u] >= (unsigned int)kDenseCell) mine += (unsigned long long)dense_tiles(a[u]) << 32;
         }
     }
     unsigned long long incl = mine;
@@ -259,8 +259,11 @@ __global__ void __launch_bounds__(kCellSortThreads) cell_sort_kernel(
         for (int u = 0; u < 4; ++u) {
             const unsigned int cnt = a[u];
             a[u] = run;
-            if (cnt >= (unsigned int)kDenseCell && cnt <= (unsigned int)kDenseMax)
-                dense_list[drun++] = (unsigned int)(cell0 + c_lo + k + u);
+            if (cnt >= (unsigned int)kDenseCell) {  // one work item per (dense cell, tile of <= 32 particles)
+                const unsigned int nt = dense_tiles(cnt);
+                for (unsigned int t = 0; t < nt; ++t)
+                    dense_list[drun++] = ((unsigned long long)(cell0 + c_lo + k + u) << 32) | t;
+            }
             run += cnt;
         }
         v = make_uint4(a[0], a[1], a[2], a[3]);
@@ -302,7 +305,7 @@ static inline cudaError_t set_smem(const void *fn, size_t bytes)
 
 cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp, int ctas, unsigned int *cta_hist,
                         unsigned int *bin_base, float4 *part, unsigned int *cell_start, float4 *sorted,
-                        unsigned int *rel, int *idx_s, int *minidx, unsigned int *dense_list, Ctrl *ctrl,
+                        unsigned int *rel, int *idx_s, int *minidx, unsigned long long *dense_list, Ctrl *ctrl,
                         StageHook &hook, cudaStream_t s)
 {
     if (N <= 0) return cudaSuccess;
