@@ -30,7 +30,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", tmp,
+    extra = os.environ.get("FOF_NVCC_EXTRA", "").split()  # e.g. -DFOF_TILES_MINB=6 (tuning experiments)
+    cmd = [nvcc, *NVCC_FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []), "-o", tmp,
            *[os.path.join(CSRC, f) for f in SOURCES]]
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)

@@ -258,7 +258,7 @@ int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *s
                        minidx, dense, ctrl, hook, s), "sort kernels");
     }
     {
-        StageTimer t(h, s, kLinkPairs, 2 * has);
+        StageTimer t(h, s, kLinkPairs, has);
         CK(launch_link(sorted, h->N, h->grid, cell, dense, rel, ctrl, h->num_sms, s), "link kernels");
     }
     { StageTimer t(h, s, kLinkFlatten, has); CK(launch_flatten_min(rel, idx_s, minidx, h->N, s), "flatten_min_kernel"); }

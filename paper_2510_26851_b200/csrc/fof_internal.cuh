@@ -33,7 +33,9 @@ struct Ctrl {
     long long K;                    // kept groups (written by fof_groups)
     unsigned long long grid_pairs;  // candidate pairs of the unfiltered half stencil on this grid
     unsigned int ndense;            // work items (dense cell, tile) listed by cell_sort_kernel
-    unsigned int pad1[5];
+    unsigned int tile_ticket;       // next (dense cell, tile) item of link_kernel
+    unsigned int sparse_ticket;     // next 32-particle chunk of link_kernel
+    unsigned int pad1[3];
 };
 static_assert(sizeof(Ctrl) <= 256, "Ctrl must fit its 256-byte slot");
 

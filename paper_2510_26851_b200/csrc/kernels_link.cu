@@ -76,6 +76,15 @@ __device__ __forceinline__ int unite_rel(unsigned int *rel, int a, int b)
     return ra;
 }
 
+#ifndef FOF_LINK_MINB
+#define FOF_LINK_MINB 6   // resident CTAs per SM the link kernel is compiled for (register cap)
+#endif
+#ifndef FOF_START_ROLE
+#define FOF_START_ROLE 0  // every warp starts on the tile queue (see link_kernel)
+#endif
+#ifndef FOF_LONG_RANGE
+#define FOF_LONG_RANGE 16
+#endif
 constexpr int kWarpsPerCta = kLinkBlock / 32;
 constexpr unsigned int kFull = 0xffffffffu;
 
@@ -87,22 +96,21 @@ __device__ __forceinline__ unsigned int lanemask_lt()
 }
 
 // =============================================================================================
-// link_tiles_kernel: pairs that involve a dense cell.
+// Tile role: pairs whose home cell is dense.
 // =============================================================================================
 
 // Tile I (one particle per lane, `me`; idle lanes sit at +inf) against a batch of `cnt` <= 32
 // candidates staged in shared memory.  Returns, in lane k, the mask of tile lanes linked to
-// candidate k; `nedges` (warp-uniform) counts the set bits of all masks.
+// candidate k.
 template <bool WRAP>
 __device__ __forceinline__ unsigned int batch_adjacency(const float4 &me, const float4 *s_pj, int cnt, const Grid &g,
-                                                        int lane, unsigned int &nedges)
+                                                        int lane)
 {
     unsigned int adjT = 0;
-#pragma unroll 4
+#pragma unroll 8
     for (int k = 0; k < cnt; ++k) {
         const unsigned int bal = __ballot_sync(kFull, linked_t<WRAP>(me, s_pj[k], g));
         if (lane == k) adjT = bal;
-        nedges += (unsigned int)__popc(bal);
     }
     return adjT;
 }
@@ -124,8 +132,24 @@ __device__ __forceinline__ void batch_unions(unsigned int adjT, const float4 *s_
     }
 }
 
-// Neighbour cells of a dense cell: candidates from the 26 cells around (cx, cy, cz), filtered to
-// those within `reach` of the cell, compacted into batches of 32.
+// The 13 forward neighbour cells q = 0..12 of a cell: +x, then the rows (dy, dz) = (+1, 0), (-1, +1),
+// (0, +1), (+1, +1) with dx = -1, 0, +1 each; offsets + 1 packed two bits per cell.
+constexpr unsigned int pack13(int axis)
+{
+    unsigned int v = 0;
+    for (int q = 0; q < 13; ++q) {
+        const int dx = q == 0 ? 1 : (q - 1) % 3 - 1;
+        const int dy = q == 0 ? 0 : (q < 4 ? 1 : (q - 4) / 3 - 1);
+        const int dz = q < 4 ? 0 : 1;
+        const int d = axis == 0 ? dx : (axis == 1 ? dy : dz);
+        v |= (unsigned int)(d + 1) << (2 * q);
+    }
+    return v;
+}
+constexpr unsigned int kFwdX = pack13(0), kFwdY = pack13(1), kFwdZ = pack13(2);
+
+// Candidates from the 13 forward cells around (cx, cy, cz), filtered to those within `reach` of
+// the cell, compacted into batches of 32 and tested against the tile.
 template <bool WRAP>
 __device__ __forceinline__ void tile_neighbours(const float4 *__restrict__ sorted,
                                                 const unsigned int *__restrict__ cs, unsigned int *rel, float4 *s_pj,
@@ -134,30 +158,28 @@ __device__ __forceinline__ void tile_neighbours(const float4 *__restrict__ sorte
                                                 unsigned int &nedges, unsigned int &ntests)
 {
     const int n = g.n;
-    // lane q < 27 looks up neighbour cell q = (dx + 1) + 3 (dy + 1) + 9 (dz + 1); q > 13 is the forward half
-    int nx = 0, ny = 0, nz = 0, beg = 0, len = 0;
-    if (lane < 27 && lane != 13) {
-        nx = cx + lane % 3 - 1;
-        ny = cy + (lane / 3) % 3 - 1;
-        nz = cz + lane / 9 - 1;
+    int beg = 0, len = 0;
+    if (lane < 13) {
+        int nx = cx + (int)((kFwdX >> (2 * lane)) & 3u) - 1;
+        int ny = cy + (int)((kFwdY >> (2 * lane)) & 3u) - 1;
+        int nz = cz + (int)((kFwdZ >> (2 * lane)) & 3u) - 1;
         if (WRAP) {
             nx = nx < 0 ? n - 1 : (nx >= n ? 0 : nx);
             ny = ny < 0 ? n - 1 : (ny >= n ? 0 : ny);
-            nz = nz < 0 ? n - 1 : (nz >= n ? 0 : nz);
+            nz = nz >= n ? 0 : nz;
         }
         const unsigned int c = cell_id(nx, ny, nz, n);
         beg = (int)__ldg(cs + c);
         len = (int)__ldg(cs + c + 1) - beg;
-        // a dense neighbour in my backward half owns our pairs itself
-        if (len >= kDenseCell && lane < 13) len = 0;
     }
     int incl = len;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
+    for (int o = 1; o < 16; o <<= 1) {  // lanes >= 13 hold 0: a 16-lane scan is enough
         const int v = __shfl_up_sync(kFull, incl, o);
         if (lane >= o) incl += v;
     }
-    const int total = __shfl_sync(kFull, incl, 31);
+    const int total = __shfl_sync(kFull, incl, 15);
+    if (total == 0) return;
     const int excl = incl - len;
     const float lo = g.reach, hi = 1.0f - g.reach;
     int nc = 0;  // candidates waiting in s_pj (warp-uniform)
@@ -167,25 +189,27 @@ __device__ __forceinline__ void tile_neighbours(const float4 *__restrict__ sorte
         // owner q of slot p: the first lane whose inclusive prefix exceeds p
         int q = 0;
 #pragma unroll
-        for (int st = 16; st > 0; st >>= 1) {
+        for (int st = 8; st > 0; st >>= 1) {
             const int v = __shfl_sync(kFull, incl, q + st - 1);
             if (v <= p) q += st;
         }
-        q = min(q, 31);
         const int j = __shfl_sync(kFull, beg, q) + (p - __shfl_sync(kFull, excl, q));
-        const int qx = __shfl_sync(kFull, nx, q), qy = __shfl_sync(kFull, ny, q), qz = __shfl_sync(kFull, nz, q);
         bool pass = false;
         float4 pj = make_float4(0.f, 0.f, 0.f, 0.f);
         if (has) {
             pj = __ldg(sorted + j);
-            // position of the candidate inside ITS cell; it can reach my cell only from within
-            // `reach` of the face(s) it shares with it (the same margins as the sparse kernel's flags)
-            const float fx = __fmul_rn(pj.x, g.inv_cell) - (float)qx;
-            const float fy = __fmul_rn(pj.y, g.inv_cell) - (float)qy;
-            const float fz = __fmul_rn(pj.z, g.inv_cell) - (float)qz;
-            const int dx = q % 3 - 1, dy = (q / 3) % 3 - 1, dz = q / 9 - 1;
+            // position of the candidate inside ITS cell (the fractional part of its cell coordinate):
+            // it can reach my cell only from within `reach` of the face(s) it shares with it
+            // (the same margins as the sparse kernel's flags)
+            const float ux = __fmul_rn(pj.x, g.inv_cell), uy = __fmul_rn(pj.y, g.inv_cell),
+                        uz = __fmul_rn(pj.z, g.inv_cell);
+            const float fx = ux - (float)min(__float2int_rd(ux), g.n_minus_1);
+            const float fy = uy - (float)min(__float2int_rd(uy), g.n_minus_1);
+            const float fz = uz - (float)min(__float2int_rd(uz), g.n_minus_1);
+            const int dx = (int)((kFwdX >> (2 * q)) & 3u) - 1, dy = (int)((kFwdY >> (2 * q)) & 3u) - 1,
+                      dz = (int)((kFwdZ >> (2 * q)) & 3u) - 1;
             pass = (dx == 0 || (dx < 0 ? fx > hi : fx < lo)) && (dy == 0 || (dy < 0 ? fy > hi : fy < lo)) &&
-                   (dz == 0 || (dz < 0 ? fz > hi : fz < lo));
+                   (dz == 0 || fz < lo);
             pj.w = __int_as_float(j);
         }
         const unsigned int bal = __ballot_sync(kFull, pass);
@@ -193,8 +217,9 @@ __device__ __forceinline__ void tile_neighbours(const float4 *__restrict__ sorte
         nc += __popc(bal);
         __syncwarp();
         if (nc >= 32) {
-            const unsigned int adjT = batch_adjacency<WRAP>(me, s_pj, 32, g, lane, nedges);
-            ntests += 32u * (unsigned int)cntI;
+            const unsigned int adjT = batch_adjacency<WRAP>(me, s_pj, 32, g, lane);
+            nedges += (unsigned int)__popc(adjT);
+            if (lane == 0) ntests += 32u * (unsigned int)cntI;
             batch_unions(adjT, s_pj, 32, rel, ib, grp, leader, lane);
             const float4 keep = s_pj[32 + lane];
             __syncwarp();
@@ -204,163 +229,198 @@ __device__ __forceinline__ void tile_neighbours(const float4 *__restrict__ sorte
         }
     }
     if (nc) {
-        const unsigned int adjT = batch_adjacency<WRAP>(me, s_pj, nc, g, lane, nedges);
-        ntests += (unsigned int)(nc * cntI);
+        const unsigned int adjT = batch_adjacency<WRAP>(me, s_pj, nc, g, lane);
+        nedges += (unsigned int)__popc(adjT);
+        if (lane == 0) ntests += (unsigned int)(nc * cntI);
         batch_unions(adjT, s_pj, nc, rel, ib, grp, leader, lane);
     }
     __syncwarp();
 }
 
-__global__ void __launch_bounds__(kLinkBlock) link_tiles_kernel(const float4 *__restrict__ sorted, Grid g,
-                                                                const unsigned int *__restrict__ cell_start,
-                                                                const unsigned long long *__restrict__ items,
-                                                                unsigned int *rel, Ctrl *ctrl)
+// One work item: tile `t` (ts particles) of dense cell `c`.
+__device__ __forceinline__ void tile_item(const float4 *__restrict__ sorted, const Grid &g,
+                                          const unsigned int *__restrict__ cell_start, unsigned long long item,
+                                          unsigned int *rel, float4 *s_pj, int lane, unsigned int &nedges,
+                                          unsigned int &ntests)
 {
-    __shared__ float4 s_pj_all[kWarpsPerCta][64];
-    float4 *s_pj = s_pj_all[threadIdx.x >> 5];
-    const int lane = threadIdx.x & 31;
-    const unsigned int nitems = ctrl->ndense;
-    const unsigned int nwarps = gridDim.x * kWarpsPerCta;
     const float inf = __int_as_float(0x7f800000);
     const int n = g.n;
-    unsigned int nedges = 0, ntests = 0;  // warp-uniform
-    for (unsigned int it = blockIdx.x * kWarpsPerCta + (threadIdx.x >> 5); it < nitems; it += nwarps) {
-        const unsigned long long item = __ldg(items + it);
-        const unsigned int c = (unsigned int)(item >> 32);
-        const int t = (int)(unsigned int)item;
-        const int b0 = (int)__ldg(cell_start + c), e0 = (int)__ldg(cell_start + c + 1);
-        const int ts = (int)dense_tile_size((unsigned int)(e0 - b0));
-        const int ib = b0 + t * ts;
-        const int cntI = min(ts, e0 - ib);
-        // a lane without a particle sits at +inf: d2 = inf (or NaN) fails every test
-        float4 me = make_float4(inf, inf, inf, 0.0f);
-        if (lane < cntI) me = __ldg(sorted + ib + lane);
-        me.w = __int_as_float(ib + lane);
+    const unsigned int c = (unsigned int)(item >> 32);
+    const int t = (int)(((unsigned int)item) >> 5), ts = (int)(((unsigned int)item) & 31u) + 1;
+    const int b0 = (int)__ldg(cell_start + c), e0 = (int)__ldg(cell_start + c + 1);
+    const int ib = b0 + t * ts;
+    const int cntI = min(ts, e0 - ib);
+    // a lane without a particle sits at +inf: d2 = inf (or NaN) fails every test
+    float4 me = make_float4(inf, inf, inf, 0.0f);
+    if (lane < cntI) me = __ldg(sorted + ib + lane);
+    me.w = __int_as_float(ib + lane);
 
-        // ---- the tile against itself (pairs inside one cell never wrap: cell side <= L/3)
-        __syncwarp();
-        s_pj[lane] = me;
-        __syncwarp();
-        unsigned int e_diag = 0;
-        unsigned int adj = batch_adjacency<false>(me, s_pj, cntI, g, lane, e_diag) & ~(1u << lane);
-        // every real particle is linked to itself (d2 = 0) and every pair shows up twice; a lane at
-        // +inf gives inf - inf = NaN and is linked to nothing
-        nedges += (e_diag - (unsigned int)cntI) >> 1;
-        ntests += (unsigned int)(cntI * (cntI - 1) / 2);
-        int lab = lane;  // lowest lane of my component inside the tile
-        if (__any_sync(kFull, adj != 0u)) {
-            // breadth-first from the lowest unlabelled lane; one warp OR-reduction per level
-            const unsigned int self = 1u << lane;
-            unsigned int todo = cntI >= 32 ? kFull : ((1u << cntI) - 1u);
-            while (todo) {
-                const int r = __ffs((int)todo) - 1;
-                unsigned int vis = 1u << r;
-                while (true) {
-                    const unsigned int nxt = vis | __reduce_or_sync(kFull, (vis & self) ? adj : 0u);
-                    if (nxt == vis) break;
-                    vis = nxt;
-                }
-                if (vis & self) lab = r;
-                todo &= ~vis;
+    // ---- the tile against itself (pairs inside one cell never wrap: cell side <= L/3)
+    __syncwarp();
+    s_pj[lane] = me;
+    __syncwarp();
+    const unsigned int adj = batch_adjacency<false>(me, s_pj, cntI, g, lane) & ~(1u << lane);
+    nedges += (unsigned int)__popc(adj & lanemask_lt());
+    if (lane == 0) ntests += (unsigned int)(cntI * (cntI - 1) / 2);
+    int lab = lane;  // lowest lane of my component inside the tile
+    if (__any_sync(kFull, adj != 0u)) {
+        // breadth-first from the lowest unlabelled lane; one warp OR-reduction per level
+        const unsigned int self = 1u << lane;
+        unsigned int todo = cntI >= 32 ? kFull : ((1u << cntI) - 1u);
+        while (todo) {
+            const int r = __ffs((int)todo) - 1;
+            unsigned int vis = 1u << r;
+            while (true) {
+                const unsigned int nxt = vis | __reduce_or_sync(kFull, (vis & self) ? adj : 0u);
+                if (nxt == vis) break;
+                vis = nxt;
             }
-            if (lab != lane) unite_rel(rel, ib + lane, ib + lab);
+            if (vis & self) lab = r;
+            todo &= ~vis;
         }
-        const unsigned int grp = __match_any_sync(kFull, lab);
-        const bool leader = lab == lane;
+        if (lab != lane) unite_rel(rel, ib + lane, ib + lab);
+    }
+    const unsigned int grp = __match_any_sync(kFull, lab);
+    const bool leader = lab == lane;
 
-        // ---- the earlier tiles of my cell (all full: ts particles)
-        for (int jt = 0; jt < t; ++jt) {
-            const int jb = b0 + jt * ts;
-            __syncwarp();
-            if (lane < ts) {
-                float4 pj = __ldg(sorted + jb + lane);
-                pj.w = __int_as_float(jb + lane);
-                s_pj[lane] = pj;
-            }
-            __syncwarp();
-            const unsigned int adjT = batch_adjacency<false>(me, s_pj, ts, g, lane, nedges);
-            ntests += (unsigned int)(ts * cntI);
-            batch_unions(adjT, s_pj, ts, rel, ib, grp, leader, lane);
+    // ---- the earlier tiles of my cell (all full: ts particles)
+    for (int jt = 0; jt < t; ++jt) {
+        const int jb = b0 + jt * ts;
+        __syncwarp();
+        if (lane < ts) {
+            float4 pj = __ldg(sorted + jb + lane);
+            pj.w = __int_as_float(jb + lane);
+            s_pj[lane] = pj;
         }
         __syncwarp();
+        const unsigned int adjT = batch_adjacency<false>(me, s_pj, ts, g, lane);
+        nedges += (unsigned int)__popc(adjT);
+        if (lane == 0) ntests += (unsigned int)(ts * cntI);
+        batch_unions(adjT, s_pj, ts, rel, ib, grp, leader, lane);
+    }
+    __syncwarp();
 
-        // ---- the 26 neighbour cells
-        const int cx = (int)(c % (unsigned int)n), cy = (int)((c / (unsigned int)n) % (unsigned int)n),
-                  cz = (int)(c / ((unsigned int)n * (unsigned int)n));
-        const bool wrap = n < 6 || cx == 0 || cx == n - 1 || cy == 0 || cy == n - 1 || cz == 0 || cz == n - 1;
-        if (wrap) tile_neighbours<true>(sorted, cell_start, rel, s_pj, me, ib, cntI, grp, leader, cx, cy, cz, g, lane, nedges, ntests);
-        else tile_neighbours<false>(sorted, cell_start, rel, s_pj, me, ib, cntI, grp, leader, cx, cy, cz, g, lane, nedges, ntests);
-    }
-    if (lane == 0) {
-        if (nedges) atomicAdd(&ctrl->edges, (unsigned long long)nedges);
-        if (ntests) atomicAdd(&ctrl->pair_tests, (unsigned long long)ntests);
-    }
+    // ---- the 13 forward neighbour cells; the cell coordinates come from a member's position
+    // (the binning expression of H1, so they are the coordinates the sort used)
+    const float3 p0 = make_float3(__shfl_sync(kFull, me.x, 0), __shfl_sync(kFull, me.y, 0),
+                                  __shfl_sync(kFull, me.z, 0));
+    const int cx = min(__float2int_rd(__fmul_rn(p0.x, g.inv_cell)), g.n_minus_1);
+    const int cy = min(__float2int_rd(__fmul_rn(p0.y, g.inv_cell)), g.n_minus_1);
+    const int cz = min(__float2int_rd(__fmul_rn(p0.z, g.inv_cell)), g.n_minus_1);
+    const bool wrap = n < 6 || cx == 0 || cx == n - 1 || cy == 0 || cy == n - 1 || cz == n - 1;
+    if (wrap) tile_neighbours<true>(sorted, cell_start, rel, s_pj, me, ib, cntI, grp, leader, cx, cy, cz, g, lane, nedges, ntests);
+    else tile_neighbours<false>(sorted, cell_start, rel, s_pj, me, ib, cntI, grp, leader, cx, cy, cz, g, lane, nedges, ntests);
 }
 
 // =============================================================================================
-// link_sparse_kernel: pairs of two sparse cells.
+// Sparse role: pairs whose home cell is sparse.
 // =============================================================================================
-constexpr int kStencil = 14;                        // own cell + 13 forward cells
-constexpr int kMaxRanges = 32 * kStencil;           // candidate ranges of one warp
-constexpr int kMaxSlots = kMaxRanges * (kDenseCell - 1);  // a sparse cell holds < kDenseCell particles
+constexpr int kLongRange = FOF_LONG_RANGE;  // longer candidate ranges (dense neighbour cells) are walked by the whole warp
+constexpr int kRangesNoWrap = 5, kRangesWrap = 7;  // with wrap: the 14 stencil cells in two passes of 7
+constexpr int kMaxRanges = 32 * kRangesWrap;
+constexpr int kMaxSlots = kMaxRanges * kLongRange;  // < 2^16: slot and range counts share one packed scan
 constexpr int kBitmapWords = (kMaxSlots + 31) / 32;
 
-// Stencil order: q = 0 own cell, 1 the +x cell, then the rows (dy, dz) = (+1, 0), (-1, +1), (0, +1),
-// (+1, +1) with dx = -1, 0, +1 each.
 struct SparseSmem {
-    int2 range[kMaxRanges];            // (first candidate, first slot << 5 | owner lane)
-    unsigned int bitmap[kBitmapWords]; // bit p set: a range starts at slot p
+    int2 range[kMaxRanges];             // (first candidate, first slot << 5 | owner lane)
+    unsigned int bitmap[kBitmapWords];  // bit p set: a range starts at slot p
 };
 
-template <bool WRAP>
+// One home particle per lane.  Candidate ranges: without wrap, one run of `sorted` per stencil row
+// (the rest of my cell [+ the +x cell]; then up to three cells of the rows (dy, dz) = (+1, 0),
+// (-1, +1), (0, +1), (+1, +1)); with wrap, one range per stencil cell.  A neighbour cell is
+// visited only if I am within `reach` of every face between us.
+template <bool WRAP, int PASS>
 __device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, const unsigned int *__restrict__ cs,
                                             unsigned int *rel, int si, bool valid, const float4 &me, int cx, int cy,
                                             int cz, float fx, float fy, float fz, const Grid &g, SparseSmem &sm,
                                             int lane, unsigned int &nedges, unsigned int &ntests)
 {
+    constexpr int NR = WRAP ? kRangesWrap : kRangesNoWrap;
     const int n = g.n;
     const float lo = g.reach, hi = 1.0f - g.reach;
     const bool xl = fx < lo, xh = fx > hi, yl = fy < lo, yh = fy > hi, zh = fz > hi;
-    int beg[kStencil], len[kStencil];
-    bool live = valid;
+    int beg[NR], len[NR];
 #pragma unroll
-    for (int q = 0; q < kStencil; ++q) {
-        const int dx = q == 0 ? 0 : (q == 1 ? 1 : (q - 2) % 3 - 1);
-        const int dy = q < 2 ? 0 : (q < 5 ? 1 : (q < 8 ? -1 : (q < 11 ? 0 : 1)));
-        const int dz = q < 5 ? 0 : 1;
-        // the cell can hold a partner only if I am within `reach` of every face between us
-        const bool want = live && (dx == 0 || (dx < 0 ? xl : xh)) && (dy == 0 || (dy < 0 ? yl : yh)) && (dz == 0 || zh);
-        beg[q] = 0;
-        len[q] = 0;
-        if (want) {
-            int ax = cx + dx, ay = cy + dy, az = cz + dz;
-            if (WRAP) {
-                ax = ax < 0 ? n - 1 : (ax >= n ? 0 : ax);
-                ay = ay < 0 ? n - 1 : (ay >= n ? 0 : ay);
-                az = az >= n ? 0 : az;
-            }
-            const unsigned int c = cell_id(ax, ay, az, n);
-            const int b = (int)__ldg(cs + c), e = (int)__ldg(cs + c + 1);
-            if (e - b < kDenseCell) {  // pairs with a dense cell belong to link_tiles_kernel
-                beg[q] = q == 0 ? si + 1 : b;
-                len[q] = e - beg[q];
-            } else if (q == 0) {
-                live = false;  // my own cell is dense: nothing to do here
+    for (int r = 0; r < NR; ++r) beg[r] = len[r] = 0;
+    if (valid) {
+        const unsigned int *home = cs + cell_id(cx, cy, cz, n);
+        const int c0 = (int)__ldg(home), c1 = (int)__ldg(home + 1);
+        if (c1 - c0 < kDenseCell) {  // a dense home cell belongs to link_tiles_kernel
+            if (!WRAP) {
+                // the loads below stay inside the row: a lane that needs the cell behind an x face
+                // has sent its whole warp to the WRAP variant
+                beg[0] = si + 1;
+                len[0] = (xh ? (int)__ldg(home + 2) : c1) - beg[0];
+                const int nn = n * n;
+                const int off_lo = xl ? -1 : 0, off_hi = xh ? 2 : 1;
+                const bool on[4] = {yh, zh && yl, zh, zh && yh};
+                const int row[4] = {n, nn - n, nn, nn + n};
+#pragma unroll
+                for (int r = 0; r < 4; ++r)
+                    if (on[r]) {
+                        beg[r + 1] = (int)__ldg(home + row[r] + off_lo);
+                        len[r + 1] = (int)__ldg(home + row[r] + off_hi) - beg[r + 1];
+                    }
+            } else {
+                if (PASS == 0) {
+                    beg[0] = si + 1;
+                    len[0] = c1 - beg[0];
+                }
+#pragma unroll
+                for (int k = (PASS == 0 ? 1 : 0); k < kRangesWrap; ++k) {
+                    const int q = k + PASS * kRangesWrap;
+                    const int dx = q == 1 ? 1 : (q - 2) % 3 - 1;
+                    const int dy = q < 2 ? 0 : (q < 5 ? 1 : (q < 8 ? -1 : (q < 11 ? 0 : 1)));
+                    const int dz = q < 5 ? 0 : 1;
+                    if ((dx == 0 || (dx < 0 ? xl : xh)) && (dy == 0 || (dy < 0 ? yl : yh)) && (dz == 0 || zh)) {
+                        int ax = cx + dx, ay = cy + dy, az = cz + dz;
+                        ax = ax < 0 ? n - 1 : (ax >= n ? 0 : ax);
+                        ay = ay < 0 ? n - 1 : (ay >= n ? 0 : ay);
+                        az = az >= n ? 0 : az;
+                        const unsigned int *p = cs + cell_id(ax, ay, az, n);
+                        beg[k] = (int)__ldg(p);
+                        len[k] = (int)__ldg(p + 1) - beg[k];
+                    }
+                }
             }
         }
     }
-    // flatten: one packed warp scan gives every lane its first slot (low 16 bits) and range id (high)
+    // ---- long ranges: the whole warp walks them, 32 candidates per trip
+#pragma unroll
+    for (int r = 0; r < NR; ++r) {
+        unsigned int lng = __ballot_sync(kFull, len[r] > kLongRange);
+        while (lng) {
+            const int owner = __ffs((int)lng) - 1;
+            lng &= lng - 1u;
+            const int b = __shfl_sync(kFull, beg[r], owner), l = __shfl_sync(kFull, len[r], owner);
+            const int osi = __shfl_sync(kFull, si, owner);
+            float4 o4;
+            o4.x = __shfl_sync(kFull, me.x, owner);
+            o4.y = __shfl_sync(kFull, me.y, owner);
+            o4.z = __shfl_sync(kFull, me.z, owner);
+            o4.w = 0.0f;
+            if (lane == 0) ntests += (unsigned int)l;
+            for (int j = b + lane; j < b + l; j += 32)
+                if (linked_t<WRAP>(o4, __ldg(sorted + j), g)) {
+                    ++nedges;
+                    unite_rel(rel, osi, j);
+                }
+        }
+        if (len[r] > kLongRange) len[r] = 0;
+    }
+    // ---- the rest is flattened: one packed warp scan gives every lane its first slot (low 16 bits)
+    // and its first range id (high bits)
     unsigned int mine = 0;
 #pragma unroll
-    for (int q = 0; q < kStencil; ++q) mine += (unsigned int)len[q] + (len[q] > 0 ? 0x10000u : 0u);
+    for (int r = 0; r < NR; ++r) mine += (unsigned int)len[r] + (len[r] > 0 ? 0x10000u : 0u);
     unsigned int incl = mine;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
         const unsigned int v = __shfl_up_sync(kFull, incl, o);
         if (lane >= o) incl += v;
     }
-    const unsigned int all = __shfl_sync(kFull, incl, 31);
-    const int total = (int)(all & 0xffffu);
+    const int total = (int)(__shfl_sync(kFull, incl, 31) & 0xffffu);
     if (total == 0) return;
     const int words = (total + 31) >> 5;
     for (int w = lane; w < words; w += 32) sm.bitmap[w] = 0u;
@@ -368,11 +428,11 @@ __device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, c
     {
         int slot = (int)((incl - mine) & 0xffffu), rid = (int)((incl - mine) >> 16);
 #pragma unroll
-        for (int q = 0; q < kStencil; ++q)
-            if (len[q] > 0) {
-                sm.range[rid++] = make_int2(beg[q], (slot << 5) | lane);
+        for (int r = 0; r < NR; ++r)
+            if (len[r] > 0) {
+                sm.range[rid++] = make_int2(beg[r], (slot << 5) | lane);
                 atomicOr(&sm.bitmap[slot >> 5], 1u << (slot & 31));
-                slot += len[q];
+                slot += len[r];
             }
     }
     __syncwarp();
@@ -382,7 +442,7 @@ __device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, c
     for (int w = 0; w < words; ++w) {
         const unsigned int bits = sm.bitmap[w];
         const int p = (w << 5) + lane;
-        const int2 r = sm.range[before + __popc(bits & le) - 1];  // p >= 0 has a range: slot 0 starts one
+        const int2 r = sm.range[before + __popc(bits & le) - 1];  // slot 0 starts a range: never -1
         before += __popc(bits);
         const int owner = r.y & 31;
         float4 o4;
@@ -393,8 +453,7 @@ __device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, c
         const int osi = __shfl_sync(kFull, si, owner);
         if (p < total) {
             const int j = r.x + (p - (r.y >> 5));
-            const float4 pj = __ldg(sorted + j);
-            if (linked_t<WRAP>(o4, pj, g)) {
+            if (linked_t<WRAP>(o4, __ldg(sorted + j), g)) {
                 ++nedges;
                 unite_rel(rel, osi, j);
             }
@@ -403,42 +462,96 @@ __device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, c
     __syncwarp();
 }
 
-// Persistent grid: each warp walks chunks of 32 consecutive cell-sorted particles.
-__global__ void __launch_bounds__(kLinkBlock) link_sparse_kernel(const float4 *__restrict__ sorted, int64_t N, Grid g,
-                                                                 const unsigned int *__restrict__ cell_start,
-                                                                 unsigned int *rel, Ctrl *ctrl)
+// 32 consecutive cell-sorted particles, one per lane.
+__device__ __forceinline__ void sparse_chunk(const float4 *__restrict__ sorted, int64_t N, const Grid &g,
+                                             const unsigned int *__restrict__ cell_start, unsigned int *rel,
+                                             int64_t base, SparseSmem &sm, int lane, unsigned int &nedges,
+                                             unsigned int &ntests)
 {
-    __shared__ SparseSmem s_all[kWarpsPerCta];
-    SparseSmem &sm = s_all[threadIdx.x >> 5];
-    const int lane = threadIdx.x & 31;
-    unsigned int nedges = 0, ntests = 0;  // per lane
     const int n = g.n;
     const float lo = g.reach, hi = 1.0f - g.reach;
-    for (int64_t base = (int64_t)blockIdx.x * kLinkBlock; base < N; base += (int64_t)gridDim.x * kLinkBlock) {
-        const int64_t s64 = base + threadIdx.x;
-        const bool valid = s64 < N;
-        const int si = (int)s64;
-        float4 me = make_float4(0.f, 0.f, 0.f, 0.f);
-        int cx = 0, cy = 0, cz = 0;
-        float fx = 0.5f, fy = 0.5f, fz = 0.5f;
-        bool needwrap = false;
-        if (valid) {
-            me = __ldg(sorted + si);
-            const float ux = __fmul_rn(me.x, g.inv_cell), uy = __fmul_rn(me.y, g.inv_cell),
-                        uz = __fmul_rn(me.z, g.inv_cell);
-            cx = min(__float2int_rd(ux), g.n_minus_1);
-            cy = min(__float2int_rd(uy), g.n_minus_1);
-            cz = min(__float2int_rd(uz), g.n_minus_1);
-            fx = ux - (float)cx;
-            fy = uy - (float)cy;
-            fz = uz - (float)cz;
-            needwrap = n < 6 || (fx < lo && cx == 0) || (fx > hi && cx == n - 1) || (fy < lo && cy == 0) ||
-                       (fy > hi && cy == n - 1) || (fz > hi && cz == n - 1);
+    const int64_t s64 = base + lane;
+    const bool valid = s64 < N;
+    const int si = (int)s64;
+    float4 me = make_float4(0.f, 0.f, 0.f, 0.f);
+    int cx = 0, cy = 0, cz = 0;
+    float fx = 0.5f, fy = 0.5f, fz = 0.5f;
+    bool needwrap = false;
+    if (valid) {
+        me = __ldg(sorted + si);
+        const float ux = __fmul_rn(me.x, g.inv_cell), uy = __fmul_rn(me.y, g.inv_cell), uz = __fmul_rn(me.z, g.inv_cell);
+        cx = min(__float2int_rd(ux), g.n_minus_1);
+        cy = min(__float2int_rd(uy), g.n_minus_1);
+        cz = min(__float2int_rd(uz), g.n_minus_1);
+        fx = ux - (float)cx;
+        fy = uy - (float)cy;
+        fz = uz - (float)cz;
+        needwrap = n < 6 || (fx < lo && cx == 0) || (fx > hi && cx == n - 1) || (fy < lo && cy == 0) ||
+                   (fy > hi && cy == n - 1) || (fz > hi && cz == n - 1);
+    }
+    if (__any_sync(kFull, needwrap)) {
+        sparse_warp<true, 0>(sorted, cell_start, rel, si, valid, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
+        sparse_warp<true, 1>(sorted, cell_start, rel, si, valid, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
+    } else {
+        sparse_warp<false, 0>(sorted, cell_start, rel, si, valid, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
+    }
+}
+
+// =============================================================================================
+// H4: one persistent kernel.  Every warp draws work through atomic tickets, first from the queue
+// of (dense cell, tile) items listed by cell_sort_kernel, then, when that runs dry, from the queue
+// of 32 x kSparseBatch consecutive cell-sorted particles of the sparse role: no grid-wide barrier
+// between the two, the tail of one overlaps the head of the other.  All hooks are atomicCAS on
+// roots, so any interleaving gives the same partition.  (Measured at cfg2: two back-to-back
+// kernels 0.99 ms, this kernel 0.87 ms; letting half of the warps START on the sparse queue costs
+// 1.69 ms -- the two roles together are ~170 KB of SASS and evict each other from the instruction
+// caches when they share an SM.)
+// =============================================================================================
+constexpr int kTileBatch = 4;     // items per ticket
+constexpr int kSparseBatch = 8;   // 32-particle chunks per ticket
+
+union LinkSmem {
+    float4 pj[64];
+    SparseSmem sp;
+};
+
+__global__ void __launch_bounds__(kLinkBlock, FOF_LINK_MINB) link_kernel(const float4 *__restrict__ sorted, int64_t N,
+                                                                         Grid g,
+                                                                         const unsigned int *__restrict__ cell_start,
+                                                                         const unsigned long long *__restrict__ items,
+                                                                         unsigned int *rel, Ctrl *ctrl)
+{
+    __shared__ LinkSmem s_all[kWarpsPerCta];
+    LinkSmem &sm = s_all[threadIdx.x >> 5];
+    const int lane = threadIdx.x & 31;
+    const unsigned int nitems = ctrl->ndense;
+    unsigned int nedges = 0, ntests = 0;  // per lane
+    int role = FOF_START_ROLE;
+    for (int phase = 0; phase < 2; ++phase, role ^= 1) {
+        if (role == 0) {
+            while (true) {
+                unsigned int it0 = 0;
+                if (lane == 0) it0 = atomicAdd(&ctrl->tile_ticket, (unsigned int)kTileBatch);
+                it0 = __shfl_sync(kFull, it0, 0);
+                if (it0 >= nitems) break;
+                const unsigned int it1 = min(it0 + (unsigned int)kTileBatch, nitems);
+                for (unsigned int it = it0; it < it1; ++it)
+                    tile_item(sorted, g, cell_start, __ldg(items + it), rel, sm.pj, lane, nedges, ntests);
+            }
+        } else {
+            while (true) {
+                unsigned int k0 = 0;
+                if (lane == 0) k0 = atomicAdd(&ctrl->sparse_ticket, (unsigned int)kSparseBatch);
+                k0 = __shfl_sync(kFull, k0, 0);
+                const int64_t base0 = (int64_t)k0 * 32;
+                if (base0 >= N) break;
+                for (int k = 0; k < kSparseBatch; ++k) {
+                    const int64_t base = base0 + 32 * k;
+                    if (base >= N) break;
+                    sparse_chunk(sorted, N, g, cell_start, rel, base, sm.sp, lane, nedges, ntests);
+                }
+            }
         }
-        if (__any_sync(kFull, needwrap))
-            sparse_warp<true>(sorted, cell_start, rel, si, valid, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
-        else
-            sparse_warp<false>(sorted, cell_start, rel, si, valid, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
     }
     for (int o = 16; o > 0; o >>= 1) {
         nedges += __shfl_xor_sync(kFull, nedges, o);
@@ -524,9 +637,8 @@ cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned 
                         cudaStream_t s)
 {
     if (N <= 0) return cudaSuccess;
-    const unsigned int grid = (unsigned int)min((int64_t)blocks_for(N, kLinkBlock), (int64_t)num_sms * 32);
-    link_tiles_kernel<<<(unsigned int)num_sms * 8, kLinkBlock, 0, s>>>(sorted, g, cell_start, dense_list, rel, ctrl);
-    link_sparse_kernel<<<grid, kLinkBlock, 0, s>>>(sorted, N, g, cell_start, rel, ctrl);
+    const unsigned int grid = (unsigned int)min((int64_t)blocks_for(N, kLinkBlock), (int64_t)num_sms * FOF_LINK_MINB);
+    link_kernel<<<grid, kLinkBlock, 0, s>>>(sorted, N, g, cell_start, dense_list, rel, ctrl);
     return cudaGetLastError();
 }
 

@@ -260,9 +260,9 @@ __global__ void __launch_bounds__(kCellSortThreads) cell_sort_kernel(
             const unsigned int cnt = a[u];
             a[u] = run;
             if (cnt >= (unsigned int)kDenseCell) {  // one work item per (dense cell, tile of <= 32 particles)
-                const unsigned int nt = dense_tiles(cnt);
+                const unsigned int nt = dense_tiles(cnt), ts = dense_tile_size(cnt);
                 for (unsigned int t = 0; t < nt; ++t)
-                    dense_list[drun++] = ((unsigned long long)(cell0 + c_lo + k + u) << 32) | t;
+                    dense_list[drun++] = ((unsigned long long)(cell0 + c_lo + k + u) << 32) | (t << 5) | (ts - 1u);
             }
             run += cnt;
         }
