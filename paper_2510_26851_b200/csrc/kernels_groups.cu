@@ -2,24 +2,49 @@
 // PAPER.md:93-95 (§2 step vi), PAPER.md:172 ("accumulates particle counts per halo via a parallel
 // histogram"), PAPER.md:227 (Alg. 2 "Compaction"), PAPER.md:259 (Eq. 4, halo position = mean of
 // member positions; made periodic per DESIGN.md R11), PAPER.md:263/369 (minimum particle cut).
+//
+// All three passes are latency-bound gathers / atomics over N particles, so every thread takes
+// four consecutive particles and issues their loads together (128-bit where the pointers allow).
 #include "fof_internal.cuh"
 
 namespace fof {
 
+constexpr int kPer = 4;  // particles per thread in the streaming passes
+
+template <bool VEC>
+__device__ __forceinline__ void load4(const int *__restrict__ p, int64_t i, int64_t N, int v[4], int fill)
+{
+    if (VEC && i + 3 < N) {
+        const int4 t = __ldg(reinterpret_cast<const int4 *>(p + i));
+        v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+    } else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) v[k] = (i + k < N) ? __ldg(p + i + k) : fill;
+    }
+}
+
 // H6: cnt[g] = number of members of group g other than its canonical particle (labels[i] != i).
 // Singletons (most of the background) issue no atomic at all.
+template <bool VEC>
 __global__ void __launch_bounds__(kBlock) group_count_kernel(const int *__restrict__ labels, int64_t N,
                                                              int *__restrict__ cnt)
 {
-    const int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+    const int64_t i = ((int64_t)blockIdx.x * kBlock + threadIdx.x) * kPer;
     if (i >= N) return;
-    const int l = labels[i];
-    if (l != (int)i) atomicAdd(cnt + l, 1);
+    int l[4];
+    load4<VEC>(labels, i, N, l, -1);
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+        if (l[k] >= 0 && l[k] != (int)(i + k)) atomicAdd(cnt + l[k], 1);
 }
 
-// H7: kept[i] = (labels[i] == i && cnt[i] + 1 >= N_min); exclusive scan of kept over i gives the
-// compact id, ascending in the canonical label.  Same single-pass look-back scan as the cell scan.
-// In place: cnt[i] becomes gid[i] (compact id of the group whose canonical particle is i, else -1).
+// H7: a canonical particle i (labels[i] == i) heads a kept group iff cnt[i] + 1 >= N_min; the
+// exclusive scan of that flag over i is the compact id, ascending in the canonical label.  Single
+// pass with decoupled look-back: state[tile] = (flag << 32) | value, flag 1 = tile aggregate,
+// 2 = inclusive prefix; tiles are handed out by an atomic ticket, so a tile only ever waits on
+// tiles that already started.  In place: the entry of a kept canonical particle becomes
+// -1 - gid; every other entry stays >= 0 (a count), which H8 reads as "dropped".
+// For N_min >= 2 the labels are not read at all: cnt[i] > 0 already says that i is canonical.
 __device__ __forceinline__ unsigned int lookback_g(unsigned long long *state, unsigned int tile,
                                                    unsigned int aggregate, int lane)
 {
@@ -59,16 +84,24 @@ __global__ void __launch_bounds__(kBlock) group_compact_kernel(const int *__rest
     const unsigned int tile = s_tile;
     const int64_t base = (int64_t)tile * kScanTile + (int64_t)tid * kScanItems;
 
-    int sz[kScanItems];
-    unsigned int keep = 0;  // bit k: item k is the canonical particle of a kept group
+    int c[kScanItems];
+    if (base + kScanItems <= N) {  // cnt is a workspace array: 16-byte aligned
+        const int4 a = *reinterpret_cast<const int4 *>(cnt_to_gid + base);
+        const int4 b = *reinterpret_cast<const int4 *>(cnt_to_gid + base + 4);
+        c[0] = a.x; c[1] = a.y; c[2] = a.z; c[3] = a.w; c[4] = b.x; c[5] = b.y; c[6] = b.z; c[7] = b.w;
+    } else {
 #pragma unroll
-    for (int k = 0; k < kScanItems; ++k) {
-        const int64_t i = base + k;
-        sz[k] = 0;
-        if (i < N) {
-            const int c = cnt_to_gid[i];
-            if (labels[i] == (int)i && c + 1 >= N_min) { keep |= 1u << k; sz[k] = c + 1; }
-        }
+        for (int k = 0; k < kScanItems; ++k) c[k] = (base + k < N) ? cnt_to_gid[base + k] : -1;
+    }
+    unsigned int keep = 0;  // bit k: item k is the canonical particle of a kept group
+    if (N_min >= 2) {
+#pragma unroll
+        for (int k = 0; k < kScanItems; ++k)
+            if (c[k] + 1 >= N_min) keep |= 1u << k;
+    } else {
+#pragma unroll
+        for (int k = 0; k < kScanItems; ++k)
+            if (base + k < N && labels[base + k] == (int)(base + k)) keep |= 1u << k;
     }
     const unsigned int sum = __popc(keep);
     unsigned int incl = sum;
@@ -100,21 +133,17 @@ __global__ void __launch_bounds__(kBlock) group_compact_kernel(const int *__rest
     if (tile == last_tile && tid == kBlock - 1) ctrl->K = (long long)s_prefix + total;
 #pragma unroll
     for (int k = 0; k < kScanItems; ++k) {
+        if (!(keep & (1u << k))) continue;
         const int64_t i = base + k;
-        if (i >= N) break;
-        int gid = -1;
-        if (keep & (1u << k)) {
-            gid = (int)k_out++;
-            if (gid < cap) {
-                group_label[gid] = (int)i;
-                group_size[gid] = sz[k];
-                acc[4 * (int64_t)gid + 0] = 0.0;
-                acc[4 * (int64_t)gid + 1] = 0.0;
-                acc[4 * (int64_t)gid + 2] = 0.0;
-                acc[4 * (int64_t)gid + 3] = 0.0;
-            }
+        const int gid = (int)k_out++;
+        cnt_to_gid[i] = -1 - gid;
+        if (gid < cap) {
+            group_label[gid] = (int)i;
+            group_size[gid] = c[k] + 1;
+            double2 *a2 = reinterpret_cast<double2 *>(acc + 4 * (int64_t)gid);
+            a2[0] = make_double2(0.0, 0.0);
+            a2[1] = make_double2(0.0, 0.0);
         }
-        cnt_to_gid[i] = gid;
     }
 }
 
@@ -127,34 +156,50 @@ __device__ __forceinline__ double min_image_d(double d, double L, double h)
     return d;
 }
 
+template <bool VEC>
 __global__ void __launch_bounds__(kBlock) group_reduce_kernel(const float *__restrict__ pos,
                                                               const float *__restrict__ mass,
                                                               const int *__restrict__ labels, int64_t N, Grid g,
                                                               const int *__restrict__ gid_of, int64_t cap,
                                                               double *acc, int *__restrict__ particle_group)
 {
-    const int64_t i = (int64_t)blockIdx.x * kBlock + threadIdx.x;
-    if (i >= N) return;
-    const int l = labels[i];
-    const int gid = gid_of[l];
-    if (particle_group) particle_group[i] = gid;
-    if (gid < 0 || gid >= cap) return;
-    const double L = (double)g.L, h = 0.5 * (double)g.L;
-    const double m = mass ? (double)mass[i] : 1.0;
-    double d[3];
+    const int64_t i0 = ((int64_t)blockIdx.x * kBlock + threadIdx.x) * kPer;
+    if (i0 >= N) return;
+    int l[4], gid[4];
+    load4<VEC>(labels, i0, N, l, -1);
 #pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        const float wi = wrap1(pos[3 * i + a], g.L);
-        const float wr = wrap1(pos[3 * (int64_t)l + a], g.L);
-        d[a] = min_image_d((double)wi - (double)wr, L, h);
+    for (int k = 0; k < 4; ++k) gid[k] = l[k] >= 0 ? -1 - __ldg(gid_of + l[k]) : -1;  // < 0: dropped
+    if (particle_group) {
+        if (VEC && i0 + 3 < N) {
+            *reinterpret_cast<int4 *>(particle_group + i0) =
+                make_int4(max(gid[0], -1), max(gid[1], -1), max(gid[2], -1), max(gid[3], -1));
+        } else {
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (i0 + k < N) particle_group[i0 + k] = max(gid[k], -1);
+        }
     }
-    double *dst = acc + 4 * (int64_t)gid;
-    if (l != (int)i) {  // the canonical particle itself has delta = 0
-        atomicAdd(dst + 0, m * d[0]);
-        atomicAdd(dst + 1, m * d[1]);
-        atomicAdd(dst + 2, m * d[2]);
+    const double L = (double)g.L, h = 0.5 * (double)g.L;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        if (gid[k] < 0 || gid[k] >= cap) continue;
+        const int64_t i = i0 + k;
+        const double m = mass ? (double)__ldg(mass + i) : 1.0;
+        double *dst = acc + 4 * (int64_t)gid[k];
+        if (l[k] != (int)i) {  // the canonical particle itself has delta = 0
+            double d[3];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const float wi = wrap1(__ldg(pos + 3 * i + a), g.L);
+                const float wr = wrap1(__ldg(pos + 3 * (int64_t)l[k] + a), g.L);
+                d[a] = min_image_d((double)wi - (double)wr, L, h);
+            }
+            atomicAdd(dst + 0, m * d[0]);
+            atomicAdd(dst + 1, m * d[1]);
+            atomicAdd(dst + 2, m * d[2]);
+        }
+        if (mass) atomicAdd(dst + 3, m);
     }
-    if (mass) atomicAdd(dst + 3, m);
 }
 
 // H8 finish: one thread per kept group.
@@ -187,10 +232,14 @@ __global__ void __launch_bounds__(kBlock) group_finish_kernel(const float *__res
 }
 
 static inline unsigned int blocks_for(int64_t n, int per_block) { return (unsigned int)((n + per_block - 1) / per_block); }
+static inline bool aligned16(const void *p) { return ((uintptr_t)p & 15) == 0; }
 
 cudaError_t launch_group_count(const int *labels, int64_t N, int *cnt, cudaStream_t s)
 {
-    if (N > 0) group_count_kernel<<<blocks_for(N, kBlock), kBlock, 0, s>>>(labels, N, cnt);
+    if (N <= 0) return cudaSuccess;
+    const unsigned int grid = blocks_for(N, kBlock * kPer);
+    if (aligned16(labels)) group_count_kernel<true><<<grid, kBlock, 0, s>>>(labels, N, cnt);
+    else group_count_kernel<false><<<grid, kBlock, 0, s>>>(labels, N, cnt);
     return cudaGetLastError();
 }
 
@@ -208,9 +257,12 @@ cudaError_t launch_group_compact(const int *labels, int64_t N, int N_min, int *c
 cudaError_t launch_group_reduce(const float *pos, const float *mass, const int *labels, int64_t N, Grid g,
                                 const int *gid, int64_t cap, double *acc, int *particle_group, cudaStream_t s)
 {
-    if (N > 0)
-        group_reduce_kernel<<<blocks_for(N, kBlock), kBlock, 0, s>>>(pos, mass, labels, N, g, gid, cap, acc,
-                                                                     particle_group);
+    if (N <= 0) return cudaSuccess;
+    const unsigned int grid = blocks_for(N, kBlock * kPer);
+    if (aligned16(labels) && aligned16(particle_group))
+        group_reduce_kernel<true><<<grid, kBlock, 0, s>>>(pos, mass, labels, N, g, gid, cap, acc, particle_group);
+    else
+        group_reduce_kernel<false><<<grid, kBlock, 0, s>>>(pos, mass, labels, N, g, gid, cap, acc, particle_group);
     return cudaGetLastError();
 }
 

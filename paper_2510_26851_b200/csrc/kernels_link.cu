@@ -567,17 +567,41 @@ __global__ void __launch_bounds__(kLinkBlock, FOF_LINK_MINB) link_kernel(const f
 // minidx to the smallest ORIGINAL index of its members ("minimum label", PAPER.md:180
 // "minimum global particle ID").  The chase is read-only; a concurrent reader sees either the old
 // offset (an ancestor) or the root.  Roots have nothing to do: minidx[root] starts as its own index.
+// Four consecutive particles per thread, so that four chases are in flight.
 __global__ void __launch_bounds__(kBlock) flatten_min_kernel(unsigned int *rel, const int *__restrict__ idx_s,
                                                              int *minidx, int64_t N)
 {
-    const int64_t s = (int64_t)blockIdx.x * kBlock + threadIdx.x;
-    if (s >= N) return;
-    unsigned int d = rel[s];
-    if (d == 0u) return;
-    int r = (int)s - (int)d;
-    while ((d = rel[r]) != 0u) r -= (int)d;
-    rel[s] = (unsigned int)((int)s - r);
-    atomicMin(minidx + r, idx_s[s]);
+    const int64_t s0 = ((int64_t)blockIdx.x * kBlock + threadIdx.x) * 4;
+    if (s0 >= N) return;
+    unsigned int d[4];
+    if (s0 + 3 < N) {
+        const uint4 t = *reinterpret_cast<const uint4 *>(rel + s0);
+        d[0] = t.x; d[1] = t.y; d[2] = t.z; d[3] = t.w;
+    } else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) d[k] = (s0 + k < N) ? rel[s0 + k] : 0u;
+    }
+    if ((d[0] | d[1] | d[2] | d[3]) == 0u) return;
+    int r[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) r[k] = (int)(s0 + k) - (int)d[k];
+    // lock-step chase: one round issues the (up to four) loads together
+    bool more = true;
+    while (more) {
+        unsigned int e[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) e[k] = d[k] ? rel[r[k]] : 0u;
+        more = false;
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            if (e[k]) { r[k] -= (int)e[k]; more = true; }
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+        if (d[k]) {
+            rel[s0 + k] = (unsigned int)((int)(s0 + k) - r[k]);
+            atomicMin(minidx + r[k], idx_s[s0 + k]);
+        }
 }
 
 // H5b: labels[original index] = minimum original index of the component.
@@ -586,10 +610,21 @@ __global__ void __launch_bounds__(kBlock) write_labels_kernel(const unsigned int
                                                               const int *__restrict__ minidx, int *__restrict__ labels,
                                                               int64_t N)
 {
-    const int64_t s = (int64_t)blockIdx.x * kBlock + threadIdx.x;
-    if (s >= N) return;
-    const int r = (int)s - (int)__ldg(rel + s);
-    labels[__ldg(idx_s + s)] = __ldg(minidx + r);
+    const int64_t s0 = ((int64_t)blockIdx.x * kBlock + threadIdx.x) * 4;
+    if (s0 >= N) return;
+    if (s0 + 3 < N) {
+        const uint4 d = __ldg(reinterpret_cast<const uint4 *>(rel + s0));
+        const int4 oi = __ldg(reinterpret_cast<const int4 *>(idx_s + s0));
+        const int s = (int)s0;
+        const int m0 = __ldg(minidx + (s - (int)d.x)), m1 = __ldg(minidx + (s + 1 - (int)d.y)),
+                  m2 = __ldg(minidx + (s + 2 - (int)d.z)), m3 = __ldg(minidx + (s + 3 - (int)d.w));
+        labels[oi.x] = m0;
+        labels[oi.y] = m1;
+        labels[oi.z] = m2;
+        labels[oi.w] = m3;
+    } else {
+        for (int64_t s = s0; s < N; ++s) labels[__ldg(idx_s + s)] = __ldg(minidx + ((int)s - (int)__ldg(rel + s)));
+    }
 }
 
 // P_exec of DESIGN.md §7: candidate pairs the unfiltered half stencil implies on this grid,
@@ -644,14 +679,14 @@ cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned 
 
 cudaError_t launch_flatten_min(unsigned int *rel, const int *idx_s, int *minidx, int64_t N, cudaStream_t s)
 {
-    if (N > 0) flatten_min_kernel<<<blocks_for(N, kBlock), kBlock, 0, s>>>(rel, idx_s, minidx, N);
+    if (N > 0) flatten_min_kernel<<<blocks_for(N, kBlock * 4), kBlock, 0, s>>>(rel, idx_s, minidx, N);
     return cudaGetLastError();
 }
 
 cudaError_t launch_write_labels(const unsigned int *rel, const int *idx_s, const int *minidx, int *labels, int64_t N,
                                 cudaStream_t s)
 {
-    if (N > 0) write_labels_kernel<<<blocks_for(N, kBlock), kBlock, 0, s>>>(rel, idx_s, minidx, labels, N);
+    if (N > 0) write_labels_kernel<<<blocks_for(N, kBlock * 4), kBlock, 0, s>>>(rel, idx_s, minidx, labels, N);
     return cudaGetLastError();
 }
 
