@@ -52,7 +52,10 @@ struct Grid {
 };
 
 constexpr int kLinkBlock = 256;     // threads per CTA of the link kernels
-constexpr int kDenseCell = 8;       // cells with >= kDenseCell particles are DENSE: every pair that involves one of
+#ifndef FOF_DENSE_CELL
+#define FOF_DENSE_CELL 8
+#endif
+constexpr int kDenseCell = FOF_DENSE_CELL;       // cells with >= kDenseCell particles are DENSE: every pair that involves one of
                                     // their particles belongs to link_tiles_kernel, all others to link_sparse_kernel
 
 // A dense cell of m particles is cut into dense_tiles(m) tiles of dense_tile_size(m) <= 32
