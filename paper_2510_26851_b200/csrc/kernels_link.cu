@@ -266,7 +266,7 @@ __device__ __forceinline__ void tile_item(const float4 *__restrict__ sorted, con
     if (__any_sync(kFull, adj != 0u)) {
         // breadth-first from the lowest unlabelled lane; one warp OR-reduction per level
         const unsigned int self = 1u << lane;
-        unsigned int todo = cntI >= 32 ? kFull : ((1u << cntI) - 1u);
+        unsigned int todo = __ballot_sync(kFull, adj != 0u);  // lanes without a link are their own component
         while (todo) {
             const int r = __ffs((int)todo) - 1;
             unsigned int vis = 1u << r;
@@ -332,10 +332,12 @@ struct SparseSmem {
 // visited only if I am within `reach` of every face between us.
 template <bool WRAP, int PASS>
 __device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, const unsigned int *__restrict__ cs,
-                                            unsigned int *rel, int si, bool valid, const float4 &me, int cx, int cy,
-                                            int cz, float fx, float fy, float fz, const Grid &g, SparseSmem &sm,
-                                            int lane, unsigned int &nedges, unsigned int &ntests)
+                                            unsigned int *rel, int si, bool live, const unsigned int *home, int c1,
+                                            const float4 &me, int cx, int cy, int cz, float fx, float fy, float fz,
+                                            const Grid &g, SparseSmem &sm, int lane, unsigned int &nedges,
+                                            unsigned int &ntests)
 {
+    // live: a real particle whose home cell (cell_start entry `home`, end `c1`) is sparse
     constexpr int NR = WRAP ? kRangesWrap : kRangesNoWrap;
     const int n = g.n;
     const float lo = g.reach, hi = 1.0f - g.reach;
@@ -343,10 +345,8 @@ __device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, c
     int beg[NR], len[NR];
 #pragma unroll
     for (int r = 0; r < NR; ++r) beg[r] = len[r] = 0;
-    if (valid) {
-        const unsigned int *home = cs + cell_id(cx, cy, cz, n);
-        const int c0 = (int)__ldg(home), c1 = (int)__ldg(home + 1);
-        if (c1 - c0 < kDenseCell) {  // a dense home cell belongs to link_tiles_kernel
+    {
+        if (live) {
             if (!WRAP) {
                 // the loads below stay inside the row: a lane that needs the cell behind an x face
                 // has sent its whole warp to the WRAP variant
@@ -387,27 +387,32 @@ __device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, c
         }
     }
     // ---- long ranges: the whole warp walks them, 32 candidates per trip
+    int longest = len[0];
 #pragma unroll
-    for (int r = 0; r < NR; ++r) {
-        unsigned int lng = __ballot_sync(kFull, len[r] > kLongRange);
-        while (lng) {
-            const int owner = __ffs((int)lng) - 1;
-            lng &= lng - 1u;
-            const int b = __shfl_sync(kFull, beg[r], owner), l = __shfl_sync(kFull, len[r], owner);
-            const int osi = __shfl_sync(kFull, si, owner);
-            float4 o4;
-            o4.x = __shfl_sync(kFull, me.x, owner);
-            o4.y = __shfl_sync(kFull, me.y, owner);
-            o4.z = __shfl_sync(kFull, me.z, owner);
-            o4.w = 0.0f;
-            if (lane == 0) ntests += (unsigned int)l;
-            for (int j = b + lane; j < b + l; j += 32)
-                if (linked_t<WRAP>(o4, __ldg(sorted + j), g)) {
-                    ++nedges;
-                    unite_rel(rel, osi, j);
-                }
+    for (int r = 1; r < NR; ++r) longest = max(longest, len[r]);
+    if (__any_sync(kFull, longest > kLongRange)) {
+#pragma unroll
+        for (int r = 0; r < NR; ++r) {
+            unsigned int lng = __ballot_sync(kFull, len[r] > kLongRange);
+            while (lng) {
+                const int owner = __ffs((int)lng) - 1;
+                lng &= lng - 1u;
+                const int b = __shfl_sync(kFull, beg[r], owner), l = __shfl_sync(kFull, len[r], owner);
+                const int osi = __shfl_sync(kFull, si, owner);
+                float4 o4;
+                o4.x = __shfl_sync(kFull, me.x, owner);
+                o4.y = __shfl_sync(kFull, me.y, owner);
+                o4.z = __shfl_sync(kFull, me.z, owner);
+                o4.w = 0.0f;
+                if (lane == 0) ntests += (unsigned int)l;
+                for (int j = b + lane; j < b + l; j += 32)
+                    if (linked_t<WRAP>(o4, __ldg(sorted + j), g)) {
+                        ++nedges;
+                        unite_rel(rel, osi, j);
+                    }
+            }
+            if (len[r] > kLongRange) len[r] = 0;
         }
-        if (len[r] > kLongRange) len[r] = 0;
     }
     // ---- the rest is flattened: one packed warp scan gives every lane its first slot (low 16 bits)
     // and its first range id (high bits)
@@ -423,7 +428,10 @@ __device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, c
     const int total = (int)(__shfl_sync(kFull, incl, 31) & 0xffffu);
     if (total == 0) return;
     const int words = (total + 31) >> 5;
-    for (int w = lane; w < words; w += 32) sm.bitmap[w] = 0u;
+    static_assert(kBitmapWords <= 4 * 32, "bitmap zeroing below covers 128 words");
+#pragma unroll
+    for (int k = 0; k < (kBitmapWords + 31) / 32; ++k)
+        if (lane + 32 * k < words) sm.bitmap[lane + 32 * k] = 0u;
     __syncwarp();
     {
         int slot = (int)((incl - mine) & 0xffffu), rid = (int)((incl - mine) >> 16);
@@ -476,7 +484,9 @@ __device__ __forceinline__ void sparse_chunk(const float4 *__restrict__ sorted, 
     float4 me = make_float4(0.f, 0.f, 0.f, 0.f);
     int cx = 0, cy = 0, cz = 0;
     float fx = 0.5f, fy = 0.5f, fz = 0.5f;
-    bool needwrap = false;
+    bool needwrap = false, live = false;
+    const unsigned int *home = cell_start;
+    int c1 = 0;
     if (valid) {
         me = __ldg(sorted + si);
         const float ux = __fmul_rn(me.x, g.inv_cell), uy = __fmul_rn(me.y, g.inv_cell), uz = __fmul_rn(me.z, g.inv_cell);
@@ -486,14 +496,18 @@ __device__ __forceinline__ void sparse_chunk(const float4 *__restrict__ sorted, 
         fx = ux - (float)cx;
         fy = uy - (float)cy;
         fz = uz - (float)cz;
-        needwrap = n < 6 || (fx < lo && cx == 0) || (fx > hi && cx == n - 1) || (fy < lo && cy == 0) ||
-                   (fy > hi && cy == n - 1) || (fz > hi && cz == n - 1);
+        home = cell_start + cell_id(cx, cy, cz, n);
+        c1 = (int)__ldg(home + 1);
+        live = c1 - (int)__ldg(home) < kDenseCell;  // a dense home cell belongs to the tile role
+        needwrap = live && (n < 6 || (fx < lo && cx == 0) || (fx > hi && cx == n - 1) || (fy < lo && cy == 0) ||
+                            (fy > hi && cy == n - 1) || (fz > hi && cz == n - 1));
     }
+    if (!__any_sync(kFull, live)) return;
     if (__any_sync(kFull, needwrap)) {
-        sparse_warp<true, 0>(sorted, cell_start, rel, si, valid, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
-        sparse_warp<true, 1>(sorted, cell_start, rel, si, valid, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
+        sparse_warp<true, 0>(sorted, cell_start, rel, si, live, home, c1, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
+        sparse_warp<true, 1>(sorted, cell_start, rel, si, live, home, c1, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
     } else {
-        sparse_warp<false, 0>(sorted, cell_start, rel, si, valid, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
+        sparse_warp<false, 0>(sorted, cell_start, rel, si, live, home, c1, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
     }
 }
 
