@@ -317,3 +317,85 @@ def test_run_host_path(B):
     d = np.abs(gc.numpy()[:K].astype(np.float64) - og["group_com"])
     assert np.minimum(d, w.L - d).max() <= 1e-5 * w.L
     B.fof_destroy(h)
+
+
+@pytest.mark.parametrize("n_particles", [4099, 65537])
+def test_unaligned_caller_pointers(B, n_particles):
+    """pos / labels / particle_group that are only 4-byte aligned (views one element into a buffer) and
+    an N that is not a multiple of 4: the kernels must take their scalar load/store paths."""
+    rng = np.random.default_rng(77)
+    L, b, N_min = 50.0, 1.0, 3
+    N = n_particles
+    clump = rng.standard_normal((N // 3, 3)) * 0.8 + 25.0
+    p = np.concatenate([rng.random((N - N // 3, 3)) * L, clump]).astype(np.float32) % np.float32(L)
+    p = p[rng.permutation(N)]
+    m = rng.uniform(0.5, 1.5, N).astype(np.float32)
+    lab, E = oracle.labels_cells(p, L, b)
+    og = oracle.groups(p, lab, L, N_min, mass=m)
+
+    f = B.FoF(N, L, b, N_min)
+    buf_p = torch.empty(3 * N + 1, dtype=torch.float32, device="cuda")
+    dpos = buf_p[1:].view(N, 3)
+    dpos.copy_(torch.from_numpy(p))
+    buf_l = torch.empty(N + 1, dtype=torch.int32, device="cuda")
+    labels = buf_l[1:]
+    buf_g = torch.empty(N + 3, dtype=torch.int32, device="cuda")
+    pg = buf_g[3:]
+    buf_m = torch.empty(N + 1, dtype=torch.float32, device="cuda")
+    dm = buf_m[1:]
+    dm.copy_(torch.from_numpy(m))
+    assert dpos.data_ptr() % 16 == 4 and labels.data_ptr() % 16 == 4 and pg.data_ptr() % 16 == 12
+    B.fof_link(f.h, dpos, labels, f.ws)
+    assert f.status() == 0
+    assert np.array_equal(labels.cpu().numpy(), lab)
+    assert f.link_stats()[0] == E
+    out = f.alloc_groups()
+    K = B.fof_groups(f.h, dpos, dm, labels, f.ws, out["group_label"], out["group_size"], out["group_mass"],
+                     out["group_com"], pg, out["cap"])
+    assert K == og["K"]
+    assert np.array_equal(out["group_size"][:K].cpu().numpy(), og["group_size"])
+    assert np.array_equal(pg.cpu().numpy(), og["particle_group"])
+    gm = out["group_mass"][:K].cpu().numpy()
+    assert np.all(np.abs(gm - og["group_mass"]) <= 1e-5 * og["group_mass"])
+    d = np.abs(out["group_com"][:K].cpu().numpy().astype(np.float64) - og["group_com"])
+    assert np.minimum(d, L - d).max() <= 1e-5 * L
+    f.close()
+
+
+def test_stress_full_size_sampled(B):
+    """Full-size strongly clustered set (256^3, Zel'dovich past shell crossing, b = 0.4 spacing): checked
+    by properties that hold at any size plus sampled components recomputed by brute force."""
+    w = inputs.CONFIGS["stress_b0.4"]
+    p = inputs.make_positions(w)
+    N = len(p)
+    f = B.FoF(N, w.L, w.b, w.N_min)
+    dpos = torch.from_numpy(p).cuda()
+    labels = f.link(dpos)
+    g = f.groups(dpos, labels, particle_group=True)
+    lab = labels.cpu().numpy()
+    f.close()
+    idx = np.arange(N, dtype=np.int32)
+    assert (lab <= idx).all() and (lab[lab] == lab).all()
+    sizes = np.bincount(lab, minlength=N)
+    assert sizes.sum() == N
+    kept = np.flatnonzero(sizes >= w.N_min)
+    assert g["K"] == len(kept)
+    assert np.array_equal(g["group_label"].cpu().numpy(), kept.astype(np.int32))
+    assert np.array_equal(g["group_size"].cpu().numpy(), sizes[kept].astype(np.int32))
+    # sampled groups: the members found by the GPU must form exactly one brute-force component, and no
+    # outside particle within the group's bounding box (+ b) may link to it
+    rng = np.random.default_rng(3)
+    for gl in rng.choice(kept, size=8, replace=False):
+        mem = np.flatnonzero(lab == gl)
+        if len(mem) > 3000:
+            continue
+        q = p[mem]
+        sub, _ = oracle.labels_brute(q, w.L, w.b)
+        assert (sub == 0).all(), "a GPU group is not connected"
+        lo, hi = q.min(0) - w.b, q.max(0) + w.b
+        if (lo < 0).any() or (hi > w.L).any():
+            continue  # groups touching the box faces are covered by the small wrapped cases
+        near = np.flatnonzero(((p >= lo) & (p <= hi)).all(1))
+        both, _ = oracle.labels_brute(p[near], w.L, w.b)
+        inside = np.isin(near, mem)
+        assert len(set(both[inside])) == 1 and not np.isin(both[~inside], both[inside]).any()
