@@ -124,6 +124,23 @@ def workload_for_rank(name: str, rank: int) -> inputs.Workload:
     return dataclasses.replace(w, seed=w.seed + 1000 * rank) if rank else w
 
 
+def max_over_ranks_ms(ms: float, world: int, device) -> float:
+    """Device time of the slowest rank (the contract's "max over ranks"); identity at world 1."""
+    if world == 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, n_per_rank: int, ms_step: float) -> float:
+    """Replicas only: every rank links its own n_per_rank particles per step."""
+    return world * n_per_rank / (ms_step * 1e-3)
+
+
 def time_oracle(pos, w, mass=None):
     """One pass of the oracle (cell list + union-find + groups), wall clock, single thread."""
     import oracle
@@ -228,11 +245,8 @@ def run_ours(args):
     stages = B.fof_profile_read(f.h)
     B.fof_profile_enable(f.h, 0)
     E, pair_tests, grid_pairs = f.link_stats()
-    t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_step = float(t.item()) / args.steps
-    value = world * N / (ms_step * 1e-3)
+    ms_step = max_over_ranks_ms(ms_total, world, dev) / args.steps
+    value = whole_job_value(world, N, ms_step)
 
     # ---- end to end: host buffers through the C ABI (fof_run_host), copies inside the timed region
     cap = out["cap"]
@@ -254,10 +268,7 @@ def run_ours(args):
     e1.record(stream)
     torch.cuda.synchronize()
     barrier()
-    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_ms = float(t.item()) / e2e_steps
+    e2e_ms = max_over_ranks_ms(e0.elapsed_time(e1), world, dev) / e2e_steps
     B.fof_destroy(h2)
     assert Kh == K_groups, (Kh, K_groups)
     assert torch.equal(hl.to(dev), labels), "host-path labels differ from device-path labels"
@@ -331,7 +342,7 @@ def run_ours(args):
         "grid_pairs_per_s": grid_pairs / (stages["link.pairs"] * 1e-3) if stages.get("link.pairs") else None,
         "stage_ms": {k: round(v, 5) for k, v in stages.items()},
         "roofline": roofline, "cpu_baseline": cpu, "parity_vs_oracle_in_this_run": parity,
-        "e2e": {"value": world * N / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
+        "e2e": {"value": whole_job_value(world, N, e2e_ms), "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
                 "h2d_bytes_per_step": int(hpos.numel() * 4),
                 "d2h_bytes_per_step": int(N * 4 + Kh * (4 + 4 + 4 + 12) + 8)},
         "gpu_launches": int(launches), "clocks": clk.summary(),

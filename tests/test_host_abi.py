@@ -1,0 +1,134 @@
+"""CPU-only checks of the boundary: the C-ABI library loads and exports every symbol that
+include/fof.h declares, the host-only calls behave as the header says (no compute call is made:
+there is no GPU here), and the multi-rank bookkeeping of bench.py works under gloo, world size 2."""
+from __future__ import annotations
+
+import ctypes
+import json
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2510_26851_b200 import binding, build
+
+    build.build()
+    binding.lib()
+    return binding
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "fof.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(fof_[a-z_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol(B):
+    names = declared_symbols()
+    assert len(names) >= 18 and "fof_link" in names and "fof_groups" in names and "fof_create" in names
+    raw = ctypes.CDLL(B.LIB_PATH)
+    for n in names:
+        assert hasattr(raw, n), f"{n} is declared in include/fof.h but not exported"
+
+
+def test_plan_and_argument_errors(B):
+    # Eq. 1: b = b_frac L / N^(1/3), evaluated in double, rounded once
+    assert B.fof_linking_length(0.2, 1000.0, 256 ** 3) == float(np.float32(0.2 * 1000.0 / 256))
+    h = B.fof_create(256 ** 3, 1000.0, 0.78125, 20)
+    n, cells, n_max = B.fof_get_grid(h)
+    assert n == 256 and cells == 256 ** 3 and n_max == 1024   # floor(1280 / 1.001) = 1278, capped at 1024
+    ws = B.fof_workspace_bytes(h)
+    assert 256 ** 3 * 50 < ws < 256 ** 3 * 120
+    B.fof_set_grid(h, 128)
+    assert B.fof_get_grid(h)[0] == 128 and B.fof_workspace_bytes(h) < ws
+    with pytest.raises(B.FofError) as e:
+        B.fof_set_grid(h, 2000)
+    assert e.value.code == B.FOF_ERR_INVALID_ARG
+    B.fof_destroy(h)
+    for bad in [(-1, 1.0, 0.1, 20), (10, 0.0, 0.1, 20), (10, 1.0, -0.1, 20), (10, 1.0, 0.1, 0), (2 ** 31, 1.0, 0.1, 20)]:
+        with pytest.raises(B.FofError) as e:
+            B.fof_create(*bad)
+        assert e.value.code == B.FOF_ERR_INVALID_ARG
+    with pytest.raises(B.FofError) as e:      # fewer than 3 cells of side >= b per axis
+        B.fof_create(100, 1.0, 0.4, 20)
+    assert e.value.code == B.FOF_ERR_UNSUPPORTED
+    h = B.fof_create(0, 1.0, 0.1, 20)          # N = 0 is a valid plan
+    assert B.fof_workspace_bytes(h) > 0
+    B.fof_destroy(h)
+    assert B.lib().fof_error_string(B.FOF_ERR_CAPACITY).decode() == "more groups than capacity"
+    assert B.lib().fof_error_string(12345).decode() == "unknown error"
+
+
+def test_grid_choice_keeps_cell_side_above_b(B):
+    """H0: cell side L/n >= 1.001 b for every plan (R3), n >= 3."""
+    rng = np.random.default_rng(1)
+    for _ in range(200):
+        L = float(np.float32(10 ** rng.uniform(-2, 4)))
+        b = float(np.float32(L / rng.uniform(3.2, 5000)))
+        N = int(10 ** rng.uniform(0, 9))
+        h = B.fof_create(N, L, b, 20)
+        n, cells, n_max = B.fof_get_grid(h)
+        assert 3 <= n <= n_max <= 1024 and cells == n ** 3
+        assert L / n_max >= b * 1.001 * (1 - 1e-6)
+        B.fof_destroy(h)
+
+
+def _gloo_worker(rank, world, port, out):
+    import torch.distributed as dist
+
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port))
+    sys.path.insert(0, ROOT)
+    import bench
+
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    assert bench.dist_env() == (rank, rank, world)
+    w = bench.workload_for_rank("cfg0", rank)
+    ms = bench.max_over_ranks_ms(10.0 + 5.0 * rank, world, "cpu")   # rank 1 is the slow one
+    out.put((rank, w.seed, w.N, ms, bench.whole_job_value(world, w.N, ms)))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_replica_bookkeeping_under_gloo_world_2():
+    import torch.multiprocessing as mp
+
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = 29500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_gloo_worker, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    rows = sorted(out.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    (r0, s0, n0, ms0, v0), (r1, s1, n1, ms1, v1) = rows
+    assert s0 != s1 and n0 == n1 == 32 ** 3            # independent replicas of the same workload
+    assert ms0 == ms1 == 15.0                           # max over ranks
+    assert v0 == v1 == 2 * 32 ** 3 / 15.0e-3            # whole-job aggregate
+
+
+def test_reference_arm_other_ranks_exit_silently():
+    env = dict(os.environ, RANK="1", LOCAL_RANK="1", WORLD_SIZE="2")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
+                        "--steps", "1", "--warmup", "0"], env=env, capture_output=True, text=True, timeout=120)
+    assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_reference_arm_prints_the_contract_line():
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1",
+                        "--warmup", "0", "--workload", "cfg0"], capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr
+    line = json.loads(r.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["metric"] == "fof_linked_particles_per_s"
+    assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
+    assert line["value"] > 0 and line["config"]["workload"] == "cfg0"
