@@ -44,8 +44,8 @@ ALG_BYTES_PER_PARTICLE = {
     "link.partition": 12,          # read pos (reorder); the bin-contiguous intermediate is not counted
     "link.cell_sort": 16,          # write sorted (x, y, z, idx)
     "link.pairs": 16 + 4,          # read sorted once, write parent
-    "link.flatten": 4 + 4 + 4 + 4, # flatten parent read + write; read idx, min-per-root RMW
-    "link.labels": 4 + 4,          # gather the root's minimum, write labels (original order)
+    "link.labels": 16 + 4 + 4,     # the model's flatten (8) + canonicalise (8) streams, then gather the root's
+                                   # label and write labels (original order)
     "groups.clear": 0,
     "groups.count": 4 + 4,         # read labels, size RMW
     "groups.compact": 4 + 4,       # read sizes, write id map

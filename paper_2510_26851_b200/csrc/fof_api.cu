@@ -34,7 +34,6 @@ void layout(fof_handle *h)
     h->off_bin_base = off;    off += align256(((size_t)h->sort.bins + 2) * sizeof(unsigned int));
     h->off_part = off;        off += align256((N + 1) * sizeof(float4));
     h->off_idx = off;         off += align256((N + 1) * sizeof(int));
-    h->off_minidx = off;      off += align256((N + 1) * sizeof(int));
     h->off_dense = off;       off += align256((N / kDenseCell + N / 32 + 2) * sizeof(unsigned long long));
     h->off_sorted = off;      off += align256((N + 1) * sizeof(float4));
     h->off_cnt = off;         off += align256((N + 1) * sizeof(int));
@@ -69,10 +68,10 @@ int cuda_fail(fof_handle *h, cudaError_t e, const char *where)
     } while (0)
 
 // Profiled stages, in execution order (fof_profile_name).
-enum Stage { kLinkClear = 0, kLinkHist, kLinkOffsets, kLinkPartition, kLinkCellSort, kLinkPairs, kLinkFlatten, kLinkLabels,
+enum Stage { kLinkClear = 0, kLinkHist, kLinkOffsets, kLinkPartition, kLinkCellSort, kLinkPairs, kLinkLabels,
              kGroupsClear, kGroupsCount, kGroupsCompact, kGroupsReduce, kGroupsFinish, kNumStages };
 const char *const kStageName[kNumStages] = {
-    "link.clear", "link.hist", "link.offsets", "link.partition", "link.cell_sort", "link.pairs", "link.flatten", "link.labels",
+    "link.clear", "link.hist", "link.offsets", "link.partition", "link.cell_sort", "link.pairs", "link.labels",
     "groups.clear", "groups.count", "groups.compact", "groups.reduce", "groups.finish"};
 static_assert(kNumStages <= kMaxStages, "raise kMaxStages");
 
@@ -239,7 +238,7 @@ int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *s
     unsigned int *cell = at<unsigned int>(ws, h->off_cell);
     float4 *sorted = at<float4>(ws, h->off_sorted);
     unsigned int *rel = at<unsigned int>(ws, h->off_rel);
-    int *idx_s = at<int>(ws, h->off_idx), *minidx = at<int>(ws, h->off_minidx);
+    int *idx_s = at<int>(ws, h->off_idx);
     unsigned long long *dense = at<unsigned long long>(ws, h->off_dense);
     h->linked = false;
     const int has = h->N > 0;
@@ -255,14 +254,13 @@ int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *s
         StageHook hook{h, s, kLinkHist};
         CK(launch_sort(pos, h->N, h->grid, h->sort, h->part_ctas, at<unsigned int>(ws, h->off_cta_hist),
                        at<unsigned int>(ws, h->off_bin_base), at<float4>(ws, h->off_part), cell, sorted, rel, idx_s,
-                       minidx, dense, ctrl, hook, s), "sort kernels");
+                       dense, ctrl, hook, s), "sort kernels");
     }
     {
         StageTimer t(h, s, kLinkPairs, has);
-        CK(launch_link(sorted, h->N, h->grid, cell, dense, rel, ctrl, h->num_sms, s), "link kernels");
+        CK(launch_link(sorted, h->N, h->grid, cell, dense, rel, idx_s, ctrl, h->num_sms, s), "link kernels");
     }
-    { StageTimer t(h, s, kLinkFlatten, has); CK(launch_flatten_min(rel, idx_s, minidx, h->N, s), "flatten_min_kernel"); }
-    { StageTimer t(h, s, kLinkLabels, has); CK(launch_write_labels(rel, idx_s, minidx, labels, h->N, s), "write_labels_kernel"); }
+    { StageTimer t(h, s, kLinkLabels, has); CK(launch_write_labels(rel, idx_s, labels, h->N, s), "write_labels_kernel"); }
     h->linked = true;
     h->linked_ws = ws;
     return FOF_OK;

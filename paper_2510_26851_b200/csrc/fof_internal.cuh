@@ -86,7 +86,7 @@ struct fof_handle {
     // workspace layout (byte offsets, 256-B aligned)
     fof::SortPlan sort;
     size_t off_ctrl, off_cell, off_part, off_cta_hist, off_bin_base, off_sorted, off_cnt, off_acc, off_gscan_state;
-    size_t off_rel, off_idx, off_minidx, off_dense;  // union-find (cell-sorted space), original index, min original index
+    size_t off_rel, off_idx, off_dense;  // union-find (cell-sorted space), original index of each slot, work items
     size_t ws_bytes;
     int64_t gscan_tiles, max_groups;
     int num_sms, part_ctas;
@@ -170,15 +170,13 @@ struct StageHook {
 // kernels (one launcher per step; all asynchronous on `s`)
 cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp, int ctas, unsigned int *cta_hist,
                         unsigned int *bin_base, float4 *part, unsigned int *cell_start, float4 *sorted,
-                        unsigned int *rel, int *idx_s, int *minidx, unsigned long long *dense_list, Ctrl *ctrl,
+                        unsigned int *rel, int *idx_s, unsigned long long *dense_list, Ctrl *ctrl,
                         StageHook &hook, cudaStream_t s);
 cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
-                        const unsigned long long *dense_list, unsigned int *rel, Ctrl *ctrl, int num_sms,
-                        cudaStream_t s);
+                        const unsigned long long *dense_list, unsigned int *rel, const int *idx_s, Ctrl *ctrl,
+                        int num_sms, cudaStream_t s);
 cudaError_t launch_grid_pairs(const unsigned int *cell_start, Grid g, Ctrl *ctrl, int num_sms, cudaStream_t s);
-cudaError_t launch_flatten_min(unsigned int *rel, const int *idx_s, int *minidx, int64_t N, cudaStream_t s);
-cudaError_t launch_write_labels(const unsigned int *rel, const int *idx_s, const int *minidx, int *labels, int64_t N,
-                                cudaStream_t s);
+cudaError_t launch_write_labels(const unsigned int *rel, const int *idx_s, int *labels, int64_t N, cudaStream_t s);
 
 cudaError_t launch_group_count(const int *labels, int64_t N, int *cnt, cudaStream_t s);
 cudaError_t launch_group_compact(const int *labels, int64_t N, int N_min, int *cnt_to_gid, int64_t cap,

@@ -2,8 +2,8 @@
 // What is linked: PAPER.md:85-87 (§2 step iv) and PAPER.md:200-214 (Alg. 2 candidate cells and
 // mask); the 27-cell stencil with indices mod n is PAPER.md:202.  The T label sweeps of
 // PAPER.md:221-225 are replaced by their fixed point, computed with a lock-free union-find
-// (ECL-CC style: atomicCAS hooks at roots, path halving) whose root is the minimum index of its
-// set, the converged min-label of PAPER.md:91.
+// (ECL-CC style: atomicCAS hooks at roots, path halving) whose root is the member with the
+// minimum original index, the converged min-label of PAPER.md:91.
 //
 // Design.  The union-find runs in CELL-SORTED index space: a component is a
 // spatially compact object, so its parent entries sit in a few cache lines.  Every unordered
@@ -23,9 +23,8 @@
 //                       the ranges of a warp are flattened into one list of candidate slots that
 //                       the 32 lanes walk together, so a lane with many candidates does not hold
 //                       the others hostage.
-// The canonical label (minimum ORIGINAL index of the component) is produced by two streaming
-// passes: flatten + atomicMin of the original index at the root, then a scatter of that minimum
-// to labels[original index].
+// The root of a set is its member with the smallest ORIGINAL index, so the canonical label is
+// read off the root by one streaming pass (chase + scatter to labels[original index]).
 #include "fof_internal.cuh"
 
 namespace fof {
@@ -46,29 +45,32 @@ __device__ __forceinline__ bool linked_t(const float4 &a, const float4 &b, const
     return d2 <= g.b2;
 }
 
-// ---- union-find on `rel`: rel[s] = s - parent(s) >= 0 (a root has rel 0; the root of a set is
-// its smallest cell-sorted index).  Hooks are atomicCAS(rel + root, 0, distance) and can only
+// ---- union-find on `rel`: rel[s] = s - parent(s) as a signed offset (a root has rel 0, which
+// cell_sort_kernel writes for every slot).  The root of a set is its member with the smallest
+// ORIGINAL index (`idx`), i.e. the canonical label of PAPER.md:91 / 180 itself, so H5 needs no
+// minimum pass: a root hooks under another one only if its original index is the larger of the
+// two (a strict total order: no cycles).  Hooks are atomicCAS(rel + root, 0, offset) and can only
 // succeed on a true root; every plain load may return a stale value, which is always the offset
 // to SOME ancestor (links only ever move up), so staleness costs hops, never correctness.  Plain
 // path-halving stores at non-roots are benign.
 __device__ __forceinline__ int find_rel(unsigned int *rel, int x)
 {
-    unsigned int d = rel[x];
+    int d = (int)rel[x];
     while (d) {
-        const int p = x - (int)d;
-        const unsigned int dp = rel[p];
-        if (dp) rel[x] = d + dp;  // halve: x -> grandparent
+        const int p = x - d;
+        const int dp = (int)rel[p];
+        if (dp) rel[x] = (unsigned int)(d + dp);  // halve: x -> grandparent
         x = p;
         d = dp;
     }
     return x;
 }
 
-__device__ __forceinline__ int unite_rel(unsigned int *rel, int a, int b)
+__device__ __forceinline__ int unite_rel(unsigned int *rel, const int *__restrict__ idx, int a, int b)
 {
     int ra = find_rel(rel, a), rb = find_rel(rel, b);
     while (ra != rb) {
-        if (ra < rb) { const int t = ra; ra = rb; rb = t; }  // ra is the larger root
+        if (__ldg(idx + ra) < __ldg(idx + rb)) { const int t = ra; ra = rb; rb = t; }  // ra: larger original index
         const unsigned int old = atomicCAS(rel + ra, 0u, (unsigned int)(ra - rb));
         if (old == 0u) return rb;
         ra = find_rel(rel, ra - (int)old);
@@ -117,7 +119,8 @@ __device__ __forceinline__ unsigned int batch_adjacency(const float4 &me, const 
 
 // Hooks of one batch: candidate k (cell-sorted index in s_pj[k].w) joins every component of the
 // tile it is linked to.  `grp` = lanes of my tile component, `leader` = I am its lowest lane.
-__device__ __forceinline__ void batch_unions(unsigned int adjT, const float4 *s_pj, int cnt, unsigned int *rel, int ib,
+__device__ __forceinline__ void batch_unions(unsigned int adjT, const float4 *s_pj, int cnt, unsigned int *rel,
+                                             const int *__restrict__ idx_s, int ib,
                                              unsigned int grp, bool leader, int lane)
 {
     const unsigned int active = __reduce_or_sync(kFull, adjT);  // tile lanes with any link into the batch
@@ -128,7 +131,7 @@ __device__ __forceinline__ void batch_unions(unsigned int adjT, const float4 *s_
         const int gl = __ffs((int)lead) - 1;
         lead &= lead - 1u;
         const unsigned int members = __shfl_sync(kFull, grp, gl);
-        if (adjT & members) unite_rel(rel, j, ib + gl);
+        if (adjT & members) unite_rel(rel, idx_s, j, ib + gl);
     }
 }
 
@@ -152,8 +155,8 @@ constexpr unsigned int kFwdX = pack13(0), kFwdY = pack13(1), kFwdZ = pack13(2);
 // the cell, compacted into batches of 32 and tested against the tile.
 template <bool WRAP>
 __device__ __forceinline__ void tile_neighbours(const float4 *__restrict__ sorted,
-                                                const unsigned int *__restrict__ cs, unsigned int *rel, float4 *s_pj,
-                                                const float4 &me, int ib, int cntI, unsigned int grp, bool leader,
+                                                const unsigned int *__restrict__ cs, unsigned int *rel,
+                                                const int *__restrict__ idx_s, float4 *s_pj, const float4 &me, int ib, int cntI, unsigned int grp, bool leader,
                                                 int cx, int cy, int cz, const Grid &g, int lane,
                                                 unsigned int &nedges, unsigned int &ntests)
 {
@@ -220,7 +223,7 @@ __device__ __forceinline__ void tile_neighbours(const float4 *__restrict__ sorte
             const unsigned int adjT = batch_adjacency<WRAP>(me, s_pj, 32, g, lane);
             nedges += (unsigned int)__popc(adjT);
             if (lane == 0) ntests += 32u * (unsigned int)cntI;
-            batch_unions(adjT, s_pj, 32, rel, ib, grp, leader, lane);
+            batch_unions(adjT, s_pj, 32, rel, idx_s, ib, grp, leader, lane);
             const float4 keep = s_pj[32 + lane];
             __syncwarp();
             s_pj[lane] = keep;
@@ -232,7 +235,7 @@ __device__ __forceinline__ void tile_neighbours(const float4 *__restrict__ sorte
         const unsigned int adjT = batch_adjacency<WRAP>(me, s_pj, nc, g, lane);
         nedges += (unsigned int)__popc(adjT);
         if (lane == 0) ntests += (unsigned int)(nc * cntI);
-        batch_unions(adjT, s_pj, nc, rel, ib, grp, leader, lane);
+        batch_unions(adjT, s_pj, nc, rel, idx_s, ib, grp, leader, lane);
     }
     __syncwarp();
 }
@@ -240,7 +243,7 @@ __device__ __forceinline__ void tile_neighbours(const float4 *__restrict__ sorte
 // One work item: tile `t` (ts particles) of dense cell `c`.
 __device__ __forceinline__ void tile_item(const float4 *__restrict__ sorted, const Grid &g,
                                           const unsigned int *__restrict__ cell_start, unsigned long long item,
-                                          unsigned int *rel, float4 *s_pj, int lane, unsigned int &nedges,
+                                          unsigned int *rel, const int *__restrict__ idx_s, float4 *s_pj, int lane, unsigned int &nedges,
                                           unsigned int &ntests)
 {
     const float inf = __int_as_float(0x7f800000);
@@ -278,10 +281,17 @@ __device__ __forceinline__ void tile_item(const float4 *__restrict__ sorted, con
             if (vis & self) lab = r;
             todo &= ~vis;
         }
-        if (lab != lane) unite_rel(rel, ib + lane, ib + lab);
     }
+    // every member hooks straight under the member of its component with the smallest original index
+    // (the union-find's order): no retries, depth one
     const unsigned int grp = __match_any_sync(kFull, lab);
-    const bool leader = lab == lane;
+    const int my_oi = lane < cntI ? __ldg(idx_s + ib + lane) : 0x7fffffff;
+    const int min_oi = __reduce_min_sync(grp, my_oi);
+    const int head = __ffs((int)(__ballot_sync(kFull, my_oi == min_oi) & grp)) - 1;
+    const bool leader = head == lane;
+    // (a parent that is no longer a root is fine: original indices still fall along every path)
+    if (!leader && atomicCAS(rel + ib + lane, 0u, (unsigned int)(lane - head)) != 0u)
+        unite_rel(rel, idx_s, ib + lane, ib + head);  // somebody hooked me first: general path
 
     // ---- the earlier tiles of my cell (all full: ts particles)
     for (int jt = 0; jt < t; ++jt) {
@@ -296,7 +306,7 @@ __device__ __forceinline__ void tile_item(const float4 *__restrict__ sorted, con
         const unsigned int adjT = batch_adjacency<false>(me, s_pj, ts, g, lane);
         nedges += (unsigned int)__popc(adjT);
         if (lane == 0) ntests += (unsigned int)(ts * cntI);
-        batch_unions(adjT, s_pj, ts, rel, ib, grp, leader, lane);
+        batch_unions(adjT, s_pj, ts, rel, idx_s, ib, grp, leader, lane);
     }
     __syncwarp();
 
@@ -308,8 +318,8 @@ __device__ __forceinline__ void tile_item(const float4 *__restrict__ sorted, con
     const int cy = min(__float2int_rd(__fmul_rn(p0.y, g.inv_cell)), g.n_minus_1);
     const int cz = min(__float2int_rd(__fmul_rn(p0.z, g.inv_cell)), g.n_minus_1);
     const bool wrap = n < 6 || cx == 0 || cx == n - 1 || cy == 0 || cy == n - 1 || cz == n - 1;
-    if (wrap) tile_neighbours<true>(sorted, cell_start, rel, s_pj, me, ib, cntI, grp, leader, cx, cy, cz, g, lane, nedges, ntests);
-    else tile_neighbours<false>(sorted, cell_start, rel, s_pj, me, ib, cntI, grp, leader, cx, cy, cz, g, lane, nedges, ntests);
+    if (wrap) tile_neighbours<true>(sorted, cell_start, rel, idx_s, s_pj, me, ib, cntI, grp, leader, cx, cy, cz, g, lane, nedges, ntests);
+    else tile_neighbours<false>(sorted, cell_start, rel, idx_s, s_pj, me, ib, cntI, grp, leader, cx, cy, cz, g, lane, nedges, ntests);
 }
 
 // =============================================================================================
@@ -332,7 +342,8 @@ struct SparseSmem {
 // visited only if I am within `reach` of every face between us.
 template <bool WRAP, int PASS>
 __device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, const unsigned int *__restrict__ cs,
-                                            unsigned int *rel, int si, bool live, const unsigned int *home, int c1,
+                                            unsigned int *rel, const int *__restrict__ idx_s, int si, bool live,
+                                            const unsigned int *home, int c1,
                                             const float4 &me, int cx, int cy, int cz, float fx, float fy, float fz,
                                             const Grid &g, SparseSmem &sm, int lane, unsigned int &nedges,
                                             unsigned int &ntests)
@@ -408,7 +419,7 @@ __device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, c
                 for (int j = b + lane; j < b + l; j += 32)
                     if (linked_t<WRAP>(o4, __ldg(sorted + j), g)) {
                         ++nedges;
-                        unite_rel(rel, osi, j);
+                        unite_rel(rel, idx_s, osi, j);
                     }
             }
             if (len[r] > kLongRange) len[r] = 0;
@@ -463,7 +474,7 @@ __device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, c
             const int j = r.x + (p - (r.y >> 5));
             if (linked_t<WRAP>(o4, __ldg(sorted + j), g)) {
                 ++nedges;
-                unite_rel(rel, osi, j);
+                unite_rel(rel, idx_s, osi, j);
             }
         }
     }
@@ -473,7 +484,7 @@ __device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, c
 // 32 consecutive cell-sorted particles, one per lane.
 __device__ __forceinline__ void sparse_chunk(const float4 *__restrict__ sorted, int64_t N, const Grid &g,
                                              const unsigned int *__restrict__ cell_start, unsigned int *rel,
-                                             int64_t base, SparseSmem &sm, int lane, unsigned int &nedges,
+                                             const int *__restrict__ idx_s, int64_t base, SparseSmem &sm, int lane, unsigned int &nedges,
                                              unsigned int &ntests)
 {
     const int n = g.n;
@@ -504,10 +515,10 @@ __device__ __forceinline__ void sparse_chunk(const float4 *__restrict__ sorted, 
     }
     if (!__any_sync(kFull, live)) return;
     if (__any_sync(kFull, needwrap)) {
-        sparse_warp<true, 0>(sorted, cell_start, rel, si, live, home, c1, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
-        sparse_warp<true, 1>(sorted, cell_start, rel, si, live, home, c1, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
+        sparse_warp<true, 0>(sorted, cell_start, rel, idx_s, si, live, home, c1, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
+        sparse_warp<true, 1>(sorted, cell_start, rel, idx_s, si, live, home, c1, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
     } else {
-        sparse_warp<false, 0>(sorted, cell_start, rel, si, live, home, c1, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
+        sparse_warp<false, 0>(sorted, cell_start, rel, idx_s, si, live, home, c1, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
     }
 }
 
@@ -533,7 +544,8 @@ __global__ void __launch_bounds__(kLinkBlock, FOF_LINK_MINB) link_kernel(const f
                                                                          Grid g,
                                                                          const unsigned int *__restrict__ cell_start,
                                                                          const unsigned long long *__restrict__ items,
-                                                                         unsigned int *rel, Ctrl *ctrl)
+                                                                         unsigned int *rel,
+                                                                         const int *__restrict__ idx_s, Ctrl *ctrl)
 {
     __shared__ LinkSmem s_all[kWarpsPerCta];
     LinkSmem &sm = s_all[threadIdx.x >> 5];
@@ -550,7 +562,7 @@ __global__ void __launch_bounds__(kLinkBlock, FOF_LINK_MINB) link_kernel(const f
                 if (it0 >= nitems) break;
                 const unsigned int it1 = min(it0 + (unsigned int)kTileBatch, nitems);
                 for (unsigned int it = it0; it < it1; ++it)
-                    tile_item(sorted, g, cell_start, __ldg(items + it), rel, sm.pj, lane, nedges, ntests);
+                    tile_item(sorted, g, cell_start, __ldg(items + it), rel, idx_s, sm.pj, lane, nedges, ntests);
             }
         } else {
             while (true) {
@@ -562,7 +574,7 @@ __global__ void __launch_bounds__(kLinkBlock, FOF_LINK_MINB) link_kernel(const f
                 for (int k = 0; k < kSparseBatch; ++k) {
                     const int64_t base = base0 + 32 * k;
                     if (base >= N) break;
-                    sparse_chunk(sorted, N, g, cell_start, rel, base, sm.sp, lane, nedges, ntests);
+                    sparse_chunk(sorted, N, g, cell_start, rel, idx_s, base, sm.sp, lane, nedges, ntests);
                 }
             }
         }
@@ -577,68 +589,41 @@ __global__ void __launch_bounds__(kLinkBlock, FOF_LINK_MINB) link_kernel(const f
     }
 }
 
-// H5a: flatten ("after convergence"): rel[s] <- s - root(s), and lower the root's
-// minidx to the smallest ORIGINAL index of its members ("minimum label", PAPER.md:180
-// "minimum global particle ID").  The chase is read-only; a concurrent reader sees either the old
-// offset (an ancestor) or the root.  Roots have nothing to do: minidx[root] starts as its own index.
-// Four consecutive particles per thread, so that four chases are in flight.
-__global__ void __launch_bounds__(kBlock) flatten_min_kernel(unsigned int *rel, const int *__restrict__ idx_s,
-                                                             int *minidx, int64_t N)
-{
-    const int64_t s0 = ((int64_t)blockIdx.x * kBlock + threadIdx.x) * 4;
-    if (s0 >= N) return;
-    unsigned int d[4];
-    if (s0 + 3 < N) {
-        const uint4 t = *reinterpret_cast<const uint4 *>(rel + s0);
-        d[0] = t.x; d[1] = t.y; d[2] = t.z; d[3] = t.w;
-    } else {
-#pragma unroll
-        for (int k = 0; k < 4; ++k) d[k] = (s0 + k < N) ? rel[s0 + k] : 0u;
-    }
-    if ((d[0] | d[1] | d[2] | d[3]) == 0u) return;
-    int r[4];
-#pragma unroll
-    for (int k = 0; k < 4; ++k) r[k] = (int)(s0 + k) - (int)d[k];
-    // lock-step chase: one round issues the (up to four) loads together
-    bool more = true;
-    while (more) {
-        unsigned int e[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) e[k] = d[k] ? rel[r[k]] : 0u;
-        more = false;
-#pragma unroll
-        for (int k = 0; k < 4; ++k)
-            if (e[k]) { r[k] -= (int)e[k]; more = true; }
-    }
-#pragma unroll
-    for (int k = 0; k < 4; ++k)
-        if (d[k]) {
-            rel[s0 + k] = (unsigned int)((int)(s0 + k) - r[k]);
-            atomicMin(minidx + r[k], idx_s[s0 + k]);
-        }
-}
-
-// H5b: labels[original index] = minimum original index of the component.
+// H5 ("after convergence"): labels[original index] = original index of the root =
+// the minimum original index of the component ("minimum label", "minimum
+// global particle ID").  Four consecutive slots per thread, chased in lock step so that the (up to
+// four) loads of one round are in flight together; the chase is read-only.
 __global__ void __launch_bounds__(kBlock) write_labels_kernel(const unsigned int *__restrict__ rel,
-                                                              const int *__restrict__ idx_s,
-                                                              const int *__restrict__ minidx, int *__restrict__ labels,
+                                                              const int *__restrict__ idx_s, int *__restrict__ labels,
                                                               int64_t N)
 {
     const int64_t s0 = ((int64_t)blockIdx.x * kBlock + threadIdx.x) * 4;
     if (s0 >= N) return;
+    int d[4], oi[4];
     if (s0 + 3 < N) {
-        const uint4 d = __ldg(reinterpret_cast<const uint4 *>(rel + s0));
-        const int4 oi = __ldg(reinterpret_cast<const int4 *>(idx_s + s0));
-        const int s = (int)s0;
-        const int m0 = __ldg(minidx + (s - (int)d.x)), m1 = __ldg(minidx + (s + 1 - (int)d.y)),
-                  m2 = __ldg(minidx + (s + 2 - (int)d.z)), m3 = __ldg(minidx + (s + 3 - (int)d.w));
-        labels[oi.x] = m0;
-        labels[oi.y] = m1;
-        labels[oi.z] = m2;
-        labels[oi.w] = m3;
+        const uint4 t = __ldg(reinterpret_cast<const uint4 *>(rel + s0));
+        const int4 o = __ldg(reinterpret_cast<const int4 *>(idx_s + s0));
+        d[0] = (int)t.x; d[1] = (int)t.y; d[2] = (int)t.z; d[3] = (int)t.w;
+        oi[0] = o.x; oi[1] = o.y; oi[2] = o.z; oi[3] = o.w;
     } else {
-        for (int64_t s = s0; s < N; ++s) labels[__ldg(idx_s + s)] = __ldg(minidx + ((int)s - (int)__ldg(rel + s)));
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            d[k] = (s0 + k < N) ? (int)__ldg(rel + s0 + k) : 0;
+            oi[k] = (s0 + k < N) ? __ldg(idx_s + s0 + k) : 0;
+        }
     }
+    int r[4], e[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { r[k] = (int)(s0 + k) - d[k]; e[k] = d[k]; }
+    while (e[0] | e[1] | e[2] | e[3]) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) e[k] = e[k] ? (int)__ldg(rel + r[k]) : 0;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) r[k] -= e[k];
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+        if (s0 + k < N) labels[oi[k]] = d[k] ? __ldg(idx_s + r[k]) : oi[k];
 }
 
 // P_exec of DESIGN.md §7: candidate pairs the unfiltered half stencil implies on this grid,
@@ -682,25 +667,18 @@ cudaError_t launch_grid_pairs(const unsigned int *cell_start, Grid g, Ctrl *ctrl
 static inline unsigned int blocks_for(int64_t n, int per_block) { return (unsigned int)((n + per_block - 1) / per_block); }
 
 cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
-                        const unsigned long long *dense_list, unsigned int *rel, Ctrl *ctrl, int num_sms,
-                        cudaStream_t s)
+                        const unsigned long long *dense_list, unsigned int *rel, const int *idx_s, Ctrl *ctrl,
+                        int num_sms, cudaStream_t s)
 {
     if (N <= 0) return cudaSuccess;
     const unsigned int grid = (unsigned int)min((int64_t)blocks_for(N, kLinkBlock), (int64_t)num_sms * FOF_LINK_MINB);
-    link_kernel<<<grid, kLinkBlock, 0, s>>>(sorted, N, g, cell_start, dense_list, rel, ctrl);
+    link_kernel<<<grid, kLinkBlock, 0, s>>>(sorted, N, g, cell_start, dense_list, rel, idx_s, ctrl);
     return cudaGetLastError();
 }
 
-cudaError_t launch_flatten_min(unsigned int *rel, const int *idx_s, int *minidx, int64_t N, cudaStream_t s)
+cudaError_t launch_write_labels(const unsigned int *rel, const int *idx_s, int *labels, int64_t N, cudaStream_t s)
 {
-    if (N > 0) flatten_min_kernel<<<blocks_for(N, kBlock * 4), kBlock, 0, s>>>(rel, idx_s, minidx, N);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_write_labels(const unsigned int *rel, const int *idx_s, const int *minidx, int *labels, int64_t N,
-                                cudaStream_t s)
-{
-    if (N > 0) write_labels_kernel<<<blocks_for(N, kBlock * 4), kBlock, 0, s>>>(rel, idx_s, minidx, labels, N);
+    if (N > 0) write_labels_kernel<<<blocks_for(N, kBlock * 4), kBlock, 0, s>>>(rel, idx_s, labels, N);
     return cudaGetLastError();
 }
 

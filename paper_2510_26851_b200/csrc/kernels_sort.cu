@@ -182,7 +182,7 @@ __global__ void __launch_bounds__(kPartThreads) part_scatter_kernel(const float 
 //   1. histogram of the bin's records over its cells (shared-memory atomics);
 //   2. exclusive scan -> cell_start[] (coalesced), work items of link_tiles_kernel (dense cells);
 //   3. records re-read (L2) and moved to their final slot; rel = 0 (every particle a root),
-//      idx_s = minidx = original index (inputs of H5).
+//      idx_s = original index (the order of the union-find, input of H5).
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ unsigned int cell_of(const float4 &v, const Grid &g)
 {
@@ -192,7 +192,7 @@ __device__ __forceinline__ unsigned int cell_of(const float4 &v, const Grid &g)
 __global__ void __launch_bounds__(kCellSortThreads) cell_sort_kernel(
     const float4 *__restrict__ part, const unsigned int *__restrict__ bin_base, Grid g, int shift, int64_t C,
     unsigned int *__restrict__ cell_start, float4 *sorted, unsigned int *__restrict__ rel,
-    int *__restrict__ idx_s, int *__restrict__ minidx, unsigned long long *__restrict__ dense_list, Ctrl *ctrl)
+    int *__restrict__ idx_s, unsigned long long *__restrict__ dense_list, Ctrl *ctrl)
 {
     extern __shared__ unsigned int s_cell[];  // [2^shift]
     __shared__ unsigned long long s_warp[kCellSortThreads / 32];
@@ -293,7 +293,6 @@ __global__ void __launch_bounds__(kCellSortThreads) cell_sort_kernel(
         const int oi = __float_as_int(__ldcg(&sorted[p].w));
         rel[p] = 0u;
         idx_s[p] = oi;
-        minidx[p] = oi;
     }
 }
 
@@ -305,7 +304,7 @@ static inline cudaError_t set_smem(const void *fn, size_t bytes)
 
 cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp, int ctas, unsigned int *cta_hist,
                         unsigned int *bin_base, float4 *part, unsigned int *cell_start, float4 *sorted,
-                        unsigned int *rel, int *idx_s, int *minidx, unsigned long long *dense_list, Ctrl *ctrl,
+                        unsigned int *rel, int *idx_s, unsigned long long *dense_list, Ctrl *ctrl,
                         StageHook &hook, cudaStream_t s)
 {
     if (N <= 0) return cudaSuccess;
@@ -332,7 +331,7 @@ cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp,
     hook.end(2);
     hook.begin(3, 1);
     cell_sort_kernel<<<sp.bins, kCellSortThreads, smem_cells, s>>>(part, bin_base, g, sp.shift, C, cell_start, sorted,
-                                                                  rel, idx_s, minidx, dense_list, ctrl);
+                                                                  rel, idx_s, dense_list, ctrl);
     hook.end(3);
     return cudaGetLastError();
 }
