@@ -254,7 +254,7 @@ int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *s
         StageHook hook{h, s, kLinkHist};
         CK(launch_sort(pos, h->N, h->grid, h->sort, h->part_ctas, at<unsigned int>(ws, h->off_cta_hist),
                        at<unsigned int>(ws, h->off_bin_base), at<float4>(ws, h->off_part), cell, sorted, rel, idx_s,
-                       dense, ctrl, hook, s), "sort kernels");
+                       dense, labels, ctrl, hook, s), "sort kernels");
     }
     {
         StageTimer t(h, s, kLinkPairs, has);

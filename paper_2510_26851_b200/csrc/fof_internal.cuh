@@ -11,7 +11,10 @@
 namespace fof {
 
 constexpr int kBlock = 256;           // threads per CTA for the streaming kernels
-constexpr int kScanItems = 8;         // items per thread in the single-pass scan
+#ifndef FOF_SCAN_ITEMS
+#define FOF_SCAN_ITEMS 16
+#endif
+constexpr int kScanItems = FOF_SCAN_ITEMS;  // items per thread in the single-pass scan (multiple of 4)
 constexpr int kScanTile = kBlock * kScanItems;
 constexpr float kCellMargin = 1.001f; // cell side >= b * kCellMargin  (R3)
 constexpr int kMaxGrid = 1024;        // n^3 <= 2^30: at most kMaxBins bins of 2^15 cells
@@ -170,7 +173,7 @@ struct StageHook {
 // kernels (one launcher per step; all asynchronous on `s`)
 cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp, int ctas, unsigned int *cta_hist,
                         unsigned int *bin_base, float4 *part, unsigned int *cell_start, float4 *sorted,
-                        unsigned int *rel, int *idx_s, unsigned long long *dense_list, Ctrl *ctrl,
+                        unsigned int *rel, int *idx_s, unsigned long long *dense_list, int *labels, Ctrl *ctrl,
                         StageHook &hook, cudaStream_t s);
 cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
                         const unsigned long long *dense_list, unsigned int *rel, const int *idx_s, Ctrl *ctrl,

@@ -86,9 +86,11 @@ __global__ void __launch_bounds__(kBlock) group_compact_kernel(const int *__rest
 
     int c[kScanItems];
     if (base + kScanItems <= N) {  // cnt is a workspace array: 16-byte aligned
-        const int4 a = *reinterpret_cast<const int4 *>(cnt_to_gid + base);
-        const int4 b = *reinterpret_cast<const int4 *>(cnt_to_gid + base + 4);
-        c[0] = a.x; c[1] = a.y; c[2] = a.z; c[3] = a.w; c[4] = b.x; c[5] = b.y; c[6] = b.z; c[7] = b.w;
+#pragma unroll
+        for (int q = 0; q < kScanItems / 4; ++q) {
+            const int4 a = *reinterpret_cast<const int4 *>(cnt_to_gid + base + 4 * q);
+            c[4 * q] = a.x; c[4 * q + 1] = a.y; c[4 * q + 2] = a.z; c[4 * q + 3] = a.w;
+        }
     } else {
 #pragma unroll
         for (int k = 0; k < kScanItems; ++k) c[k] = (base + k < N) ? cnt_to_gid[base + k] : -1;

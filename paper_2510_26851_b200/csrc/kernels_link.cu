@@ -591,8 +591,9 @@ __global__ void __launch_bounds__(kLinkBlock, FOF_LINK_MINB) link_kernel(const f
 
 // H5 ("after convergence"): labels[original index] = original index of the root =
 // the minimum original index of the component ("minimum label", "minimum
-// global particle ID").  Four consecutive slots per thread, chased in lock step so that the (up to
-// four) loads of one round are in flight together; the chase is read-only.
+// global particle ID").  part_scatter_kernel has already written labels[i] = i, which is final for
+// every root, so only non-roots are scattered here.  Four consecutive slots per thread, chased in
+// lock step so that the (up to four) loads of one round are in flight together; read-only chase.
 __global__ void __launch_bounds__(kBlock) write_labels_kernel(const unsigned int *__restrict__ rel,
                                                               const int *__restrict__ idx_s, int *__restrict__ labels,
                                                               int64_t N)
@@ -602,8 +603,9 @@ __global__ void __launch_bounds__(kBlock) write_labels_kernel(const unsigned int
     int d[4], oi[4];
     if (s0 + 3 < N) {
         const uint4 t = __ldg(reinterpret_cast<const uint4 *>(rel + s0));
-        const int4 o = __ldg(reinterpret_cast<const int4 *>(idx_s + s0));
         d[0] = (int)t.x; d[1] = (int)t.y; d[2] = (int)t.z; d[3] = (int)t.w;
+        if ((d[0] | d[1] | d[2] | d[3]) == 0) return;  // four roots
+        const int4 o = __ldg(reinterpret_cast<const int4 *>(idx_s + s0));
         oi[0] = o.x; oi[1] = o.y; oi[2] = o.z; oi[3] = o.w;
     } else {
 #pragma unroll
@@ -623,7 +625,7 @@ __global__ void __launch_bounds__(kBlock) write_labels_kernel(const unsigned int
     }
 #pragma unroll
     for (int k = 0; k < 4; ++k)
-        if (s0 + k < N) labels[oi[k]] = d[k] ? __ldg(idx_s + r[k]) : oi[k];
+        if (d[k]) labels[oi[k]] = __ldg(idx_s + r[k]);
 }
 
 // P_exec of DESIGN.md §7: candidate pairs the unfiltered half stencil implies on this grid,

@@ -161,7 +161,8 @@ __global__ void __launch_bounds__(kPartThreads) part_scatter_kernel(const float 
                                                                     int shift, int bins, int64_t chunk,
                                                                     const unsigned int *__restrict__ cta_hist,
                                                                     const unsigned int *__restrict__ bin_base,
-                                                                    float4 *__restrict__ part)
+                                                                    float4 *__restrict__ part, int *__restrict__ labels,
+                                                                    bool labels_vec)
 {
     extern __shared__ unsigned int s_bin[];
     const unsigned int *src = cta_hist + (int64_t)blockIdx.x * bins;
@@ -175,6 +176,16 @@ __global__ void __launch_bounds__(kPartThreads) part_scatter_kernel(const float 
         const unsigned int dst = atomicAdd(&s_bin[c >> shift], 1u);
         part[dst] = make_float4(x, y, z, __int_as_float((int)i));
     });
+    // H5, first half: labels[i] = i, coalesced, while this CTA walks its chunk in the original order.
+    // That is already the final label of every root (singletons above all); write_labels_kernel then
+    // scatters only the labels of non-roots.
+    for (int64_t i = i0 + 4 * (int64_t)threadIdx.x; i < i1; i += 4 * (int64_t)kPartThreads) {
+        if (labels_vec && i + 4 <= i1) {
+            *reinterpret_cast<int4 *>(labels + i) = make_int4((int)i, (int)i + 1, (int)i + 2, (int)i + 3);
+        } else {
+            for (int k = 0; k < 4 && i + k < i1; ++k) labels[i + k] = (int)(i + k);
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -304,7 +315,7 @@ static inline cudaError_t set_smem(const void *fn, size_t bytes)
 
 cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp, int ctas, unsigned int *cta_hist,
                         unsigned int *bin_base, float4 *part, unsigned int *cell_start, float4 *sorted,
-                        unsigned int *rel, int *idx_s, unsigned long long *dense_list, Ctrl *ctrl,
+                        unsigned int *rel, int *idx_s, unsigned long long *dense_list, int *labels, Ctrl *ctrl,
                         StageHook &hook, cudaStream_t s)
 {
     if (N <= 0) return cudaSuccess;
@@ -327,7 +338,7 @@ cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp,
     hook.end(1);
     hook.begin(2, 1);
     scat<<<ctas, kPartThreads, smem_bins, s>>>(pos, N, g, sp.shift, sp.bins, chunk, cta_hist, bin_base,
-                                                             part);
+                                                             part, labels, ((uintptr_t)labels & 15) == 0);
     hook.end(2);
     hook.begin(3, 1);
     cell_sort_kernel<<<sp.bins, kCellSortThreads, smem_cells, s>>>(part, bin_base, g, sp.shift, C, cell_start, sorted,
