@@ -304,12 +304,12 @@ int fof_groups(fof_handle *h, const float *pos, const float *mass, const int32_t
         for (int k = kGroupsClear; k <= kGroupsFinish; ++k) h->ev_valid[h->prof_cur * kMaxStages + k] = false;
     {
         StageTimer t(h, s, kGroupsClear, 0);
-        CK(cudaMemsetAsync(&ctrl->gscan_ticket, 0, sizeof(unsigned int), s), "memset ticket");
-        CK(cudaMemsetAsync(&ctrl->K, 0, sizeof(long long), s), "memset K");
         CK(cudaMemsetAsync(cnt, 0, (size_t)(h->N + 1) * sizeof(int), s), "memset cnt");
-        CK(cudaMemsetAsync(state, 0, (size_t)h->gscan_tiles * sizeof(unsigned long long), s), "memset gscan state");
     }
-    { StageTimer t(h, s, kGroupsCount, has); CK(launch_group_count(labels, h->N, cnt, s), "group_count_kernel"); }
+    {   // also clears the compaction's ticket, K and scan state
+        StageTimer t(h, s, kGroupsCount, 1);
+        CK(launch_group_count(labels, h->N, cnt, state, h->gscan_tiles, ctrl, s), "group_count_kernel");
+    }
     {
         StageTimer t(h, s, kGroupsCompact, has);
         CK(launch_group_compact(labels, h->N, h->N_min, cnt, cap, group_label, group_size, acc, state, ctrl,

@@ -181,7 +181,8 @@ cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned 
 cudaError_t launch_grid_pairs(const unsigned int *cell_start, Grid g, Ctrl *ctrl, int num_sms, cudaStream_t s);
 cudaError_t launch_write_labels(const unsigned int *rel, const int *idx_s, int *labels, int64_t N, cudaStream_t s);
 
-cudaError_t launch_group_count(const int *labels, int64_t N, int *cnt, cudaStream_t s);
+cudaError_t launch_group_count(const int *labels, int64_t N, int *cnt, unsigned long long *state,
+                               int64_t state_items, Ctrl *ctrl, cudaStream_t s);
 cudaError_t launch_group_compact(const int *labels, int64_t N, int N_min, int *cnt_to_gid, int64_t cap,
                                  int *group_label, int *group_size, double *acc, unsigned long long *state,
                                  Ctrl *ctrl, int64_t tiles, cudaStream_t s);

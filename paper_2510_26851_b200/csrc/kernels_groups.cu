@@ -9,17 +9,23 @@
 
 namespace fof {
 
-constexpr int kPer = 4;  // particles per thread in the streaming passes
+#ifndef FOF_GROUP_PER
+#define FOF_GROUP_PER 4
+#endif
+constexpr int kPer = FOF_GROUP_PER;  // particles per thread in the streaming passes (multiple of 4)
 
 template <bool VEC>
-__device__ __forceinline__ void load4(const int *__restrict__ p, int64_t i, int64_t N, int v[4], int fill)
+__device__ __forceinline__ void load_per(const int *__restrict__ p, int64_t i, int64_t N, int v[kPer], int fill)
 {
-    if (VEC && i + 3 < N) {
-        const int4 t = __ldg(reinterpret_cast<const int4 *>(p + i));
-        v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+    if (VEC && i + kPer <= N) {
+#pragma unroll
+        for (int q = 0; q < kPer / 4; ++q) {
+            const int4 t = __ldg(reinterpret_cast<const int4 *>(p + i + 4 * q));
+            v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
+        }
     } else {
 #pragma unroll
-        for (int k = 0; k < 4; ++k) v[k] = (i + k < N) ? __ldg(p + i + k) : fill;
+        for (int k = 0; k < kPer; ++k) v[k] = (i + k < N) ? __ldg(p + i + k) : fill;
     }
 }
 
@@ -27,14 +33,19 @@ __device__ __forceinline__ void load4(const int *__restrict__ p, int64_t i, int6
 // Singletons (most of the background) issue no atomic at all.
 template <bool VEC>
 __global__ void __launch_bounds__(kBlock) group_count_kernel(const int *__restrict__ labels, int64_t N,
-                                                             int *__restrict__ cnt)
+                                                             int *__restrict__ cnt, unsigned long long *state,
+                                                             int64_t state_items, Ctrl *ctrl)
 {
-    const int64_t i = ((int64_t)blockIdx.x * kBlock + threadIdx.x) * kPer;
+    // also clears what group_compact_kernel (the next launch) needs: its ticket, K and scan state
+    const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+    if (tid == 0) { ctrl->gscan_ticket = 0u; ctrl->K = 0; }
+    for (int64_t k = tid; k < state_items; k += (int64_t)gridDim.x * kBlock) state[k] = 0ull;
+    const int64_t i = tid * kPer;
     if (i >= N) return;
-    int l[4];
-    load4<VEC>(labels, i, N, l, -1);
+    int l[kPer];
+    load_per<VEC>(labels, i, N, l, -1);
 #pragma unroll
-    for (int k = 0; k < 4; ++k)
+    for (int k = 0; k < kPer; ++k)
         if (l[k] >= 0 && l[k] != (int)(i + k)) atomicAdd(cnt + l[k], 1);
 }
 
@@ -167,23 +178,26 @@ __global__ void __launch_bounds__(kBlock) group_reduce_kernel(const float *__res
 {
     const int64_t i0 = ((int64_t)blockIdx.x * kBlock + threadIdx.x) * kPer;
     if (i0 >= N) return;
-    int l[4], gid[4];
-    load4<VEC>(labels, i0, N, l, -1);
+    int l[kPer], gid[kPer];
+    load_per<VEC>(labels, i0, N, l, -1);
 #pragma unroll
-    for (int k = 0; k < 4; ++k) gid[k] = l[k] >= 0 ? -1 - __ldg(gid_of + l[k]) : -1;  // < 0: dropped
+    for (int k = 0; k < kPer; ++k) gid[k] = l[k] >= 0 ? -1 - __ldg(gid_of + l[k]) : -1;  // < 0: dropped
     if (particle_group) {
-        if (VEC && i0 + 3 < N) {
-            *reinterpret_cast<int4 *>(particle_group + i0) =
-                make_int4(max(gid[0], -1), max(gid[1], -1), max(gid[2], -1), max(gid[3], -1));
+        if (VEC && i0 + kPer <= N) {
+#pragma unroll
+            for (int q = 0; q < kPer / 4; ++q)
+                *reinterpret_cast<int4 *>(particle_group + i0 + 4 * q) =
+                    make_int4(max(gid[4 * q], -1), max(gid[4 * q + 1], -1), max(gid[4 * q + 2], -1),
+                              max(gid[4 * q + 3], -1));
         } else {
 #pragma unroll
-            for (int k = 0; k < 4; ++k)
+            for (int k = 0; k < kPer; ++k)
                 if (i0 + k < N) particle_group[i0 + k] = max(gid[k], -1);
         }
     }
     const double L = (double)g.L, h = 0.5 * (double)g.L;
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
+    for (int k = 0; k < kPer; ++k) {
         if (gid[k] < 0 || gid[k] >= cap) continue;
         const int64_t i = i0 + k;
         const double m = mass ? (double)__ldg(mass + i) : 1.0;
@@ -236,12 +250,12 @@ __global__ void __launch_bounds__(kBlock) group_finish_kernel(const float *__res
 static inline unsigned int blocks_for(int64_t n, int per_block) { return (unsigned int)((n + per_block - 1) / per_block); }
 static inline bool aligned16(const void *p) { return ((uintptr_t)p & 15) == 0; }
 
-cudaError_t launch_group_count(const int *labels, int64_t N, int *cnt, cudaStream_t s)
+cudaError_t launch_group_count(const int *labels, int64_t N, int *cnt, unsigned long long *state,
+                               int64_t state_items, Ctrl *ctrl, cudaStream_t s)
 {
-    if (N <= 0) return cudaSuccess;
-    const unsigned int grid = blocks_for(N, kBlock * kPer);
-    if (aligned16(labels)) group_count_kernel<true><<<grid, kBlock, 0, s>>>(labels, N, cnt);
-    else group_count_kernel<false><<<grid, kBlock, 0, s>>>(labels, N, cnt);
+    const unsigned int grid = N > 0 ? blocks_for(N, kBlock * kPer) : 1u;
+    if (aligned16(labels)) group_count_kernel<true><<<grid, kBlock, 0, s>>>(labels, N, cnt, state, state_items, ctrl);
+    else group_count_kernel<false><<<grid, kBlock, 0, s>>>(labels, N, cnt, state, state_items, ctrl);
     return cudaGetLastError();
 }
 
