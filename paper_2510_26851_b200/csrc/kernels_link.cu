@@ -340,15 +340,32 @@ struct SparseSmem {
 // (the rest of my cell [+ the +x cell]; then up to three cells of the rows (dy, dz) = (+1, 0),
 // (-1, +1), (0, +1), (+1, +1)); with wrap, one range per stencil cell.  A neighbour cell is
 // visited only if I am within `reach` of every face between us.
-template <bool WRAP, int PASS>
+// the 14 stencil cells of the sparse role (own, +x, rows (+1,0), (-1,+1), (0,+1), (+1,+1)), offsets + 1
+// packed two bits per cell
+constexpr unsigned int pack14(int axis)
+{
+    unsigned int v = 0;
+    for (int q = 0; q < 14; ++q) {
+        const int dx = q == 0 ? 0 : (q == 1 ? 1 : (q - 2) % 3 - 1);
+        const int dy = q < 2 ? 0 : (q < 5 ? 1 : (q < 8 ? -1 : (q < 11 ? 0 : 1)));
+        const int dz = q < 5 ? 0 : 1;
+        const int d = axis == 0 ? dx : (axis == 1 ? dy : dz);
+        v |= (unsigned int)(d + 1) << (2 * q);
+    }
+    return v;
+}
+constexpr unsigned int kStX = pack14(0), kStY = pack14(1), kStZ = pack14(2);
+
+template <bool WRAP>
 __device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, const unsigned int *__restrict__ cs,
                                             unsigned int *rel, const int *__restrict__ idx_s, int si, bool live,
                                             const unsigned int *home, int c1,
                                             const float4 &me, int cx, int cy, int cz, float fx, float fy, float fz,
                                             const Grid &g, SparseSmem &sm, int lane, unsigned int &nedges,
-                                            unsigned int &ntests)
+                                            unsigned int &ntests, int pass)
 {
-    // live: a real particle whose home cell (cell_start entry `home`, end `c1`) is sparse
+    // live: a real particle whose home cell (cell_start entry `home`, end `c1`) is sparse;
+    // pass: with WRAP the stencil cells 7 pass .. 7 pass + 6 are walked (two calls), else unused
     constexpr int NR = WRAP ? kRangesWrap : kRangesNoWrap;
     const int n = g.n;
     const float lo = g.reach, hi = 1.0f - g.reach;
@@ -374,17 +391,15 @@ __device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, c
                         len[r + 1] = (int)__ldg(home + row[r] + off_hi) - beg[r + 1];
                     }
             } else {
-                if (PASS == 0) {
-                    beg[0] = si + 1;
-                    len[0] = c1 - beg[0];
-                }
 #pragma unroll
-                for (int k = (PASS == 0 ? 1 : 0); k < kRangesWrap; ++k) {
-                    const int q = k + PASS * kRangesWrap;
-                    const int dx = q == 1 ? 1 : (q - 2) % 3 - 1;
-                    const int dy = q < 2 ? 0 : (q < 5 ? 1 : (q < 8 ? -1 : (q < 11 ? 0 : 1)));
-                    const int dz = q < 5 ? 0 : 1;
-                    if ((dx == 0 || (dx < 0 ? xl : xh)) && (dy == 0 || (dy < 0 ? yl : yh)) && (dz == 0 || zh)) {
+                for (int k = 0; k < kRangesWrap; ++k) {
+                    const int q = k + pass * kRangesWrap;
+                    const int dx = (int)((kStX >> (2 * q)) & 3u) - 1, dy = (int)((kStY >> (2 * q)) & 3u) - 1,
+                              dz = (int)((kStZ >> (2 * q)) & 3u) - 1;
+                    if (q == 0) {
+                        beg[0] = si + 1;
+                        len[0] = c1 - beg[0];
+                    } else if ((dx == 0 || (dx < 0 ? xl : xh)) && (dy == 0 || (dy < 0 ? yl : yh)) && (dz == 0 || zh)) {
                         int ax = cx + dx, ay = cy + dy, az = cz + dz;
                         ax = ax < 0 ? n - 1 : (ax >= n ? 0 : ax);
                         ay = ay < 0 ? n - 1 : (ay >= n ? 0 : ay);
@@ -515,10 +530,11 @@ __device__ __forceinline__ void sparse_chunk(const float4 *__restrict__ sorted, 
     }
     if (!__any_sync(kFull, live)) return;
     if (__any_sync(kFull, needwrap)) {
-        sparse_warp<true, 0>(sorted, cell_start, rel, idx_s, si, live, home, c1, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
-        sparse_warp<true, 1>(sorted, cell_start, rel, idx_s, si, live, home, c1, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
+#pragma unroll 1
+        for (int pass = 0; pass < 2; ++pass)
+            sparse_warp<true>(sorted, cell_start, rel, idx_s, si, live, home, c1, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests, pass);
     } else {
-        sparse_warp<false, 0>(sorted, cell_start, rel, idx_s, si, live, home, c1, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests);
+        sparse_warp<false>(sorted, cell_start, rel, idx_s, si, live, home, c1, me, cx, cy, cz, fx, fy, fz, g, sm, lane, nedges, ntests, 0);
     }
 }
 
