@@ -265,11 +265,17 @@ __device__ __forceinline__ void tile_item(const float4 *__restrict__ sorted, con
     const unsigned int adj = batch_adjacency<false>(me, s_pj, cntI, g, lane) & ~(1u << lane);
     nedges += (unsigned int)__popc(adj & lanemask_lt());
     if (lane == 0) ntests += (unsigned int)(cntI * (cntI - 1) / 2);
-    int lab = lane;  // lowest lane of my component inside the tile
+    // Components of the tile: breadth-first from the lowest unlabelled lane, one warp OR-reduction
+    // per level.  Lanes without a link are their own component and are never visited.  `head` is
+    // the member with the smallest original index (the union-find's order): every other member
+    // hooks straight under it, depth one, no retries.  (A parent that is no longer a root is fine:
+    // original indices still fall along every path.)
+    const unsigned int self = 1u << lane;
+    unsigned int grp = self;
+    int head = lane;
     if (__any_sync(kFull, adj != 0u)) {
-        // breadth-first from the lowest unlabelled lane; one warp OR-reduction per level
-        const unsigned int self = 1u << lane;
-        unsigned int todo = __ballot_sync(kFull, adj != 0u);  // lanes without a link are their own component
+        const int my_oi = lane < cntI ? __ldg(idx_s + ib + lane) : 0x7fffffff;
+        unsigned int todo = __ballot_sync(kFull, adj != 0u);
         while (todo) {
             const int r = __ffs((int)todo) - 1;
             unsigned int vis = 1u << r;
@@ -278,18 +284,14 @@ __device__ __forceinline__ void tile_item(const float4 *__restrict__ sorted, con
                 if (nxt == vis) break;
                 vis = nxt;
             }
-            if (vis & self) lab = r;
+            const bool in = (vis & self) != 0u;
+            const int m = __reduce_min_sync(kFull, in ? my_oi : 0x7fffffff);
+            const unsigned int hb = __ballot_sync(kFull, in && my_oi == m);
+            if (in) { grp = vis; head = __ffs((int)hb) - 1; }
             todo &= ~vis;
         }
     }
-    // every member hooks straight under the member of its component with the smallest original index
-    // (the union-find's order): no retries, depth one
-    const unsigned int grp = __match_any_sync(kFull, lab);
-    const int my_oi = lane < cntI ? __ldg(idx_s + ib + lane) : 0x7fffffff;
-    const int min_oi = __reduce_min_sync(grp, my_oi);
-    const int head = __ffs((int)(__ballot_sync(kFull, my_oi == min_oi) & grp)) - 1;
     const bool leader = head == lane;
-    // (a parent that is no longer a root is fine: original indices still fall along every path)
     if (!leader && atomicCAS(rel + ib + lane, 0u, (unsigned int)(lane - head)) != 0u)
         unite_rel(rel, idx_s, ib + lane, ib + head);  // somebody hooked me first: general path
 
