@@ -52,6 +52,13 @@ def _load():
         lib.oracle_groups.restype = ctypes.c_int64
         lib.oracle_groups.argtypes = [f32p, f32p, i32p, ctypes.c_int64, ctypes.c_float, ctypes.c_int32,
                                       ctypes.c_int64, i32p, i32p, f64p, f64p, i32p]
+        f64p_ = ctypes.POINTER(ctypes.c_double)
+        lib.oracle_group_sigma.restype = ctypes.c_int
+        lib.oracle_group_sigma.argtypes = [f32p, f32p, i32p, ctypes.c_int64, ctypes.c_float, ctypes.c_int64, f64p_,
+                                           f64p_]
+        lib.oracle_groups_backward.restype = ctypes.c_int
+        lib.oracle_groups_backward.argtypes = [f32p, f32p, i32p, ctypes.c_int64, ctypes.c_float, ctypes.c_int64,
+                                               f64p_, f64p_, f64p_, f64p_, f64p_, f64p_]
         lib.oracle_pref.restype = ctypes.c_int
         lib.oracle_pref.argtypes = [f32p, ctypes.c_int64, ctypes.c_float, ctypes.c_float, u64p]
         lib.oracle_linking_length.restype = ctypes.c_float
@@ -144,6 +151,49 @@ def groups(pos, labels, L: float, N_min: int, mass=None):
     K = int(K)
     return dict(K=K, group_label=gl[:K].copy(), group_size=gs[:K].copy(), group_mass=gm[:K].copy(),
                 group_com=gc[:K].copy(), particle_group=pg)
+
+
+def _f64(a):
+    if a is None:
+        return None, None
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def group_sigma(pos, particle_group, L: float, group_com, mass=None) -> np.ndarray:
+    """sigma_g = sqrt(sum m |min-image(w_i - X_g)|^2 / M_g), float64 [K] (section 3.1.1, reading R23)."""
+    pos, p = _pos(pos)
+    pg = np.ascontiguousarray(particle_group, dtype=np.int32)
+    gc, gcp = _f64(group_com)
+    K = gc.shape[0]
+    out = np.zeros(max(K, 1), np.float64)
+    mp = None
+    if mass is not None:
+        mass, mp = _f32(mass)
+    _check(_load().oracle_group_sigma(p, mp, pg.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), pos.shape[0], _f(L),
+                                      K, gcp, out.ctypes.data_as(ctypes.POINTER(ctypes.c_double))))
+    return out[:K]
+
+
+def groups_backward(pos, particle_group, L: float, group_mass, group_com, grad_com, group_sigma=None,
+                    grad_sigma=None, mass=None) -> np.ndarray:
+    """Frozen-assignment backward (Eq. 4; Eq. 5 through sigma): float64 [N,3]."""
+    pos, p = _pos(pos)
+    N = pos.shape[0]
+    pg = np.ascontiguousarray(particle_group, dtype=np.int32)
+    gm, gmp = _f64(group_mass)
+    gc, gcp = _f64(group_com)
+    gs, gsp = _f64(group_sigma)
+    dx, dxp = _f64(grad_com)
+    ds, dsp = _f64(grad_sigma)
+    out = np.zeros((max(N, 1), 3), np.float64)
+    mp = None
+    if mass is not None:
+        mass, mp = _f32(mass)
+    _check(_load().oracle_groups_backward(p, mp, pg.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), N, _f(L),
+                                          gm.shape[0], gmp, gcp, gsp, dxp, dsp,
+                                          out.ctypes.data_as(ctypes.POINTER(ctypes.c_double))))
+    return out[:N]
 
 
 def pref(pos, L: float, b: float) -> int:

@@ -281,6 +281,83 @@ int64_t oracle_groups(const float *pos, const float *mass, const int32_t *labels
     return K;
 }
 
+/* ---- NEXT-1: halo decoration and frozen-assignment backward ------------------
+ * PAPER.md:255-261 (section 3.1 "Frozen Assignment", Eq. 4): membership is held fixed and
+ *     X^h = (1/N) sum_i x_i   ->   dX^h/dtheta = (1/N) sum_i dx_i/dtheta,
+ * i.e. dL/dx_i = (m_i / M_g) dL/dX_g for a member i of group g (mass-weighted as the forward is,
+ * DESIGN.md R12) and 0 for a particle of a dropped group.
+ * PAPER.md:283-290 (section 3.1.1 "Decorated Frozen Assignment", Eq. 5): the decoration is the
+ * "particle standard deviation (sigma)" of a halo.  The paper gives no formula; reading R23
+ * (DESIGN.md): sigma_g = sqrt( sum_i m_i |delta_i|^2 / M_g ) with delta_i the minimum-image
+ * displacement of member i from the periodic centre of mass X_g, all in float64.  Its derivative
+ * at fixed membership is d sigma_g / d x_i = (m_i / (M_g sigma_g)) delta_i (the terms through X_g
+ * cancel because sum_i m_i delta_i = 0); it is taken as 0 where sigma_g = 0.
+ * Both functions follow the definition with one plain pass over the particles.
+ * Pins (tests/test_oracle_next1.py): numpy mean / std for groups away from the box faces,
+ * translation across a face, closed forms (unit masses: gradient = G/N_g), and central finite
+ * differences of an independent numpy forward.                                                  */
+int oracle_group_sigma(const float *pos, const float *mass, const int32_t *particle_group, int64_t N, float L,
+                       int64_t K, const double *group_com, double *group_sigma)
+{
+    if (N < 0 || K < 0 || !(L > 0.0f)) return ORACLE_ERR_ARG;
+    float *w = (float *)malloc(sizeof(float) * 3 * (size_t)(N > 0 ? N : 1));
+    double *sq = (double *)calloc((size_t)(K > 0 ? K : 1) * 2, sizeof(double));
+    if (!w || !sq) { free(w); free(sq); return ORACLE_ERR_NOMEM; }
+    int rc = oracle_wrap(pos, N, L, w);
+    if (rc) { free(w); free(sq); return rc; }
+    const double Ld = (double)L, hd = 0.5 * (double)L;
+    for (int64_t i = 0; i < N; ++i) {
+        const int32_t k = particle_group[i];
+        if (k < 0) continue;
+        if (k >= K) { free(w); free(sq); return ORACLE_ERR_ARG; }
+        const double m = mass ? (double)mass[i] : 1.0;
+        double d2 = 0.0;
+        for (int a = 0; a < 3; ++a) {
+            double d = (double)w[3 * i + a] - group_com[3 * k + a];
+            if (d > hd) d = d - Ld; else if (d < -hd) d = d + Ld;
+            d2 += d * d;
+        }
+        sq[2 * k] += m * d2;
+        sq[2 * k + 1] += m;
+    }
+    for (int64_t k = 0; k < K; ++k) group_sigma[k] = sq[2 * k + 1] > 0.0 ? sqrt(sq[2 * k] / sq[2 * k + 1]) : 0.0;
+    free(w); free(sq);
+    return ORACLE_OK;
+}
+
+int oracle_groups_backward(const float *pos, const float *mass, const int32_t *particle_group, int64_t N, float L,
+                           int64_t K, const double *group_mass, const double *group_com,
+                           const double *group_sigma, const double *grad_com, const double *grad_sigma,
+                           double *grad_pos)
+{
+    if (N < 0 || K < 0 || !(L > 0.0f)) return ORACLE_ERR_ARG;
+    if (grad_sigma && !group_sigma) return ORACLE_ERR_ARG;
+    float *w = (float *)malloc(sizeof(float) * 3 * (size_t)(N > 0 ? N : 1));
+    if (!w) return ORACLE_ERR_NOMEM;
+    int rc = oracle_wrap(pos, N, L, w);
+    if (rc) { free(w); return rc; }
+    const double Ld = (double)L, hd = 0.5 * (double)L;
+    for (int64_t i = 0; i < N; ++i) {
+        const int32_t k = particle_group[i];
+        for (int a = 0; a < 3; ++a) grad_pos[3 * i + a] = 0.0;
+        if (k < 0) continue;
+        if (k >= K) { free(w); return ORACLE_ERR_ARG; }
+        const double m = mass ? (double)mass[i] : 1.0;
+        const double wgt = m / group_mass[k];
+        for (int a = 0; a < 3; ++a) {
+            double g = grad_com ? wgt * grad_com[3 * k + a] : 0.0;
+            if (grad_sigma && group_sigma[k] > 0.0) {
+                double d = (double)w[3 * i + a] - group_com[3 * k + a];
+                if (d > hd) d = d - Ld; else if (d < -hd) d = d + Ld;
+                g += grad_sigma[k] * wgt * d / group_sigma[k];
+            }
+            grad_pos[3 * i + a] = g;
+        }
+    }
+    free(w);
+    return ORACLE_OK;
+}
+
 /* ---- P_ref: candidate pairs of the linked-cell method on the tightest grid n_ref = floor(L/b) ---
  * (27-cell stencil, each unordered particle pair counted once).  Metric denominator only
  * (DESIGN.md §6); sorted keys + run lengths, no dense cell array.                               */
