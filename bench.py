@@ -248,6 +248,37 @@ def run_ours(args):
     ms_step = max_over_ranks_ms(ms_total, world, dev) / args.steps
     value = whole_job_value(world, N, ms_step)
 
+    # ---- NEXT-1: halo decoration sigma + frozen-assignment backward, timed on their own
+    # (not part of the step: the BASELINE metric is fof_link + fof_groups)
+    next1 = None
+    if not args.no_next1:
+        og = f.groups(dpos, labels, particle_group=True)
+        Kk = og["K"]
+        gcom = torch.randn((max(Kk, 1), 3), device=dev)[:Kk]
+        gsig = torch.randn(max(Kk, 1), device=dev)[:Kk]
+        for _ in range(2):
+            sig = f.group_sigma(dpos, og)
+            gp = f.groups_backward(dpos, og, grad_com=gcom, group_sigma=sig, grad_sigma=gsig)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        reps = 10
+        torch.cuda.synchronize()
+        ev[0].record(stream)
+        for _ in range(reps):
+            sig = f.group_sigma(dpos, og)
+        ev[1].record(stream)
+        for _ in range(reps):
+            gp = f.groups_backward(dpos, og, grad_com=gcom, group_sigma=sig, grad_sigma=gsig)
+        ev[2].record(stream)
+        torch.cuda.synchronize()
+        t_sig, t_bwd = ev[0].elapsed_time(ev[1]) / reps, ev[1].elapsed_time(ev[2]) / reps
+        pk = peaks()[0]
+        next1 = {"sigma_ms": t_sig, "backward_ms": t_bwd,
+                 "sigma_alg_GBps": 16 * N / (t_sig * 1e-3) / 1e9, "backward_alg_GBps": 28 * N / (t_bwd * 1e-3) / 1e9,
+                 "sigma_frac_of_hbm_peak": 16 * N / (t_sig * 1e-3) / 1e9 / pk,
+                 "backward_frac_of_hbm_peak": 28 * N / (t_bwd * 1e-3) / 1e9 / pk,
+                 "alg_bytes": "sigma: pos 12 + group id 4 per particle; backward: pos 12 + group id 4 + grad 12"}
+        del gp, sig, og
+
     # ---- end to end: host buffers through the C ABI (fof_run_host), copies inside the timed region
     cap = out["cap"]
     h2 = B.fof_create(N, w.L, w.b, w.N_min)
@@ -345,7 +376,7 @@ def run_ours(args):
         "e2e": {"value": whole_job_value(world, N, e2e_ms), "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
                 "h2d_bytes_per_step": int(hpos.numel() * 4),
                 "d2h_bytes_per_step": int(N * 4 + Kh * (4 + 4 + 4 + 12) + 8)},
-        "gpu_launches": int(launches), "clocks": clk.summary(),
+        "gpu_launches": int(launches), "clocks": clk.summary(), "next1": next1,
     }
     print(json.dumps(line), flush=True)
     if world > 1:
@@ -361,6 +392,7 @@ def main():
     ap.add_argument("--workload", default="cfg2", choices=sorted(inputs.CONFIGS))
     ap.add_argument("--grid", type=int, default=None, help="force n cells per axis (tuning knob)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-next1", action="store_true", help="skip the sigma / backward timing")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -97,6 +97,29 @@ int fof_groups(fof_handle *h, const float *pos, const float *mass, const int32_t
                int32_t *group_label, int32_t *group_size, float *group_mass, float *group_com,
                int32_t *particle_group, int64_t cap, int64_t *K_host, void *stream);
 
+/* Halo decoration (section 3.1.1 "Decorated Frozen Assignment": "particle standard deviation
+ * (sigma)" as the surrogate of halo mass; R23):
+ *   group_sigma[k] = sqrt( sum_i m_i |delta_i|^2 / M_k ),  delta_i = minimum-image displacement of
+ * member i from group_com[k], accumulated in float64.  Downstream of fof_groups: particle_group,
+ * group_mass, group_com are its outputs (dev), K its *K_host.  `ws` as in fof_groups (scratch).
+ *   group_sigma  dev [K] float32, written.
+ * Asynchronous on `stream`. */
+int fof_group_sigma(fof_handle *h, const float *pos, const float *mass, const int32_t *particle_group,
+                    const float *group_mass, const float *group_com, int64_t K, void *ws, float *group_sigma,
+                    void *stream);
+
+/* Frozen-assignment backward (section 3.1, Eq. 4: dX^h/dtheta = (1/N) sum_i dx_i/dtheta;
+ * Eq. 5 for the decoration; R24).  Membership is held fixed:
+ *   grad_pos[i] = (m_i / M_k) (grad_com[k] + grad_sigma[k] delta_i / group_sigma[k]),  k = particle_group[i],
+ * and 0 for a particle of a dropped group (k < 0); the sigma term is 0 where group_sigma[k] = 0.
+ *   grad_com    dev [K,3] float32 dL/dX_k, or NULL (= 0)
+ *   grad_sigma  dev [K] float32 dL/dsigma_k, or NULL (= 0; then group_sigma may be NULL too)
+ *   grad_pos    dev [N,3] float32, written (every element).
+ * Asynchronous on `stream`; needs no workspace. */
+int fof_groups_backward(fof_handle *h, const float *pos, const float *mass, const int32_t *particle_group,
+                        const float *group_mass, const float *group_com, const float *group_sigma,
+                        const float *grad_com, const float *grad_sigma, int64_t K, float *grad_pos, void *stream);
+
 /* Host-buffer entry point (the end-to-end call): copies pos (and mass) host -> device, runs
  * fof_link + fof_groups, copies labels and the K group records device -> host.
  *   *_host  host buffers (pinned for full copy speed); mass_host / particle_group_host may be NULL.

@@ -60,6 +60,10 @@ def lib():
                                      ctypes.POINTER(ctypes.c_uint64)]
         L.fof_groups.restype = ctypes.c_int
         L.fof_groups.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, ctypes.POINTER(i64), vp]
+        L.fof_group_sigma.restype = ctypes.c_int
+        L.fof_group_sigma.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp]
+        L.fof_groups_backward.restype = ctypes.c_int
+        L.fof_groups_backward.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, vp, vp]
         L.fof_host_device_bytes.restype = ctypes.c_size_t
         L.fof_host_device_bytes.argtypes = [vp, i64]
         L.fof_run_host.restype = ctypes.c_int
@@ -156,6 +160,18 @@ def fof_groups(h, pos, mass, labels, ws, group_label, group_size, group_mass, gr
                             _ptr(group_mass), _ptr(group_com), _ptr(particle_group), int(cap), ctypes.byref(K),
                             _stream_ptr(stream)), h)
     return int(K.value)
+
+
+def fof_group_sigma(h, pos, mass, particle_group, group_mass, group_com, K, ws, group_sigma, stream=None):
+    _check(lib().fof_group_sigma(h, _ptr(pos), _ptr(mass), _ptr(particle_group), _ptr(group_mass), _ptr(group_com),
+                                 int(K), _ptr(ws), _ptr(group_sigma), _stream_ptr(stream)), h)
+
+
+def fof_groups_backward(h, pos, mass, particle_group, group_mass, group_com, group_sigma, grad_com, grad_sigma, K,
+                        grad_pos, stream=None):
+    _check(lib().fof_groups_backward(h, _ptr(pos), _ptr(mass), _ptr(particle_group), _ptr(group_mass),
+                                     _ptr(group_com), _ptr(group_sigma), _ptr(grad_com), _ptr(grad_sigma), int(K),
+                                     _ptr(grad_pos), _stream_ptr(stream)), h)
 
 
 def fof_host_device_bytes(h, cap: int) -> int:
@@ -261,6 +277,27 @@ class FoF:
                    group_mass=torch.empty(cap, dtype=torch.float32, device=d),
                    group_com=torch.empty((cap, 3), dtype=torch.float32, device=d),
                    particle_group=torch.empty(self.N, dtype=torch.int32, device=d) if particle_group else None)
+        return out
+
+    def group_sigma(self, pos, g, mass=None, stream=None):
+        """Halo decoration sigma [K] of the groups `g` returned by groups(..., particle_group=True)."""
+        import torch
+
+        K = g["K"]
+        sig = torch.empty(K, dtype=torch.float32, device=pos.device)
+        with torch.cuda.device(self.device):
+            fof_group_sigma(self.h, pos, mass, g["particle_group"], g["group_mass"], g["group_com"], K, self.ws, sig,
+                            stream)
+        return sig
+
+    def groups_backward(self, pos, g, grad_com=None, group_sigma=None, grad_sigma=None, mass=None, stream=None):
+        """Frozen-assignment backward: grad_pos [N,3] from dL/dX [K,3] (and dL/dsigma [K])."""
+        import torch
+
+        out = torch.empty((self.N, 3), dtype=torch.float32, device=pos.device)
+        with torch.cuda.device(self.device):
+            fof_groups_backward(self.h, pos, mass, g["particle_group"], g["group_mass"], g["group_com"], group_sigma,
+                                grad_com, grad_sigma, g["K"], out, stream)
         return out
 
     def groups(self, pos, labels, mass=None, out=None, particle_group=False, stream=None):

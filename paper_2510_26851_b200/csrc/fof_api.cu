@@ -334,6 +334,35 @@ int fof_groups(fof_handle *h, const float *pos, const float *mass, const int32_t
     return FOF_OK;
 }
 
+int fof_group_sigma(fof_handle *h, const float *pos, const float *mass, const int32_t *particle_group,
+                    const float *group_mass, const float *group_com, int64_t K, void *ws, float *group_sigma,
+                    void *stream)
+{
+    if (!h || !ws || ((uintptr_t)ws & 255) || K < 0 || K > h->max_groups) return FOF_ERR_INVALID_ARG;
+    if (h->N > 0 && (!pos || !particle_group)) return FOF_ERR_INVALID_ARG;
+    if (K > 0 && (!group_mass || !group_com || !group_sigma)) return FOF_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    h->launches += K > 0 ? 2 : 0;
+    CK(launch_group_sigma(pos, mass, particle_group, h->N, h->grid, group_mass, group_com, K,
+                          at<double>(ws, h->off_acc), group_sigma, s), "sigma kernels");
+    return FOF_OK;
+}
+
+int fof_groups_backward(fof_handle *h, const float *pos, const float *mass, const int32_t *particle_group,
+                        const float *group_mass, const float *group_com, const float *group_sigma,
+                        const float *grad_com, const float *grad_sigma, int64_t K, float *grad_pos, void *stream)
+{
+    if (!h || K < 0) return FOF_ERR_INVALID_ARG;
+    if (h->N > 0 && (!pos || !particle_group || !grad_pos)) return FOF_ERR_INVALID_ARG;
+    if (K > 0 && (!group_mass || !group_com)) return FOF_ERR_INVALID_ARG;
+    if (grad_sigma && !group_sigma) return FOF_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    h->launches += h->N > 0 ? 1 : 0;
+    CK(launch_groups_backward(pos, mass, particle_group, h->N, h->grid, group_mass, group_com, group_sigma, grad_com,
+                              grad_sigma, K, grad_pos, s), "groups_backward_kernel");
+    return FOF_OK;
+}
+
 size_t fof_host_device_bytes(const fof_handle *h, int64_t cap)
 {
     if (!h || cap < 0) return 0;

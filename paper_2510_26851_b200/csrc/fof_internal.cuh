@@ -70,6 +70,8 @@ __host__ __device__ __forceinline__ unsigned int dense_tile_size(unsigned int m)
     return T <= 16u ? (m + T - 1u) / T : 32u;
 }
 
+
+
 }  // namespace fof
 
 namespace fof {
@@ -77,6 +79,8 @@ struct SortPlan {
     int shift;  // cells per bin = 2^shift
     int bins;   // ceil(C / 2^shift) <= kMaxBins
 };
+
+
 }  // namespace fof
 
 struct fof_handle {
@@ -191,5 +195,14 @@ cudaError_t launch_group_reduce(const float *pos, const float *mass, const int *
 cudaError_t launch_group_finish(const float *pos, const int *group_label, const int *group_size,
                                 const double *acc, bool has_mass, Grid g, int64_t cap, const Ctrl *ctrl,
                                 float *group_mass, float *group_com, cudaStream_t s);
+
+
+cudaError_t launch_group_sigma(const float *pos, const float *mass, const int *particle_group, int64_t N, Grid g,
+                               const float *group_mass, const float *group_com, int64_t K, double *acc,
+                               float *group_sigma, cudaStream_t s);
+cudaError_t launch_groups_backward(const float *pos, const float *mass, const int *particle_group, int64_t N, Grid g,
+                                   const float *group_mass, const float *group_com, const float *group_sigma,
+                                   const float *grad_com, const float *grad_sigma, int64_t K, float *grad_pos,
+                                   cudaStream_t s);
 
 }  // namespace fof

@@ -399,3 +399,65 @@ def test_stress_full_size_sampled(B):
         both, _ = oracle.labels_brute(p[near], w.L, w.b)
         inside = np.isin(near, mem)
         assert len(set(both[inside])) == 1 and not np.isin(both[~inside], both[inside]).any()
+
+
+# --------------------------------------------------------------------------- NEXT-1: decoration + backward
+@pytest.mark.parametrize("weighted", [False, True])
+def test_sigma_and_backward_against_oracle(B, weighted):
+    """fof_group_sigma / fof_groups_backward (section 3.1 Eq. 4, 3.1.1 Eq. 5) on a clustered set
+    with groups that cross the box faces.  Tolerances: the CUDA path reads the float32 group_com /
+    group_mass / group_sigma that fof_groups / fof_group_sigma wrote (rounded once, <= ulp/2), the
+    oracle its own float64 values; a shift e of the centre changes sigma^2 by |e|^2 only (sum m delta
+    = 0), so sigma agrees to float32 rounding; in the backward, delta / sigma inherits
+    |e| / sigma <= ulp(L) / sigma per axis."""
+    w = inputs.scaled(inputs.CONFIGS["cfg1"], 48)
+    p = inputs.make_positions(w)
+    m = inputs.make_masses(w) if weighted else None
+    lab, _ = oracle.labels_cells(p, w.L, w.b)
+    og = oracle.groups(p, lab, w.L, w.N_min, mass=m)
+    osig = oracle.group_sigma(p, og["particle_group"], w.L, og["group_com"], mass=m)
+    rng = np.random.default_rng(8)
+    K = og["K"]
+    assert K > 50
+    G = rng.standard_normal((K, 3)).astype(np.float32)
+    C = rng.standard_normal(K).astype(np.float32)
+    ograd = oracle.groups_backward(p, og["particle_group"], w.L, og["group_mass"], og["group_com"], G,
+                                   group_sigma=osig, grad_sigma=C, mass=m)
+    ograd_x = oracle.groups_backward(p, og["particle_group"], w.L, og["group_mass"], og["group_com"], G, mass=m)
+
+    f = B.FoF(len(p), w.L, w.b, w.N_min)
+    dpos = torch.from_numpy(p).cuda()
+    dm = None if m is None else torch.from_numpy(m).cuda()
+    labels = f.link(dpos)
+    g = f.groups(dpos, labels, mass=dm, particle_group=True)
+    assert g["K"] == K
+    sig = f.group_sigma(dpos, g, mass=dm)
+    s_gpu = sig.cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(s_gpu - osig) <= 2e-6 * osig + 1e-7 * w.L)
+    dG, dC = torch.from_numpy(G).cuda(), torch.from_numpy(C).cuda()
+    gx = f.groups_backward(dpos, g, grad_com=dG, mass=dm).cpu().numpy().astype(np.float64)
+    assert np.abs(gx - ograd_x).max() <= 2e-6 * np.abs(ograd_x).max()
+    assert (gx[og["particle_group"] < 0] == 0).all()
+    gall = f.groups_backward(dpos, g, grad_com=dG, group_sigma=sig, grad_sigma=dC, mass=dm).cpu().numpy().astype(np.float64)
+    ulp_L = float(np.spacing(np.float32(w.L)))
+    pg = og["particle_group"]
+    member = pg >= 0
+    mm = np.ones(len(p)) if m is None else m.astype(np.float64)
+    wgt = np.zeros(len(p))
+    wgt[member] = mm[member] / og["group_mass"][pg[member]]
+    bound = np.zeros(len(p))
+    bound[member] = 4e-6 * np.abs(ograd).max() + 2.0 * np.abs(C[pg[member]]) * wgt[member] * ulp_L / osig[pg[member]]
+    assert np.all(np.abs(gall - ograd).max(1) <= bound + 1e-30)
+    f.close()
+
+
+def test_backward_without_groups_is_zero(B):
+    rng = np.random.default_rng(12)
+    p = (rng.random((5000, 3)) * 100.0).astype(np.float32)   # sparse: no group reaches N_min
+    f = B.FoF(len(p), 100.0, 0.5, 20)
+    dpos = torch.from_numpy(p).cuda()
+    g = f.groups(dpos, f.link(dpos), particle_group=True)
+    assert g["K"] == 0
+    assert f.group_sigma(dpos, g).numel() == 0
+    assert (f.groups_backward(dpos, g) == 0).all()
+    f.close()
