@@ -379,19 +379,29 @@ __device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, c
         if (live) {
             if (!WRAP) {
                 // the loads below stay inside the row: a lane that needs the cell behind an x face
-                // has sent its whole warp to the WRAP variant
+                // has sent its whole warp to the WRAP variant.  Flags are consumed where they are
+                // computed (short predicate lifetimes).
+                const int off_lo = xl ? -1 : 0, off_hi = xh ? 2 : 1;
                 beg[0] = si + 1;
                 len[0] = (xh ? (int)__ldg(home + 2) : c1) - beg[0];
-                const int nn = n * n;
-                const int off_lo = xl ? -1 : 0, off_hi = xh ? 2 : 1;
-                const bool on[4] = {yh, zh && yl, zh, zh && yh};
-                const int row[4] = {n, nn - n, nn, nn + n};
-#pragma unroll
-                for (int r = 0; r < 4; ++r)
-                    if (on[r]) {
-                        beg[r + 1] = (int)__ldg(home + row[r] + off_lo);
-                        len[r + 1] = (int)__ldg(home + row[r] + off_hi) - beg[r + 1];
+                if (yh) {
+                    const unsigned int *row = home + n;
+                    beg[1] = (int)__ldg(row + off_lo);
+                    len[1] = (int)__ldg(row + off_hi) - beg[1];
+                }
+                if (zh) {
+                    const unsigned int *row = home + n * n;
+                    beg[3] = (int)__ldg(row + off_lo);
+                    len[3] = (int)__ldg(row + off_hi) - beg[3];
+                    if (yl) {
+                        beg[2] = (int)__ldg(row - n + off_lo);
+                        len[2] = (int)__ldg(row - n + off_hi) - beg[2];
                     }
+                    if (yh) {
+                        beg[4] = (int)__ldg(row + n + off_lo);
+                        len[4] = (int)__ldg(row + n + off_hi) - beg[4];
+                    }
+                }
             } else {
 #pragma unroll
                 for (int k = 0; k < kRangesWrap; ++k) {
@@ -444,9 +454,10 @@ __device__ __forceinline__ void sparse_warp(const float4 *__restrict__ sorted, c
     }
     // ---- the rest is flattened: one packed warp scan gives every lane its first slot (low 16 bits)
     // and its first range id (high bits)
-    unsigned int mine = 0;
+    int tot = 0, cnt = 0;  // every len is >= 0
 #pragma unroll
-    for (int r = 0; r < NR; ++r) mine += (unsigned int)len[r] + (len[r] > 0 ? 0x10000u : 0u);
+    for (int r = 0; r < NR; ++r) { tot += len[r]; cnt += min(len[r], 1); }
+    const unsigned int mine = (unsigned int)tot | ((unsigned int)cnt << 16);
     unsigned int incl = mine;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -508,28 +519,22 @@ __device__ __forceinline__ void sparse_chunk(const float4 *__restrict__ sorted, 
     const float lo = g.reach, hi = 1.0f - g.reach;
     const int64_t s64 = base + lane;
     const bool valid = s64 < N;
-    const int si = (int)s64;
-    float4 me = make_float4(0.f, 0.f, 0.f, 0.f);
-    int cx = 0, cy = 0, cz = 0;
-    float fx = 0.5f, fy = 0.5f, fz = 0.5f;
-    bool needwrap = false, live = false;
-    const unsigned int *home = cell_start;
-    int c1 = 0;
-    if (valid) {
-        me = __ldg(sorted + si);
-        const float ux = __fmul_rn(me.x, g.inv_cell), uy = __fmul_rn(me.y, g.inv_cell), uz = __fmul_rn(me.z, g.inv_cell);
-        cx = min(__float2int_rd(ux), g.n_minus_1);
-        cy = min(__float2int_rd(uy), g.n_minus_1);
-        cz = min(__float2int_rd(uz), g.n_minus_1);
-        fx = ux - (float)cx;
-        fy = uy - (float)cy;
-        fz = uz - (float)cz;
-        home = cell_start + cell_id(cx, cy, cz, n);
-        c1 = (int)__ldg(home + 1);
-        live = c1 - (int)__ldg(home) < kDenseCell;  // a dense home cell belongs to the tile role
-        needwrap = live && (n < 6 || (fx < lo && cx == 0) || (fx > hi && cx == n - 1) || (fy < lo && cy == 0) ||
-                            (fy > hi && cy == n - 1) || (fz > hi && cz == n - 1));
-    }
+    const int si = (int)min(s64, N - 1);  // idle lanes of the last chunk shadow the last particle (never live)
+    const float4 me = __ldg(sorted + si);
+    const float ux = __fmul_rn(me.x, g.inv_cell), uy = __fmul_rn(me.y, g.inv_cell), uz = __fmul_rn(me.z, g.inv_cell);
+    const int cx = min(__float2int_rd(ux), g.n_minus_1);
+    const int cy = min(__float2int_rd(uy), g.n_minus_1);
+    const int cz = min(__float2int_rd(uz), g.n_minus_1);
+    const float fx = ux - (float)cx, fy = uy - (float)cy, fz = uz - (float)cz;
+    const unsigned int *home = cell_start + cell_id(cx, cy, cz, n);
+    const int c1 = (int)__ldg(home + 1);
+    const bool live = valid & (c1 - (int)__ldg(home) < kDenseCell);  // a dense home cell belongs to the tile role
+    // wrap is needed if a face I am within reach of is a box face (x: exact test; y, z: any particle of a
+    // boundary row takes the wrapped variant, 3 rows in 256), or if the grid is too small for |d| < L/2
+    const unsigned int edge_yz = ((unsigned int)(cy - 1) >= (unsigned int)(n - 2)) | (unsigned int)(cz == n - 1);
+    const unsigned int edge_x = ((unsigned int)(fx < lo) & (unsigned int)(cx == 0)) |
+                                ((unsigned int)(fx > hi) & (unsigned int)(cx == n - 1));
+    const bool needwrap = live & (((unsigned int)(n < 6) | edge_yz | edge_x) != 0u);
     if (!__any_sync(kFull, live)) return;
     if (__any_sync(kFull, needwrap)) {
 #pragma unroll 1
