@@ -461,3 +461,19 @@ def test_backward_without_groups_is_zero(B):
     assert f.group_sigma(dpos, g).numel() == 0
     assert (f.groups_backward(dpos, g) == 0).all()
     f.close()
+
+
+@pytest.mark.parametrize("grid", [600, 1024])
+def test_large_grids_take_the_wide_bin_paths(B, grid):
+    """n = 600 (2.2e8 cells: bins of 2^13 cells) and n = 1024 (2^30 cells: bins of 2^15 cells, 128 KB of
+    shared-memory counters per CTA): the sort's wide-bin configurations, far more cells than particles."""
+    rng = np.random.default_rng(91)
+    L, b, N_min = 2000.0, 1.0, 5
+    bg = rng.random((150000, 3)) * L
+    centres = rng.random((300, 3)) * L
+    clumps = (centres[:, None, :] + rng.standard_normal((300, 40, 3)) * 0.6).reshape(-1, 3)
+    p = (np.concatenate([bg, clumps]) % L).astype(np.float32)
+    p[p >= np.float32(L)] = 0.0
+    p = p[rng.permutation(len(p))]
+    got, lab, og = check_against_oracle(B, p, L, b, N_min, grid=grid)
+    assert got["grid"][0] == grid and og["K"] >= 250
