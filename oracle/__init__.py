@@ -16,6 +16,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "fof_oracle.c")
+_SRC2 = os.path.join(_HERE, "fof_oracle_stochastic.c")  # NEXT-3: stochastic-edge FoF
 _LIB = os.path.join(_HERE, "libfof_oracle.so")
 # -ffp-contract=off: the float32 link predicate must not be contracted into FMAs.
 CFLAGS = ["-O2", "-std=c99", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC"]
@@ -25,9 +26,10 @@ _lib = None
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (building the checker is not using it)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_SRC2))
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < newest:
         tmp = _LIB + f".tmp{os.getpid()}"
-        subprocess.check_call(["gcc", *CFLAGS, "-o", tmp, _SRC, "-lm"])
+        subprocess.check_call(["gcc", *CFLAGS, "-o", tmp, _SRC, _SRC2, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -59,6 +61,19 @@ def _load():
         lib.oracle_groups_backward.restype = ctypes.c_int
         lib.oracle_groups_backward.argtypes = [f32p, f32p, i32p, ctypes.c_int64, ctypes.c_float, ctypes.c_int64,
                                                f64p_, f64p_, f64p_, f64p_, f64p_, f64p_]
+        f64q = ctypes.POINTER(ctypes.c_double)
+        lib.oracle_sigmoid_fixed.restype = ctypes.c_float
+        lib.oracle_sigmoid_fixed.argtypes = [ctypes.c_float]
+        lib.oracle_rng_u24.restype = ctypes.c_uint32
+        lib.oracle_rng_u24.argtypes = [ctypes.c_uint64, ctypes.c_uint32, ctypes.c_uint32, ctypes.c_uint32]
+        for fn in (lib.oracle_stochastic_brute, lib.oracle_stochastic_cells):
+            fn.restype = ctypes.c_int
+            fn.argtypes = [f32p, ctypes.c_int64, ctypes.c_float, ctypes.c_float, ctypes.c_float, ctypes.c_float,
+                           ctypes.c_uint64, ctypes.c_uint32, i32p, f64q, f64q, u64p, u64p]
+        lib.oracle_stochastic_edges.restype = ctypes.c_int64
+        lib.oracle_stochastic_edges.argtypes = [f32p, ctypes.c_int64, ctypes.c_float, ctypes.c_float, ctypes.c_float,
+                                                ctypes.c_float, ctypes.c_uint64, ctypes.c_uint32, ctypes.c_int64,
+                                                i32p, i32p, f32p]
         lib.oracle_pref.restype = ctypes.c_int
         lib.oracle_pref.argtypes = [f32p, ctypes.c_int64, ctypes.c_float, ctypes.c_float, u64p]
         lib.oracle_linking_length.restype = ctypes.c_float
@@ -194,6 +209,51 @@ def groups_backward(pos, particle_group, L: float, group_mass, group_com, grad_c
                                           gm.shape[0], gmp, gcp, gsp, dxp, dsp,
                                           out.ctypes.data_as(ctypes.POINTER(ctypes.c_double))))
     return out[:N]
+
+
+def sigmoid_fixed(t: float) -> float:
+    """The fixed float32 logistic of reading R26 (NEXT-3)."""
+    return float(_load().oracle_sigmoid_fixed(_f(t)))
+
+
+def rng_u24(seed: int, sample: int, lo: int, hi: int) -> int:
+    """24 random bits of the counter-based generator of reading R27 (NEXT-3)."""
+    return int(_load().oracle_rng_u24(int(seed), int(sample), int(lo), int(hi)))
+
+
+def stochastic(pos, L: float, b_cand: float, b_link: float, alpha: float, seed: int, sample: int, brute=False,
+               want_grad=True):
+    """One Monte Carlo sample of stochastic-edge FoF (Eq. 8): dict(labels, logp, grad [N,3] f64,
+    n_cand, n_edge)."""
+    pos, p = _pos(pos)
+    N = pos.shape[0]
+    labels = np.empty(max(N, 1), np.int32)
+    grad = np.zeros((max(N, 1), 3), np.float64) if want_grad else None
+    logp = ctypes.c_double(0.0)
+    nc, ne = ctypes.c_uint64(0), ctypes.c_uint64(0)
+    fn = _load().oracle_stochastic_brute if brute else _load().oracle_stochastic_cells
+    f64q = ctypes.POINTER(ctypes.c_double)
+    _check(fn(p, N, _f(L), _f(b_cand), _f(b_link), _f(alpha), int(seed), int(sample),
+              labels.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), ctypes.byref(logp),
+              grad.ctypes.data_as(f64q) if want_grad else None, ctypes.byref(nc), ctypes.byref(ne)))
+    return dict(labels=labels[:N], logp=float(logp.value), grad=None if grad is None else grad[:N],
+                n_cand=int(nc.value), n_edge=int(ne.value))
+
+
+def stochastic_edges(pos, L: float, b_cand: float, b_link: float, alpha: float, seed: int, sample: int):
+    """Potential edges of one sample (tiny inputs): (ij int32 [P,2], y int32 [P], p float32 [P])."""
+    pos, pp = _pos(pos)
+    N = pos.shape[0]
+    cap = max(1, N * (N - 1) // 2)
+    ij = np.empty((cap, 2), np.int32)
+    y = np.empty(cap, np.int32)
+    pr = np.empty(cap, np.float32)
+    i32p = ctypes.POINTER(ctypes.c_int32)
+    k = _load().oracle_stochastic_edges(pp, N, _f(L), _f(b_cand), _f(b_link), _f(alpha), int(seed), int(sample), cap,
+                                        ij.ctypes.data_as(i32p), y.ctypes.data_as(i32p),
+                                        pr.ctypes.data_as(ctypes.POINTER(ctypes.c_float)))
+    k = int(_check(k))
+    return ij[:k].copy(), y[:k].copy(), pr[:k].copy()
 
 
 def pref(pos, L: float, b: float) -> int:
