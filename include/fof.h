@@ -97,6 +97,24 @@ int fof_groups(fof_handle *h, const float *pos, const float *mass, const int32_t
                int32_t *group_label, int32_t *group_size, float *group_mass, float *group_com,
                int32_t *particle_group, int64_t cap, int64_t *K_host, void *stream);
 
+/* Stochastic-edge FoF, one Monte Carlo sample (section 3.2, Eq. 6-8; R25-R28).
+ * Every pair of particles closer than the plan's linking length (fof_create's `b`, here the
+ * CANDIDATE radius) is a potential edge, kept with probability
+ *     p = sigma(alpha (b_link^2 - d^2) / b_link^2),   0 < b_link <= b,
+ * (sigma: logistic by a fixed float32 recipe; the decision u < p uses a counter-based generator
+ * keyed on (seed, sample, the pair's original indices), so it does not depend on the device or
+ * the traversal).  Must follow a fof_link on the same (h, ws): it re-uses that call's cell-sorted
+ * arrays, so S samples share one binning; it overwrites the union-find state and the counters of
+ * fof_link_stats (edges = sampled edges, pair tests = potential edges of this sample).
+ *   labels    dev [N] int32, written: minimum original index of the particle's component in the
+ *             sampled graph.
+ *   logp      dev, one float64, written: log p(y) = sum over potential edges of
+ *             y log p + (1 - y) log(1 - p).
+ *   grad_pos  dev [N,3] float32 or NULL: d log p(y) / d pos (the score function of Eq. 7).
+ * Asynchronous on `stream`.  FOF_ERR_STATE without a preceding fof_link on (h, ws). */
+int fof_link_stochastic(fof_handle *h, float b_link, float alpha, uint64_t seed, uint32_t sample, int32_t *labels,
+                        double *logp, float *grad_pos, void *ws, void *stream);
+
 /* Halo decoration (section 3.1.1 "Decorated Frozen Assignment": "particle standard deviation
  * (sigma)" as the surrogate of halo mass; R23):
  *   group_sigma[k] = sqrt( sum_i m_i |delta_i|^2 / M_k ),  delta_i = minimum-image displacement of

@@ -60,6 +60,8 @@ def lib():
                                      ctypes.POINTER(ctypes.c_uint64)]
         L.fof_groups.restype = ctypes.c_int
         L.fof_groups.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, ctypes.POINTER(i64), vp]
+        L.fof_link_stochastic.restype = ctypes.c_int
+        L.fof_link_stochastic.argtypes = [vp, f32, f32, ctypes.c_uint64, ctypes.c_uint32, vp, vp, vp, vp, vp]
         L.fof_group_sigma.restype = ctypes.c_int
         L.fof_group_sigma.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp]
         L.fof_groups_backward.restype = ctypes.c_int
@@ -160,6 +162,12 @@ def fof_groups(h, pos, mass, labels, ws, group_label, group_size, group_mass, gr
                             _ptr(group_mass), _ptr(group_com), _ptr(particle_group), int(cap), ctypes.byref(K),
                             _stream_ptr(stream)), h)
     return int(K.value)
+
+
+def fof_link_stochastic(h, b_link, alpha, seed, sample, labels, logp, grad_pos, ws, stream=None):
+    """labels: cuda int32 [N]; logp: cuda float64 [1]; grad_pos: cuda float32 [N,3] or None."""
+    _check(lib().fof_link_stochastic(h, _f(b_link), _f(alpha), int(seed), int(sample), _ptr(labels), _ptr(logp),
+                                     _ptr(grad_pos), _ptr(ws), _stream_ptr(stream)), h)
 
 
 def fof_group_sigma(h, pos, mass, particle_group, group_mass, group_com, K, ws, group_sigma, stream=None):
@@ -278,6 +286,18 @@ class FoF:
                    group_com=torch.empty((cap, 3), dtype=torch.float32, device=d),
                    particle_group=torch.empty(self.N, dtype=torch.int32, device=d) if particle_group else None)
         return out
+
+    def link_stochastic(self, b_link, alpha, seed, sample, want_grad=True, stream=None):
+        """One stochastic-edge sample on the binning of the last link(): (labels, logp tensor, grad or None)."""
+        import torch
+
+        d = self.device
+        labels = torch.empty(self.N, dtype=torch.int32, device=d)
+        logp = torch.zeros(1, dtype=torch.float64, device=d)
+        grad = torch.empty((self.N, 3), dtype=torch.float32, device=d) if want_grad else None
+        with torch.cuda.device(d):
+            fof_link_stochastic(self.h, b_link, alpha, seed, sample, labels, logp, grad, self.ws, stream)
+        return labels, logp, grad
 
     def group_sigma(self, pos, g, mass=None, stream=None):
         """Halo decoration sigma [K] of the groups `g` returned by groups(..., particle_group=True)."""

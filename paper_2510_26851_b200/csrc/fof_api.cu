@@ -334,6 +334,21 @@ int fof_groups(fof_handle *h, const float *pos, const float *mass, const int32_t
     return FOF_OK;
 }
 
+int fof_link_stochastic(fof_handle *h, float b_link, float alpha, uint64_t seed, uint32_t sample, int32_t *labels,
+                        double *logp, float *grad_pos, void *ws, void *stream)
+{
+    if (!h || !ws || ((uintptr_t)ws & 255) || !logp) return FOF_ERR_INVALID_ARG;
+    if (!(b_link > 0.0f) || !(b_link <= h->b) || !isfinite(alpha)) return FOF_ERR_INVALID_ARG;
+    if (h->N > 0 && !labels) return FOF_ERR_INVALID_ARG;
+    if (!h->linked || h->linked_ws != ws) return FOF_ERR_STATE;  // needs the sort of a fof_link on (h, ws)
+    cudaStream_t s = (cudaStream_t)stream;
+    h->launches += h->N > 0 ? 3 : 0;
+    CK(launch_link_stochastic(at<float4>(ws, h->off_sorted), h->N, h->grid, at<unsigned int>(ws, h->off_cell),
+                              at<int>(ws, h->off_idx), at<unsigned int>(ws, h->off_rel), b_link, alpha, seed, sample,
+                              labels, logp, grad_pos, at<Ctrl>(ws, h->off_ctrl), s), "stochastic link kernels");
+    return FOF_OK;
+}
+
 int fof_group_sigma(fof_handle *h, const float *pos, const float *mass, const int32_t *particle_group,
                     const float *group_mass, const float *group_com, int64_t K, void *ws, float *group_sigma,
                     void *stream)

@@ -153,6 +153,39 @@ __device__ __forceinline__ bool linked(float xi, float yi, float zi, float xj, f
     return d2 <= g.b2;
 }
 
+// ---- union-find on `rel`: rel[s] = s - parent(s) as a signed offset (a root has rel 0, which
+// cell_sort_kernel writes for every slot).  The root of a set is its member with the smallest
+// ORIGINAL index (`idx`), i.e. the canonical label of PAPER.md:91 / 180 itself, so H5 needs no
+// minimum pass: a root hooks under another one only if its original index is the larger of the
+// two (a strict total order: no cycles).  Hooks are atomicCAS(rel + root, 0, offset) and can only
+// succeed on a true root; every plain load may return a stale value, which is always the offset
+// to SOME ancestor (links only ever move up), so staleness costs hops, never correctness.  Plain
+// path-halving stores at non-roots are benign.
+__device__ __forceinline__ int find_rel(unsigned int *rel, int x)
+{
+    int d = (int)rel[x];
+    while (d) {
+        const int p = x - d;
+        const int dp = (int)rel[p];
+        if (dp) rel[x] = (unsigned int)(d + dp);  // halve: x -> grandparent
+        x = p;
+        d = dp;
+    }
+    return x;
+}
+
+__device__ __forceinline__ int unite_rel(unsigned int *rel, const int *__restrict__ idx, int a, int b)
+{
+    int ra = find_rel(rel, a), rb = find_rel(rel, b);
+    while (ra != rb) {
+        if (__ldg(idx + ra) < __ldg(idx + rb)) { const int t = ra; ra = rb; rb = t; }  // ra: larger original index
+        const unsigned int old = atomicCAS(rel + ra, 0u, (unsigned int)(ra - rb));
+        if (old == 0u) return rb;
+        ra = find_rel(rel, ra - (int)old);
+    }
+    return ra;
+}
+
 __device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long *p)
 {
     unsigned long long v;
@@ -204,5 +237,10 @@ cudaError_t launch_groups_backward(const float *pos, const float *mass, const in
                                    const float *group_mass, const float *group_com, const float *group_sigma,
                                    const float *grad_com, const float *grad_sigma, int64_t K, float *grad_pos,
                                    cudaStream_t s);
+
+cudaError_t launch_link_stochastic(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
+                                   const int *idx_s, unsigned int *rel, float b_link, float alpha,
+                                   unsigned long long seed, unsigned int sample, int *labels, double *logp, float *grad,
+                                   Ctrl *ctrl, cudaStream_t s);
 
 }  // namespace fof

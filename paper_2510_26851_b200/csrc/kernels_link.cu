@@ -45,38 +45,7 @@ __device__ __forceinline__ bool linked_t(const float4 &a, const float4 &b, const
     return d2 <= g.b2;
 }
 
-// ---- union-find on `rel`: rel[s] = s - parent(s) as a signed offset (a root has rel 0, which
-// cell_sort_kernel writes for every slot).  The root of a set is its member with the smallest
-// ORIGINAL index (`idx`), i.e. the canonical label of PAPER.md:91 / 180 itself, so H5 needs no
-// minimum pass: a root hooks under another one only if its original index is the larger of the
-// two (a strict total order: no cycles).  Hooks are atomicCAS(rel + root, 0, offset) and can only
-// succeed on a true root; every plain load may return a stale value, which is always the offset
-// to SOME ancestor (links only ever move up), so staleness costs hops, never correctness.  Plain
-// path-halving stores at non-roots are benign.
-__device__ __forceinline__ int find_rel(unsigned int *rel, int x)
-{
-    int d = (int)rel[x];
-    while (d) {
-        const int p = x - d;
-        const int dp = (int)rel[p];
-        if (dp) rel[x] = (unsigned int)(d + dp);  // halve: x -> grandparent
-        x = p;
-        d = dp;
-    }
-    return x;
-}
-
-__device__ __forceinline__ int unite_rel(unsigned int *rel, const int *__restrict__ idx, int a, int b)
-{
-    int ra = find_rel(rel, a), rb = find_rel(rel, b);
-    while (ra != rb) {
-        if (__ldg(idx + ra) < __ldg(idx + rb)) { const int t = ra; ra = rb; rb = t; }  // ra: larger original index
-        const unsigned int old = atomicCAS(rel + ra, 0u, (unsigned int)(ra - rb));
-        if (old == 0u) return rb;
-        ra = find_rel(rel, ra - (int)old);
-    }
-    return ra;
-}
+// (the union-find, find_rel / unite_rel, lives in fof_internal.cuh: kernels_stochastic.cu uses it too)
 
 #ifndef FOF_LINK_MINB
 #define FOF_LINK_MINB 6   // resident CTAs per SM the link kernel is compiled for (register cap)

@@ -477,3 +477,49 @@ def test_large_grids_take_the_wide_bin_paths(B, grid):
     p = p[rng.permutation(len(p))]
     got, lab, og = check_against_oracle(B, p, L, b, N_min, grid=grid)
     assert got["grid"][0] == grid and og["K"] >= 250
+
+
+# --------------------------------------------------------------------------- NEXT-3: stochastic-edge FoF
+@pytest.mark.parametrize("alpha,kappa", [(5.0, 1.5), (0.5, 1.25), (50.0, 1.0)])
+def test_stochastic_link_against_oracle(B, alpha, kappa):
+    """fof_link_stochastic (section 3.2 Eq. 8): labels of every sample and the numbers of potential and
+    sampled edges bit-exact (both sides take u < p on identical float32 bits), log p(y) to float64
+    summation order, the score function to float32 accumulation (atomics, arbitrary order)."""
+    w = inputs.scaled(inputs.CONFIGS["cfg1"], 40)
+    p = inputs.make_positions(w)
+    b_link = w.b
+    b_cand = float(np.float32(kappa * w.b))
+    f = B.FoF(len(p), w.L, b_cand, w.N_min)
+    dpos = torch.from_numpy(p).cuda()
+    f.link(dpos)                                   # the binning every sample re-uses
+    for sample in (0, 1, 7):
+        o = oracle.stochastic(p, w.L, b_cand, b_link, alpha, 1234, sample)
+        labels, logp, grad = f.link_stochastic(b_link, alpha, 1234, sample)
+        E, ncand, _ = f.link_stats()
+        assert ncand == o["n_cand"] and E == o["n_edge"]
+        assert np.array_equal(labels.cpu().numpy(), o["labels"]), "sampled components differ"
+        assert abs(float(logp.item()) - o["logp"]) <= 1e-9 * abs(o["logp"]) + 1e-9
+        g = grad.cpu().numpy().astype(np.float64)
+        assert np.abs(g - o["grad"]).max() <= 2e-5 * np.abs(o["grad"]).max()
+    # samples differ from each other, and a different seed gives a different graph
+    a = f.link_stochastic(b_link, alpha, 1234, 0, want_grad=False)[0]
+    c = f.link_stochastic(b_link, alpha, 1235, 0, want_grad=False)[0]
+    assert alpha >= 50.0 or not torch.equal(a, c)
+    f.close()
+
+
+def test_stochastic_link_wraps_and_needs_a_link_first(B):
+    rng = np.random.default_rng(17)
+    L, b = 8.0, 1.0
+    p = (rng.random((3000, 3)) * L).astype(np.float32)          # n = 5 cells per axis at b_cand = 1.5: every pair wraps
+    f = B.FoF(len(p), L, 1.5, 5)
+    with pytest.raises(B.FofError) as e:
+        f.link_stochastic(b, 3.0, 1, 0)
+    assert e.value.code == B.FOF_ERR_STATE
+    f.link(torch.from_numpy(p).cuda())
+    o = oracle.stochastic(p, L, 1.5, b, 3.0, 1, 0, brute=True)
+    labels, logp, grad = f.link_stochastic(b, 3.0, 1, 0)
+    assert np.array_equal(labels.cpu().numpy(), o["labels"])
+    assert abs(float(logp.item()) - o["logp"]) <= 1e-9 * abs(o["logp"])
+    assert np.abs(grad.cpu().numpy() - o["grad"]).max() <= 2e-5 * np.abs(o["grad"]).max()
+    f.close()
