@@ -279,6 +279,36 @@ def run_ours(args):
                  "alg_bytes": "sigma: pos 12 + group id 4 per particle; backward: pos 12 + group id 4 + grad 12"}
         del gp, sig, og
 
+    # ---- NEXT-3: S = 16 stochastic-edge samples on one binning (PAPER.md 3.2: S = 16;
+    # candidate radius 1.5 b, alpha = 5), timed on their own
+    next3 = None
+    if not args.no_next3:
+        S = 16
+        f3 = B.FoF(N, w.L, float(np.float32(1.5 * w.b)), w.N_min, device=dev)
+        lab3 = torch.empty(N, dtype=torch.int32, device=dev)
+        f3.link(dpos, lab3)
+        lp3 = torch.zeros(1, dtype=torch.float64, device=dev)
+        g3 = torch.empty((N, 3), dtype=torch.float32, device=dev)
+        for smp in range(2):
+            B.fof_link_stochastic(f3.h, w.b, 5.0, 2024, smp, lab3, lp3, g3, f3.ws)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        torch.cuda.synchronize()
+        ev[0].record(stream)
+        f3.link(dpos, lab3)
+        ev[1].record(stream)
+        for smp in range(S):
+            B.fof_link_stochastic(f3.h, w.b, 5.0, 2024, smp, lab3, lp3, g3, f3.ws)
+        ev[2].record(stream)
+        torch.cuda.synchronize()
+        e3, cand3, _ = f3.link_stats()
+        t_bin, t_smp = ev[0].elapsed_time(ev[1]), ev[1].elapsed_time(ev[2]) / S
+        next3 = {"samples": S, "binning_ms": t_bin, "ms_per_sample": t_smp,
+                 "potential_edges": cand3, "sampled_edges_last": e3,
+                 "potential_edges_per_s": cand3 / (t_smp * 1e-3), "particles_per_s_per_sample": N / (t_smp * 1e-3),
+                 "config": "b_cand = 1.5 b, alpha = 5, log p(y) and score function on"}
+        f3.close()
+        del f3, lab3, g3
+
     # ---- end to end: host buffers through the C ABI (fof_run_host), copies inside the timed region
     cap = out["cap"]
     h2 = B.fof_create(N, w.L, w.b, w.N_min)
@@ -376,7 +406,7 @@ def run_ours(args):
         "e2e": {"value": whole_job_value(world, N, e2e_ms), "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
                 "h2d_bytes_per_step": int(hpos.numel() * 4),
                 "d2h_bytes_per_step": int(N * 4 + Kh * (4 + 4 + 4 + 12) + 8)},
-        "gpu_launches": int(launches), "clocks": clk.summary(), "next1": next1,
+        "gpu_launches": int(launches), "clocks": clk.summary(), "next1": next1, "next3": next3,
     }
     print(json.dumps(line), flush=True)
     if world > 1:
@@ -393,6 +423,7 @@ def main():
     ap.add_argument("--grid", type=int, default=None, help="force n cells per axis (tuning knob)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-next1", action="store_true", help="skip the sigma / backward timing")
+    ap.add_argument("--no-next3", action="store_true", help="skip the stochastic-edge sample timing")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

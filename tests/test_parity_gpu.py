@@ -498,7 +498,7 @@ def test_stochastic_link_against_oracle(B, alpha, kappa):
         E, ncand, _ = f.link_stats()
         assert ncand == o["n_cand"] and E == o["n_edge"]
         assert np.array_equal(labels.cpu().numpy(), o["labels"]), "sampled components differ"
-        assert abs(float(logp.item()) - o["logp"]) <= 1e-9 * abs(o["logp"]) + 1e-9
+        assert abs(float(logp.item()) - o["logp"]) <= 2e-6 * abs(o["logp"]) + 1e-6   # float32 log terms
         g = grad.cpu().numpy().astype(np.float64)
         assert np.abs(g - o["grad"]).max() <= 2e-5 * np.abs(o["grad"]).max()
     # samples differ from each other, and a different seed gives a different graph
@@ -520,6 +520,6 @@ def test_stochastic_link_wraps_and_needs_a_link_first(B):
     o = oracle.stochastic(p, L, 1.5, b, 3.0, 1, 0, brute=True)
     labels, logp, grad = f.link_stochastic(b, 3.0, 1, 0)
     assert np.array_equal(labels.cpu().numpy(), o["labels"])
-    assert abs(float(logp.item()) - o["logp"]) <= 1e-9 * abs(o["logp"])
+    assert abs(float(logp.item()) - o["logp"]) <= 2e-6 * abs(o["logp"])
     assert np.abs(grad.cpu().numpy() - o["grad"]).max() <= 2e-5 * np.abs(o["grad"]).max()
     f.close()
