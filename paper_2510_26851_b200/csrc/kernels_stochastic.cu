@@ -97,8 +97,9 @@ __global__ void __launch_bounds__(kBlock) link_stochastic_kernel(const float4 *_
     unsigned int ncand = 0, nedge = 0;
     s_g[wib][lane][0] = s_g[wib][lane][1] = s_g[wib][lane][2] = 0.0f;
     __syncwarp();
+    int dx = -2, dy = -1, dz = -1;
     for (int q = 0; q < 27; ++q) {
-        const int dx = q % 3 - 1, dy = (q / 3) % 3 - 1, dz = q / 9 - 1;
+        if (++dx > 1) { dx = -1; if (++dy > 1) { dy = -1; ++dz; } }  // q = (dx + 1) + 3 (dy + 1) + 9 (dz + 1)
         const bool forward = q > 13;  // dz > 0, or dz == 0 and dy > 0, or dz == dy == 0 and dx > 0
         if (!forward && q != 13 && !grad) continue;  // the backward half only feeds the gradient
         int beg = 0, len = 0;
@@ -169,7 +170,7 @@ __global__ void __launch_bounds__(kBlock) link_stochastic_kernel(const float4 *_
                     }
                 }
             }
-            if (grad) {
+            if (grad && __any_sync(0xffffffffu, gx != 0.0f || gy != 0.0f || gz != 0.0f)) {
                 // segmented inclusive scan over runs of equal owner, then one add per home particle
                 const int key = has ? owner : -1 - lane;
 #pragma unroll
