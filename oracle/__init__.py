@@ -17,6 +17,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "fof_oracle.c")
 _SRC2 = os.path.join(_HERE, "fof_oracle_stochastic.c")  # NEXT-3: stochastic-edge FoF
+_SRC3 = os.path.join(_HERE, "fof_oracle_subhalo.c")     # NEXT-4: six-dimensional sub-halo pass
 _LIB = os.path.join(_HERE, "libfof_oracle.so")
 # -ffp-contract=off: the float32 link predicate must not be contracted into FMAs.
 CFLAGS = ["-O2", "-std=c99", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC"]
@@ -26,10 +27,10 @@ _lib = None
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (building the checker is not using it)."""
-    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_SRC2))
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_SRC2), os.path.getmtime(_SRC3))
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < newest:
         tmp = _LIB + f".tmp{os.getpid()}"
-        subprocess.check_call(["gcc", *CFLAGS, "-o", tmp, _SRC, _SRC2, "-lm"])
+        subprocess.check_call(["gcc", *CFLAGS, "-o", tmp, _SRC, _SRC2, _SRC3, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -62,6 +63,9 @@ def _load():
         lib.oracle_groups_backward.argtypes = [f32p, f32p, i32p, ctypes.c_int64, ctypes.c_float, ctypes.c_int64,
                                                f64p_, f64p_, f64p_, f64p_, f64p_, f64p_]
         f64q = ctypes.POINTER(ctypes.c_double)
+        lib.oracle_subgroups.restype = ctypes.c_int
+        lib.oracle_subgroups.argtypes = [f32p, f32p, i32p, ctypes.c_int64, ctypes.c_float, ctypes.c_float,
+                                         ctypes.c_float, ctypes.c_float, i32p, u64p]
         lib.oracle_sigmoid_fixed.restype = ctypes.c_float
         lib.oracle_sigmoid_fixed.argtypes = [ctypes.c_float]
         lib.oracle_rng_u24.restype = ctypes.c_uint32
@@ -209,6 +213,20 @@ def groups_backward(pos, particle_group, L: float, group_mass, group_com, grad_c
                                           gm.shape[0], gmp, gcp, gsp, dxp, dsp,
                                           out.ctypes.data_as(ctypes.POINTER(ctypes.c_double))))
     return out[:N]
+
+
+def subgroups(pos, vel, particle_group, L: float, sigma_x: float, sigma_v: float, ell: float):
+    """Six-dimensional FoF inside every kept halo (Eq. 3): (sub_labels int32 [N], E6)."""
+    pos, p = _pos(pos)
+    vel, v = _f32(vel)
+    N = pos.shape[0]
+    pg = np.ascontiguousarray(particle_group, dtype=np.int32)
+    out = np.empty(max(N, 1), np.int32)
+    E = ctypes.c_uint64(0)
+    i32p = ctypes.POINTER(ctypes.c_int32)
+    _check(_load().oracle_subgroups(p, v, pg.ctypes.data_as(i32p), N, _f(L), _f(sigma_x), _f(sigma_v), _f(ell),
+                                    out.ctypes.data_as(i32p), ctypes.byref(E)))
+    return out[:N], int(E.value)
 
 
 def sigmoid_fixed(t: float) -> float:
