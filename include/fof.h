@@ -115,6 +115,21 @@ int fof_groups(fof_handle *h, const float *pos, const float *mass, const int32_t
 int fof_link_stochastic(fof_handle *h, float b_link, float alpha, uint64_t seed, uint32_t sample, int32_t *labels,
                         double *logp, float *grad_pos, void *ws, void *stream);
 
+/* Six-dimensional sub-halo pass (section 2.1.1, Eq. 3; R29-R31): inside every
+ * kept halo a second FoF in phase space, two members linked iff
+ *     (x_i - x_j)^2 / sigma_x + (v_i - v_j)^2 / sigma_v <= ell^2
+ * (minimum-image position differences, float32 without FMA).  Downstream of fof_groups:
+ * particle_group (dev [N]) and group_size (dev [K]) are its outputs, K its *K_host.
+ *   vel         dev [N,3] float32 velocities.
+ *   sub_labels  dev [N] int32, written: minimum original index of the particle's 6-D component; a
+ *               particle of a dropped halo (particle_group < 0) gets its own index.
+ *   ws          the plan's workspace (scratch: the cell-sorted state of fof_link is overwritten, so a
+ *               later fof_link_stochastic / fof_link_stats needs a new fof_link first).
+ * Work is O(sum over halos of size^2).  Asynchronous on `stream`. */
+int fof_subgroups(fof_handle *h, const float *pos, const float *vel, const int32_t *particle_group,
+                  const int32_t *group_size, int64_t K, float sigma_x, float sigma_v, float ell, int32_t *sub_labels,
+                  void *ws, void *stream);
+
 /* Halo decoration (section 3.1.1 "Decorated Frozen Assignment": "particle standard deviation
  * (sigma)" as the surrogate of halo mass; R23):
  *   group_sigma[k] = sqrt( sum_i m_i |delta_i|^2 / M_k ),  delta_i = minimum-image displacement of

@@ -62,6 +62,8 @@ def lib():
         L.fof_groups.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, ctypes.POINTER(i64), vp]
         L.fof_link_stochastic.restype = ctypes.c_int
         L.fof_link_stochastic.argtypes = [vp, f32, f32, ctypes.c_uint64, ctypes.c_uint32, vp, vp, vp, vp, vp]
+        L.fof_subgroups.restype = ctypes.c_int
+        L.fof_subgroups.argtypes = [vp, vp, vp, vp, vp, i64, f32, f32, f32, vp, vp, vp]
         L.fof_group_sigma.restype = ctypes.c_int
         L.fof_group_sigma.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp]
         L.fof_groups_backward.restype = ctypes.c_int
@@ -168,6 +170,11 @@ def fof_link_stochastic(h, b_link, alpha, seed, sample, labels, logp, grad_pos, 
     """labels: cuda int32 [N]; logp: cuda float64 [1]; grad_pos: cuda float32 [N,3] or None."""
     _check(lib().fof_link_stochastic(h, _f(b_link), _f(alpha), int(seed), int(sample), _ptr(labels), _ptr(logp),
                                      _ptr(grad_pos), _ptr(ws), _stream_ptr(stream)), h)
+
+
+def fof_subgroups(h, pos, vel, particle_group, group_size, K, sigma_x, sigma_v, ell, sub_labels, ws, stream=None):
+    _check(lib().fof_subgroups(h, _ptr(pos), _ptr(vel), _ptr(particle_group), _ptr(group_size), int(K), _f(sigma_x),
+                               _f(sigma_v), _f(ell), _ptr(sub_labels), _ptr(ws), _stream_ptr(stream)), h)
 
 
 def fof_group_sigma(h, pos, mass, particle_group, group_mass, group_com, K, ws, group_sigma, stream=None):
@@ -298,6 +305,16 @@ class FoF:
         with torch.cuda.device(d):
             fof_link_stochastic(self.h, b_link, alpha, seed, sample, labels, logp, grad, self.ws, stream)
         return labels, logp, grad
+
+    def subgroups(self, pos, vel, g, sigma_x, sigma_v, ell, stream=None):
+        """6-D sub-halo labels [N] inside the groups `g` returned by groups(..., particle_group=True)."""
+        import torch
+
+        sub = torch.empty(self.N, dtype=torch.int32, device=pos.device)
+        with torch.cuda.device(self.device):
+            fof_subgroups(self.h, pos, vel, g["particle_group"], g["group_size"], g["K"], sigma_x, sigma_v, ell, sub,
+                          self.ws, stream)
+        return sub
 
     def group_sigma(self, pos, g, mass=None, stream=None):
         """Halo decoration sigma [K] of the groups `g` returned by groups(..., particle_group=True)."""

@@ -349,6 +349,30 @@ int fof_link_stochastic(fof_handle *h, float b_link, float alpha, uint64_t seed,
     return FOF_OK;
 }
 
+int fof_subgroups(fof_handle *h, const float *pos, const float *vel, const int32_t *particle_group,
+                  const int32_t *group_size, int64_t K, float sigma_x, float sigma_v, float ell, int32_t *sub_labels,
+                  void *ws, void *stream)
+{
+    if (!h || !ws || ((uintptr_t)ws & 255) || K < 0 || K > h->N) return FOF_ERR_INVALID_ARG;
+    if (!(sigma_x > 0.0f) || !(sigma_v > 0.0f) || !(ell > 0.0f)) return FOF_ERR_INVALID_ARG;
+    if (h->N > 0 && (!pos || !vel || !particle_group || !sub_labels)) return FOF_ERR_INVALID_ARG;
+    if (K > 0 && !group_size) return FOF_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (h->num_sms == 0) {
+        int dev = 0, sms = 0;
+        CK(cudaGetDevice(&dev), "cudaGetDevice");
+        CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute");
+        h->num_sms = sms;
+    }
+    h->linked = false;  // the member lists and their union-find re-use the link's arrays
+    h->launches += h->N > 0 ? (K > 0 ? 4 : 2) : 0;
+    CK(launch_subgroups(pos, vel, particle_group, group_size, h->N, K, h->L, sigma_x, sigma_v, ell,
+                        at<unsigned int>(ws, h->off_cnt), at<unsigned int>(ws, h->off_part), at<int>(ws, h->off_idx),
+                        at<unsigned int>(ws, h->off_rel), sub_labels, at<Ctrl>(ws, h->off_ctrl), h->num_sms, s),
+       "sub-halo kernels");
+    return FOF_OK;
+}
+
 int fof_group_sigma(fof_handle *h, const float *pos, const float *mass, const int32_t *particle_group,
                     const float *group_mass, const float *group_com, int64_t K, void *ws, float *group_sigma,
                     void *stream)

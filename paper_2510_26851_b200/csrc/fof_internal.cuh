@@ -243,4 +243,9 @@ cudaError_t launch_link_stochastic(const float4 *sorted, int64_t N, Grid g, cons
                                    unsigned long long seed, unsigned int sample, int *labels, double *logp, float *grad,
                                    Ctrl *ctrl, cudaStream_t s);
 
+cudaError_t launch_subgroups(const float *pos, const float *vel, const int *particle_group, const int *group_size,
+                             int64_t N, int64_t K, float L, float sigma_x, float sigma_v, float ell,
+                             unsigned int *offsets, unsigned int *cursor, int *members, unsigned int *sub_rel,
+                             int *sub_labels, Ctrl *ctrl, int num_sms, cudaStream_t s);
+
 }  // namespace fof

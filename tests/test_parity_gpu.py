@@ -523,3 +523,63 @@ def test_stochastic_link_wraps_and_needs_a_link_first(B):
     assert abs(float(logp.item()) - o["logp"]) <= 2e-6 * abs(o["logp"])
     assert np.abs(grad.cpu().numpy() - o["grad"]).max() <= 2e-5 * np.abs(o["grad"]).max()
     f.close()
+
+
+# --------------------------------------------------------------------------- NEXT-4: 6-D sub-halo pass
+@pytest.mark.parametrize("sv_scale", [120.0, 1e15])
+def test_subgroups_against_oracle(B, sv_scale):
+    """fof_subgroups (section 2.1.1 Eq. 3): sub-halo labels bit-exact with the oracle (the same float32
+    predicate on both sides), on halos that cross the box faces; sv -> infinity gives back the halos."""
+    w = inputs.scaled(inputs.CONFIGS["cfg1"], 48)
+    p = inputs.make_positions(w)
+    rng = np.random.default_rng(19)
+    v = (rng.standard_normal((len(p), 3)) * 50.0).astype(np.float32)
+    lab, _ = oracle.labels_cells(p, w.L, w.b)
+    og = oracle.groups(p, lab, w.L, w.N_min)
+    pgo = og["particle_group"]
+    v[(rng.random(len(p)) < 0.5) & (pgo >= 0)] += np.float32(400.0)      # a bulk flow through every halo
+    ell = float(np.float32(1.3 * w.b))
+    osub, _ = oracle.subgroups(p, v, pgo, w.L, 1.0, sv_scale ** 2, ell)
+
+    f = B.FoF(len(p), w.L, w.b, w.N_min)
+    dpos, dvel = torch.from_numpy(p).cuda(), torch.from_numpy(v).cuda()
+    labels = f.link(dpos)
+    g = f.groups(dpos, labels, particle_group=True)
+    assert g["K"] == og["K"]
+    sub = f.subgroups(dpos, dvel, g, 1.0, sv_scale ** 2, ell).cpu().numpy()
+    assert np.array_equal(sub, osub), "sub-halo labels differ"
+    if sv_scale > 1e10:
+        assert np.array_equal(sub[pgo >= 0], lab[pgo >= 0])
+    else:
+        assert len(np.unique(sub[pgo >= 0])) > og["K"]
+    # the link state was overwritten: a stochastic sample must ask for a new fof_link
+    with pytest.raises(B.FofError) as e:
+        f.link_stochastic(w.b, 1.0, 1, 0)
+    assert e.value.code == B.FOF_ERR_STATE
+    f.close()
+
+
+def test_subgroups_large_halo_and_no_halo(B):
+    rng = np.random.default_rng(23)
+    L, b = 50.0, 1.0
+    clump = rng.standard_normal((3000, 3)) * 1.2 + 25.0          # one halo of ~3000 members: 94 tiles
+    p = np.concatenate([rng.random((2000, 3)) * L, clump]).astype(np.float32) % np.float32(L)
+    v = (rng.standard_normal((len(p), 3)) * 30.0).astype(np.float32)
+    v[2000:3500] += np.float32(200.0)
+    lab, _ = oracle.labels_cells(p, L, b)
+    og = oracle.groups(p, lab, L, 20)
+    osub, _ = oracle.subgroups(p, v, og["particle_group"], L, 1.0, 60.0 ** 2, 0.9)
+    f = B.FoF(len(p), L, b, 20)
+    dpos, dvel = torch.from_numpy(p).cuda(), torch.from_numpy(v).cuda()
+    g = f.groups(dpos, f.link(dpos), particle_group=True)
+    assert g["group_size"].max().item() > 2000
+    assert np.array_equal(f.subgroups(dpos, dvel, g, 1.0, 60.0 ** 2, 0.9).cpu().numpy(), osub)
+    f.close()
+    q = (rng.random((4000, 3)) * 100.0).astype(np.float32)        # no halo at all
+    f = B.FoF(len(q), 100.0, 0.5, 20)
+    dq = torch.from_numpy(q).cuda()
+    g = f.groups(dq, f.link(dq), particle_group=True)
+    assert g["K"] == 0
+    sub = f.subgroups(dq, torch.zeros_like(dq), g, 1.0, 1.0, 1.0).cpu().numpy()
+    assert np.array_equal(sub, np.arange(len(q), dtype=np.int32))
+    f.close()
