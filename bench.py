@@ -309,6 +309,34 @@ def run_ours(args):
         f3.close()
         del f3, lab3, g3
 
+    # ---- NEXT-4: six-dimensional sub-halo pass inside every kept halo, timed on its own
+    next4 = None
+    if not args.no_next4:
+        og = f.groups(dpos, labels, particle_group=True)
+        gen = torch.Generator(device=dev).manual_seed(4)
+        dvel = torch.randn((N, 3), device=dev, generator=gen) * 50.0      # synthetic velocities, 50 per axis
+        sub = torch.empty(N, dtype=torch.int32, device=dev)
+        args6 = (f.h, dpos, dvel, og["particle_group"], og["group_size"], og["K"], 1.0, 100.0 ** 2, float(w.b), sub, f.ws)
+        for _ in range(2):
+            B.fof_subgroups(*args6)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize()
+        ev[0].record(stream)
+        for _ in range(5):
+            B.fof_subgroups(*args6)
+        ev[1].record(stream)
+        torch.cuda.synchronize()
+        sizes = og["group_size"].to(torch.float64)
+        pairs = float((sizes * (sizes - 1) / 2).sum().item())
+        t6 = ev[0].elapsed_time(ev[1]) / 5
+        members = int(sizes.sum().item())
+        nsub = int(torch.unique(sub[og["particle_group"] >= 0]).numel())
+        next4 = {"ms": t6, "halos": og["K"], "members": members, "pairs_in_halos": pairs,
+                 "pair_tests_per_s": pairs / (t6 * 1e-3), "sub_halos": nsub,
+                 "config": "sigma_x = 1, sigma_v = 100^2 (velocities ~ N(0, 50)), ell = b"}
+        f.link(dpos, labels)  # restore the link state that fof_subgroups overwrote
+        del dvel, sub, og
+
     # ---- end to end: host buffers through the C ABI (fof_run_host), copies inside the timed region
     cap = out["cap"]
     h2 = B.fof_create(N, w.L, w.b, w.N_min)
@@ -406,7 +434,7 @@ def run_ours(args):
         "e2e": {"value": whole_job_value(world, N, e2e_ms), "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
                 "h2d_bytes_per_step": int(hpos.numel() * 4),
                 "d2h_bytes_per_step": int(N * 4 + Kh * (4 + 4 + 4 + 12) + 8)},
-        "gpu_launches": int(launches), "clocks": clk.summary(), "next1": next1, "next3": next3,
+        "gpu_launches": int(launches), "clocks": clk.summary(), "next1": next1, "next3": next3, "next4": next4,
     }
     print(json.dumps(line), flush=True)
     if world > 1:
@@ -424,6 +452,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-next1", action="store_true", help="skip the sigma / backward timing")
     ap.add_argument("--no-next3", action="store_true", help="skip the stochastic-edge sample timing")
+    ap.add_argument("--no-next4", action="store_true", help="skip the sub-halo pass timing")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -5,7 +5,7 @@
 // Readings R29-R31 of DESIGN.md: float32 predicate without FMA, d2 <= ell2; labels = minimum original
 // index of the 6-D component inside one kept halo; particles of dropped halos keep their own index.
 // Steps: member lists per halo (exclusive scan of the group sizes, atomic fill), all pairs inside
-// each halo tile by tile (one CTA per halo, one warp per tile of 32 members, the partner tile staged
+// each halo tile by tile (one warp per tile of 32 members, the partner tile staged
 // in shared memory), lock-free union-find over member slots ordered by original index, labels.
 // Cost is O(sum of squared halo sizes): meant for halos, not for a percolating component.
 #include "fof_internal.cuh"
@@ -81,8 +81,13 @@ __device__ __forceinline__ bool linked6(const float *a, const float *b, const Su
 
 constexpr int kSubWarps = kBlock / 32;
 
-// One CTA per kept halo (grid-stride), one warp per tile of 32 member slots; the tile meets itself
-// and every earlier tile.  A pair is taken by its later slot.
+// One warp per tile of 32 member slots; the tile meets itself and every earlier tile; a pair is
+// taken by its later slot.  Two launches share the halos by size: WIDE = false, one warp per halo of
+// at most kSubSmall members (eight halos per CTA: a typical halo has two tiles); WIDE = true, one CTA
+// per larger halo, its warps striding over the tiles.
+constexpr int kSubSmall = 256;
+
+template <bool WIDE>
 __global__ void __launch_bounds__(kBlock) subhalo_link_kernel(const float *__restrict__ pos,
                                                               const float *__restrict__ vel, int64_t K, Sub6 q,
                                                               const unsigned int *__restrict__ offsets,
@@ -92,10 +97,13 @@ __global__ void __launch_bounds__(kBlock) subhalo_link_kernel(const float *__res
     __shared__ float s_j[kSubWarps][32][6];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     unsigned int nedges = 0;
-    for (int64_t k = blockIdx.x; k < K; k += gridDim.x) {
+    const int64_t k0 = WIDE ? (int64_t)blockIdx.x : (int64_t)blockIdx.x * kSubWarps + warp;
+    const int64_t kstep = WIDE ? (int64_t)gridDim.x : (int64_t)gridDim.x * kSubWarps;
+    for (int64_t k = k0; k < K; k += kstep) {
         const int off = (int)offsets[k], M = (int)offsets[k + 1] - off;
+        if ((M > kSubSmall) != WIDE) continue;
         const int tiles = (M + 31) >> 5;
-        for (int it = warp; it < tiles; it += kSubWarps) {
+        for (int it = WIDE ? warp : 0; it < tiles; it += WIDE ? kSubWarps : 1) {
             const int myslot = off + it * 32 + lane;
             const bool valid = it * 32 + lane < M;
             float me[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
@@ -172,8 +180,11 @@ cudaError_t launch_subgroups(const float *pos, const float *vel, const int *part
     sub_fill_kernel<<<(unsigned int)((N + kBlock - 1) / kBlock), kBlock, 0, s>>>(particle_group, N, K, offsets, cursor,
                                                                                 members, sub_rel, sub_labels);
     if (K > 0) {
-        const unsigned int grid = (unsigned int)(K < (int64_t)num_sms * 16 ? K : (int64_t)num_sms * 16);
-        subhalo_link_kernel<<<grid, kBlock, 0, s>>>(pos, vel, K, q, offsets, members, sub_rel, ctrl);
+        const int64_t cap = (int64_t)num_sms * 16;
+        const unsigned int grid_small = (unsigned int)((K + kSubWarps - 1) / kSubWarps < cap ? (K + kSubWarps - 1) / kSubWarps : cap);
+        const unsigned int grid_wide = (unsigned int)(K < cap ? K : cap);
+        subhalo_link_kernel<false><<<grid_small, kBlock, 0, s>>>(pos, vel, K, q, offsets, members, sub_rel, ctrl);
+        subhalo_link_kernel<true><<<grid_wide, kBlock, 0, s>>>(pos, vel, K, q, offsets, members, sub_rel, ctrl);
         sub_labels_kernel<<<(unsigned int)num_sms * 8, kBlock, 0, s>>>(sub_rel, members, offsets + K, sub_labels);
     }
     return cudaGetLastError();
