@@ -130,6 +130,22 @@ int fof_subgroups(fof_handle *h, const float *pos, const float *vel, const int32
                   const int32_t *group_size, int64_t K, float sigma_x, float sigma_v, float ell, int32_t *sub_labels,
                   void *ws, void *stream);
 
+/* Device steps of the slab-decomposed multi-GPU FoF (section 2.3).  They need
+ * no plan; the exchange between devices is done by the caller (paper_2510_26851_b200/slab.py).
+ * fof_layer_select: indices i (dev out_idx, capacity N) of the particles whose wrapped coordinate along
+ *   `axis` lies in [lo, lo + width) modulo L; *count (dev uint32) = how many; order arbitrary.
+ * fof_component_min: out[i] = minimum of ids[] over i's component, given canonical local labels
+ *   (labels[labels[i]] == labels[i]); tmp = dev scratch [N].  Turns local labels into the "minimum
+ *   global particle ID" of PAPER.md:180.
+ * fof_merge_labels: union-find over global ids 0..G-1 (parent = dev scratch [G]), hooked by the P
+ *   equivalence pairs (dev [P,2], the smaller id wins), then labels[i] <- root(labels[i]) for the N
+ *   labels given (in place).  All asynchronous on `stream`. */
+int fof_layer_select(const float *pos, int64_t N, float L, int32_t axis, float lo, float width, int32_t *out_idx,
+                     uint32_t *count, void *stream);
+int fof_component_min(const int32_t *labels, const int32_t *ids, int64_t N, int32_t *tmp, int32_t *out, void *stream);
+int fof_merge_labels(const int32_t *pairs, int64_t P, int32_t *parent, int64_t G, int32_t *labels, int64_t N,
+                     void *stream);
+
 /* Halo decoration (section 3.1.1 "Decorated Frozen Assignment": "particle standard deviation
  * (sigma)" as the surrogate of halo mass; R23):
  *   group_sigma[k] = sqrt( sum_i m_i |delta_i|^2 / M_k ),  delta_i = minimum-image displacement of

@@ -64,6 +64,12 @@ def lib():
         L.fof_link_stochastic.argtypes = [vp, f32, f32, ctypes.c_uint64, ctypes.c_uint32, vp, vp, vp, vp, vp]
         L.fof_subgroups.restype = ctypes.c_int
         L.fof_subgroups.argtypes = [vp, vp, vp, vp, vp, i64, f32, f32, f32, vp, vp, vp]
+        L.fof_layer_select.restype = ctypes.c_int
+        L.fof_layer_select.argtypes = [vp, i64, f32, i32, f32, f32, vp, vp, vp]
+        L.fof_component_min.restype = ctypes.c_int
+        L.fof_component_min.argtypes = [vp, vp, i64, vp, vp, vp]
+        L.fof_merge_labels.restype = ctypes.c_int
+        L.fof_merge_labels.argtypes = [vp, i64, vp, i64, vp, i64, vp]
         L.fof_group_sigma.restype = ctypes.c_int
         L.fof_group_sigma.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp]
         L.fof_groups_backward.restype = ctypes.c_int
@@ -175,6 +181,21 @@ def fof_link_stochastic(h, b_link, alpha, seed, sample, labels, logp, grad_pos, 
 def fof_subgroups(h, pos, vel, particle_group, group_size, K, sigma_x, sigma_v, ell, sub_labels, ws, stream=None):
     _check(lib().fof_subgroups(h, _ptr(pos), _ptr(vel), _ptr(particle_group), _ptr(group_size), int(K), _f(sigma_x),
                                _f(sigma_v), _f(ell), _ptr(sub_labels), _ptr(ws), _stream_ptr(stream)), h)
+
+
+def fof_layer_select(pos, L, axis, lo, width, out_idx, count, stream=None):
+    _check(lib().fof_layer_select(_ptr(pos), int(pos.shape[0]), _f(L), int(axis), _f(lo), _f(width), _ptr(out_idx),
+                                  _ptr(count), _stream_ptr(stream)))
+
+
+def fof_component_min(labels, ids, tmp, out, stream=None):
+    _check(lib().fof_component_min(_ptr(labels), _ptr(ids), int(labels.shape[0]), _ptr(tmp), _ptr(out),
+                                   _stream_ptr(stream)))
+
+
+def fof_merge_labels(pairs, parent, labels, stream=None):
+    _check(lib().fof_merge_labels(_ptr(pairs), int(pairs.shape[0]), _ptr(parent), int(parent.shape[0]), _ptr(labels),
+                                  int(labels.shape[0]), _stream_ptr(stream)))
 
 
 def fof_group_sigma(h, pos, mass, particle_group, group_mass, group_com, K, ws, group_sigma, stream=None):

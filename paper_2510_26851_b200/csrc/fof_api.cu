@@ -373,6 +373,30 @@ int fof_subgroups(fof_handle *h, const float *pos, const float *vel, const int32
     return FOF_OK;
 }
 
+int fof_layer_select(const float *pos, int64_t N, float L, int32_t axis, float lo, float width, int32_t *out_idx,
+                     uint32_t *count, void *stream)
+{
+    if (N < 0 || !(L > 0.0f) || axis < 0 || axis > 2 || !(width >= 0.0f) || !count) return FOF_ERR_INVALID_ARG;
+    if (N > 0 && (!pos || !out_idx)) return FOF_ERR_INVALID_ARG;
+    return launch_layer_select(pos, N, L, axis, lo, width, out_idx, count, (cudaStream_t)stream) == cudaSuccess
+               ? FOF_OK : FOF_ERR_CUDA;
+}
+
+int fof_component_min(const int32_t *labels, const int32_t *ids, int64_t N, int32_t *tmp, int32_t *out, void *stream)
+{
+    if (N < 0 || (N > 0 && (!labels || !ids || !tmp || !out))) return FOF_ERR_INVALID_ARG;
+    return launch_component_min(labels, ids, N, tmp, out, (cudaStream_t)stream) == cudaSuccess ? FOF_OK : FOF_ERR_CUDA;
+}
+
+int fof_merge_labels(const int32_t *pairs, int64_t P, int32_t *parent, int64_t G, int32_t *labels, int64_t N,
+                     void *stream)
+{
+    if (P < 0 || G < 0 || N < 0 || (G > 0 && !parent) || (P > 0 && !pairs) || (N > 0 && !labels))
+        return FOF_ERR_INVALID_ARG;
+    return launch_merge_labels(pairs, P, parent, G, labels, N, (cudaStream_t)stream) == cudaSuccess ? FOF_OK
+                                                                                                    : FOF_ERR_CUDA;
+}
+
 int fof_group_sigma(fof_handle *h, const float *pos, const float *mass, const int32_t *particle_group,
                     const float *group_mass, const float *group_com, int64_t K, void *ws, float *group_sigma,
                     void *stream)

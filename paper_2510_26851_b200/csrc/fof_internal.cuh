@@ -248,4 +248,10 @@ cudaError_t launch_subgroups(const float *pos, const float *vel, const int *part
                              unsigned int *offsets, unsigned int *cursor, int *members, unsigned int *sub_rel,
                              int *sub_labels, Ctrl *ctrl, int num_sms, cudaStream_t s);
 
+cudaError_t launch_layer_select(const float *pos, int64_t N, float L, int axis, float lo, float width, int *out_idx,
+                                unsigned int *count, cudaStream_t s);
+cudaError_t launch_component_min(const int *labels, const int *ids, int64_t N, int *tmp, int *out, cudaStream_t s);
+cudaError_t launch_merge_labels(const int *pairs, int64_t P, int *parent, int64_t G, int *labels, int64_t N,
+                                cudaStream_t s);
+
 }  // namespace fof

@@ -583,3 +583,33 @@ def test_subgroups_large_halo_and_no_halo(B):
     sub = f.subgroups(dq, torch.zeros_like(dq), g, 1.0, 1.0, 1.0).cpu().numpy()
     assert np.array_equal(sub, np.arange(len(q), dtype=np.int32))
     f.close()
+
+
+# --------------------------------------------------------------------------- NEXT-2: slab-decomposed FoF
+@pytest.mark.parametrize("world", [2, 3, 4])
+def test_slab_fof_equals_monolithic(B, world):
+    """slabs + ghost layer + label-equivalence merge give exactly the monolithic labels
+    (minimum global particle id).  All ranks are played in turn on this one GPU; the exchange is emulated."""
+    from paper_2510_26851_b200 import slab
+
+    w = inputs.scaled(inputs.CONFIGS["cfg1"], 48)
+    p = inputs.make_positions(w)
+    rng = np.random.default_rng(5)
+    # a chain of particles 0.8 b apart along z through the whole box: one group that crosses every face
+    nz = int(w.L / (0.8 * w.b))
+    chain = np.stack([np.full(nz, 0.37 * w.L), np.full(nz, 0.61 * w.L), (np.arange(nz) + 0.5) * (w.L / nz)], 1)
+    p = np.concatenate([p, chain.astype(np.float32)])
+    p = p[rng.permutation(len(p))]
+    N = len(p)
+    f = B.FoF(N, w.L, w.b, w.N_min)
+    mono = f.link(torch.from_numpy(p).cuda()).cpu().numpy()
+    f.close()
+    own = slab.split_into_slabs(p, w.L, world)
+    assert sum(len(o) for o in own) == N
+    parts = [(torch.from_numpy(p[o]).cuda(), torch.from_numpy(o.astype(np.int32)).cuda()) for o in own]
+    out = slab.slab_fof_emulated(parts, w.L, w.b, N)
+    crossing = 0
+    for o, lab in zip(own, out):
+        assert np.array_equal(lab.cpu().numpy(), mono[o]), "slab labels differ from the monolithic run"
+        crossing += int((~np.isin(mono[o], o)).sum())
+    assert crossing > nz // 2          # many particles whose canonical particle lives on another rank
