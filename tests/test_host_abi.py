@@ -132,3 +132,50 @@ def test_reference_arm_prints_the_contract_line():
     assert line["impl"] == "reference" and line["metric"] == "fof_linked_particles_per_s"
     assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
     assert line["value"] > 0 and line["config"]["workload"] == "cfg0"
+
+
+def _ring_worker(rank, world, port, out):
+    import torch
+    import torch.distributed as dist
+
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port))
+    sys.path.insert(0, ROOT)
+    from paper_2510_26851_b200.slab import RingExchange
+
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    ex = RingExchange()
+    # rank r lends r + 1 rows (rank 0: also tests the empty case when world == 3 via rank 2 -> 0 rows)
+    rows = 0 if (world == 3 and rank == 2) else rank + 1
+    t = torch.full((rows, 3), float(rank)) + torch.arange(3.0)
+    got = ex.send_down_recv_up(t)                       # rows lent by rank + 1
+    ids = ex.send_down_recv_up(torch.arange(rows, dtype=torch.int32) + 100 * rank)
+    pairs = torch.tensor([[rank, 10 + rank]] * rank, dtype=torch.int32).reshape(rank, 2)
+    allp = ex.all_gather_rows(pairs)
+    out.put((rank, got.tolist(), ids.tolist(), allp.tolist()))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_slab_ring_exchange_under_gloo(world):
+    """The plumbing of the slab-decomposed FoF (NEXT-2): variable-length ring send/recv (who lends to whom,
+    empty messages) and the all-gather of the equivalence pairs, on CPU tensors over gloo."""
+    import torch.multiprocessing as mp
+
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = 31500 + (os.getpid() + world) % 2000
+    procs = [ctx.Process(target=_ring_worker, args=(r, world, port, out)) for r in range(world)]
+    for p in procs:
+        p.start()
+    rows = sorted(out.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for rank, got, ids, allp in rows:
+        up = (rank + 1) % world
+        n_up = 0 if (world == 3 and up == 2) else up + 1
+        assert got == [[float(up), float(up) + 1, float(up) + 2]] * n_up      # what rank + 1 lent
+        assert ids == [100 * up + k for k in range(n_up)]
+        assert allp == [[r, 10 + r] for r in range(world) for _ in range(r)]    # rank-major concatenation
