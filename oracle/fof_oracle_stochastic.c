@@ -16,13 +16,15 @@
  *      bc have p = 0 and contribute nothing.
  *  R26 sigma ("smooth sigmoidal thresholding function", its form is left open): the logistic
  *      function evaluated by a FIXED float32 recipe so that both sides take the Bernoulli decision
- *      on identical bits:  t = alpha * ((b2 - d2) / b2), clamped to [-30, 30];  z = (-t) * log2(e);
+ *      on identical bits:  t = c * (b2 - d2) with c = fl(alpha / b2), clamped to [-30, 30];  z = (-t) * log2(e);
  *      n = rint(z); f = z - n (exact);  2^f by the degree-6 Taylor polynomial in Horner form with
  *      separate multiply and add;  e = 2^f * 2^n (exact scaling);  p = 1 / (1 + e).
- *  R27 randomness: counter-based.  u = (top 24 bits of mix(seed, sample, lo, hi)) * 2^-24 with
- *      lo < hi the ORIGINAL indices of the pair and mix = two rounds of the splitmix64 finaliser;
+ *  R27 randomness: counter-based, 32-bit.  h = mix(fold(seed) ^ (sample * 0x9E3779B9)); h = mix(h + lo);
+ *      h = mix(h ^ (hi * 0x85EBCA6B)); u = (h >> 8) * 2^-24, with lo < hi the ORIGINAL indices of the
+ *      pair, fold(seed) = low word ^ high word, and mix the 32-bit finaliser
+ *      x ^= x >> 16; x *= 0x7FEB352D; x ^= x >> 15; x *= 0x846CA68B; x ^= x >> 16.
  *      y = (u < p).  Independent of traversal order, grid and device.
- *  R28 d log p(y) / d x_i = sum_j (y_ij - p_ij) dt/dx_i,  dt/dx_i = -2 alpha delta_ij / b2
+ *  R28 d log p(y) / d x_i = sum_j (y_ij - p_ij) dt/dx_i,  dt/dx_i = -2 c delta_ij
  *      (delta = minimum-image x_i - x_j), and 0 for a pair whose t was clamped.  float64 sums.
  */
 #include <math.h>
@@ -56,20 +58,20 @@ float oracle_sigmoid_fixed(float t)
 }
 
 /* ---- R27: counter-based uniform, 24 bits ------------------------------------------------------- */
-static uint64_t splitmix_fin(uint64_t z)
+static uint32_t mix32(uint32_t x)
 {
-    z ^= z >> 30; z *= 0xBF58476D1CE4E5B9ULL;
-    z ^= z >> 27; z *= 0x94D049BB133111EBULL;
-    z ^= z >> 31;
-    return z;
+    x ^= x >> 16; x *= 0x7FEB352DU;
+    x ^= x >> 15; x *= 0x846CA68BU;
+    x ^= x >> 16;
+    return x;
 }
 
 uint32_t oracle_rng_u24(uint64_t seed, uint32_t sample, uint32_t lo, uint32_t hi)
 {
-    uint64_t x = seed ^ (0x9E3779B97F4A7C15ULL * ((uint64_t)sample + 1ULL));
-    x = splitmix_fin(x + (uint64_t)lo);
-    x = splitmix_fin(x ^ ((uint64_t)hi * 0xD1B54A32D192ED03ULL));
-    return (uint32_t)(x >> 40);
+    uint32_t h = mix32((uint32_t)(seed ^ (seed >> 32)) ^ (sample * 0x9E3779B9U));   /* per-sample key */
+    h = mix32(h + lo);
+    h = mix32(h ^ (hi * 0x85EBCA6BU));
+    return h >> 8;
 }
 
 /* ---- one potential edge: candidate test (R25), p (R26), decision (R27), log-probability term and
@@ -77,7 +79,7 @@ uint32_t oracle_rng_u24(uint64_t seed, uint32_t sample, uint32_t lo, uint32_t hi
 typedef struct { int cand; int y; float p; double logp; double gi[3]; } pair_term;
 
 static pair_term pair_eval(const float *wi, const float *wj, int32_t i, int32_t j, float L, float bc2, float b2,
-                           float alpha, uint64_t seed, uint32_t sample)
+                           float alpha, uint64_t seed, uint32_t sample)  /* R26: c = fl(alpha / b2) */
 {
     pair_term r;
     memset(&r, 0, sizeof(r));
@@ -94,17 +96,17 @@ static pair_term pair_eval(const float *wi, const float *wj, int32_t i, int32_t 
     float d2 = s + zz;
     if (!(d2 <= bc2)) return r;
     r.cand = 1;
+    float c = alpha / b2;
     float num = b2 - d2;
-    float rat = num / b2;
-    float t = alpha * rat;
+    float t = c * num;
     r.p = oracle_sigmoid_fixed(t);
     const uint32_t lo = (uint32_t)(i < j ? i : j), hi = (uint32_t)(i < j ? j : i);
     const float u = (float)oracle_rng_u24(seed, sample, lo, hi) * 5.9604644775390625e-8f;  /* 2^-24 */
     r.y = u < r.p;
     r.logp = r.y ? log((double)r.p) : log1p(-(double)r.p);
     if (t <= 30.0f && t >= -30.0f) {
-        const double c = ((double)r.y - (double)r.p) * (-2.0 * (double)alpha / (double)b2);
-        for (int k = 0; k < 3; ++k) r.gi[k] = c * (double)d[k];
+        const double gc = ((double)r.y - (double)r.p) * (-2.0 * (double)c);   /* dt/dx_i = -2 c delta */
+        for (int k = 0; k < 3; ++k) r.gi[k] = gc * (double)d[k];
     }
     return r;
 }

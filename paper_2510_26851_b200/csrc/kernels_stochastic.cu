@@ -29,33 +29,30 @@ __device__ __forceinline__ float sigmoid_fixed(float t, float &e_out)
     q = __fadd_rn(__fmul_rn(q, f), 1.0f);
     const float e = __fmul_rn(q, __int_as_float(((int)n + 127) << 23));  // exact: |n| <= 44
     e_out = e;
-    return __fdiv_rn(1.0f, __fadd_rn(1.0f, e));
+    return __frcp_rn(__fadd_rn(1.0f, e));  // correctly rounded 1 / x: the bits of the oracle's division
 }
 
-// R27: 24 random bits from (seed, sample, lo, hi), two rounds of the splitmix64 finaliser.
-__device__ __forceinline__ unsigned long long splitmix_fin(unsigned long long z)
+// R27: 24 random bits from (folded seed, sample, lo, hi): two rounds of a 32-bit finaliser.
+__device__ __forceinline__ unsigned int mix32(unsigned int x)
 {
-    z ^= z >> 30; z *= 0xBF58476D1CE4E5B9ULL;
-    z ^= z >> 27; z *= 0x94D049BB133111EBULL;
-    z ^= z >> 31;
-    return z;
+    x ^= x >> 16; x *= 0x7FEB352DU;
+    x ^= x >> 15; x *= 0x846CA68BU;
+    x ^= x >> 16;
+    return x;
 }
 
-__device__ __forceinline__ unsigned int rng_u24(unsigned long long seed, unsigned int sample, unsigned int lo,
-                                                unsigned int hi)
+__device__ __forceinline__ unsigned int rng_u24(unsigned int key, unsigned int lo, unsigned int hi)
 {
-    unsigned long long x = seed ^ (0x9E3779B97F4A7C15ULL * ((unsigned long long)sample + 1ULL));
-    x = splitmix_fin(x + (unsigned long long)lo);
-    x = splitmix_fin(x ^ ((unsigned long long)hi * 0xD1B54A32D192ED03ULL));
-    return (unsigned int)(x >> 40);
+    unsigned int h = mix32(key + lo);
+    h = mix32(h ^ (hi * 0x85EBCA6BU));
+    return h >> 8;
 }
 
 struct StochParams {
-    float b2;       // fl(b_link * b_link): the scale of Eq. 8
-    float alpha;
-    float gscale;   // -2 alpha / b2
-    unsigned long long seed;
-    unsigned int sample;
+    float b2;          // fl(b_link * b_link): the scale of Eq. 8
+    float c;           // fl(alpha / b2): t = c (b2 - d2)
+    float gscale;      // -2 c
+    unsigned int key;  // mix32(fold(seed) ^ (sample * 0x9E3779B9))
 };
 
 __global__ void __launch_bounds__(kBlock) iota_kernel(int *__restrict__ labels, int64_t N)
@@ -93,7 +90,7 @@ __global__ void __launch_bounds__(kBlock) link_stochastic_kernel(const float4 *_
               cz = min(__float2int_rd(uz), g.n_minus_1);
     const float fx = ux - (float)cx, fy = uy - (float)cy, fz = uz - (float)cz;
     const float lo = g.reach, hi = 1.0f - g.reach;
-    double lp = 0.0;
+    float lp = 0.0f;  // a lane adds at most a few thousand O(1) terms: float32 is enough before the float64 reduction
     unsigned int ncand = 0, nedge = 0;
     s_g[wib][lane][0] = s_g[wib][lane][1] = s_g[wib][lane][2] = 0.0f;
     __syncwarp();
@@ -144,12 +141,11 @@ __global__ void __launch_bounds__(kBlock) link_stochastic_kernel(const float4 *_
                 const float ddz = min_image(__fsub_rn(oz, pj.z), g.L, g.h);
                 const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(ddx, ddx), __fmul_rn(ddy, ddy)), __fmul_rn(ddz, ddz));
                 if (d2 <= g.b2) {  // R25: beyond the candidate radius p = 0
-                    const float tt = __fmul_rn(sp.alpha, __fdiv_rn(__fsub_rn(sp.b2, d2), sp.b2));
+                    const float tt = __fmul_rn(sp.c, __fsub_rn(sp.b2, d2));
                     float e;
                     const float pr = sigmoid_fixed(tt, e);
                     const unsigned int oj = (unsigned int)__ldg(idx_s + j);
-                    const float u = __fmul_rn((float)rng_u24(sp.seed, sp.sample, min(ooi, oj), max(ooi, oj)),
-                                              5.9604644775390625e-8f);
+                    const float u = __fmul_rn((float)rng_u24(sp.key, min(ooi, oj), max(ooi, oj)), 5.9604644775390625e-8f);
                     const bool y = u < pr;
                     const float tc = fminf(fmaxf(tt, -30.0f), 30.0f);
                     if (grad && tt == tc) {
@@ -160,8 +156,8 @@ __global__ void __launch_bounds__(kBlock) link_stochastic_kernel(const float4 *_
                     }
                     if (forward || (q == 13 && j > osi)) {
                         ++ncand;
-                        // log p = -log1p(e); log(1 - p) = log(e / (1 + e)) = log p - t; float32 terms, float64 sum
-                        lp += (double)(-log1pf(e) - (y ? 0.0f : tc));
+                        // log p = -log(1 + e); log(1 - p) = log(e / (1 + e)) = log p - t; float32 terms
+                        lp += -__logf(__fadd_rn(1.0f, e)) - (y ? 0.0f : tc);
                         if (y) {
                             ++nedge;
                             const int pa = osi - (int)rel[osi], pb = j - (int)rel[j];
@@ -196,13 +192,14 @@ __global__ void __launch_bounds__(kBlock) link_stochastic_kernel(const float4 *_
         grad[3 * (int64_t)oi + 1] = s_g[wib][lane][1];
         grad[3 * (int64_t)oi + 2] = s_g[wib][lane][2];
     }
+    double lpd = (double)lp;
     for (int o = 16; o > 0; o >>= 1) {
-        lp += __shfl_xor_sync(0xffffffffu, lp, o);
+        lpd += __shfl_xor_sync(0xffffffffu, lpd, o);
         ncand += __shfl_xor_sync(0xffffffffu, ncand, o);
         nedge += __shfl_xor_sync(0xffffffffu, nedge, o);
     }
     if (lane == 0) {
-        if (lp != 0.0) atomicAdd(logp, lp);
+        if (lpd != 0.0) atomicAdd(logp, lpd);
         if (ncand) atomicAdd(&ctrl->pair_tests, (unsigned long long)ncand);  // potential edges of this sample
         if (nedge) atomicAdd(&ctrl->edges, (unsigned long long)nedge);       // sampled edges
     }
@@ -222,10 +219,13 @@ cudaError_t launch_link_stochastic(const float4 *sorted, int64_t N, Grid g, cons
     if ((e = cudaMemsetAsync(rel, 0, (size_t)N * sizeof(unsigned int), s)) != cudaSuccess) return e;
     StochParams sp;
     sp.b2 = b_link * b_link;
-    sp.alpha = alpha;
-    sp.gscale = (float)(-2.0 * (double)alpha / (double)sp.b2);
-    sp.seed = seed;
-    sp.sample = sample;
+    sp.c = alpha / sp.b2;
+    sp.gscale = -2.0f * sp.c;
+    unsigned int k = (unsigned int)(seed ^ (seed >> 32)) ^ (sample * 0x9E3779B9U);  // per-sample key: mix32 on the host
+    k ^= k >> 16; k *= 0x7FEB352DU;
+    k ^= k >> 15; k *= 0x846CA68BU;
+    k ^= k >> 16;
+    sp.key = k;
     iota_kernel<<<blocks_for(N, kBlock), kBlock, 0, s>>>(labels, N);
     link_stochastic_kernel<<<blocks_for(N, kBlock), kBlock, 0, s>>>(sorted, N, g, cell_start, idx_s, rel, sp, logp, grad,
                                                                     ctrl);
