@@ -227,7 +227,21 @@ def run_ours(args):
         K_groups = step()
     torch.cuda.synchronize()
 
-    # ---- timed region: device-resident inputs; K steps bracketed by barrier + synchronize
+    # ---- stage breakdown: a pass of its own with events around every stage (they cost ~0.06 ms per step,
+    # so they stay out of the timed region); it also tells which stage dominates
+    n_break = max(3, min(args.steps, 10))
+    B.fof_profile_only(f.h, None)
+    B.fof_profile_enable(f.h, n_break)
+    for _ in range(n_break):
+        step()
+    torch.cuda.synchronize()
+    stages = B.fof_profile_read(f.h)
+    B.fof_profile_enable(f.h, 0)
+    top = max(stages, key=lambda k: stages[k])
+
+    # ---- timed region: device-resident inputs; K steps bracketed by barrier + synchronize; only the
+    # dominant stage carries events (two per step), its live time feeds the roofline
+    B.fof_profile_only(f.h, top)
     B.fof_profile_enable(f.h, args.steps)
     launches0 = B.fof_launch_count(f.h)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -242,8 +256,9 @@ def run_ours(args):
     barrier()
     ms_total = e0.elapsed_time(e1)
     launches = B.fof_launch_count(f.h) - launches0
-    stages = B.fof_profile_read(f.h)
+    top_ms_live = B.fof_profile_read(f.h)[top]
     B.fof_profile_enable(f.h, 0)
+    B.fof_profile_only(f.h, None)
     E, pair_tests, grid_pairs = f.link_stats()
     ms_step = max_over_ranks_ms(ms_total, world, dev) / args.steps
     value = whole_job_value(world, N, ms_step)
@@ -369,9 +384,8 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel (live CUDA-event times from inside the timed region)
     peak, peak_src = peaks()
-    top = max(stages, key=lambda k: stages[k])
     alg = ALG_BYTES_PER_PARTICLE.get(top, 0) * N
-    hbm_achieved = alg / (stages[top] * 1e-3) / 1e9 if stages[top] > 0 else 0.0
+    hbm_achieved = alg / (top_ms_live * 1e-3) / 1e9 if top_ms_live > 0 else 0.0
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")  # written by hand from the ncu --set full capture
     if os.path.exists(tpath):
@@ -395,18 +409,18 @@ def run_ours(args):
         except Exception:
             mhz = 1965.0
         alu_peak = sms * 4 * 32 * mhz * 1e6 / 1e9  # G lane-operations / s
-        alu_achieved = 9.0 * pair_tests / (stages[top] * 1e-3) / 1e9
+        alu_achieved = 9.0 * pair_tests / (top_ms_live * 1e-3) / 1e9
         roofline = {"bound": "alu", "kernel": top, "achieved": alu_achieved, "peak": alu_peak, "unit": "GOP/s",
                     "frac": alu_achieved / alu_peak, "traffic": traffic,
                     "peak_source": f"{sms} SMs x 4 schedulers x 32 lanes x {mhz:.0f} MHz (DESIGN.md 6)",
-                    "alg_ops_per_launch": 9 * pair_tests, "kernel_ms": stages[top],
+                    "alg_ops_per_launch": 9 * pair_tests, "kernel_ms": top_ms_live,
                     "hbm": {"alg_bytes_per_launch": alg, "achieved": hbm_achieved, "peak": peak, "unit": "GB/s",
                             "frac": hbm_achieved / peak, "peak_source": peak_src},
                     "path": path}
     else:
         roofline = {"bound": "hbm", "kernel": top, "achieved": hbm_achieved, "peak": peak, "unit": "GB/s",
                     "frac": hbm_achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                    "alg_bytes_per_launch": alg, "kernel_ms": stages[top], "path": path}
+                    "alg_bytes_per_launch": alg, "kernel_ms": top_ms_live, "path": path}
 
     # ---- the oracle timed beside it on the host cores (a reported baseline, not the target)
     cpu = None
@@ -430,6 +444,8 @@ def run_ours(args):
         "pair_tests_per_s": pair_tests / (stages["link.pairs"] * 1e-3) if stages.get("link.pairs") else None,
         "grid_pairs_per_s": grid_pairs / (stages["link.pairs"] * 1e-3) if stages.get("link.pairs") else None,
         "stage_ms": {k: round(v, 5) for k, v in stages.items()},
+        "stage_ms_note": f"separate pass of {n_break} steps with events around every stage; the timed region carries "
+                         f"events around {top} only (roofline.kernel_ms)",
         "roofline": roofline, "cpu_baseline": cpu, "parity_vs_oracle_in_this_run": parity,
         "e2e": {"value": whole_job_value(world, N, e2e_ms), "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
                 "h2d_bytes_per_step": int(hpos.numel() * 4),

@@ -194,6 +194,9 @@ int fof_status(fof_handle *h, void *ws, void *stream);
  * fof_profile_name(h, k) is a static string ("link.bin", "groups.reduce", ...).
  * fof_launch_count: kernels this handle has launched so far (memsets and copies not counted). */
 int fof_profile_enable(fof_handle *h, int slots);
+/* Restrict the recorded events to stage `stage` (0 <= stage < fof_profile_count), or -1 for every stage
+ * (the default): two events per step instead of two per stage keep the timed region undisturbed. */
+int fof_profile_only(fof_handle *h, int stage);
 int fof_profile_count(const fof_handle *h);
 const char *fof_profile_name(const fof_handle *h, int k);
 int fof_profile_read(fof_handle *h, float *ms, int cap);

@@ -82,6 +82,8 @@ def lib():
         L.fof_status.argtypes = [vp, vp, vp]
         L.fof_profile_enable.restype = ctypes.c_int
         L.fof_profile_enable.argtypes = [vp, ctypes.c_int]
+        L.fof_profile_only.restype = ctypes.c_int
+        L.fof_profile_only.argtypes = [vp, ctypes.c_int]
         L.fof_profile_count.restype = ctypes.c_int
         L.fof_profile_count.argtypes = [vp]
         L.fof_profile_name.restype = ctypes.c_char_p
@@ -231,6 +233,12 @@ def fof_status(h, ws, stream=None) -> int:
 
 def fof_profile_enable(h, slots: int):
     _check(lib().fof_profile_enable(h, int(slots)), h)
+
+
+def fof_profile_only(h, stage_name=None):
+    """Record events for one stage only (by name), or for every stage (None)."""
+    k = -1 if stage_name is None else fof_profile_names(h).index(stage_name)
+    _check(lib().fof_profile_only(h, k), h)
 
 
 def fof_profile_names(h):

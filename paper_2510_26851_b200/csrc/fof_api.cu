@@ -80,12 +80,13 @@ struct StageTimer {  // records the two events of a stage around its launches
     StageTimer(fof_handle *h_, cudaStream_t s_, int k_, int kernels) : h(h_), s(s_), k(k_)
     {
         h->launches += (unsigned long long)kernels;
-        if (h->prof_slots) {
+        if (on()) {
             cudaEventRecord(h->ev[(h->prof_cur * kMaxStages + k) * 2], s);
             h->ev_valid[h->prof_cur * kMaxStages + k] = true;
         }
     }
-    ~StageTimer() { if (h->prof_slots) cudaEventRecord(h->ev[(h->prof_cur * kMaxStages + k) * 2 + 1], s); }
+    ~StageTimer() { if (on()) cudaEventRecord(h->ev[(h->prof_cur * kMaxStages + k) * 2 + 1], s); }
+    bool on() const { return h->prof_slots && (h->prof_only < 0 || h->prof_only == k); }
 };
 
 }  // namespace
@@ -94,14 +95,15 @@ namespace fof {
 void StageHook::begin(int k, int kernels)
 {
     h->launches += (unsigned long long)kernels;
-    if (h->prof_slots) {
+    if (h->prof_slots && (h->prof_only < 0 || h->prof_only == base + k)) {
         cudaEventRecord(h->ev[(h->prof_cur * kMaxStages + base + k) * 2], s);
         h->ev_valid[h->prof_cur * kMaxStages + base + k] = true;
     }
 }
 void StageHook::end(int k)
 {
-    if (h->prof_slots) cudaEventRecord(h->ev[(h->prof_cur * kMaxStages + base + k) * 2 + 1], s);
+    if (h->prof_slots && (h->prof_only < 0 || h->prof_only == base + k))
+        cudaEventRecord(h->ev[(h->prof_cur * kMaxStages + base + k) * 2 + 1], s);
 }
 }  // namespace fof
 
@@ -135,6 +137,7 @@ int fof_create(int64_t N, float L, float b, int32_t N_min, fof_handle **out)
     if (!h) return FOF_ERR_INVALID_ARG;
     memset(h, 0, sizeof(*h));
     h->N = N; h->L = L; h->b = b; h->N_min = N_min;
+    h->prof_only = -1;
     h->n_max = n_max;
     h->n = n_occ < n_max ? n_occ : n_max;
     if (h->n < 3) h->n = 3;
@@ -170,6 +173,13 @@ int fof_profile_enable(fof_handle *h, int slots)
         h->prof_cur = slots - 1;
         h->prof_slots = slots;
     }
+    return FOF_OK;
+}
+
+int fof_profile_only(fof_handle *h, int stage)
+{
+    if (!h || stage < -1 || stage >= kNumStages) return FOF_ERR_INVALID_ARG;
+    h->prof_only = stage;
     return FOF_OK;
 }
 

@@ -102,6 +102,7 @@ struct fof_handle {
     char cuda_err[256];
     // measurement aids
     int prof_slots;        // 0 = profiling off; else event sets used round-robin, one per fof_link call
+    int prof_only;         // -1: every stage is timed; k: only stage k (fof_profile_only)
     int prof_cur;          // slot of the current (last) fof_link
     cudaEvent_t *ev;       // [slot][2k] before, [slot][2k+1] after stage k
     bool *ev_valid;        // [slot][k]
