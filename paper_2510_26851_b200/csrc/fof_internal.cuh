@@ -58,8 +58,8 @@ constexpr int kLinkBlock = 256;     // threads per CTA of the link kernels
 #ifndef FOF_DENSE_CELL
 #define FOF_DENSE_CELL 8
 #endif
-constexpr int kDenseCell = FOF_DENSE_CELL;       // cells with >= kDenseCell particles are DENSE: every pair that involves one of
-                                    // their particles belongs to link_tiles_kernel, all others to link_sparse_kernel
+constexpr int kDenseCell = FOF_DENSE_CELL;  // cells with >= kDenseCell particles are DENSE: the pairs whose home cell is
+                                            // dense belong to the tile role of link_kernel, all others to its sparse role
 
 // A dense cell of m particles is cut into dense_tiles(m) tiles of dense_tile_size(m) <= 32
 // consecutive particles (balanced: 43 -> 22 + 21, not 32 + 11); one work item per tile.

@@ -1,4 +1,4 @@
-// kernels_link.cu — H4 half-stencil pair tests + union, H5 flatten + canonical labels.
+// kernels_link.cu — H4 half-stencil pair tests + union, H5 canonical labels.
 // What is linked: PAPER.md:85-87 (§2 step iv) and PAPER.md:200-214 (Alg. 2 candidate cells and
 // mask); the 27-cell stencil with indices mod n is PAPER.md:202.  The T label sweeps of
 // PAPER.md:221-225 are replaced by their fixed point, computed with a lock-free union-find
@@ -7,22 +7,22 @@
 //
 // Design.  The union-find runs in CELL-SORTED index space: a component is a
 // spatially compact object, so its parent entries sit in a few cache lines.  Every unordered
-// pair of particles in the same or in adjacent cells is tested exactly once, by one of two kernels:
-//   link_tiles_kernel   pairs with at least one particle in a DENSE cell (>= kDenseCell particles).
-//                       One warp per (dense cell, tile of <= 32 of its particles): the tile sits in
-//                       registers, one particle per lane; the candidates (the tile itself, the
-//                       earlier tiles of the cell, and the particles of the 26 neighbour cells that
-//                       lie within b of the cell) are staged 32 at a time in shared memory and
-//                       broadcast, so one trip of 11 instructions tests 32 pairs.  The adjacency
-//                       comes out as ballot bitmasks; components of the tile are closed in registers
-//                       and only one hook per (component, adjacent candidate) reaches the union-find.
-//                       A pair of two dense cells belongs to the one that sees the other in its
-//                       forward half stencil.
-//   link_sparse_kernel  pairs of two sparse cells.  One thread per particle collects its candidate
-//                       ranges (own cell after itself + the 13 forward cells, reach-filtered);
-//                       the ranges of a warp are flattened into one list of candidate slots that
-//                       the 32 lanes walk together, so a lane with many candidates does not hold
-//                       the others hostage.
+// pair of particles in the same or in adjacent cells is tested exactly once, by one of the two roles
+// of link_kernel, the one that owns the pair's HOME cell (the cell that sees the other one in its
+// forward half stencil):
+//   tile role    home cell DENSE (>= kDenseCell particles).  One warp per (dense cell, tile of <= 32
+//                of its particles): the tile sits in registers, one particle per lane; the
+//                candidates (the tile itself, the earlier tiles of the cell, and the particles of
+//                the 13 forward cells that lie within b of the cell) are staged 32 at a time in
+//                shared memory and broadcast, so one trip of ~13 instructions tests 32 pairs.  The
+//                adjacency comes out as ballot bitmasks; components of the tile are closed in
+//                registers and only one hook per (component, adjacent candidate) reaches the
+//                union-find.
+//   sparse role  home cell sparse.  One thread per particle collects its candidate ranges (own cell
+//                after itself + the forward cells, reach-filtered); the ranges of a warp are
+//                flattened into one list of candidate slots that the 32 lanes walk together, so a
+//                lane with many candidates does not hold the others hostage; ranges longer than
+//                kLongRange (dense neighbour cells) are walked by the whole warp.
 // The root of a set is its member with the smallest ORIGINAL index, so the canonical label is
 // read off the root by one streaming pass (chase + scatter to labels[original index]).
 #include "fof_internal.cuh"

@@ -191,7 +191,7 @@ __global__ void __launch_bounds__(kPartThreads) part_scatter_kernel(const float 
 // ---------------------------------------------------------------------------------------------
 // H2 + H3 (level 2): one CTA per bin.  Shared memory: one counter per cell of the bin.
 //   1. histogram of the bin's records over its cells (shared-memory atomics);
-//   2. exclusive scan -> cell_start[] (coalesced), work items of link_tiles_kernel (dense cells);
+//   2. exclusive scan -> cell_start[] (coalesced), work items of the tile role of link_kernel (dense cells);
 //   3. records re-read (L2) and moved to their final slot; rel = 0 (every particle a root),
 //      idx_s = original index (the order of the union-find, input of H5).
 // ---------------------------------------------------------------------------------------------
