@@ -613,3 +613,21 @@ def test_slab_fof_equals_monolithic(B, world):
         assert np.array_equal(lab.cpu().numpy(), mono[o]), "slab labels differ from the monolithic run"
         crossing += int((~np.isin(mono[o], o)).sum())
     assert crossing > nz // 2          # many particles whose canonical particle lives on another rank
+
+
+@pytest.mark.parametrize("grid", [3, 4, 5, 6, 7])
+def test_tiny_grids_wrap_everywhere(B, grid):
+    """n = 3 .. 5 cells per axis: every stencil wraps and the minimum-image selects are live in both roles
+    of the link kernel; n = 6, 7: the first grids where interior warps take the wrap-free variant.  Dense
+    clumps on the box corner and faces plus a sparse background."""
+    rng = np.random.default_rng(100 + grid)
+    L, b = 10.0, 1.0
+    corner = rng.standard_normal((400, 3)) * 0.5                      # straddles all three faces at 0 / L
+    face = rng.standard_normal((300, 3)) * 0.4 + np.array([5.0, 0.0, 5.0])
+    bg = rng.random((1500, 3)) * L
+    p = (np.concatenate([corner, face, bg]) % L).astype(np.float32)
+    p[p >= np.float32(L)] = 0.0
+    p = p[rng.permutation(len(p))]
+    got, lab, og = check_against_oracle(B, p, L, b, 5, grid=grid, brute=True,
+                                        mass=rng.uniform(0.5, 1.5, len(p)).astype(np.float32))
+    assert got["grid"][0] == grid and og["group_size"].max() > 300
