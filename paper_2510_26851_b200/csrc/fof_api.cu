@@ -327,7 +327,7 @@ int fof_groups(fof_handle *h, const float *pos, const float *mass, const int32_t
     }
     {
         StageTimer t(h, s, kGroupsReduce, has);
-        CK(launch_group_reduce(pos, mass, labels, h->N, h->grid, cnt, cap, acc, particle_group, s),
+        CK(launch_group_reduce(pos, mass, labels, h->N, h->grid, cnt, cap, group_size, acc, particle_group, s),
            "group_reduce_kernel");
     }
     const int64_t fin = cap < h->max_groups ? cap : h->max_groups;

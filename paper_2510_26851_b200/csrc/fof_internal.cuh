@@ -225,7 +225,8 @@ cudaError_t launch_group_compact(const int *labels, int64_t N, int N_min, int *c
                                  int *group_label, int *group_size, double *acc, unsigned long long *state,
                                  Ctrl *ctrl, int64_t tiles, cudaStream_t s);
 cudaError_t launch_group_reduce(const float *pos, const float *mass, const int *labels, int64_t N, Grid g,
-                                const int *gid, int64_t cap, double *acc, int *particle_group, cudaStream_t s);
+                                const int *gid, int64_t cap, const int *group_size, double *acc, int *particle_group,
+                                cudaStream_t s);
 cudaError_t launch_group_finish(const float *pos, const int *group_label, const int *group_size,
                                 const double *acc, bool has_mass, Grid g, int64_t cap, const Ctrl *ctrl,
                                 float *group_mass, float *group_com, cudaStream_t s);

@@ -162,6 +162,12 @@ __global__ void __launch_bounds__(kBlock) group_compact_kernel(const int *__rest
 
 // H8 accumulate: for every member of a kept group, delta = min-image(w_i - r) in double with
 // r = wrapped position of the canonical particle; acc[g] += (m dx, m dy, m dz, m).
+// The pass is bound by the L2 atomic rate (three or four float64 atomics per member), so groups of
+// fewer than kFloatAccMax members use ONE 128-bit float32 atomic per member instead (the same
+// 32-byte slot read as a float4): with deltas of at most L/2 and < 4096 terms the float32 sums stay
+// ~1e-3 ulp(L) per member away from the float64 ones, far inside the 1e-5 L tolerance; larger groups
+// (a percolating component) keep float64.
+constexpr int kFloatAccMax = 4096;
 __device__ __forceinline__ double min_image_d(double d, double L, double h)
 {
     if (d > h) d -= L;
@@ -174,7 +180,8 @@ __global__ void __launch_bounds__(kBlock) group_reduce_kernel(const float *__res
                                                               const float *__restrict__ mass,
                                                               const int *__restrict__ labels, int64_t N, Grid g,
                                                               const int *__restrict__ gid_of, int64_t cap,
-                                                              double *acc, int *__restrict__ particle_group)
+                                                              const int *__restrict__ group_size, double *acc,
+                                                              int *__restrict__ particle_group)
 {
     const int64_t i0 = ((int64_t)blockIdx.x * kBlock + threadIdx.x) * kPer;
     if (i0 >= N) return;
@@ -202,19 +209,28 @@ __global__ void __launch_bounds__(kBlock) group_reduce_kernel(const float *__res
         const int64_t i = i0 + k;
         const double m = mass ? (double)__ldg(mass + i) : 1.0;
         double *dst = acc + 4 * (int64_t)gid[k];
-        if (l[k] != (int)i) {  // the canonical particle itself has delta = 0
-            double d[3];
+        double d[3] = {0.0, 0.0, 0.0};
+        const bool member = l[k] != (int)i;  // the canonical particle itself has delta = 0
+        if (member) {
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
                 const float wi = wrap1(__ldg(pos + 3 * i + a), g.L);
                 const float wr = wrap1(__ldg(pos + 3 * (int64_t)l[k] + a), g.L);
                 d[a] = min_image_d((double)wi - (double)wr, L, h);
             }
-            atomicAdd(dst + 0, m * d[0]);
-            atomicAdd(dst + 1, m * d[1]);
-            atomicAdd(dst + 2, m * d[2]);
         }
-        if (mass) atomicAdd(dst + 3, m);
+        if (__ldg(group_size + gid[k]) < kFloatAccMax) {
+            if (member || mass)
+                atomicAdd(reinterpret_cast<float4 *>(dst),
+                          make_float4((float)(m * d[0]), (float)(m * d[1]), (float)(m * d[2]), mass ? (float)m : 0.0f));
+        } else {
+            if (member) {
+                atomicAdd(dst + 0, m * d[0]);
+                atomicAdd(dst + 1, m * d[1]);
+                atomicAdd(dst + 2, m * d[2]);
+            }
+            if (mass) atomicAdd(dst + 3, m);
+        }
     }
 }
 
@@ -232,13 +248,20 @@ __global__ void __launch_bounds__(kBlock) group_finish_kernel(const float *__res
     if (K > cap) K = cap;
     if (k >= K) return;
     const int l = group_label[k];
-    const double M = has_mass ? acc[4 * k + 3] : (double)group_size[k];
+    double sum[4];
+    if (group_size[k] < kFloatAccMax) {  // float32 slot (see group_reduce_kernel)
+        const float4 f = *reinterpret_cast<const float4 *>(acc + 4 * k);
+        sum[0] = f.x; sum[1] = f.y; sum[2] = f.z; sum[3] = f.w;
+    } else {
+        sum[0] = acc[4 * k]; sum[1] = acc[4 * k + 1]; sum[2] = acc[4 * k + 2]; sum[3] = acc[4 * k + 3];
+    }
+    const double M = has_mass ? sum[3] : (double)group_size[k];
     const double L = (double)g.L;
     group_mass[k] = (float)M;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         const float wr = wrap1(pos[3 * (int64_t)l + a], g.L);
-        double c = (double)wr + acc[4 * k + a] / M;
+        double c = (double)wr + sum[a] / M;
         if (c < 0.0) c += L;
         if (c >= L) c -= L;
         float cf = (float)c;
@@ -271,14 +294,15 @@ cudaError_t launch_group_compact(const int *labels, int64_t N, int N_min, int *c
 }
 
 cudaError_t launch_group_reduce(const float *pos, const float *mass, const int *labels, int64_t N, Grid g,
-                                const int *gid, int64_t cap, double *acc, int *particle_group, cudaStream_t s)
+                                const int *gid, int64_t cap, const int *group_size, double *acc, int *particle_group,
+                                cudaStream_t s)
 {
     if (N <= 0) return cudaSuccess;
     const unsigned int grid = blocks_for(N, kBlock * kPer);
     if (aligned16(labels) && aligned16(particle_group))
-        group_reduce_kernel<true><<<grid, kBlock, 0, s>>>(pos, mass, labels, N, g, gid, cap, acc, particle_group);
+        group_reduce_kernel<true><<<grid, kBlock, 0, s>>>(pos, mass, labels, N, g, gid, cap, group_size, acc, particle_group);
     else
-        group_reduce_kernel<false><<<grid, kBlock, 0, s>>>(pos, mass, labels, N, g, gid, cap, acc, particle_group);
+        group_reduce_kernel<false><<<grid, kBlock, 0, s>>>(pos, mass, labels, N, g, gid, cap, group_size, acc, particle_group);
     return cudaGetLastError();
 }
 
