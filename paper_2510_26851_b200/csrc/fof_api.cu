@@ -31,7 +31,8 @@ void layout(fof_handle *h)
     h->off_cell = off;        off += align256(((size_t)cell_items + 8) * sizeof(unsigned int));
     h->off_rel = off;         off += align256((N + 1) * sizeof(unsigned int));
     h->off_cta_hist = off;    off += align256((size_t)kMaxPartCtas * h->sort.bins * sizeof(unsigned int));
-    h->off_bin_base = off;    off += align256(((size_t)h->sort.bins + 2) * sizeof(unsigned int));
+    // fine bin offsets, and behind them the coarse ones of the two-pass partition (<= bins / 64 + 2 entries)
+    h->off_bin_base = off;    off += align256(((size_t)h->sort.bins + 2 + (size_t)h->sort.bins / 64 + 4) * sizeof(unsigned int));
     h->off_part = off;        off += align256((N + 1) * sizeof(float4));
     h->off_idx = off;         off += align256((N + 1) * sizeof(int));
     h->off_dense = off;       off += align256((N / kDenseCell + N / 32 + 2) * sizeof(unsigned long long));

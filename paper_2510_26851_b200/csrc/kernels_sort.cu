@@ -307,6 +307,62 @@ __global__ void __launch_bounds__(kCellSortThreads) cell_sort_kernel(
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Second partition pass (only when there are more than kTwoPassBins bins): the input is the
+// coarse-bin-contiguous record array of a first pass over bins 2^kCoarseShift times wider (a few
+// dozen write streams per CTA, each a long run), so a CTA's contiguous chunk only touches ~1000 fine
+// bins inside one coarse bin (tens of MB): the open write streams stay in the L2 and in the TLB.  At
+// 512^3 a single pass has 148 CTAs x 32768 streams spread over 2 GB: 4.7 ms; two passes: 3.3 ms
+// (measured with 2^6 .. 2^11: 5.0, 5.2 (2^8), 3.6, 3.3, 3.8 ms).
+// ---------------------------------------------------------------------------------------------
+constexpr int kTwoPassBins = 8192;
+#ifndef FOF_COARSE_SHIFT
+#define FOF_COARSE_SHIFT 10
+#endif
+constexpr int kCoarseShift = FOF_COARSE_SHIFT;
+
+__global__ void __launch_bounds__(kPartThreads) rec_hist_kernel(const float4 *__restrict__ rec, int64_t N, Grid g,
+                                                                int shift, int bins, int64_t chunk,
+                                                                unsigned int *__restrict__ cta_hist)
+{
+    extern __shared__ unsigned int s_bin[];
+    for (int b = threadIdx.x; b < bins; b += kPartThreads) s_bin[b] = 0u;
+    __syncthreads();
+    const int64_t i0 = (int64_t)blockIdx.x * chunk, i1 = min(N, i0 + chunk);
+    for (int64_t i = i0 + threadIdx.x; i < i1; i += 4 * kPartThreads) {
+        float4 v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = __ldg(rec + min(i + u * kPartThreads, i1 - 1));
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (i + u * kPartThreads < i1) atomicAdd(&s_bin[cell_of(v[u], g) >> shift], 1u);
+    }
+    __syncthreads();
+    unsigned int *dst = cta_hist + (int64_t)blockIdx.x * bins;
+    for (int b = threadIdx.x; b < bins; b += kPartThreads) dst[b] = s_bin[b];
+}
+
+__global__ void __launch_bounds__(kPartThreads) rec_scatter_kernel(const float4 *__restrict__ rec, int64_t N, Grid g,
+                                                                   int shift, int bins, int64_t chunk,
+                                                                   const unsigned int *__restrict__ cta_hist,
+                                                                   const unsigned int *__restrict__ bin_base,
+                                                                   float4 *__restrict__ out)
+{
+    extern __shared__ unsigned int s_bin[];
+    const unsigned int *src = cta_hist + (int64_t)blockIdx.x * bins;
+    for (int b = threadIdx.x; b < bins; b += kPartThreads) s_bin[b] = src[b] + bin_base[b];
+    __syncthreads();
+    const int64_t i0 = (int64_t)blockIdx.x * chunk, i1 = min(N, i0 + chunk);
+    for (int64_t i = i0 + threadIdx.x; i < i1; i += 4 * kPartThreads) {
+        float4 v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = __ldg(rec + min(i + u * kPartThreads, i1 - 1));
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (i + u * kPartThreads < i1) out[atomicAdd(&s_bin[cell_of(v[u], g) >> shift], 1u)] = v[u];
+    }
+}
+
 static inline cudaError_t set_smem(const void *fn, size_t bytes)
 {
     if (bytes <= 48 * 1024) return cudaSuccess;
@@ -330,16 +386,42 @@ cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp,
     if ((e = set_smem((const void *)cell_sort_kernel, smem_cells)) != cudaSuccess) return e;
     const int64_t chunk = ((N + ctas - 1) / ctas + 3) & ~(int64_t)3;  // a multiple of 4: quads stay aligned
     const int64_t C = (int64_t)g.n * g.n * g.n;
-    hook.begin(0, 1);
-    hist<<<ctas, kPartThreads, smem_bins, s>>>(pos, N, g, sp.shift, sp.bins, chunk, cta_hist, ctrl);
-    hook.end(0);
-    hook.begin(1, 1);
-    part_offsets_kernel<<<(sp.bins + 31) / 32, 32 * kOffGroups, 0, s>>>(cta_hist, ctas, sp.bins, bin_base, ctrl);
-    hook.end(1);
-    hook.begin(2, 1);
-    scat<<<ctas, kPartThreads, smem_bins, s>>>(pos, N, g, sp.shift, sp.bins, chunk, cta_hist, bin_base,
-                                                             part, labels, ((uintptr_t)labels & 15) == 0);
-    hook.end(2);
+    const bool labels_vec = ((uintptr_t)labels & 15) == 0;
+    if (sp.bins <= kTwoPassBins) {
+        hook.begin(0, 1);
+        hist<<<ctas, kPartThreads, smem_bins, s>>>(pos, N, g, sp.shift, sp.bins, chunk, cta_hist, ctrl);
+        hook.end(0);
+        hook.begin(1, 1);
+        part_offsets_kernel<<<(sp.bins + 31) / 32, 32 * kOffGroups, 0, s>>>(cta_hist, ctas, sp.bins, bin_base, ctrl);
+        hook.end(1);
+        hook.begin(2, 1);
+        scat<<<ctas, kPartThreads, smem_bins, s>>>(pos, N, g, sp.shift, sp.bins, chunk, cta_hist, bin_base, part, labels,
+                                                   labels_vec);
+        hook.end(2);
+    } else {
+        // pass 1 over bins 2^kCoarseShift times wider: pos -> `sorted` (used as scratch); pass 2: -> `part`
+        const int cshift = sp.shift + kCoarseShift;
+        const int cbins = (int)((C + ((int64_t)1 << cshift) - 1) >> cshift);
+        unsigned int *cbase = bin_base + sp.bins + 2;  // the coarse bin offsets live behind the fine ones
+        if ((e = set_smem((const void *)rec_hist_kernel, smem_bins)) != cudaSuccess) return e;
+        if ((e = set_smem((const void *)rec_scatter_kernel, smem_bins)) != cudaSuccess) return e;
+        const size_t smem_c = (size_t)cbins * sizeof(unsigned int);
+        hook.begin(0, 1);
+        hist<<<ctas, kPartThreads, smem_c, s>>>(pos, N, g, cshift, cbins, chunk, cta_hist, ctrl);
+        hook.end(0);
+        hook.begin(1, 2);
+        part_offsets_kernel<<<(cbins + 31) / 32, 32 * kOffGroups, 0, s>>>(cta_hist, ctas, cbins, cbase, ctrl);
+        hook.end(1);
+        hook.begin(2, 3);
+        scat<<<ctas, kPartThreads, smem_c, s>>>(pos, N, g, cshift, cbins, chunk, cta_hist, cbase, sorted, labels,
+                                                labels_vec);
+        rec_hist_kernel<<<ctas, kPartThreads, smem_bins, s>>>(sorted, N, g, sp.shift, sp.bins, chunk, cta_hist);
+        if ((e = cudaMemsetAsync(&ctrl->scan_ticket, 0, sizeof(unsigned int), s)) != cudaSuccess) return e;
+        part_offsets_kernel<<<(sp.bins + 31) / 32, 32 * kOffGroups, 0, s>>>(cta_hist, ctas, sp.bins, bin_base, ctrl);
+        rec_scatter_kernel<<<ctas, kPartThreads, smem_bins, s>>>(sorted, N, g, sp.shift, sp.bins, chunk, cta_hist,
+                                                                 bin_base, part);
+        hook.end(2);
+    }
     hook.begin(3, 1);
     cell_sort_kernel<<<sp.bins, kCellSortThreads, smem_cells, s>>>(part, bin_base, g, sp.shift, C, cell_start, sorted,
                                                                   rel, idx_s, dense_list, ctrl);
