@@ -315,7 +315,10 @@ __global__ void __launch_bounds__(kCellSortThreads) cell_sort_kernel(
 // 512^3 a single pass has 148 CTAs x 32768 streams spread over 2 GB: 4.7 ms; two passes: 3.3 ms
 // (measured with 2^6 .. 2^11: 5.0, 5.2 (2^8), 3.6, 3.3, 3.8 ms).
 // ---------------------------------------------------------------------------------------------
-constexpr int kTwoPassBins = 8192;
+#ifndef FOF_TWO_PASS_BINS
+#define FOF_TWO_PASS_BINS 8192
+#endif
+constexpr int kTwoPassBins = FOF_TWO_PASS_BINS;
 #ifndef FOF_COARSE_SHIFT
 #define FOF_COARSE_SHIFT 10
 #endif
