@@ -12,6 +12,14 @@
 using namespace fof;
 
 namespace {
+// Most work items the cell sort can list: every dense cell of m particles gives at most m / kDenseCell
+// tiles, a heavy one (m >= kHeavyCell) at most (m / 32 + 1) kHeavyParts items.
+size_t dense_items_max(size_t N)
+{
+    const size_t plain = N / kDenseCell, heavy = (N / 32 + N / kHeavyCell + 1) * kHeavyParts;
+    return (plain > heavy ? plain : heavy) + 2;
+}
+
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -35,7 +43,7 @@ void layout(fof_handle *h)
     h->off_bin_base = off;    off += align256(((size_t)h->sort.bins + 2 + (size_t)h->sort.bins / 64 + 4) * sizeof(unsigned int));
     h->off_part = off;        off += align256((N + 1) * sizeof(float4));
     h->off_idx = off;         off += align256((N + 1) * sizeof(int));
-    h->off_dense = off;       off += align256((N / kDenseCell + N / 32 + 2) * sizeof(unsigned long long));
+    h->off_dense = off;       off += align256(dense_items_max(N) * sizeof(unsigned long long));
     h->off_sorted = off;      off += align256((N + 1) * sizeof(float4));
     h->off_cnt = off;         off += align256((N + 1) * sizeof(int));
     h->off_acc = off;         off += align256(((size_t)h->max_groups + 1) * 4 * sizeof(double));

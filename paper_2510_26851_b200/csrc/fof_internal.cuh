@@ -69,6 +69,20 @@ __host__ __device__ __forceinline__ unsigned int dense_tile_size(unsigned int m)
     const unsigned int T = dense_tiles(m);
     return T <= 16u ? (m + T - 1u) / T : 32u;
 }
+// A tile of a HEAVY cell (>= kHeavyCell particles: a clump core) meets thousands of candidates; its
+// candidate stream (earlier tiles of the cell + 13 forward cells) is dealt round-robin to
+// dense_parts(m) work items so that no single warp carries it (the tail of the link kernel).
+#ifndef FOF_HEAVY_CELL
+#define FOF_HEAVY_CELL 128
+#endif
+#ifndef FOF_HEAVY_PARTS
+#define FOF_HEAVY_PARTS 8
+#endif
+constexpr unsigned int kHeavyCell = FOF_HEAVY_CELL, kHeavyParts = FOF_HEAVY_PARTS;  // parts: a power of two <= 8
+__host__ __device__ __forceinline__ unsigned int dense_parts(unsigned int m)
+{
+    return (m >= kHeavyCell && m < (1u << 29)) ? kHeavyParts : 1u;  // item word: part:3 | tile:24 | size:5
+}
 
 
 

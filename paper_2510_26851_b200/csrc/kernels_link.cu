@@ -127,11 +127,11 @@ __device__ __forceinline__ void tile_neighbours(const float4 *__restrict__ sorte
                                                 const unsigned int *__restrict__ cs, unsigned int *rel,
                                                 const int *__restrict__ idx_s, float4 *s_pj, const float4 &me, int ib, int cntI, unsigned int grp, bool leader,
                                                 int cx, int cy, int cz, const Grid &g, int lane,
-                                                unsigned int &nedges, unsigned int &ntests)
+                                                int part, int nparts, unsigned int &nedges, unsigned int &ntests)
 {
     const int n = g.n;
     int beg = 0, len = 0;
-    if (lane < 13) {
+    if (lane < 13 && (nparts == 1 || (lane & (nparts - 1)) == part)) {  // nparts is a power of two
         int nx = cx + (int)((kFwdX >> (2 * lane)) & 3u) - 1;
         int ny = cy + (int)((kFwdY >> (2 * lane)) & 3u) - 1;
         int nz = cz + (int)((kFwdZ >> (2 * lane)) & 3u) - 1;
@@ -218,8 +218,12 @@ __device__ __forceinline__ void tile_item(const float4 *__restrict__ sorted, con
     const float inf = __int_as_float(0x7f800000);
     const int n = g.n;
     const unsigned int c = (unsigned int)(item >> 32);
-    const int t = (int)(((unsigned int)item) >> 5), ts = (int)(((unsigned int)item) & 31u) + 1;
+    const int ts = (int)(((unsigned int)item) & 31u) + 1;
     const int b0 = (int)__ldg(cell_start + c), e0 = (int)__ldg(cell_start + c + 1);
+    // a heavy cell's tile comes as nparts items, each with every nparts-th batch of its candidates
+    const int nparts = (int)dense_parts((unsigned int)(e0 - b0));
+    const int part = nparts == 1 ? 0 : (int)(((unsigned int)item) >> 29);
+    const int t = nparts == 1 ? (int)(((unsigned int)item) >> 5) : (int)((((unsigned int)item) >> 5) & 0xffffffu);
     const int ib = b0 + t * ts;
     const int cntI = min(ts, e0 - ib);
     // a lane without a particle sits at +inf: d2 = inf (or NaN) fails every test
@@ -232,8 +236,10 @@ __device__ __forceinline__ void tile_item(const float4 *__restrict__ sorted, con
     s_pj[lane] = me;
     __syncwarp();
     const unsigned int adj = batch_adjacency<false>(me, s_pj, cntI, g, lane) & ~(1u << lane);
-    nedges += (unsigned int)__popc(adj & lanemask_lt());
-    if (lane == 0) ntests += (unsigned int)(cntI * (cntI - 1) / 2);
+    if (part == 0) {
+        nedges += (unsigned int)__popc(adj & lanemask_lt());
+        if (lane == 0) ntests += (unsigned int)(cntI * (cntI - 1) / 2);
+    }
     // Components of the tile: breadth-first from the lowest unlabelled lane, one warp OR-reduction
     // per level.  Lanes without a link are their own component and are never visited.  `head` is
     // the member with the smallest original index (the union-find's order): every other member
@@ -261,11 +267,11 @@ __device__ __forceinline__ void tile_item(const float4 *__restrict__ sorted, con
         }
     }
     const bool leader = head == lane;
-    if (!leader && atomicCAS(rel + ib + lane, 0u, (unsigned int)(lane - head)) != 0u)
+    if (part == 0 && !leader && atomicCAS(rel + ib + lane, 0u, (unsigned int)(lane - head)) != 0u)
         unite_rel(rel, idx_s, ib + lane, ib + head);  // somebody hooked me first: general path
 
     // ---- the earlier tiles of my cell (all full: ts particles)
-    for (int jt = 0; jt < t; ++jt) {
+    for (int jt = part; jt < t; jt += nparts) {
         const int jb = b0 + jt * ts;
         __syncwarp();
         if (lane < ts) {
@@ -289,8 +295,8 @@ __device__ __forceinline__ void tile_item(const float4 *__restrict__ sorted, con
     const int cy = min(__float2int_rd(__fmul_rn(p0.y, g.inv_cell)), g.n_minus_1);
     const int cz = min(__float2int_rd(__fmul_rn(p0.z, g.inv_cell)), g.n_minus_1);
     const bool wrap = n < 6 || cx == 0 || cx == n - 1 || cy == 0 || cy == n - 1 || cz == n - 1;
-    if (wrap) tile_neighbours<true>(sorted, cell_start, rel, idx_s, s_pj, me, ib, cntI, grp, leader, cx, cy, cz, g, lane, nedges, ntests);
-    else tile_neighbours<false>(sorted, cell_start, rel, idx_s, s_pj, me, ib, cntI, grp, leader, cx, cy, cz, g, lane, nedges, ntests);
+    if (wrap) tile_neighbours<true>(sorted, cell_start, rel, idx_s, s_pj, me, ib, cntI, grp, leader, cx, cy, cz, g, lane, part, nparts, nedges, ntests);
+    else tile_neighbours<false>(sorted, cell_start, rel, idx_s, s_pj, me, ib, cntI, grp, leader, cx, cy, cz, g, lane, part, nparts, nedges, ntests);
 }
 
 // =============================================================================================

@@ -237,7 +237,7 @@ __global__ void __launch_bounds__(kCellSortThreads) cell_sort_kernel(
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             mine += a[u];
-            if (a[u] >= (unsigned int)kDenseCell) mine += (unsigned long long)dense_tiles(a[u]) << 32;
+            if (a[u] >= (unsigned int)kDenseCell) mine += (unsigned long long)(dense_tiles(a[u]) * dense_parts(a[u])) << 32;
         }
     }
     unsigned long long incl = mine;
@@ -270,10 +270,13 @@ __global__ void __launch_bounds__(kCellSortThreads) cell_sort_kernel(
         for (int u = 0; u < 4; ++u) {
             const unsigned int cnt = a[u];
             a[u] = run;
-            if (cnt >= (unsigned int)kDenseCell) {  // one work item per (dense cell, tile of <= 32 particles)
-                const unsigned int nt = dense_tiles(cnt), ts = dense_tile_size(cnt);
+            if (cnt >= (unsigned int)kDenseCell) {
+                // one work item per (dense cell, tile of <= 32 particles, part of the tile's candidate stream)
+                const unsigned int nt = dense_tiles(cnt), ts = dense_tile_size(cnt), np = dense_parts(cnt);
                 for (unsigned int t = 0; t < nt; ++t)
-                    dense_list[drun++] = ((unsigned long long)(cell0 + c_lo + k + u) << 32) | (t << 5) | (ts - 1u);
+                    for (unsigned int part = 0; part < np; ++part)
+                        dense_list[drun++] = ((unsigned long long)(cell0 + c_lo + k + u) << 32) | (part << 29) |
+                                             (t << 5) | (ts - 1u);
             }
             run += cnt;
         }
