@@ -384,7 +384,7 @@ int fof_subgroups(fof_handle *h, const float *pos, const float *vel, const int32
         h->num_sms = sms;
     }
     h->linked = false;  // the member lists and their union-find re-use the link's arrays
-    h->launches += h->N > 0 ? (K > 0 ? 5 : 2) : 0;
+    h->launches += h->N > 0 ? (K > 0 ? 6 : 3) : 0;
     CK(launch_subgroups(pos, vel, particle_group, group_size, h->N, K, h->L, sigma_x, sigma_v, ell,
                         at<unsigned int>(ws, h->off_cnt), at<unsigned int>(ws, h->off_part), at<int>(ws, h->off_idx),
                         at<unsigned int>(ws, h->off_rel), sub_labels, at<Ctrl>(ws, h->off_ctrl), h->num_sms, s),

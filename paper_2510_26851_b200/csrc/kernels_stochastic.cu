@@ -7,7 +7,7 @@
 // keyed on (seed, sample, original indices); d log p / d x_i = sum_j (y - p)(-2 alpha delta / b^2).
 // The binning is NOT redone: the kernel walks the cell-sorted arrays that the last fof_link left in
 // the workspace ("we do not rebuild the neighbor list", and S samples share one sort).
-// One warp per 32 home particles; per stencil cell the candidate ranges are flattened across the warp.
+// One warp per 32 home particles (a tile); candidates staged in shared memory, potential edges flattened over the lanes.
 #include "fof_internal.cuh"
 
 namespace fof {
@@ -61,142 +61,319 @@ __global__ void __launch_bounds__(kBlock) iota_kernel(int *__restrict__ labels, 
     if (i < N) labels[i] = (int)i;
 }
 
-// One warp per 32 consecutive cell-sorted home particles, one per lane.  For each of the 27 stencil
-// cells in turn, the lanes' candidate ranges (reach-filtered) are flattened into slots that the 32
-// lanes walk together, so a home particle in a dense cell does not serialise its warp.  A pair is
-// "owned" (counted, added to log p, hooked) by the particle that sees the other one later in its
-// own cell or in its forward half stencil; seen from the other side the same pair (same p, same y:
-// the generator is keyed on the pair) only feeds the home particle's gradient.  The gradient terms
-// of one batch are summed per home particle by a segmented warp scan (slots of one home particle
-// are consecutive) and kept in shared memory: no atomics, fixed summation order.
 constexpr int kStochWarps = kBlock / 32;
 
-__global__ void __launch_bounds__(kBlock) link_stochastic_kernel(const float4 *__restrict__ sorted, int64_t N, Grid g,
+struct StochAcc {
+    float lp;  // a lane adds at most a few thousand O(1) terms: float32 is enough before the float64 reduction
+    unsigned int ncand, nedge;
+};
+
+// One warp per 32 consecutive cell-sorted home particles.  Homes of
+// one grid row (same cy, cz: consecutive lanes, their cells consecutive in x) form a segment; its
+// candidates are the nine rows around it, each one contiguous run of `sorted` (cells xa - 1 .. xb + 1;
+// the periodic images of the end cells as runs of their own).  Candidates that cannot be within the
+// candidate radius of the segment (too far from the face(s) they share with it) are dropped, the
+// rest are staged 32 at a time in shared memory and every home tests every candidate (broadcast
+// reads, ~13 instructions per 32 tests).  The pairs that pass — the potential edges — are then
+// flattened home by home over the lanes for the expensive part (logistic, random draw, log p,
+// gradient, hook), so that this part runs with full lanes and a home particle's gradient terms are
+// consecutive (segmented warp scan, no atomics, fixed summation order).  A pair is owned (counted,
+// log p, hooked) by the member that sees the other one in its forward half stencil (in one cell:
+// the earlier slot); seen from the other side the same pair (same p, same y: the generator is keyed
+// on the pair) only feeds the home particle's gradient.
+struct StochSmem {
+    float4 home[32];  // x, y, z, original index
+    float4 cand[64];  // x, y, z, cell-sorted slot
+    float g[32][3];
+    int selfk[32];    // 1 + position in the batch of the home's own slot, 0 if it is not there
+};
+
+// Lane h: the candidates of the batch within the candidate radius of home h (bit k: candidate k).
+template <bool WRAP>
+__device__ __forceinline__ unsigned int stoch_adjacency(const float4 *cand, int cnt, const float4 &mine, const Grid &g)
+{
+    unsigned int adjH = 0;
+#pragma unroll 4
+    for (int k = 0; k < cnt; ++k) {
+        const float4 pj = cand[k];
+        float ddx = __fsub_rn(mine.x, pj.x), ddy = __fsub_rn(mine.y, pj.y), ddz = __fsub_rn(mine.z, pj.z);
+        if (WRAP) {
+            ddx = min_image(ddx, g.L, g.h);
+            ddy = min_image(ddy, g.L, g.h);
+            ddz = min_image(ddz, g.L, g.h);
+        }
+        const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(ddx, ddx), __fmul_rn(ddy, ddy)), __fmul_rn(ddz, ddz));
+        if (d2 <= g.b2) adjH |= 1u << k;  // R25: beyond the radius p = 0
+    }
+    return adjH;
+}
+
+// position of the (r + 1)-th set bit of m (r < popc(m))
+__device__ __forceinline__ int nth_set_bit(unsigned int m, int r)
+{
+    int pos = 0;
+#pragma unroll
+    for (int w = 16; w > 0; w >>= 1) {
+        const int c = __popc(m & ((1u << w) - 1u));
+        if (r >= c) { r -= c; pos += w; m >>= w; }
+    }
+    return pos;
+}
+
+__device__ __forceinline__ void stoch_batch(StochSmem &sm, int cnt, bool wrap, const float4 &mine, int myslot, int s0,
+                                            const Grid &g, const StochParams &sp, const int *__restrict__ idx_s,
+                                            unsigned int *rel, bool want_grad, int lane, StochAcc &acc)
+{
+    constexpr unsigned int kAll = 0xffffffffu;
+    // ---- every home against every candidate of the batch; a home's own slot is taken out afterwards
+    sm.selfk[lane] = 0;
+    __syncwarp();
+    if (lane < cnt) {
+        const unsigned int d = (unsigned int)(__float_as_int(sm.cand[lane].w) - s0);
+        if (d < 32u) sm.selfk[d] = lane + 1;
+    }
+    unsigned int adjH = wrap ? stoch_adjacency<true>(sm.cand, cnt, mine, g) : stoch_adjacency<false>(sm.cand, cnt, mine, g);
+    __syncwarp();
+    const int sk = sm.selfk[lane];
+    if (sk) adjH &= ~(1u << (sk - 1));
+    // ---- the potential edges, home-major, 32 at a time
+    const int mine_n = __popc(adjH);
+    int incl = mine_n;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(kAll, incl, o);
+        if (lane >= o) incl += v;
+    }
+    const int total = __shfl_sync(kAll, incl, 31);
+    const int excl = incl - mine_n;
+    for (int p0 = 0; p0 < total; p0 += 32) {
+        const int p = p0 + lane;
+        const bool has = p < total;
+        int owner = 0;  // the first lane whose inclusive prefix exceeds p
+#pragma unroll
+        for (int st = 16; st > 0; st >>= 1) {
+            const int v = __shfl_sync(kAll, incl, owner + st - 1);
+            if (v <= p) owner += st;
+        }
+        owner = min(owner, 31);
+        const unsigned int mask = __shfl_sync(kAll, adjH, owner);
+        const int rank = p - __shfl_sync(kAll, excl, owner);
+        const int osi = s0 + owner;
+        float gx = 0.0f, gy = 0.0f, gz = 0.0f;
+        if (has) {
+            const float4 ph = sm.home[owner], pj = sm.cand[nth_set_bit(mask, rank)];
+            const int j = __float_as_int(pj.w);
+            // the owner of a pair: the member that sees the other one in its forward
+            // half stencil (cell offsets under the periodic wrap), in one cell the earlier slot
+            int ex = cell1(pj.x, g) - cell1(ph.x, g), ey = cell1(pj.y, g) - cell1(ph.y, g),
+                ez = cell1(pj.z, g) - cell1(ph.z, g);
+            ex = ex > 1 ? ex - g.n : (ex < -1 ? ex + g.n : ex);
+            ey = ey > 1 ? ey - g.n : (ey < -1 ? ey + g.n : ey);
+            ez = ez > 1 ? ez - g.n : (ez < -1 ? ez + g.n : ez);
+            const int order = 9 * ez + 3 * ey + ex;
+            const bool owned = order > 0 || (order == 0 && j > osi);
+            if (want_grad || owned) {  // without the gradient only the owning side has work
+                const float ddx = min_image(__fsub_rn(ph.x, pj.x), g.L, g.h);
+                const float ddy = min_image(__fsub_rn(ph.y, pj.y), g.L, g.h);
+                const float ddz = min_image(__fsub_rn(ph.z, pj.z), g.L, g.h);
+                const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(ddx, ddx), __fmul_rn(ddy, ddy)), __fmul_rn(ddz, ddz));
+                const float tt = __fmul_rn(sp.c, __fsub_rn(sp.b2, d2));
+                float e;
+                const float pr = sigmoid_fixed(tt, e);
+                const unsigned int ooi = (unsigned int)__float_as_int(ph.w), oj = (unsigned int)__ldg(idx_s + j);
+                const float u = __fmul_rn((float)rng_u24(sp.key, min(ooi, oj), max(ooi, oj)), 5.9604644775390625e-8f);
+                const bool y = u < pr;
+                const float tc = fminf(fmaxf(tt, -30.0f), 30.0f);
+                if (want_grad && tt == tc) {
+                    const float cgr = ((y ? 1.0f : 0.0f) - pr) * sp.gscale;
+                    gx = cgr * ddx;
+                    gy = cgr * ddy;
+                    gz = cgr * ddz;
+                }
+                if (owned) {
+                    ++acc.ncand;
+                    // log p = -log(1 + e); log(1 - p) = log(e / (1 + e)) = log p - t; float32 terms
+                    acc.lp += -__logf(__fadd_rn(1.0f, e)) - (y ? 0.0f : tc);
+                    if (y) {
+                        ++acc.nedge;
+                        const int pa = osi - (int)rel[osi], pb = j - (int)rel[j];
+                        if (pa != pb) unite_rel(rel, idx_s, osi, j);  // same parent: already one set
+                    }
+                }
+            }
+        }
+        if (want_grad && __any_sync(kAll, gx != 0.0f || gy != 0.0f || gz != 0.0f)) {
+            // segmented inclusive scan over runs of equal owner, then one add per home particle
+            const int key = has ? owner : -1 - lane;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const float vx = __shfl_up_sync(kAll, gx, o), vy = __shfl_up_sync(kAll, gy, o),
+                            vz = __shfl_up_sync(kAll, gz, o);
+                const int kk = __shfl_up_sync(kAll, key, o);
+                if (lane >= o && kk == key) { gx += vx; gy += vy; gz += vz; }
+            }
+            const int knext = __shfl_down_sync(kAll, key, 1);
+            if (has && (lane == 31 || knext != key)) {
+                sm.g[owner][0] += gx;
+                sm.g[owner][1] += gy;
+                sm.g[owner][2] += gz;
+            }
+            __syncwarp();
+        }
+    }
+}
+
+__device__ __forceinline__ void stoch_tile_warp(const float4 *__restrict__ sorted, const Grid &g,
+                                                const unsigned int *__restrict__ cs, const int *__restrict__ idx_s,
+                                                unsigned int *rel, const StochParams &sp, bool want_grad,
+                                                StochSmem &sm, const float4 &me, int myslot, unsigned int oi,
+                                                bool valid, int cx, int cy, int cz, int lane, StochAcc &acc)
+{
+    constexpr unsigned int kAll = 0xffffffffu;
+    const float inf = __int_as_float(0x7f800000);
+    const int n = g.n;
+    const int row = cy + n * cz;
+    const int s0 = __shfl_sync(kAll, myslot, 0);  // slot of lane 0 (lanes past the end of the array repeat the last slot)
+    const float lo = g.reach, hi = 1.0f - g.reach;
+    sm.home[lane] = make_float4(me.x, me.y, me.z, __int_as_float((int)oi));
+    __syncwarp();
+
+    unsigned int todo = __ballot_sync(kAll, valid);
+    while (todo) {
+        const int l0 = __ffs((int)todo) - 1;
+        const int r0 = __shfl_sync(kAll, row, l0);
+        const unsigned int seg = __ballot_sync(kAll, valid && row == r0) & todo;
+        todo &= ~seg;
+        const bool inseg = (seg >> lane) & 1u;
+        const int xa = __shfl_sync(kAll, cx, l0), xb = __shfl_sync(kAll, cx, 31 - __clz((int)seg));
+        const int cy0 = __shfl_sync(kAll, cy, l0), cz0 = __shfl_sync(kAll, cz, l0);
+        // a lane outside the segment sits at +inf: d2 = inf (or NaN) fails every test
+        const float4 mine = inseg ? me : make_float4(inf, inf, inf, 0.0f);
+        const int span = xb - xa + 1;
+        const int xl = xa > 0 ? xa - 1 : n - 1, xr = xb < n - 1 ? xb + 1 : 0;  // the cells beside the segment
+        const bool edges = span <= n - 2;  // otherwise the end cells are inside the segment or coincide
+        // away from the box faces no pair of the segment needs the minimum image (cf. link_kernel)
+        const bool wrap = n < 6 || xa == 0 || xb == n - 1 || cy0 == 0 || cy0 == n - 1 || cz0 == 0 || cz0 == n - 1;
+        // candidate runs: lane q < 27 = 3 (row of the stencil) + part; part 0: cells max(xa - 1, 0) ..
+        // min(xb + 1, n - 1), part 1: cell n - 1 as the left image, part 2: cell 0 as the right image
+        int beg = 0, len = 0;
+        if (lane < 27) {
+            const int rq = lane / 3, part = lane - 3 * rq;
+            const int dy = rq % 3 - 1, dz = rq / 3 - 1;
+            int ay = cy0 + dy, az = cz0 + dz;
+            ay = ay < 0 ? n - 1 : (ay >= n ? 0 : ay);
+            az = az < 0 ? n - 1 : (az >= n ? 0 : az);
+            const int m0 = max(xa - 1, 0), m1 = min(xb + 1, n - 1);
+            int c0 = -1, c1 = -1;
+            if (part == 0) { c0 = m0; c1 = m1; }
+            else if (part == 1) { if (xa == 0 && m1 < n - 1) c0 = c1 = n - 1; }
+            else { if (xb == n - 1 && m0 > 0) c0 = c1 = 0; }
+            if (c0 >= 0) {
+                beg = (int)__ldg(cs + cell_id(c0, ay, az, n));
+                len = (int)__ldg(cs + cell_id(c1, ay, az, n) + 1) - beg;
+            }
+        }
+        int incl = len;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(kAll, incl, o);
+            if (lane >= o) incl += v;
+        }
+        const int total = __shfl_sync(kAll, incl, 31);
+        const int excl = incl - len;
+        int nc = 0;  // candidates waiting in sm.cand (warp-uniform)
+        for (int base = 0;; base += 32) {
+            if (base < total) {
+                const int p = base + lane;
+                const bool has = p < total;
+                int q = 0;  // owner run of slot p: the first lane whose inclusive prefix exceeds p
+#pragma unroll
+                for (int st = 16; st > 0; st >>= 1) {
+                    const int v = __shfl_sync(kAll, incl, q + st - 1);
+                    if (v <= p) q += st;
+                }
+                q = min(q, 31);
+                const int j = __shfl_sync(kAll, beg, q) + (p - __shfl_sync(kAll, excl, q));
+                bool pass = false;
+                float4 pj = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (has) {
+                    pj = __ldg(sorted + j);
+                    // position of the candidate inside ITS cell: it can reach the segment only from within
+                    // `reach` of the face(s) between its cell and the segment's cells
+                    const float ux = __fmul_rn(pj.x, g.inv_cell), uy = __fmul_rn(pj.y, g.inv_cell),
+                                uz = __fmul_rn(pj.z, g.inv_cell);
+                    const int jx = min(__float2int_rd(ux), g.n_minus_1);
+                    const float fx = ux - (float)jx;
+                    const float fy = uy - (float)min(__float2int_rd(uy), g.n_minus_1);
+                    const float fz = uz - (float)min(__float2int_rd(uz), g.n_minus_1);
+                    const int rq = q / 3;
+                    const int dy = rq % 3 - 1, dz = rq / 3 - 1;
+                    pass = (dy == 0 || (dy < 0 ? fy > hi : fy < lo)) && (dz == 0 || (dz < 0 ? fz > hi : fz < lo));
+                    if (edges) {
+                        if (jx == xl) pass = pass && fx > hi;
+                        if (jx == xr) pass = pass && fx < lo;
+                    }
+                    pj.w = __int_as_float(j);
+                }
+                const unsigned int bal = __ballot_sync(kAll, pass);
+                if (pass) sm.cand[nc + __popc(bal & ((1u << lane) - 1u))] = pj;
+                nc += __popc(bal);
+                __syncwarp();
+            }
+            const bool last = base + 32 >= total;
+            if (nc >= 32 || (last && nc)) {
+                const int cnt = min(nc, 32);
+                stoch_batch(sm, cnt, wrap, mine, myslot, s0, g, sp, idx_s, rel, want_grad, lane, acc);
+                const float4 keep = sm.cand[32 + lane];
+                __syncwarp();
+                sm.cand[lane] = keep;
+                nc -= cnt;
+                __syncwarp();
+            }
+            if (last && nc == 0) break;
+        }
+    }
+    __syncwarp();
+}
+
+#ifndef FOF_STOCH_MINB
+#define FOF_STOCH_MINB 6  // resident CTAs per SM the kernel is compiled for (register cap 40)
+#endif
+__global__ void __launch_bounds__(kBlock, FOF_STOCH_MINB) link_stochastic_kernel(const float4 *__restrict__ sorted, int64_t N, Grid g,
                                                                  const unsigned int *__restrict__ cs,
                                                                  const int *__restrict__ idx_s, unsigned int *rel,
                                                                  StochParams sp, double *logp, float *grad,
                                                                  Ctrl *ctrl)
 {
-    __shared__ float s_g[kStochWarps][32][3];
+    constexpr unsigned int kAll = 0xffffffffu;
+    __shared__ StochSmem s_all[kStochWarps];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    StochSmem &sm = s_all[wib];
     const int64_t s64 = ((int64_t)blockIdx.x * kStochWarps + wib) * 32 + lane;
     const bool valid = s64 < N;
-    const int si = (int)min(s64, N - 1);
-    const float4 me = __ldg(sorted + si);
-    const unsigned int oi = (unsigned int)__ldg(idx_s + si);
-    const int n = g.n;
-    const float ux = __fmul_rn(me.x, g.inv_cell), uy = __fmul_rn(me.y, g.inv_cell), uz = __fmul_rn(me.z, g.inv_cell);
-    const int cx = min(__float2int_rd(ux), g.n_minus_1), cy = min(__float2int_rd(uy), g.n_minus_1),
-              cz = min(__float2int_rd(uz), g.n_minus_1);
-    const float fx = ux - (float)cx, fy = uy - (float)cy, fz = uz - (float)cz;
-    const float lo = g.reach, hi = 1.0f - g.reach;
-    float lp = 0.0f;  // a lane adds at most a few thousand O(1) terms: float32 is enough before the float64 reduction
-    unsigned int ncand = 0, nedge = 0;
-    s_g[wib][lane][0] = s_g[wib][lane][1] = s_g[wib][lane][2] = 0.0f;
+    const int myslot = (int)min(s64, N - 1);
+    const float4 me = __ldg(sorted + myslot);
+    const unsigned int oi = (unsigned int)__ldg(idx_s + myslot);
+    const int cx = min(__float2int_rd(__fmul_rn(me.x, g.inv_cell)), g.n_minus_1),
+              cy = min(__float2int_rd(__fmul_rn(me.y, g.inv_cell)), g.n_minus_1),
+              cz = min(__float2int_rd(__fmul_rn(me.z, g.inv_cell)), g.n_minus_1);
+    const bool want_grad = grad != nullptr;
+    StochAcc acc = {0.0f, 0u, 0u};
+    sm.g[lane][0] = sm.g[lane][1] = sm.g[lane][2] = 0.0f;
     __syncwarp();
-    int dx = -2, dy = -1, dz = -1;
-    for (int q = 0; q < 27; ++q) {
-        if (++dx > 1) { dx = -1; if (++dy > 1) { dy = -1; ++dz; } }  // q = (dx + 1) + 3 (dy + 1) + 9 (dz + 1)
-        const bool forward = q > 13;  // dz > 0, or dz == 0 and dy > 0, or dz == dy == 0 and dx > 0
-        if (!forward && q != 13 && !grad) continue;  // the backward half only feeds the gradient
-        int beg = 0, len = 0;
-        if (valid && !((dx < 0 && !(fx < lo)) || (dx > 0 && !(fx > hi)) || (dy < 0 && !(fy < lo)) ||
-                       (dy > 0 && !(fy > hi)) || (dz < 0 && !(fz < lo)) || (dz > 0 && !(fz > hi)))) {
-            int ax = cx + dx, ay = cy + dy, az = cz + dz;
-            ax = ax < 0 ? n - 1 : (ax >= n ? 0 : ax);
-            ay = ay < 0 ? n - 1 : (ay >= n ? 0 : ay);
-            az = az < 0 ? n - 1 : (az >= n ? 0 : az);
-            const unsigned int c = cell_id(ax, ay, az, n);
-            beg = (int)__ldg(cs + c);
-            len = (int)__ldg(cs + c + 1) - beg;
-        }
-        int incl = len;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int v = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= o) incl += v;
-        }
-        const int total = __shfl_sync(0xffffffffu, incl, 31);
-        const int excl = incl - len;
-        for (int p0 = 0; p0 < total; p0 += 32) {
-            const int p = p0 + lane;
-            const bool has = p < total;
-            int owner = 0;  // the first lane whose inclusive prefix exceeds p
-#pragma unroll
-            for (int st = 16; st > 0; st >>= 1) {
-                const int v = __shfl_sync(0xffffffffu, incl, owner + st - 1);
-                if (v <= p) owner += st;
-            }
-            owner = min(owner, 31);
-            const int j = __shfl_sync(0xffffffffu, beg, owner) + (p - __shfl_sync(0xffffffffu, excl, owner));
-            const float ox = __shfl_sync(0xffffffffu, me.x, owner), oy = __shfl_sync(0xffffffffu, me.y, owner),
-                        oz = __shfl_sync(0xffffffffu, me.z, owner);
-            const int osi = __shfl_sync(0xffffffffu, si, owner);
-            const unsigned int ooi = __shfl_sync(0xffffffffu, oi, owner);
-            float gx = 0.0f, gy = 0.0f, gz = 0.0f;
-            if (has && j != osi) {
-                const float4 pj = __ldg(sorted + j);
-                const float ddx = min_image(__fsub_rn(ox, pj.x), g.L, g.h);
-                const float ddy = min_image(__fsub_rn(oy, pj.y), g.L, g.h);
-                const float ddz = min_image(__fsub_rn(oz, pj.z), g.L, g.h);
-                const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(ddx, ddx), __fmul_rn(ddy, ddy)), __fmul_rn(ddz, ddz));
-                if (d2 <= g.b2) {  // R25: beyond the candidate radius p = 0
-                    const float tt = __fmul_rn(sp.c, __fsub_rn(sp.b2, d2));
-                    float e;
-                    const float pr = sigmoid_fixed(tt, e);
-                    const unsigned int oj = (unsigned int)__ldg(idx_s + j);
-                    const float u = __fmul_rn((float)rng_u24(sp.key, min(ooi, oj), max(ooi, oj)), 5.9604644775390625e-8f);
-                    const bool y = u < pr;
-                    const float tc = fminf(fmaxf(tt, -30.0f), 30.0f);
-                    if (grad && tt == tc) {
-                        const float cgr = ((y ? 1.0f : 0.0f) - pr) * sp.gscale;
-                        gx = cgr * ddx;
-                        gy = cgr * ddy;
-                        gz = cgr * ddz;
-                    }
-                    if (forward || (q == 13 && j > osi)) {
-                        ++ncand;
-                        // log p = -log(1 + e); log(1 - p) = log(e / (1 + e)) = log p - t; float32 terms
-                        lp += -__logf(__fadd_rn(1.0f, e)) - (y ? 0.0f : tc);
-                        if (y) {
-                            ++nedge;
-                            const int pa = osi - (int)rel[osi], pb = j - (int)rel[j];
-                            if (pa != pb) unite_rel(rel, idx_s, osi, j);  // same parent: already one set
-                        }
-                    }
-                }
-            }
-            if (grad && __any_sync(0xffffffffu, gx != 0.0f || gy != 0.0f || gz != 0.0f)) {
-                // segmented inclusive scan over runs of equal owner, then one add per home particle
-                const int key = has ? owner : -1 - lane;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const float vx = __shfl_up_sync(0xffffffffu, gx, o), vy = __shfl_up_sync(0xffffffffu, gy, o),
-                                vz = __shfl_up_sync(0xffffffffu, gz, o);
-                    const int k = __shfl_up_sync(0xffffffffu, key, o);
-                    if (lane >= o && k == key) { gx += vx; gy += vy; gz += vz; }
-                }
-                const int knext = __shfl_down_sync(0xffffffffu, key, 1);
-                if (has && (lane == 31 || knext != key)) {
-                    s_g[wib][owner][0] += gx;
-                    s_g[wib][owner][1] += gy;
-                    s_g[wib][owner][2] += gz;
-                }
-                __syncwarp();
-            }
-        }
-    }
+    stoch_tile_warp(sorted, g, cs, idx_s, rel, sp, want_grad, sm, me, myslot, oi, valid, cx, cy, cz, lane, acc);
     __syncwarp();
-    if (grad && valid) {
-        grad[3 * (int64_t)oi + 0] = s_g[wib][lane][0];
-        grad[3 * (int64_t)oi + 1] = s_g[wib][lane][1];
-        grad[3 * (int64_t)oi + 2] = s_g[wib][lane][2];
+    if (want_grad && valid) {
+        grad[3 * (int64_t)oi + 0] = sm.g[lane][0];
+        grad[3 * (int64_t)oi + 1] = sm.g[lane][1];
+        grad[3 * (int64_t)oi + 2] = sm.g[lane][2];
     }
-    double lpd = (double)lp;
+    double lpd = (double)acc.lp;
+    unsigned int ncand = acc.ncand, nedge = acc.nedge;
     for (int o = 16; o > 0; o >>= 1) {
-        lpd += __shfl_xor_sync(0xffffffffu, lpd, o);
-        ncand += __shfl_xor_sync(0xffffffffu, ncand, o);
-        nedge += __shfl_xor_sync(0xffffffffu, nedge, o);
+        lpd += __shfl_xor_sync(kAll, lpd, o);
+        ncand += __shfl_xor_sync(kAll, ncand, o);
+        nedge += __shfl_xor_sync(kAll, nedge, o);
     }
     if (lane == 0) {
         if (lpd != 0.0) atomicAdd(logp, lpd);

@@ -484,7 +484,7 @@ def test_large_grids_take_the_wide_bin_paths(B, grid):
 def test_stochastic_link_against_oracle(B, alpha, kappa):
     """fof_link_stochastic (section 3.2 Eq. 8): labels of every sample and the numbers of potential and
     sampled edges bit-exact (both sides take u < p on identical float32 bits), log p(y) to float64
-    summation order, the score function to float32 accumulation (atomics, arbitrary order)."""
+    summation order, the score function to float32 accumulation (warp scans, another order than the oracle's)."""
     w = inputs.scaled(inputs.CONFIGS["cfg1"], 40)
     p = inputs.make_positions(w)
     b_link = w.b
@@ -502,7 +502,13 @@ def test_stochastic_link_against_oracle(B, alpha, kappa):
         g = grad.cpu().numpy().astype(np.float64)
         assert np.abs(g - o["grad"]).max() <= 2e-5 * np.abs(o["grad"]).max()
     # samples differ from each other, and a different seed gives a different graph
-    a = f.link_stochastic(b_link, alpha, 1234, 0, want_grad=False)[0]
+    a, logp_a, grad_a = f.link_stochastic(b_link, alpha, 1234, 0, want_grad=False)
+    # without the score function only the owning side of each pair is evaluated: same sample, same numbers
+    o0 = oracle.stochastic(p, w.L, b_cand, b_link, alpha, 1234, 0)
+    E, ncand, _ = f.link_stats()
+    assert grad_a is None and ncand == o0["n_cand"] and E == o0["n_edge"]
+    assert np.array_equal(a.cpu().numpy(), o0["labels"])
+    assert abs(float(logp_a.item()) - o0["logp"]) <= 2e-6 * abs(o0["logp"]) + 1e-6
     c = f.link_stochastic(b_link, alpha, 1235, 0, want_grad=False)[0]
     assert alpha >= 50.0 or not torch.equal(a, c)
     f.close()
@@ -582,6 +588,54 @@ def test_subgroups_large_halo_and_no_halo(B):
     assert g["K"] == 0
     sub = f.subgroups(dq, torch.zeros_like(dq), g, 1.0, 1.0, 1.0).cpu().numpy()
     assert np.array_equal(sub, np.arange(len(q), dtype=np.int32))
+    f.close()
+
+
+def test_subgroups_many_wide_halos_and_many_halos(B):
+    """Several halos above the one-warp limit (their tile rows are dealt to the whole grid as work items found
+    by a search of the item prefix), next to small ones, two of them across box faces; then more halos
+    than one scan chunk (8192) so that the offsets come from two launches."""
+    rng = np.random.default_rng(31)
+    L, b = 60.0, 1.0
+    centres = np.array([[0.2, 30, 30], [30, 59.9, 10], [15, 15, 15], [45, 20, 50], [50, 50, 0.1], [10, 40, 40]])
+    sizes = [300, 700, 1500, 260, 257, 540]
+    parts = [rng.standard_normal((m, 3)) * 0.9 + c for m, c in zip(sizes, centres)]
+    small = [rng.standard_normal((int(m), 3)) * 0.35 + rng.random(3) * L for m in rng.integers(20, 200, 60)]
+    p = (np.concatenate(parts + small + [rng.random((3000, 3)) * L]) % L).astype(np.float32)
+    p = np.minimum(p, np.nextafter(np.float32(L), np.float32(0)))
+    p = p[rng.permutation(len(p))]
+    v = (rng.standard_normal((len(p), 3)) * 40.0).astype(np.float32)
+    v[rng.random(len(p)) < 0.4] += np.float32(250.0)
+    lab, _ = oracle.labels_cells(p, L, b)
+    og = oracle.groups(p, lab, L, 20)
+    assert (og["group_size"] > 256).sum() >= 5
+    osub, _ = oracle.subgroups(p, v, og["particle_group"], L, 1.0, 70.0 ** 2, 0.8)
+    f = B.FoF(len(p), L, b, 20)
+    dpos, dvel = torch.from_numpy(p).cuda(), torch.from_numpy(v).cuda()
+    g = f.groups(dpos, f.link(dpos), particle_group=True)
+    sub = f.subgroups(dpos, dvel, g, 1.0, 70.0 ** 2, 0.8).cpu().numpy()
+    assert np.array_equal(sub, osub)
+    assert len(np.unique(sub[og["particle_group"] >= 0])) > og["K"]
+    f.close()
+
+    # 9000 pairs-of-clumps halos of 3 members each, N_min = 3: K > 8192
+    K = 9000
+    n = 24
+    ij = np.stack(np.meshgrid(np.arange(n), np.arange(n), np.arange(n), indexing="ij"), -1).reshape(-1, 3)[:K]
+    c = (ij + 0.5) * 4.0
+    L2 = n * 4.0
+    q = (c[:, None, :] + np.array([[0, 0, 0], [0.6, 0, 0], [0, 0.6, 0]])[None]).reshape(-1, 3).astype(np.float32)
+    q = q[rng.permutation(len(q))]
+    vq = (rng.standard_normal((len(q), 3)) * 30.0).astype(np.float32)
+    lab, _ = oracle.labels_cells(q, L2, 1.0)
+    og = oracle.groups(q, lab, L2, 3)
+    assert og["K"] == K
+    osub, _ = oracle.subgroups(q, vq, og["particle_group"], L2, 1.0, 40.0 ** 2, 0.9)
+    f = B.FoF(len(q), L2, 1.0, 3)
+    dq, dv = torch.from_numpy(q).cuda(), torch.from_numpy(vq).cuda()
+    g = f.groups(dq, f.link(dq), particle_group=True)
+    assert g["K"] == K
+    assert np.array_equal(f.subgroups(dq, dv, g, 1.0, 40.0 ** 2, 0.9).cpu().numpy(), osub)
     f.close()
 
 
