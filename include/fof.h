@@ -173,7 +173,8 @@ int fof_groups_backward(fof_handle *h, const float *pos, const float *mass, cons
  * fof_link + fof_groups, copies labels and the K group records device -> host.
  *   *_host  host buffers (pinned for full copy speed); mass_host / particle_group_host may be NULL.
  *   dev_buf device scratch of fof_host_device_bytes(h, cap) bytes, 256-B aligned.
- * Synchronises `stream`. */
+ * The labels are copied back on an internal stream while the groups are built on `stream`.
+ * Synchronises `stream` (and that copy) before it returns. */
 size_t fof_host_device_bytes(const fof_handle *h, int64_t cap);
 int fof_run_host(fof_handle *h, const float *pos_host, const float *mass_host, int32_t *labels_host,
                  int32_t *group_label_host, int32_t *group_size_host, float *group_mass_host,

@@ -160,6 +160,10 @@ void fof_destroy(fof_handle *h)
 {
     if (!h) return;
     fof_profile_enable(h, 0);
+    if (h->copy_stream) {
+        (void)cudaStreamDestroy(h->copy_stream);
+        (void)cudaEventDestroy(h->ev_linked);
+    }
     delete h;
 }
 
@@ -484,10 +488,21 @@ int fof_run_host(fof_handle *h, const float *pos_host, const float *mass_host, i
     if (N && mass_host) CK(cudaMemcpyAsync(mass, mass_host, N * sizeof(float), cudaMemcpyHostToDevice, s), "H2D mass");
     int rc = fof_link(h, pos, labels, ws, s);
     if (rc != FOF_OK) return rc;
-    if (N) CK(cudaMemcpyAsync(labels_host, labels, N * sizeof(int), cudaMemcpyDeviceToHost, s), "D2H labels");
+    if (N) {  // the labels travel while the groups are built (fof_groups only reads them)
+        if (!h->copy_stream) {
+            CK(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking), "cudaStreamCreate");
+            CK(cudaEventCreateWithFlags(&h->ev_linked, cudaEventDisableTiming), "cudaEventCreate");
+        }
+        CK(cudaEventRecord(h->ev_linked, s), "cudaEventRecord");
+        CK(cudaStreamWaitEvent(h->copy_stream, h->ev_linked, 0), "cudaStreamWaitEvent");
+        CK(cudaMemcpyAsync(labels_host, labels, N * sizeof(int), cudaMemcpyDeviceToHost, h->copy_stream), "D2H labels");
+    }
     rc = fof_groups(h, pos, mass_host ? mass : nullptr, labels, ws, glabel, gsize, gmass, gcom,
                     particle_group_host ? pgroup : nullptr, cap, K_host, s);
-    if (rc != FOF_OK) return rc;
+    if (rc != FOF_OK) {
+        if (N) (void)cudaStreamSynchronize(h->copy_stream);  // no copy into the caller's buffer after the return
+        return rc;
+    }
     const size_t K = (size_t)*K_host;
     if (K) {
         CK(cudaMemcpyAsync(group_label_host, glabel, K * sizeof(int), cudaMemcpyDeviceToHost, s), "D2H group_label");
@@ -498,6 +513,7 @@ int fof_run_host(fof_handle *h, const float *pos_host, const float *mass_host, i
     if (N && particle_group_host)
         CK(cudaMemcpyAsync(particle_group_host, pgroup, N * sizeof(int), cudaMemcpyDeviceToHost, s), "D2H particle_group");
     CK(cudaStreamSynchronize(s), "sync");
+    if (N) CK(cudaStreamSynchronize(h->copy_stream), "sync labels copy");
     Ctrl c;
     CK(cudaMemcpy(&c, at<Ctrl>(ws, h->off_ctrl), sizeof(Ctrl), cudaMemcpyDeviceToHost), "copy ctrl");
     if (c.error & 1u) return FOF_ERR_NONFINITE;

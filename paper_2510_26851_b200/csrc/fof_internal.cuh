@@ -121,6 +121,9 @@ struct fof_handle {
     cudaEvent_t *ev;       // [slot][2k] before, [slot][2k+1] after stage k
     bool *ev_valid;        // [slot][k]
     unsigned long long launches;
+    // fof_run_host: the labels go back to the host on a stream of their own while the groups are built
+    cudaStream_t copy_stream;
+    cudaEvent_t ev_linked;
 };
 
 namespace fof {
