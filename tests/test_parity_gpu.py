@@ -685,3 +685,23 @@ def test_tiny_grids_wrap_everywhere(B, grid):
     got, lab, og = check_against_oracle(B, p, L, b, 5, grid=grid, brute=True,
                                         mass=rng.uniform(0.5, 1.5, len(p)).astype(np.float32))
     assert got["grid"][0] == grid and og["group_size"].max() > 300
+
+
+@pytest.mark.parametrize("grid", [3, 5, 8])
+def test_heavy_cells_across_the_wrap(B, grid):
+    """Cells of several hundred particles on both sides of the box faces: their tiles are listed as eight
+    work items each (the candidate stream of a heavy cell is shared out, kernels_link.cu), with wrapping
+    neighbours (n = 3, 5) and with the wrap-free variant next to wrapping ones (n = 8)."""
+    rng = np.random.default_rng(200 + grid)
+    L, b = 10.0, 1.0
+    corner = rng.standard_normal((2400, 3)) * 0.45                    # ~300 per cell in the eight corner cells
+    edge = rng.standard_normal((900, 3)) * 0.35 + np.array([0.0, 5.0, 0.0])
+    inner = rng.standard_normal((700, 3)) * 0.3 + np.array([5.2, 5.1, 4.9])
+    bg = rng.random((1000, 3)) * L
+    p = (np.concatenate([corner, edge, inner, bg]) % L).astype(np.float32)
+    p[p >= np.float32(L)] = 0.0
+    p = p[rng.permutation(len(p))]
+    got, lab, og = check_against_oracle(B, p, L, b, 5, grid=grid, brute=True,
+                                        mass=rng.uniform(0.5, 1.5, len(p)).astype(np.float32))
+    assert got["grid"][0] == grid and og["group_size"].max() > 2000
+
