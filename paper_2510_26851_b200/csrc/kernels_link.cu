@@ -530,8 +530,8 @@ __device__ __forceinline__ void sparse_chunk(const float4 *__restrict__ sorted, 
 // 1.69 ms -- the two roles together are ~170 KB of SASS and evict each other from the instruction
 // caches when they share an SM.)
 // =============================================================================================
-constexpr int kTileBatch = 4;     // items per ticket
-constexpr int kSparseBatch = 8;   // 32-particle chunks per ticket
+constexpr int kTileBatch = 4;     // items per ticket (at most: small inputs take fewer, see link_kernel)
+constexpr int kSparseBatch = 8;   // 32-particle chunks per ticket (at most)
 
 union LinkSmem {
     float4 pj[64];
@@ -543,7 +543,9 @@ __global__ void __launch_bounds__(kLinkBlock, FOF_LINK_MINB) link_kernel(const f
                                                                          const unsigned int *__restrict__ cell_start,
                                                                          const unsigned long long *__restrict__ items,
                                                                          unsigned int *rel,
-                                                                         const int *__restrict__ idx_s, Ctrl *ctrl)
+                                                                         const int *__restrict__ idx_s, Ctrl *ctrl,
+                                                                         unsigned int tile_batch,
+                                                                         unsigned int sparse_batch)
 {
     __shared__ LinkSmem s_all[kWarpsPerCta];
     LinkSmem &sm = s_all[threadIdx.x >> 5];
@@ -555,23 +557,23 @@ __global__ void __launch_bounds__(kLinkBlock, FOF_LINK_MINB) link_kernel(const f
         if (role == 0) {
             while (true) {
                 unsigned int it0 = 0;
-                if (lane == 0) it0 = atomicAdd(&ctrl->tile_ticket, (unsigned int)kTileBatch);
+                if (lane == 0) it0 = atomicAdd(&ctrl->tile_ticket, tile_batch);
                 it0 = __shfl_sync(kFull, it0, 0);
                 if (it0 >= nitems) break;
-                const unsigned int it1 = min(it0 + (unsigned int)kTileBatch, nitems);
+                const unsigned int it1 = min(it0 + tile_batch, nitems);
                 for (unsigned int it = it0; it < it1; ++it)
                     tile_item(sorted, g, cell_start, __ldg(items + it), rel, idx_s, sm.pj, lane, nedges, ntests);
             }
         } else {
             while (true) {
                 unsigned int k0 = 0;
-                if (lane == 0) k0 = atomicAdd(&ctrl->sparse_ticket, (unsigned int)kSparseBatch);
+                if (lane == 0) k0 = atomicAdd(&ctrl->sparse_ticket, sparse_batch);
                 k0 = __shfl_sync(kFull, k0, 0);
                 const int64_t base0 = (int64_t)k0 * 32;
                 if (base0 >= N) break;
                 for (int k = 0; k < kSparseBatch; ++k) {
                     const int64_t base = base0 + 32 * k;
-                    if (base >= N) break;
+                    if (k >= (int)sparse_batch || base >= N) break;
                     sparse_chunk(sorted, N, g, cell_start, rel, idx_s, base, sm.sp, lane, nedges, ntests);
                 }
             }
@@ -672,7 +674,13 @@ cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned 
 {
     if (N <= 0) return cudaSuccess;
     const unsigned int grid = (unsigned int)min((int64_t)blocks_for(N, kLinkBlock), (int64_t)num_sms * FOF_LINK_MINB);
-    link_kernel<<<grid, kLinkBlock, 0, s>>>(sorted, N, g, cell_start, dense_list, rel, idx_s, ctrl);
+    // tickets sized so that every warp of the grid draws at least ~4 of them: with one or two per warp
+    // (a few million particles) the slowest warp would carry twice the mean
+    const int64_t per_warp = (N / 32) / (4 * (int64_t)grid * kWarpsPerCta);
+    const unsigned int tile_batch = (unsigned int)min(max(per_warp / 2, (int64_t)1), (int64_t)kTileBatch);  // items are fewer and longer
+    const unsigned int sparse_batch = (unsigned int)min(max(per_warp, (int64_t)1), (int64_t)kSparseBatch);
+    link_kernel<<<grid, kLinkBlock, 0, s>>>(sorted, N, g, cell_start, dense_list, rel, idx_s, ctrl, tile_batch,
+                                            sparse_batch);
     return cudaGetLastError();
 }
 
