@@ -146,14 +146,45 @@ __global__ void __launch_bounds__(kBlock) sub_fill_kernel(const int *__restrict_
     sub_rel[slot] = 0u;
 }
 
+// WRAP = false: the caller knows that no coordinate difference of the two tiles exceeds L / 2, where the
+// minimum image is the identity.
+template <bool WRAP>
 __device__ __forceinline__ bool linked6(const float *a, const float *b, const Sub6 &q)
 {
-    const float dx = min_image(__fsub_rn(a[0], b[0]), q.L, q.h), dy = min_image(__fsub_rn(a[1], b[1]), q.L, q.h),
-                dz = min_image(__fsub_rn(a[2], b[2]), q.L, q.h);
+    float dx = __fsub_rn(a[0], b[0]), dy = __fsub_rn(a[1], b[1]), dz = __fsub_rn(a[2], b[2]);
+    if (WRAP) {
+        dx = min_image(dx, q.L, q.h);
+        dy = min_image(dy, q.L, q.h);
+        dz = min_image(dz, q.L, q.h);
+    }
     const float ux = __fsub_rn(a[3], b[3]), uy = __fsub_rn(a[4], b[4]), uz = __fsub_rn(a[5], b[5]);
     const float dx2 = __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
     const float dv2 = __fadd_rn(__fadd_rn(__fmul_rn(ux, ux), __fmul_rn(uy, uy)), __fmul_rn(uz, uz));
     return __fadd_rn(__fmul_rn(dx2, q.rx), __fmul_rn(dv2, q.rv)) <= q.ell2;
+}
+
+// Bounding box of the positions of a tile (wrapped into [0, L): non-negative floats order like their bits).
+struct SubBox {
+    unsigned int lo[3], hi[3];
+};
+__device__ __forceinline__ SubBox sub_box(const float *p, bool valid)
+{
+    SubBox bx;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        bx.lo[a] = __reduce_min_sync(0xffffffffu, valid ? __float_as_uint(p[a]) : 0xffffffffu);
+        bx.hi[a] = __reduce_max_sync(0xffffffffu, valid ? __float_as_uint(p[a]) : 0u);
+    }
+    return bx;
+}
+// true if some coordinate difference between (or inside) the two boxes can exceed h = L / 2
+__device__ __forceinline__ bool sub_needs_wrap(const SubBox &a, const SubBox &b, float h)
+{
+    bool w = false;
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+        w = w || __fsub_rn(__uint_as_float(max(a.hi[k], b.hi[k])), __uint_as_float(min(a.lo[k], b.lo[k]))) > h;
+    return w;
 }
 
 constexpr int kSubWarps = kBlock / 32;
@@ -196,10 +227,19 @@ __device__ __forceinline__ void sub_tile_row(const float *__restrict__ pos, cons
     __syncwarp();
     unsigned int adj = 0;
     const int dmax = min(16, cntI - 1);
-    for (int d = 1; d <= dmax; ++d) {
-        const int c = (lane + d) & 31;
-        const float pj[6] = {s_j[0][c], s_j[1][c], s_j[2][c], s_j[3][c], s_j[4][c], s_j[5][c]};
-        if (valid && c < cntI && (d < 16 || lane < 16) && linked6(me, pj, q)) adj |= 1u << c;
+    const SubBox boxI = sub_box(me, valid);
+    if (sub_needs_wrap(boxI, boxI, q.h)) {
+        for (int d = 1; d <= dmax; ++d) {
+            const int c = (lane + d) & 31;
+            const float pj[6] = {s_j[0][c], s_j[1][c], s_j[2][c], s_j[3][c], s_j[4][c], s_j[5][c]};
+            if (valid && c < cntI && (d < 16 || lane < 16) && linked6<true>(me, pj, q)) adj |= 1u << c;
+        }
+    } else {
+        for (int d = 1; d <= dmax; ++d) {
+            const int c = (lane + d) & 31;
+            const float pj[6] = {s_j[0][c], s_j[1][c], s_j[2][c], s_j[3][c], s_j[4][c], s_j[5][c]};
+            if (valid && c < cntI && (d < 16 || lane < 16) && linked6<false>(me, pj, q)) adj |= 1u << c;
+        }
     }
     const bool diag = jt1 == it;
     if (diag) nedges += (unsigned int)__popc(adj);
@@ -236,21 +276,33 @@ __device__ __forceinline__ void sub_tile_row(const float *__restrict__ pos, cons
     for (int jt = jt0; jt <= min(jt1, it - 1); ++jt) {
         const int jslot0 = off + jt * ts;
         __syncwarp();
+        float pjl[3] = {0.f, 0.f, 0.f};
         if (lane < ts) {
             const int64_t j = members[jslot0 + lane];
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
-                s_j[a][lane] = wrap1(__ldg(pos + 3 * j + a), q.L);
+                pjl[a] = wrap1(__ldg(pos + 3 * j + a), q.L);
+                s_j[a][lane] = pjl[a];
                 s_j[3 + a][lane] = __ldg(vel + 3 * j + a);
             }
         }
+        const bool wrap = sub_needs_wrap(boxI, sub_box(pjl, lane < ts), q.h);
         __syncwarp();
         unsigned int adjT = 0;  // lane k: tile lanes linked to candidate k
+        if (wrap) {
 #pragma unroll 4
-        for (int k = 0; k < ts; ++k) {
-            const float pj[6] = {s_j[0][k], s_j[1][k], s_j[2][k], s_j[3][k], s_j[4][k], s_j[5][k]};
-            const unsigned int bal = __ballot_sync(kAll, valid && linked6(me, pj, q));
-            if (lane == k) adjT = bal;
+            for (int k = 0; k < ts; ++k) {
+                const float pj[6] = {s_j[0][k], s_j[1][k], s_j[2][k], s_j[3][k], s_j[4][k], s_j[5][k]};
+                const unsigned int bal = __ballot_sync(kAll, valid && linked6<true>(me, pj, q));
+                if (lane == k) adjT = bal;
+            }
+        } else {
+#pragma unroll 4
+            for (int k = 0; k < ts; ++k) {
+                const float pj[6] = {s_j[0][k], s_j[1][k], s_j[2][k], s_j[3][k], s_j[4][k], s_j[5][k]};
+                const unsigned int bal = __ballot_sync(kAll, valid && linked6<false>(me, pj, q));
+                if (lane == k) adjT = bal;
+            }
         }
         nedges += (unsigned int)__popc(adjT);
         const unsigned int active = __reduce_or_sync(kAll, adjT);
