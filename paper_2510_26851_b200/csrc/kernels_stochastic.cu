@@ -63,9 +63,13 @@ __global__ void __launch_bounds__(kBlock) iota_kernel(int *__restrict__ labels, 
 
 constexpr int kStochWarps = kBlock / 32;
 
+#ifndef FOF_STOCH_DIRECT
+#define FOF_STOCH_DIRECT 16  // direct form when the mean number of edges per lane is at least FOF_STOCH_DIRECT / 32 of the largest
+#endif
 struct StochAcc {
     float lp;  // a lane adds at most a few thousand O(1) terms: float32 is enough before the float64 reduction
     unsigned int ncand, nedge;
+    float gx, gy, gz;  // gradient terms of this lane's own home particle gathered by the direct form of stoch_batch
 };
 
 // One warp per 32 consecutive cell-sorted home particles.  Homes of
@@ -78,9 +82,8 @@ struct StochAcc {
 // flattened home by home over the lanes for the expensive part (logistic, random draw, log p,
 // gradient, hook), so that this part runs with full lanes and a home particle's gradient terms are
 // consecutive (segmented warp scan, no atomics, fixed summation order).  A pair is owned (counted,
-// log p, hooked) by the member that sees the other one in its forward half stencil (in one cell:
-// the earlier slot); seen from the other side the same pair (same p, same y: the generator is keyed
-// on the pair) only feeds the home particle's gradient.
+// log p, hooked) by its member with the smaller cell-sorted slot; seen from the other side the same
+// pair (same p, same y: the generator is keyed on the pair) only feeds the home particle's gradient.
 struct StochSmem {
     float4 home[32];  // x, y, z, original index
     float4 cand[64];  // x, y, z, cell-sorted slot
@@ -146,6 +149,49 @@ __device__ __forceinline__ void stoch_batch(StochSmem &sm, int cnt, bool wrap, c
     }
     const int total = __shfl_sync(kAll, incl, 31);
     const int excl = incl - mine_n;
+    if (__reduce_max_sync(kAll, mine_n) * FOF_STOCH_DIRECT <= total) {
+        // Every home has about as many potential edges as the busiest one (a clump core): each lane walks
+        // its own, no flattening, the gradient stays in registers.
+        const float4 ph = sm.home[lane];
+        unsigned int m = adjH;
+        while (__any_sync(kAll, m != 0u)) {
+            if (m) {
+                const float4 pj = sm.cand[__ffs((int)m) - 1];
+                m &= m - 1u;
+                const int j = __float_as_int(pj.w);
+                const bool owned = j > myslot;
+                if (want_grad || owned) {
+                    const float ddx = min_image(__fsub_rn(ph.x, pj.x), g.L, g.h);
+                    const float ddy = min_image(__fsub_rn(ph.y, pj.y), g.L, g.h);
+                    const float ddz = min_image(__fsub_rn(ph.z, pj.z), g.L, g.h);
+                    const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(ddx, ddx), __fmul_rn(ddy, ddy)), __fmul_rn(ddz, ddz));
+                    const float tt = __fmul_rn(sp.c, __fsub_rn(sp.b2, d2));
+                    float e;
+                    const float pr = sigmoid_fixed(tt, e);
+                    const unsigned int ooi = (unsigned int)__float_as_int(ph.w), oj = (unsigned int)__ldg(idx_s + j);
+                    const float u = __fmul_rn((float)rng_u24(sp.key, min(ooi, oj), max(ooi, oj)), 5.9604644775390625e-8f);
+                    const bool y = u < pr;
+                    const float tc = fminf(fmaxf(tt, -30.0f), 30.0f);
+                    if (want_grad && tt == tc) {
+                        const float cgr = ((y ? 1.0f : 0.0f) - pr) * sp.gscale;
+                        acc.gx += cgr * ddx;
+                        acc.gy += cgr * ddy;
+                        acc.gz += cgr * ddz;
+                    }
+                    if (owned) {
+                        ++acc.ncand;
+                        acc.lp += -__logf(__fadd_rn(1.0f, e)) - (y ? 0.0f : tc);
+                        if (y) {
+                            ++acc.nedge;
+                            const int pa = myslot - (int)rel[myslot], pb = j - (int)rel[j];
+                            if (pa != pb) unite_rel(rel, idx_s, myslot, j);  // same parent: already one set
+                        }
+                    }
+                }
+            }
+        }
+        return;
+    }
     for (int p0 = 0; p0 < total; p0 += 32) {
         const int p = p0 + lane;
         const bool has = p < total;
@@ -163,15 +209,8 @@ __device__ __forceinline__ void stoch_batch(StochSmem &sm, int cnt, bool wrap, c
         if (has) {
             const float4 ph = sm.home[owner], pj = sm.cand[nth_set_bit(mask, rank)];
             const int j = __float_as_int(pj.w);
-            // the owner of a pair: the member that sees the other one in its forward
-            // half stencil (cell offsets under the periodic wrap), in one cell the earlier slot
-            int ex = cell1(pj.x, g) - cell1(ph.x, g), ey = cell1(pj.y, g) - cell1(ph.y, g),
-                ez = cell1(pj.z, g) - cell1(ph.z, g);
-            ex = ex > 1 ? ex - g.n : (ex < -1 ? ex + g.n : ex);
-            ey = ey > 1 ? ey - g.n : (ey < -1 ? ey + g.n : ey);
-            ez = ez > 1 ? ez - g.n : (ez < -1 ? ez + g.n : ez);
-            const int order = 9 * ez + 3 * ey + ex;
-            const bool owned = order > 0 || (order == 0 && j > osi);
+            // the owner of a pair: its member with the smaller cell-sorted slot
+            const bool owned = j > osi;
             if (want_grad || owned) {  // without the gradient only the owning side has work
                 const float ddx = min_image(__fsub_rn(ph.x, pj.x), g.L, g.h);
                 const float ddy = min_image(__fsub_rn(ph.y, pj.y), g.L, g.h);
@@ -358,15 +397,15 @@ __global__ void __launch_bounds__(kBlock, FOF_STOCH_MINB) link_stochastic_kernel
               cy = min(__float2int_rd(__fmul_rn(me.y, g.inv_cell)), g.n_minus_1),
               cz = min(__float2int_rd(__fmul_rn(me.z, g.inv_cell)), g.n_minus_1);
     const bool want_grad = grad != nullptr;
-    StochAcc acc = {0.0f, 0u, 0u};
+    StochAcc acc = {0.0f, 0u, 0u, 0.0f, 0.0f, 0.0f};
     sm.g[lane][0] = sm.g[lane][1] = sm.g[lane][2] = 0.0f;
     __syncwarp();
     stoch_tile_warp(sorted, g, cs, idx_s, rel, sp, want_grad, sm, me, myslot, oi, valid, cx, cy, cz, lane, acc);
     __syncwarp();
     if (want_grad && valid) {
-        grad[3 * (int64_t)oi + 0] = sm.g[lane][0];
-        grad[3 * (int64_t)oi + 1] = sm.g[lane][1];
-        grad[3 * (int64_t)oi + 2] = sm.g[lane][2];
+        grad[3 * (int64_t)oi + 0] = sm.g[lane][0] + acc.gx;
+        grad[3 * (int64_t)oi + 1] = sm.g[lane][1] + acc.gy;
+        grad[3 * (int64_t)oi + 2] = sm.g[lane][2] + acc.gz;
     }
     double lpd = (double)acc.lp;
     unsigned int ncand = acc.ncand, nedge = acc.nedge;
