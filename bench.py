@@ -317,7 +317,22 @@ def run_ours(args):
         torch.cuda.synchronize()
         e3, cand3, _ = f3.link_stats()
         t_bin, t_smp = ev[0].elapsed_time(ev[1]), ev[1].elapsed_time(ev[2]) / S
-        next3 = {"samples": S, "binning_ms": t_bin, "ms_per_sample": t_smp,
+        # the same S samples in one batched call (candidate filter, tests and p_ij shared by four samples at a time)
+        labS = torch.empty((S, N), dtype=torch.int32, device=dev)
+        lpS = torch.zeros(S, dtype=torch.float64, device=dev)
+        gS = torch.empty((S, N, 3), dtype=torch.float32, device=dev)
+        scr = torch.empty(max(B.fof_stochastic_scratch_bytes(f3.h, S), 4), dtype=torch.uint8, device=dev)
+        B.fof_link_stochastic_batch(f3.h, w.b, 5.0, 2024, 0, S, labS, lpS, gS, scr, f3.ws)
+        torch.cuda.synchronize()
+        ev[0].record(stream)
+        B.fof_link_stochastic_batch(f3.h, w.b, 5.0, 2024, 0, S, labS, lpS, gS, scr, f3.ws)
+        ev[1].record(stream)
+        torch.cuda.synchronize()
+        t_batch = ev[0].elapsed_time(ev[1]) / S
+        same = bool(torch.equal(labS[S - 1], lab3))   # the last single sample was sample S - 1
+        del labS, gS, scr
+        next3 = {"samples": S, "binning_ms": t_bin, "ms_per_sample": t_smp, "batched_ms_per_sample": t_batch,
+                 "batched_labels_equal_single": same,
                  "potential_edges": cand3, "sampled_edges_last": e3,
                  "potential_edges_per_s": cand3 / (t_smp * 1e-3), "particles_per_s_per_sample": N / (t_smp * 1e-3),
                  "config": "b_cand = 1.5 b, alpha = 5, log p(y) and score function on"}

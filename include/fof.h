@@ -115,6 +115,19 @@ int fof_groups(fof_handle *h, const float *pos, const float *mass, const int32_t
 int fof_link_stochastic(fof_handle *h, float b_link, float alpha, uint64_t seed, uint32_t sample, int32_t *labels,
                         double *logp, float *grad_pos, void *ws, void *stream);
 
+/* S samples sample .. sample + S - 1 of the same step in one call (section 3.2: the S Monte Carlo
+ * samples of one REINFORCE step share the neighbour structure).  Candidate filter, distance tests and
+ * p_ij are evaluated once for four samples at a time; sample k gives exactly the labels, log p and
+ * (to float32 summation order) the score function that fof_link_stochastic(sample + k) gives.
+ *   labels   dev [S][N]; logp dev double [S]; grad_pos dev [S][N][3] or NULL.
+ *   scratch  dev, fof_stochastic_scratch_bytes(h, S) bytes (one union-find array per sample), 4-B aligned.
+ * After the call fof_link_stats reports the potential edges (the same for every sample) as pair tests
+ * and the sampled edges summed over the S samples as E.  Same call order rules as fof_link_stochastic.
+ * Asynchronous on `stream`. */
+size_t fof_stochastic_scratch_bytes(const fof_handle *h, int32_t S);
+int fof_link_stochastic_batch(fof_handle *h, float b_link, float alpha, uint64_t seed, uint32_t sample, int32_t S,
+                              int32_t *labels, double *logp, float *grad_pos, void *scratch, void *ws, void *stream);
+
 /* Six-dimensional sub-halo pass (section 2.1.1, Eq. 3; R29-R31): inside every
  * kept halo a second FoF in phase space, two members linked iff
  *     (x_i - x_j)^2 / sigma_x + (v_i - v_j)^2 / sigma_v <= ell^2

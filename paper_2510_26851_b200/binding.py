@@ -62,6 +62,11 @@ def lib():
         L.fof_groups.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, ctypes.POINTER(i64), vp]
         L.fof_link_stochastic.restype = ctypes.c_int
         L.fof_link_stochastic.argtypes = [vp, f32, f32, ctypes.c_uint64, ctypes.c_uint32, vp, vp, vp, vp, vp]
+        L.fof_stochastic_scratch_bytes.restype = ctypes.c_size_t
+        L.fof_stochastic_scratch_bytes.argtypes = [vp, ctypes.c_int32]
+        L.fof_link_stochastic_batch.restype = ctypes.c_int
+        L.fof_link_stochastic_batch.argtypes = [vp, f32, f32, ctypes.c_uint64, ctypes.c_uint32, ctypes.c_int32, vp, vp, vp,
+                                                vp, vp, vp]
         L.fof_subgroups.restype = ctypes.c_int
         L.fof_subgroups.argtypes = [vp, vp, vp, vp, vp, i64, f32, f32, f32, vp, vp, vp]
         L.fof_layer_select.restype = ctypes.c_int
@@ -178,6 +183,16 @@ def fof_link_stochastic(h, b_link, alpha, seed, sample, labels, logp, grad_pos, 
     """labels: cuda int32 [N]; logp: cuda float64 [1]; grad_pos: cuda float32 [N,3] or None."""
     _check(lib().fof_link_stochastic(h, _f(b_link), _f(alpha), int(seed), int(sample), _ptr(labels), _ptr(logp),
                                      _ptr(grad_pos), _ptr(ws), _stream_ptr(stream)), h)
+
+
+def fof_stochastic_scratch_bytes(h, S):
+    return int(lib().fof_stochastic_scratch_bytes(h, int(S)))
+
+
+def fof_link_stochastic_batch(h, b_link, alpha, seed, sample, S, labels, logp, grad_pos, scratch, ws, stream=None):
+    """labels: cuda int32 [S,N]; logp: cuda float64 [S]; grad_pos: cuda float32 [S,N,3] or None; scratch: cuda bytes."""
+    _check(lib().fof_link_stochastic_batch(h, _f(b_link), _f(alpha), int(seed), int(sample), int(S), _ptr(labels),
+                                           _ptr(logp), _ptr(grad_pos), _ptr(scratch), _ptr(ws), _stream_ptr(stream)), h)
 
 
 def fof_subgroups(h, pos, vel, particle_group, group_size, K, sigma_x, sigma_v, ell, sub_labels, ws, stream=None):
@@ -333,6 +348,19 @@ class FoF:
         grad = torch.empty((self.N, 3), dtype=torch.float32, device=d) if want_grad else None
         with torch.cuda.device(d):
             fof_link_stochastic(self.h, b_link, alpha, seed, sample, labels, logp, grad, self.ws, stream)
+        return labels, logp, grad
+
+    def link_stochastic_batch(self, b_link, alpha, seed, sample, S, want_grad=True, stream=None):
+        """S samples sample .. sample + S - 1 in one call: (labels [S,N], logp [S], grad [S,N,3] or None)."""
+        import torch
+
+        d = self.device
+        labels = torch.empty((S, self.N), dtype=torch.int32, device=d)
+        logp = torch.zeros(S, dtype=torch.float64, device=d)
+        grad = torch.empty((S, self.N, 3), dtype=torch.float32, device=d) if want_grad else None
+        scratch = torch.empty(max(fof_stochastic_scratch_bytes(self.h, S), 4), dtype=torch.uint8, device=d)
+        with torch.cuda.device(d):
+            fof_link_stochastic_batch(self.h, b_link, alpha, seed, sample, S, labels, logp, grad, scratch, self.ws, stream)
         return labels, logp, grad
 
     def subgroups(self, pos, vel, g, sigma_x, sigma_v, ell, stream=None):

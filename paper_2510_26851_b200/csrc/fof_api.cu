@@ -372,6 +372,28 @@ int fof_link_stochastic(fof_handle *h, float b_link, float alpha, uint64_t seed,
     return FOF_OK;
 }
 
+size_t fof_stochastic_scratch_bytes(const fof_handle *h, int32_t S)
+{
+    if (!h || S <= 0) return 0;
+    return (size_t)S * ((size_t)h->N + 1) * sizeof(unsigned int);
+}
+
+int fof_link_stochastic_batch(fof_handle *h, float b_link, float alpha, uint64_t seed, uint32_t sample0, int32_t S,
+                              int32_t *labels, double *logp, float *grad_pos, void *scratch, void *ws, void *stream)
+{
+    if (!h || !ws || ((uintptr_t)ws & 255) || !logp || S <= 0 || S > 1024) return FOF_ERR_INVALID_ARG;
+    if (!(b_link > 0.0f) || !(b_link <= h->b) || !isfinite(alpha)) return FOF_ERR_INVALID_ARG;
+    if (h->N > 0 && (!labels || !scratch || ((uintptr_t)scratch & 3))) return FOF_ERR_INVALID_ARG;
+    if (!h->linked || h->linked_ws != ws) return FOF_ERR_STATE;  // needs the sort of a fof_link on (h, ws)
+    cudaStream_t s = (cudaStream_t)stream;
+    h->launches += h->N > 0 ? (unsigned long long)(S / 4 + S % 4 + 2 * S) : 0;
+    CK(launch_link_stochastic_batch(at<float4>(ws, h->off_sorted), h->N, h->grid, at<unsigned int>(ws, h->off_cell),
+                                    at<int>(ws, h->off_idx), static_cast<unsigned int *>(scratch), b_link, alpha, seed,
+                                    sample0, S, labels, logp, grad_pos, at<Ctrl>(ws, h->off_ctrl), s),
+       "stochastic link kernels (batch)");
+    return FOF_OK;
+}
+
 int fof_subgroups(fof_handle *h, const float *pos, const float *vel, const int32_t *particle_group,
                   const int32_t *group_size, int64_t K, float sigma_x, float sigma_v, float ell, int32_t *sub_labels,
                   void *ws, void *stream)

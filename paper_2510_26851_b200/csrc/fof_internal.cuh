@@ -261,6 +261,10 @@ cudaError_t launch_link_stochastic(const float4 *sorted, int64_t N, Grid g, cons
                                    const int *idx_s, unsigned int *rel, float b_link, float alpha,
                                    unsigned long long seed, unsigned int sample, int *labels, double *logp, float *grad,
                                    Ctrl *ctrl, cudaStream_t s);
+cudaError_t launch_link_stochastic_batch(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
+                                         const int *idx_s, unsigned int *rel_s, float b_link, float alpha,
+                                         unsigned long long seed, unsigned int sample0, int S, int *labels,
+                                         double *logp, float *grad, Ctrl *ctrl, cudaStream_t s);
 
 cudaError_t launch_subgroups(const float *pos, const float *vel, const int *particle_group, const int *group_size,
                              int64_t N, int64_t K, float L, float sigma_x, float sigma_v, float ell,

@@ -123,12 +123,10 @@ __device__ __forceinline__ int nth_set_bit(unsigned int m, int r)
     return pos;
 }
 
-__device__ __forceinline__ void stoch_batch(StochSmem &sm, int cnt, bool wrap, const float4 &mine, int myslot, int s0,
-                                            const Grid &g, const StochParams &sp, const int *__restrict__ idx_s,
-                                            unsigned int *rel, bool want_grad, int lane, StochAcc &acc)
+// Every home against every candidate of the batch; a home's own slot is taken out afterwards.
+__device__ __forceinline__ unsigned int stoch_batch_adjacency(StochSmem &sm, int cnt, bool wrap, const float4 &mine,
+                                                              int s0, const Grid &g, int lane)
 {
-    constexpr unsigned int kAll = 0xffffffffu;
-    // ---- every home against every candidate of the batch; a home's own slot is taken out afterwards
     sm.selfk[lane] = 0;
     __syncwarp();
     if (lane < cnt) {
@@ -139,6 +137,15 @@ __device__ __forceinline__ void stoch_batch(StochSmem &sm, int cnt, bool wrap, c
     __syncwarp();
     const int sk = sm.selfk[lane];
     if (sk) adjH &= ~(1u << (sk - 1));
+    return adjH;
+}
+
+__device__ __forceinline__ void stoch_batch(StochSmem &sm, int cnt, bool wrap, const float4 &mine, int myslot, int s0,
+                                            const Grid &g, const StochParams &sp, const int *__restrict__ idx_s,
+                                            unsigned int *rel, bool want_grad, int lane, StochAcc &acc)
+{
+    constexpr unsigned int kAll = 0xffffffffu;
+    unsigned int adjH = stoch_batch_adjacency(sm, cnt, wrap, mine, s0, g, lane);
     // ---- the potential edges, home-major, 32 at a time
     const int mine_n = __popc(adjH);
     int incl = mine_n;
@@ -262,11 +269,93 @@ __device__ __forceinline__ void stoch_batch(StochSmem &sm, int cnt, bool wrap, c
     }
 }
 
+// What happens to one staged batch: one sample (BatchOne) or several samples at once (BatchMulti).
+struct BatchOne {
+    const Grid &g;
+    const StochParams &sp;
+    const int *__restrict__ idx_s;
+    unsigned int *rel;
+    bool want_grad;
+    StochAcc &acc;
+    __device__ __forceinline__ void operator()(StochSmem &sm, int cnt, bool wrap, const float4 &mine, int myslot, int s0,
+                                               int lane) const
+    {
+        stoch_batch(sm, cnt, wrap, mine, myslot, s0, g, sp, idx_s, rel, want_grad, lane, acc);
+    }
+};
+
+// SB samples in one pass: candidate filter, distance tests and p_ij do not depend on the sample; only the
+// draw, the log terms, the gradient terms and the hooks (one union-find array per sample) do.  Each
+// lane walks the potential edges of its own home particle; all accumulators are registers.
+template <int SB>
+struct BatchMulti {
+    const Grid &g;
+    const StochParams &sp;
+    const unsigned int *keys;  // per-sample generator keys
+    const int *__restrict__ idx_s;
+    unsigned int *rel;         // SB arrays of N
+    int64_t N;
+    bool want_grad;
+    float *lp;                 // [SB]
+    unsigned int *nedge;       // [SB]
+    float (*gr)[3];            // [SB][3]
+    unsigned int &ncand;
+    __device__ __forceinline__ void operator()(StochSmem &sm, int cnt, bool wrap, const float4 &mine, int myslot, int s0,
+                                               int lane) const
+    {
+        unsigned int m = stoch_batch_adjacency(sm, cnt, wrap, mine, s0, g, lane);
+        const float4 ph = sm.home[lane];
+        while (__any_sync(0xffffffffu, m != 0u)) {
+            if (m) {
+                const float4 pj = sm.cand[__ffs((int)m) - 1];
+                m &= m - 1u;
+                const int j = __float_as_int(pj.w);
+                const bool owned = j > myslot;
+                if (want_grad || owned) {
+                    const float ddx = min_image(__fsub_rn(ph.x, pj.x), g.L, g.h);
+                    const float ddy = min_image(__fsub_rn(ph.y, pj.y), g.L, g.h);
+                    const float ddz = min_image(__fsub_rn(ph.z, pj.z), g.L, g.h);
+                    const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(ddx, ddx), __fmul_rn(ddy, ddy)), __fmul_rn(ddz, ddz));
+                    const float tt = __fmul_rn(sp.c, __fsub_rn(sp.b2, d2));
+                    float e;
+                    const float pr = sigmoid_fixed(tt, e);
+                    const unsigned int ooi = (unsigned int)__float_as_int(ph.w), oj = (unsigned int)__ldg(idx_s + j);
+                    const unsigned int klo = min(ooi, oj), khi = max(ooi, oj);
+                    const float tc = fminf(fmaxf(tt, -30.0f), 30.0f);
+                    const float lp1 = -__logf(__fadd_rn(1.0f, e));
+                    const bool gon = want_grad && tt == tc;
+                    if (owned) ++ncand;
+#pragma unroll
+                    for (int sidx = 0; sidx < SB; ++sidx) {
+                        const float u = __fmul_rn((float)rng_u24(keys[sidx], klo, khi), 5.9604644775390625e-8f);
+                        const bool y = u < pr;
+                        if (gon) {
+                            const float cgr = ((y ? 1.0f : 0.0f) - pr) * sp.gscale;
+                            gr[sidx][0] += cgr * ddx;
+                            gr[sidx][1] += cgr * ddy;
+                            gr[sidx][2] += cgr * ddz;
+                        }
+                        if (owned) {
+                            lp[sidx] += lp1 - (y ? 0.0f : tc);
+                            if (y) {
+                                ++nedge[sidx];
+                                unsigned int *r = rel + (int64_t)sidx * N;
+                                const int pa = myslot - (int)r[myslot], pb = j - (int)r[j];
+                                if (pa != pb) unite_rel(r, idx_s, myslot, j);
+                            }
+                        }
+                    }
+                }
+            }
+        }
+    }
+};
+
+template <class Batch>
 __device__ __forceinline__ void stoch_tile_warp(const float4 *__restrict__ sorted, const Grid &g,
-                                                const unsigned int *__restrict__ cs, const int *__restrict__ idx_s,
-                                                unsigned int *rel, const StochParams &sp, bool want_grad,
+                                                const unsigned int *__restrict__ cs,
                                                 StochSmem &sm, const float4 &me, int myslot, unsigned int oi,
-                                                bool valid, int cx, int cy, int cz, int lane, StochAcc &acc)
+                                                bool valid, int cx, int cy, int cz, int lane, const Batch &batch)
 {
     constexpr unsigned int kAll = 0xffffffffu;
     const float inf = __int_as_float(0x7f800000);
@@ -362,7 +451,7 @@ __device__ __forceinline__ void stoch_tile_warp(const float4 *__restrict__ sorte
             const bool last = base + 32 >= total;
             if (nc >= 32 || (last && nc)) {
                 const int cnt = min(nc, 32);
-                stoch_batch(sm, cnt, wrap, mine, myslot, s0, g, sp, idx_s, rel, want_grad, lane, acc);
+                batch(sm, cnt, wrap, mine, myslot, s0, lane);
                 const float4 keep = sm.cand[32 + lane];
                 __syncwarp();
                 sm.cand[lane] = keep;
@@ -400,7 +489,8 @@ __global__ void __launch_bounds__(kBlock, FOF_STOCH_MINB) link_stochastic_kernel
     StochAcc acc = {0.0f, 0u, 0u, 0.0f, 0.0f, 0.0f};
     sm.g[lane][0] = sm.g[lane][1] = sm.g[lane][2] = 0.0f;
     __syncwarp();
-    stoch_tile_warp(sorted, g, cs, idx_s, rel, sp, want_grad, sm, me, myslot, oi, valid, cx, cy, cz, lane, acc);
+    const BatchOne batch = {g, sp, idx_s, rel, want_grad, acc};
+    stoch_tile_warp(sorted, g, cs, sm, me, myslot, oi, valid, cx, cy, cz, lane, batch);
     __syncwarp();
     if (want_grad && valid) {
         grad[3 * (int64_t)oi + 0] = sm.g[lane][0] + acc.gx;
@@ -421,7 +511,74 @@ __global__ void __launch_bounds__(kBlock, FOF_STOCH_MINB) link_stochastic_kernel
     }
 }
 
+// SB samples of the same binning in one pass (fof_link_stochastic_batch).  keys: one generator key per
+// sample; rel: SB union-find arrays of N; logp: SB doubles; grad: SB arrays of [N][3] or nullptr.
+struct StochKeys {
+    unsigned int k[4];
+    int count_potential;  // the pass that reports the potential edges (they are the same in every pass)
+};
+
+template <int SB>
+__global__ void __launch_bounds__(kBlock, 4) link_stochastic_multi_kernel(const float4 *__restrict__ sorted, int64_t N,
+                                                                          Grid g, const unsigned int *__restrict__ cs,
+                                                                          const int *__restrict__ idx_s,
+                                                                          unsigned int *rel, StochParams sp,
+                                                                          StochKeys keys, double *logp, float *grad,
+                                                                          Ctrl *ctrl)
+{
+    constexpr unsigned int kAll = 0xffffffffu;
+    __shared__ StochSmem s_all[kStochWarps];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    StochSmem &sm = s_all[wib];
+    const int64_t s64 = ((int64_t)blockIdx.x * kStochWarps + wib) * 32 + lane;
+    const bool valid = s64 < N;
+    const int myslot = (int)min(s64, N - 1);
+    const float4 me = __ldg(sorted + myslot);
+    const unsigned int oi = (unsigned int)__ldg(idx_s + myslot);
+    const int cx = min(__float2int_rd(__fmul_rn(me.x, g.inv_cell)), g.n_minus_1),
+              cy = min(__float2int_rd(__fmul_rn(me.y, g.inv_cell)), g.n_minus_1),
+              cz = min(__float2int_rd(__fmul_rn(me.z, g.inv_cell)), g.n_minus_1);
+    float lp[SB], gr[SB][3];
+    unsigned int nedge[SB], ncand = 0;
+#pragma unroll
+    for (int k = 0; k < SB; ++k) { lp[k] = 0.0f; nedge[k] = 0u; gr[k][0] = gr[k][1] = gr[k][2] = 0.0f; }
+    const BatchMulti<SB> batch = {g, sp, keys.k, idx_s, rel, N, grad != nullptr, lp, nedge, gr, ncand};
+    stoch_tile_warp(sorted, g, cs, sm, me, myslot, oi, valid, cx, cy, cz, lane, batch);
+    __syncwarp();
+    unsigned int nedge_all = 0;
+#pragma unroll
+    for (int k = 0; k < SB; ++k) {
+        if (grad && valid) {
+            float *gk = grad + (int64_t)k * 3 * N + 3 * (int64_t)oi;
+            gk[0] = gr[k][0];
+            gk[1] = gr[k][1];
+            gk[2] = gr[k][2];
+        }
+        double lpd = (double)lp[k];
+        for (int o = 16; o > 0; o >>= 1) lpd += __shfl_xor_sync(kAll, lpd, o);
+        if (lane == 0 && lpd != 0.0) atomicAdd(logp + k, lpd);
+        nedge_all += nedge[k];
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        ncand += __shfl_xor_sync(kAll, ncand, o);
+        nedge_all += __shfl_xor_sync(kAll, nedge_all, o);
+    }
+    if (lane == 0) {
+        if (ncand && keys.count_potential) atomicAdd(&ctrl->pair_tests, (unsigned long long)ncand);  // potential edges
+        if (nedge_all) atomicAdd(&ctrl->edges, (unsigned long long)nedge_all);  // sampled edges, all samples of the call
+    }
+}
+
 static inline unsigned int blocks_for(int64_t n, int per_block) { return (unsigned int)((n + per_block - 1) / per_block); }
+
+static unsigned int stoch_key(unsigned long long seed, unsigned int sample)
+{
+    unsigned int k = (unsigned int)(seed ^ (seed >> 32)) ^ (sample * 0x9E3779B9U);  // per-sample key: mix32 on the host
+    k ^= k >> 16; k *= 0x7FEB352DU;
+    k ^= k >> 15; k *= 0x846CA68BU;
+    k ^= k >> 16;
+    return k;
+}
 
 cudaError_t launch_link_stochastic(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
                                    const int *idx_s, unsigned int *rel, float b_link, float alpha,
@@ -437,15 +594,50 @@ cudaError_t launch_link_stochastic(const float4 *sorted, int64_t N, Grid g, cons
     sp.b2 = b_link * b_link;
     sp.c = alpha / sp.b2;
     sp.gscale = -2.0f * sp.c;
-    unsigned int k = (unsigned int)(seed ^ (seed >> 32)) ^ (sample * 0x9E3779B9U);  // per-sample key: mix32 on the host
-    k ^= k >> 16; k *= 0x7FEB352DU;
-    k ^= k >> 15; k *= 0x846CA68BU;
-    k ^= k >> 16;
-    sp.key = k;
+    sp.key = stoch_key(seed, sample);
     iota_kernel<<<blocks_for(N, kBlock), kBlock, 0, s>>>(labels, N);
     link_stochastic_kernel<<<blocks_for(N, kBlock), kBlock, 0, s>>>(sorted, N, g, cell_start, idx_s, rel, sp, logp, grad,
                                                                     ctrl);
     return launch_write_labels(rel, idx_s, labels, N, s);
+}
+
+// S samples sample0 .. sample0 + S - 1 on one binning, four per pass (then one by one).
+cudaError_t launch_link_stochastic_batch(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
+                                         const int *idx_s, unsigned int *rel_s, float b_link, float alpha,
+                                         unsigned long long seed, unsigned int sample0, int S, int *labels,
+                                         double *logp, float *grad, Ctrl *ctrl, cudaStream_t s)
+{
+    cudaError_t e;
+    if ((e = cudaMemsetAsync(logp, 0, (size_t)S * sizeof(double), s)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(&ctrl->edges, 0, 2 * sizeof(unsigned long long), s)) != cudaSuccess) return e;
+    if (N <= 0) return cudaSuccess;
+    if ((e = cudaMemsetAsync(rel_s, 0, (size_t)S * (size_t)N * sizeof(unsigned int), s)) != cudaSuccess) return e;
+    StochParams sp;
+    sp.b2 = b_link * b_link;
+    sp.c = alpha / sp.b2;
+    sp.gscale = -2.0f * sp.c;
+    sp.key = 0u;
+    const unsigned int grid = blocks_for(N, kBlock);
+    for (int k0 = 0; k0 < S;) {
+        StochKeys keys = {{0u, 0u, 0u, 0u}, k0 == 0 ? 1 : 0};
+        const int sb = S - k0 >= 4 ? 4 : 1;
+        for (int k = 0; k < sb; ++k) keys.k[k] = stoch_key(seed, sample0 + (unsigned int)(k0 + k));
+        unsigned int *rel = rel_s + (size_t)k0 * (size_t)N;
+        float *gk = grad ? grad + (size_t)k0 * 3 * (size_t)N : nullptr;
+        if (sb == 4)
+            link_stochastic_multi_kernel<4><<<grid, kBlock, 0, s>>>(sorted, N, g, cell_start, idx_s, rel, sp, keys,
+                                                                    logp + k0, gk, ctrl);
+        else
+            link_stochastic_multi_kernel<1><<<grid, kBlock, 0, s>>>(sorted, N, g, cell_start, idx_s, rel, sp, keys,
+                                                                    logp + k0, gk, ctrl);
+        k0 += sb;
+    }
+    for (int k = 0; k < S; ++k) {
+        int *lab = labels + (size_t)k * (size_t)N;
+        iota_kernel<<<grid, kBlock, 0, s>>>(lab, N);
+        if ((e = launch_write_labels(rel_s + (size_t)k * (size_t)N, idx_s, lab, N, s)) != cudaSuccess) return e;
+    }
+    return cudaGetLastError();
 }
 
 }  // namespace fof

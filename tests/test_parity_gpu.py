@@ -514,6 +514,39 @@ def test_stochastic_link_against_oracle(B, alpha, kappa):
     f.close()
 
 
+@pytest.mark.parametrize("S", [1, 4, 7])
+def test_stochastic_batch_equals_single_samples_and_oracle(B, S):
+    """fof_link_stochastic_batch: sample k of the batch = fof_link_stochastic(sample0 + k) = the oracle's sample
+    (labels and edge counts bit-exact, log p and score function to summation order); S = 7 mixes a pass of four
+    samples with single ones."""
+    w = inputs.scaled(inputs.CONFIGS["cfg1"], 40)
+    p = inputs.make_positions(w)
+    b_link, alpha = w.b, 4.0
+    b_cand = float(np.float32(1.5 * w.b))
+    f = B.FoF(len(p), w.L, b_cand, w.N_min)
+    f.link(torch.from_numpy(p).cuda())
+    labels, logp, grad = f.link_stochastic_batch(b_link, alpha, 99, 3, S)
+    E_all, ncand, _ = f.link_stats()
+    E_sum = 0
+    for k in range(S):
+        o = oracle.stochastic(p, w.L, b_cand, b_link, alpha, 99, 3 + k)
+        assert ncand == o["n_cand"]
+        E_sum += o["n_edge"]
+        assert np.array_equal(labels[k].cpu().numpy(), o["labels"]), f"sample {k}: components differ"
+        assert abs(float(logp[k].item()) - o["logp"]) <= 2e-6 * abs(o["logp"]) + 1e-6
+        gk = grad[k].cpu().numpy().astype(np.float64)
+        assert np.abs(gk - o["grad"]).max() <= 2e-5 * np.abs(o["grad"]).max()
+        l1, lp1, g1 = f.link_stochastic(b_link, alpha, 99, 3 + k)
+        assert torch.equal(l1, labels[k])
+        assert abs(float(lp1.item()) - float(logp[k].item())) <= 2e-6 * abs(o["logp"]) + 1e-6
+    assert E_all == E_sum
+    # without the score function
+    labels2, logp2, grad2 = f.link_stochastic_batch(b_link, alpha, 99, 3, S, want_grad=False)
+    assert grad2 is None and torch.equal(labels2, labels)
+    assert torch.allclose(logp2, logp, rtol=2e-6, atol=1e-6)
+    f.close()
+
+
 def test_stochastic_link_wraps_and_needs_a_link_first(B):
     rng = np.random.default_rng(17)
     L, b = 8.0, 1.0
