@@ -119,7 +119,7 @@ int fof_link_stochastic(fof_handle *h, float b_link, float alpha, uint64_t seed,
  * samples of one REINFORCE step share the neighbour structure).  Candidate filter, distance tests and
  * p_ij are evaluated once for four samples at a time; sample k gives exactly the labels, log p and
  * (to float32 summation order) the score function that fof_link_stochastic(sample + k) gives.
- *   labels   dev [S][N]; logp dev double [S]; grad_pos dev [S][N][3] or NULL.
+ *   S        1 .. 1024 samples; labels dev [S][N]; logp dev double [S]; grad_pos dev [S][N][3] or NULL.
  *   scratch  dev, fof_stochastic_scratch_bytes(h, S) bytes (one union-find array per sample), 4-B aligned.
  * After the call fof_link_stats reports the potential edges (the same for every sample) as pair tests
  * and the sampled edges summed over the S samples as E.  Same call order rules as fof_link_stochastic.
