@@ -67,6 +67,28 @@ def test_plan_and_argument_errors(B):
     assert B.lib().fof_error_string(12345).decode() == "unknown error"
 
 
+def test_stochastic_batch_argument_and_state_errors(B):
+    """fof_link_stochastic_batch rejects bad arguments and a missing fof_link before it touches any memory."""
+    import ctypes
+
+    L = B.lib()
+    h = B.fof_create(1000, 10.0, 1.0, 5)
+    assert L.fof_stochastic_scratch_bytes(h, 3) == 3 * 1001 * 4
+    assert L.fof_stochastic_scratch_bytes(h, 0) == 0 and L.fof_stochastic_scratch_bytes(None, 3) == 0
+    raw = np.zeros(4096, dtype=np.uint8)
+    addr = (raw.ctypes.data + 255) & ~255            # a 256-B aligned host address: never dereferenced here
+    p = ctypes.c_void_p(addr)
+    call = lambda b_link, alpha, S, ws=p: L.fof_link_stochastic_batch(h, ctypes.c_float(b_link), ctypes.c_float(alpha), 1, 0,
+                                                                      S, p, p, None, p, ws, None)
+    assert call(1.0, 2.0, 0) == B.FOF_ERR_INVALID_ARG          # no samples
+    assert call(1.0, 2.0, 2000) == B.FOF_ERR_INVALID_ARG       # too many
+    assert call(1.5, 2.0, 2) == B.FOF_ERR_INVALID_ARG          # b_link above the plan's candidate radius
+    assert call(1.0, float("nan"), 2) == B.FOF_ERR_INVALID_ARG
+    assert call(1.0, 2.0, 2, ctypes.c_void_p(addr + 4)) == B.FOF_ERR_INVALID_ARG   # workspace not 256-B aligned
+    assert call(1.0, 2.0, 2) == B.FOF_ERR_STATE                # no fof_link on this (handle, workspace) yet
+    B.fof_destroy(h)
+
+
 def test_grid_choice_keeps_cell_side_above_b(B):
     """H0: cell side L/n >= 1.001 b for every plan (R3), n >= 3."""
     rng = np.random.default_rng(1)
