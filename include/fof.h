@@ -56,6 +56,26 @@ int fof_set_grid(fof_handle *h, int32_t n);
 /* n per axis, total cells n^3, largest admissible n. Any out pointer may be NULL. */
 int fof_get_grid(const fof_handle *h, int32_t *n, int64_t *cells, int32_t *n_max);
 
+/* Which of the two implementations of H1-H5 fof_link runs (a tuning knob: results are identical).
+ *   FOF_PATH_BLOCKS the BLOCK path where the plan admits it (>= 3 blocks of 2^k cells per axis): one
+ *                   partition pass into spatial blocks + ghost copies, one CTA per block links out of
+ *                   shared memory.  If some block holds more records than a CTA can keep (decided on the
+ *                   device, no host synchronisation), the CELL path runs instead, in the same call.
+ *   FOF_PATH_CELLS  always the CELL path: two-level counting sort into global cell-contiguous arrays and
+ *                   the persistent link kernel over them.  fof_link_stochastic[_batch] and the grid_pairs
+ *                   counter of fof_link_stats need those arrays, i.e. a plan set to FOF_PATH_CELLS (or one
+ *                   that does not admit the block path).
+ *   FOF_PATH_AUTO   (default) the faster of the two for this plan as measured on B200. */
+#define FOF_PATH_AUTO 0
+#define FOF_PATH_CELLS 1
+#define FOF_PATH_BLOCKS 2
+int fof_set_path(fof_handle *h, int32_t path);
+/* Which path the last fof_link on (h, ws) took (FOF_PATH_BLOCKS or FOF_PATH_CELLS), how many blocks the plan
+ * has (0: it does not admit the block path) and the record count of the fullest block (0 if not measured).
+ * Any out pointer may be NULL.  Synchronises `stream`. */
+int fof_link_path(fof_handle *h, void *ws, void *stream, int32_t *path_host, int32_t *blocks_host,
+                  int32_t *max_block_host);
+
 /* Bytes of device workspace fof_link / fof_groups need for this plan (0 on NULL handle). */
 size_t fof_workspace_bytes(const fof_handle *h);
 
@@ -74,7 +94,8 @@ int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *s
 
 /* Counters of the last fof_link on (h, ws): true edges E (unordered pairs with d^2 <= b^2; equal
  * to the oracle's E), distance tests executed (after the geometric reach filter), and the
- * candidate pairs the unfiltered half stencil implies on this plan's grid (P_exec of DESIGN.md §7).
+ * candidate pairs the unfiltered half stencil implies on this plan's grid (P_exec of DESIGN.md §7; 0 unless the
+ * plan is set to FOF_PATH_CELLS, see fof_set_path).
  * Any out pointer may be NULL.  Synchronises `stream`. */
 int fof_link_stats(fof_handle *h, void *ws, void *stream, uint64_t *edges_host, uint64_t *pair_tests_host,
                    uint64_t *grid_pairs_host);

@@ -51,6 +51,10 @@ def lib():
         L.fof_set_grid.argtypes = [vp, i32]
         L.fof_get_grid.restype = ctypes.c_int
         L.fof_get_grid.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i64), ctypes.POINTER(i32)]
+        L.fof_set_path.restype = ctypes.c_int
+        L.fof_set_path.argtypes = [vp, i32]
+        L.fof_link_path.restype = ctypes.c_int
+        L.fof_link_path.argtypes = [vp, vp, vp, ctypes.POINTER(i32), ctypes.POINTER(i32), ctypes.POINTER(i32)]
         L.fof_workspace_bytes.restype = ctypes.c_size_t
         L.fof_workspace_bytes.argtypes = [vp]
         L.fof_link.restype = ctypes.c_int
@@ -151,6 +155,22 @@ def fof_get_grid(h):
     n, c, m = ctypes.c_int32(), ctypes.c_int64(), ctypes.c_int32()
     _check(lib().fof_get_grid(h, ctypes.byref(n), ctypes.byref(c), ctypes.byref(m)))
     return n.value, c.value, m.value
+
+
+FOF_PATH_AUTO, FOF_PATH_CELLS, FOF_PATH_BLOCKS = 0, 1, 2
+_PATHS = {"auto": FOF_PATH_AUTO, "cells": FOF_PATH_CELLS, "blocks": FOF_PATH_BLOCKS}
+
+
+def fof_set_path(h, path):
+    """path: "auto", "cells" (always the cell path) or "blocks" (block path where the plan admits it)."""
+    _check(lib().fof_set_path(h, _PATHS[path] if isinstance(path, str) else int(path)))
+
+
+def fof_link_path(h, ws, stream=None):
+    """("blocks" | "cells" = what the last fof_link ran, blocks of the plan, records of the fullest block)"""
+    p, nb, mb = ctypes.c_int32(), ctypes.c_int32(), ctypes.c_int32()
+    _check(lib().fof_link_path(h, _ptr(ws), _stream_ptr(stream), ctypes.byref(p), ctypes.byref(nb), ctypes.byref(mb)), h)
+    return ("blocks" if p.value == FOF_PATH_BLOCKS else "cells"), int(nb.value), int(mb.value)
 
 
 def fof_workspace_bytes(h) -> int:
@@ -277,7 +297,8 @@ def fof_launch_count(h) -> int:
 class FoF:
     """Owns a plan handle and its device workspace (torch uint8 tensor)."""
 
-    def __init__(self, N: int, L: float, b: float, N_min: int = 20, device="cuda:0", grid: int | None = None):
+    def __init__(self, N: int, L: float, b: float, N_min: int = 20, device="cuda:0", grid: int | None = None,
+                 path: str = "auto"):
         import torch
 
         if not torch.cuda.is_available():
@@ -287,6 +308,8 @@ class FoF:
         self.h = fof_create(N, L, b, N_min)
         if grid is not None:
             fof_set_grid(self.h, grid)
+        if path != "auto":
+            fof_set_path(self.h, path)
         self.cap = max(1, self.N // self.N_min)
         with torch.cuda.device(self.device):
             self.ws = torch.empty(fof_workspace_bytes(self.h) + 256, dtype=torch.uint8, device=self.device)
@@ -320,6 +343,10 @@ class FoF:
     def link_stats(self, stream=None):
         with __import__("torch").cuda.device(self.device):
             return fof_link_stats(self.h, self.ws, stream)
+
+    def link_path(self, stream=None):
+        with __import__("torch").cuda.device(self.device):
+            return fof_link_path(self.h, self.ws, stream)
 
     def status(self, stream=None) -> int:
         with __import__("torch").cuda.device(self.device):

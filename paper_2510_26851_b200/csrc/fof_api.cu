@@ -23,6 +23,43 @@ size_t dense_items_max(size_t N)
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
+constexpr bool kAutoIsBlocks = false;  // what FOF_PATH_AUTO means where the plan admits the block path
+
+// H0, block path: blocks of 2^sx x 2^sy x 2^sz cells with >= 3 blocks per axis (so that the forward and the
+// backward neighbour of a block are different blocks), at most kMaxBlockBins blocks, and a mean occupancy of
+// about half of what block_link_kernel holds (kBlockCap records, own + ghost copies).
+void plan_blocks(fof_handle *h)
+{
+    h->block_ok = false;
+    BlockGeom &bg = h->bg;
+    memset(&bg, 0, sizeof(bg));
+    if (h->N <= 0 || h->n < 6) return;
+    int smax = 0;
+    while ((2 << smax) <= (h->n - 1) / 2) ++smax;  // largest s with ceil(n / 2^s) >= 3
+    if (((h->n + (1 << smax) - 1) >> smax) < 3) return;
+    int s[3] = {smax < 4 ? smax : 4, smax < 4 ? smax : 4, smax < 3 ? smax : 3};
+    const double rho = (double)h->N / ((double)h->n * h->n * h->n);
+    const double target = 0.55 * kBlockCap;
+    while ((double)(1 << (s[0] + s[1] + s[2])) * rho > target) {
+        int a = 2;  // shrink the longest side, z first
+        if (s[1] > s[a]) a = 1;
+        if (s[0] > s[a]) a = 0;
+        if (s[a] == 0) return;
+        --s[a];
+    }
+    if (s[0] < 1 || s[1] < 1 || s[2] < 1) return;  // blocks one cell wide would be mostly ghosts
+    bg.sx = s[0]; bg.sy = s[1]; bg.sz = s[2];
+    bg.nbx = (h->n + (1 << bg.sx) - 1) >> bg.sx;
+    bg.nby = (h->n + (1 << bg.sy) - 1) >> bg.sy;
+    bg.nbz = (h->n + (1 << bg.sz) - 1) >> bg.sz;
+    const int64_t bins = (int64_t)bg.nbx * bg.nby * bg.nbz;
+    if (bins > kMaxBlockBins) return;
+    bg.bins = (int)bins;
+    bg.X = (1 << bg.sx) + 2; bg.Y = (1 << bg.sy) + 2; bg.Z = (1 << bg.sz) + 1;
+    bg.ncell = bg.X * bg.Y * bg.Z;
+    h->block_ok = true;
+}
+
 // H0: workspace layout for the current grid.
 void layout(fof_handle *h)
 {
@@ -34,6 +71,7 @@ void layout(fof_handle *h)
     h->sort.bins = (int)((h->C + ((int64_t)1 << h->sort.shift) - 1) >> h->sort.shift);
     h->gscan_tiles = h->N > 0 ? (h->N + kScanTile - 1) / kScanTile : 1;
     h->max_groups = h->N / h->N_min;
+    plan_blocks(h);
     size_t off = 0;
     h->off_ctrl = off;        off += 256;
     h->off_cell = off;        off += align256(((size_t)cell_items + 8) * sizeof(unsigned int));
@@ -41,10 +79,17 @@ void layout(fof_handle *h)
     h->off_cta_hist = off;    off += align256((size_t)kMaxPartCtas * h->sort.bins * sizeof(unsigned int));
     // fine bin offsets, and behind them the coarse ones of the two-pass partition (<= bins / 64 + 2 entries)
     h->off_bin_base = off;    off += align256(((size_t)h->sort.bins + 2 + (size_t)h->sort.bins / 64 + 4) * sizeof(unsigned int));
+    // `part` and `sorted` are adjacent: the block path's record array (own + ghost copies, part_cap records)
+    // spans both; the cross-block equivalence pairs of the block path live in the idx_s array
+    h->part_cap = (int64_t)(N + N / 4 + 64);
+    if (h->part_cap > (int64_t)(2 * N + 1)) h->part_cap = (int64_t)(2 * N + 1);
     h->off_part = off;        off += align256((N + 1) * sizeof(float4));
-    h->off_idx = off;         off += align256((N + 1) * sizeof(int));
-    h->off_dense = off;       off += align256(dense_items_max(N) * sizeof(unsigned long long));
     h->off_sorted = off;      off += align256((N + 1) * sizeof(float4));
+    h->off_idx = off;         off += align256((N + 1 + 2 * (N / 4 + 64)) * sizeof(int));
+    h->off_dense = off;       off += align256(dense_items_max(N) * sizeof(unsigned long long));
+    h->off_bin_total = off;   off += align256(((size_t)kMaxBlockBins + 2) * sizeof(unsigned int));
+    h->off_bbase = off;       off += align256(((size_t)kMaxBlockBins + 2) * sizeof(unsigned int));
+    h->off_cursor = off;      off += align256(((size_t)kMaxBlockBins + 2) * sizeof(unsigned int));
     h->off_cnt = off;         off += align256((N + 1) * sizeof(int));
     h->off_acc = off;         off += align256(((size_t)h->max_groups + 1) * 4 * sizeof(double));
     h->off_gscan_state = off; off += align256((size_t)h->gscan_tiles * sizeof(unsigned long long));
@@ -77,10 +122,12 @@ int cuda_fail(fof_handle *h, cudaError_t e, const char *where)
     } while (0)
 
 // Profiled stages, in execution order (fof_profile_name).
-enum Stage { kLinkClear = 0, kLinkHist, kLinkOffsets, kLinkPartition, kLinkCellSort, kLinkPairs, kLinkLabels,
+enum Stage { kLinkClear = 0, kBlockHist, kBlockOffsets, kBlockPartition, kBlockLink, kBlockCross, kBlockFlatten,
+             kLinkHist, kLinkOffsets, kLinkPartition, kLinkCellSort, kLinkPairs, kLinkLabels,
              kGroupsClear, kGroupsCount, kGroupsCompact, kGroupsReduce, kGroupsFinish, kNumStages };
 const char *const kStageName[kNumStages] = {
-    "link.clear", "link.hist", "link.offsets", "link.partition", "link.cell_sort", "link.pairs", "link.labels",
+    "link.clear", "block.hist", "block.offsets", "block.partition", "block.link", "block.cross", "block.flatten",
+    "link.hist", "link.offsets", "link.partition", "link.cell_sort", "link.pairs", "link.labels",
     "groups.clear", "groups.count", "groups.compact", "groups.reduce", "groups.finish"};
 static_assert(kNumStages <= kMaxStages, "raise kMaxStages");
 
@@ -147,6 +194,7 @@ int fof_create(int64_t N, float L, float b, int32_t N_min, fof_handle **out)
     memset(h, 0, sizeof(*h));
     h->N = N; h->L = L; h->b = b; h->N_min = N_min;
     h->prof_only = -1;
+    h->path = FOF_PATH_AUTO;
     h->n_max = n_max;
     h->n = n_occ < n_max ? n_occ : n_max;
     if (h->n < 3) h->n = 3;
@@ -244,6 +292,30 @@ int fof_get_grid(const fof_handle *h, int32_t *n, int64_t *cells, int32_t *n_max
 
 size_t fof_workspace_bytes(const fof_handle *h) { return h ? h->ws_bytes : 0; }
 
+int fof_set_path(fof_handle *h, int32_t path)
+{
+    if (!h || (path != FOF_PATH_AUTO && path != FOF_PATH_CELLS && path != FOF_PATH_BLOCKS)) return FOF_ERR_INVALID_ARG;
+    h->path = path;
+    h->linked = false;
+    return FOF_OK;
+}
+
+int fof_link_path(fof_handle *h, void *ws, void *stream, int32_t *path_host, int32_t *blocks_host,
+                  int32_t *max_block_host)
+{
+    if (!h || !ws) return FOF_ERR_INVALID_ARG;
+    if (!h->linked || h->linked_ws != ws) return FOF_ERR_STATE;
+    cudaStream_t s = (cudaStream_t)stream;
+    Ctrl c;
+    CK(cudaMemcpyAsync(&c, at<Ctrl>(ws, h->off_ctrl), sizeof(Ctrl), cudaMemcpyDeviceToHost, s), "copy ctrl");
+    CK(cudaStreamSynchronize(s), "sync");
+    const bool blocks = !h->linked_cells && c.mode == 0u;
+    if (path_host) *path_host = blocks ? FOF_PATH_BLOCKS : FOF_PATH_CELLS;
+    if (blocks_host) *blocks_host = h->block_ok ? h->bg.bins : 0;
+    if (max_block_host) *max_block_host = h->linked_cells ? 0 : (int32_t)c.max_block;
+    return FOF_OK;
+}
+
 int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *stream)
 {
     if (!h || !ws || ((uintptr_t)ws & 255)) return FOF_ERR_INVALID_ARG;
@@ -273,19 +345,31 @@ int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *s
         StageTimer t(h, s, kLinkClear, 0);
         CK(cudaMemsetAsync(ctrl, 0, 256, s), "memset ctrl");
     }
+    // Block path first where the plan admits it; it leaves ctrl->mode = 1 (and nothing else) when a block does
+    // not fit shared memory, and the cell path below, gated on that flag, then does the work.
+    const bool blocks = h->block_ok && (h->path == FOF_PATH_BLOCKS || (h->path == FOF_PATH_AUTO && kAutoIsBlocks)) && has;
+    if (blocks) {
+        StageHook hook{h, s, kBlockHist};
+        CK(launch_block_path(pos, h->N, h->grid, h->bg, h->part_ctas, at<unsigned int>(ws, h->off_bin_total),
+                             at<unsigned int>(ws, h->off_bbase), at<unsigned int>(ws, h->off_cursor),
+                             at<float4>(ws, h->off_part), h->part_cap, at<int2>(ws, h->off_idx), labels, ctrl, hook, s),
+           "block path kernels");
+    }
+    const unsigned int *gate = blocks ? &ctrl->mode : nullptr;
     {
         StageHook hook{h, s, kLinkHist};
         CK(launch_sort(pos, h->N, h->grid, h->sort, h->part_ctas, at<unsigned int>(ws, h->off_cta_hist),
                        at<unsigned int>(ws, h->off_bin_base), at<float4>(ws, h->off_part), cell, sorted, rel, idx_s,
-                       dense, labels, ctrl, hook, s), "sort kernels");
+                       dense, labels, ctrl, gate, hook, s), "sort kernels");
     }
     {
         StageTimer t(h, s, kLinkPairs, has);
-        CK(launch_link(sorted, h->N, h->grid, cell, dense, rel, idx_s, ctrl, h->num_sms, s), "link kernels");
+        CK(launch_link(sorted, h->N, h->grid, cell, dense, rel, idx_s, ctrl, h->num_sms, gate, s), "link kernels");
     }
-    { StageTimer t(h, s, kLinkLabels, has); CK(launch_write_labels(rel, idx_s, labels, h->N, s), "write_labels_kernel"); }
+    { StageTimer t(h, s, kLinkLabels, has); CK(launch_write_labels(rel, idx_s, labels, h->N, gate, s), "write_labels_kernel"); }
     h->linked = true;
     h->linked_ws = ws;
+    h->linked_cells = !blocks;  // the cell-sorted arrays are certainly there only if the cell path ran ungated
     return FOF_OK;
 }
 
@@ -297,7 +381,7 @@ int fof_link_stats(fof_handle *h, void *ws, void *stream, uint64_t *edges_host, 
     cudaStream_t s = (cudaStream_t)stream;
     Ctrl c;
     Ctrl *ctrl = at<Ctrl>(ws, h->off_ctrl);
-    if (grid_pairs_host && h->N > 0) {  // computed on demand from the cell offsets left in the workspace
+    if (grid_pairs_host && h->N > 0 && h->linked_cells) {  // computed on demand from the cell offsets left in the workspace
         CK(cudaMemsetAsync(&ctrl->grid_pairs, 0, sizeof(unsigned long long), s), "memset grid_pairs");
         CK(launch_grid_pairs(at<unsigned int>(ws, h->off_cell), h->grid, ctrl, h->num_sms, s), "grid_pairs_kernel");
     }
@@ -363,7 +447,7 @@ int fof_link_stochastic(fof_handle *h, float b_link, float alpha, uint64_t seed,
     if (!h || !ws || ((uintptr_t)ws & 255) || !logp) return FOF_ERR_INVALID_ARG;
     if (!(b_link > 0.0f) || !(b_link <= h->b) || !isfinite(alpha)) return FOF_ERR_INVALID_ARG;
     if (h->N > 0 && !labels) return FOF_ERR_INVALID_ARG;
-    if (!h->linked || h->linked_ws != ws) return FOF_ERR_STATE;  // needs the sort of a fof_link on (h, ws)
+    if (!h->linked || h->linked_ws != ws || !h->linked_cells) return FOF_ERR_STATE;  // needs the cell sort of a fof_link on (h, ws)
     cudaStream_t s = (cudaStream_t)stream;
     h->launches += h->N > 0 ? 3 : 0;
     CK(launch_link_stochastic(at<float4>(ws, h->off_sorted), h->N, h->grid, at<unsigned int>(ws, h->off_cell),
@@ -384,7 +468,7 @@ int fof_link_stochastic_batch(fof_handle *h, float b_link, float alpha, uint64_t
     if (!h || !ws || ((uintptr_t)ws & 255) || !logp || S <= 0 || S > 1024) return FOF_ERR_INVALID_ARG;
     if (!(b_link > 0.0f) || !(b_link <= h->b) || !isfinite(alpha)) return FOF_ERR_INVALID_ARG;
     if (h->N > 0 && (!labels || !scratch || ((uintptr_t)scratch & 3))) return FOF_ERR_INVALID_ARG;
-    if (!h->linked || h->linked_ws != ws) return FOF_ERR_STATE;  // needs the sort of a fof_link on (h, ws)
+    if (!h->linked || h->linked_ws != ws || !h->linked_cells) return FOF_ERR_STATE;  // needs the cell sort of a fof_link on (h, ws)
     cudaStream_t s = (cudaStream_t)stream;
     h->launches += h->N > 0 ? (unsigned long long)(S / 4 + S % 4 + 2 * S) : 0;
     CK(launch_link_stochastic_batch(at<float4>(ws, h->off_sorted), h->N, h->grid, at<unsigned int>(ws, h->off_cell),

@@ -38,6 +38,10 @@ struct Ctrl {
     unsigned int ndense;            // work items (dense cell, tile) listed by cell_sort_kernel
     unsigned int tile_ticket;       // next (dense cell, tile) item of link_kernel
     unsigned int sparse_ticket;     // next 32-particle chunk of link_kernel
+    unsigned int mode;              // block path: 0 = every block fits shared memory, 1 = fall back to the cell path
+    unsigned int ncross;            // block path: equivalence pairs listed by block_link_kernel
+    unsigned int tile_ticket2;      // block path: next input tile of block_scatter_kernel
+    unsigned int max_block;         // block path: records (own + ghost) of the fullest block
     unsigned int pad1[3];
 };
 static_assert(sizeof(Ctrl) <= 256, "Ctrl must fit its 256-byte slot");
@@ -53,6 +57,21 @@ struct Grid {
     float reach;    // b in cell units + slack: how close to a cell face a particle must be to have
                     // a partner in the cell behind it (kernels_link.cu candidate_ranges)
 };
+
+// Block path (kernels_block.cu): the cell grid is cut into blocks of 2^sx x 2^sy x 2^sz cells; one CTA links
+// one block out of shared memory.  Local cell grid of a block: X x Y x Z cells = its own cells plus one
+// ghost layer on both x and y sides and on the upper z side (the forward half stencil never looks down in z).
+struct BlockGeom {
+    int sx, sy, sz;     // log2 of the block's cells per axis
+    int nbx, nby, nbz;  // blocks per axis = ceil(n / 2^s); >= 3 each
+    int bins;           // nbx * nby * nbz
+    int X, Y, Z;        // local grid: 2^sx + 2, 2^sy + 2, 2^sz + 1
+    int ncell;          // X * Y * Z
+};
+constexpr int kBlockCap = 4096;      // most records (own + ghost) of a block that block_link_kernel holds
+constexpr int kBlockThreads = 512;   // threads per CTA of block_link_kernel
+constexpr int kMaxBlockBins = 16384; // most blocks (one shared-memory counter each in the partition)
+constexpr unsigned int kGhostBit = 0x80000000u;  // record.w = original index | kGhostBit for a ghost copy
 
 constexpr int kLinkBlock = 256;     // threads per CTA of the link kernels
 #ifndef FOF_DENSE_CELL
@@ -106,12 +125,18 @@ struct fof_handle {
     fof::Grid grid;
     // workspace layout (byte offsets, 256-B aligned)
     fof::SortPlan sort;
+    fof::BlockGeom bg;      // block path geometry (valid if block_ok)
+    bool block_ok;          // the plan admits the block path (>= 3 blocks per axis, <= kMaxBlockBins blocks)
+    int path;               // FOF_PATH_AUTO / FOF_PATH_BLOCKS / FOF_PATH_CELLS
+    size_t off_bin_total, off_bbase, off_cursor;  // block path: records per block, exclusive offsets, write cursors
+    int64_t part_cap;       // block path: capacity of the record array (own + ghost)
     size_t off_ctrl, off_cell, off_part, off_cta_hist, off_bin_base, off_sorted, off_cnt, off_acc, off_gscan_state;
     size_t off_rel, off_idx, off_dense;  // union-find (cell-sorted space), original index of each slot, work items
     size_t ws_bytes;
     int64_t gscan_tiles, max_groups;
     int num_sms, part_ctas;
     bool linked;
+    bool linked_cells;      // the last fof_link left cell_start / sorted / idx_s / rel in the workspace for certain
     const void *linked_ws;
     char cuda_err[256];
     // measurement aids
@@ -151,6 +176,42 @@ __device__ __forceinline__ int cell1(float w, const Grid &g)
 __device__ __forceinline__ unsigned int cell_id(int cx, int cy, int cz, int n)
 {
     return (unsigned int)cx + (unsigned int)n * ((unsigned int)cy + (unsigned int)n * (unsigned int)cz);
+}
+
+// wrapped position (non-finite -> 0 and `bad`) and linear cell id of one particle
+__device__ __forceinline__ unsigned int wrap_cell(float &x, float &y, float &z, const Grid &g, bool &bad)
+{
+    if (!(isfinite(x) && isfinite(y) && isfinite(z))) { bad = true; x = y = z = 0.0f; }
+    x = wrap1(x, g.L);
+    y = wrap1(y, g.L);
+    z = wrap1(z, g.L);
+    return cell_id(cell1(x, g), cell1(y, g), cell1(z, g), g.n);
+}
+
+// Walks the particles [i0, i1) of one CTA four at a time: thread t takes the quads t, t + T, ...
+// With VEC (pos 16-byte aligned, i0 a multiple of 4) a quad is three 128-bit loads, all issued
+// before the first use, so every thread keeps 48 bytes in flight; f(x, y, z, i) is called per particle.
+template <bool VEC, int THREADS, typename F>
+__device__ __forceinline__ void for_each_particle(const float *__restrict__ pos, int64_t i0, int64_t i1, F f)
+{
+    for (int64_t i = i0 + 4 * (int64_t)threadIdx.x; i < i1; i += 4 * (int64_t)THREADS) {
+        if (VEC && i + 4 <= i1) {
+            const float4 *q = reinterpret_cast<const float4 *>(pos + 3 * i);
+            const float4 a = __ldg(q), b = __ldg(q + 1), c = __ldg(q + 2);
+            f(a.x, a.y, a.z, i);
+            f(a.w, b.x, b.y, i + 1);
+            f(b.z, b.w, c.x, i + 2);
+            f(c.y, c.z, c.w, i + 3);
+        } else {
+            const int m = (int)min((int64_t)4, i1 - i);
+            float v[12];
+#pragma unroll
+            for (int k = 0; k < 12; ++k) v[k] = (k < 3 * m) ? __ldg(pos + 3 * i + k) : 0.0f;
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (k < m) f(v[3 * k], v[3 * k + 1], v[3 * k + 2], i + k);
+        }
+    }
 }
 
 // ---- link predicate (north_star's single float32 expression):
@@ -229,12 +290,19 @@ struct StageHook {
 cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp, int ctas, unsigned int *cta_hist,
                         unsigned int *bin_base, float4 *part, unsigned int *cell_start, float4 *sorted,
                         unsigned int *rel, int *idx_s, unsigned long long *dense_list, int *labels, Ctrl *ctrl,
-                        StageHook &hook, cudaStream_t s);
+                        const unsigned int *gate, StageHook &hook, cudaStream_t s);
+// block path (kernels_block.cu): histogram + offsets + partition into blocks (with ghost copies), one CTA per
+// block links out of shared memory, equivalence pairs across blocks, flatten.  Sets ctrl->mode = 1 (and does
+// nothing else) if a block does not fit: the gated cell path then runs instead.
+cudaError_t launch_block_path(const float *pos, int64_t N, Grid g, const BlockGeom &bg, int ctas, unsigned int *bin_total,
+                              unsigned int *bin_base, unsigned int *cursor, float4 *part, int64_t part_cap, int2 *cross,
+                              int *labels, Ctrl *ctrl, StageHook &hook, cudaStream_t s);
 cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
                         const unsigned long long *dense_list, unsigned int *rel, const int *idx_s, Ctrl *ctrl,
-                        int num_sms, cudaStream_t s);
+                        int num_sms, const unsigned int *gate, cudaStream_t s);
 cudaError_t launch_grid_pairs(const unsigned int *cell_start, Grid g, Ctrl *ctrl, int num_sms, cudaStream_t s);
-cudaError_t launch_write_labels(const unsigned int *rel, const int *idx_s, int *labels, int64_t N, cudaStream_t s);
+cudaError_t launch_write_labels(const unsigned int *rel, const int *idx_s, int *labels, int64_t N,
+                                const unsigned int *gate, cudaStream_t s);
 
 cudaError_t launch_group_count(const int *labels, int64_t N, int *cnt, unsigned long long *state,
                                int64_t state_items, Ctrl *ctrl, cudaStream_t s);

@@ -545,9 +545,11 @@ __global__ void __launch_bounds__(kLinkBlock, FOF_LINK_MINB) link_kernel(const f
                                                                          unsigned int *rel,
                                                                          const int *__restrict__ idx_s, Ctrl *ctrl,
                                                                          unsigned int tile_batch,
-                                                                         unsigned int sparse_batch)
+                                                                         unsigned int sparse_batch,
+                                                                         const unsigned int *gate)
 {
     __shared__ LinkSmem s_all[kWarpsPerCta];
+    if (gate && *gate == 0u) return;  // the block path did the work
     LinkSmem &sm = s_all[threadIdx.x >> 5];
     const int lane = threadIdx.x & 31;
     const unsigned int nitems = ctrl->ndense;
@@ -596,12 +598,14 @@ __global__ void __launch_bounds__(kLinkBlock, FOF_LINK_MINB) link_kernel(const f
 // lock step so that the (up to four) loads of one round are in flight together; read-only chase.
 __global__ void __launch_bounds__(kBlock) write_labels_kernel(const unsigned int *__restrict__ rel,
                                                               const int *__restrict__ idx_s, int *__restrict__ labels,
-                                                              int64_t N)
+                                                              int64_t N, bool vec, const unsigned int *gate)
 {
+    // vec: rel and idx_s are 16-byte aligned (the workspace arrays are; the per-sample union-find arrays of
+    // fof_link_stochastic_batch, rel_s + k N, are not when N is not a multiple of 4)
     const int64_t s0 = ((int64_t)blockIdx.x * kBlock + threadIdx.x) * 4;
-    if (s0 >= N) return;
+    if (s0 >= N || (gate && *gate == 0u)) return;
     int d[4], oi[4];
-    if (s0 + 3 < N) {
+    if (vec && s0 + 3 < N) {
         const uint4 t = __ldg(reinterpret_cast<const uint4 *>(rel + s0));
         d[0] = (int)t.x; d[1] = (int)t.y; d[2] = (int)t.z; d[3] = (int)t.w;
         if ((d[0] | d[1] | d[2] | d[3]) == 0) return;  // four roots
@@ -670,7 +674,7 @@ static inline unsigned int blocks_for(int64_t n, int per_block) { return (unsign
 
 cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
                         const unsigned long long *dense_list, unsigned int *rel, const int *idx_s, Ctrl *ctrl,
-                        int num_sms, cudaStream_t s)
+                        int num_sms, const unsigned int *gate, cudaStream_t s)
 {
     if (N <= 0) return cudaSuccess;
     const unsigned int grid = (unsigned int)min((int64_t)blocks_for(N, kLinkBlock), (int64_t)num_sms * FOF_LINK_MINB);
@@ -680,13 +684,15 @@ cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned 
     const unsigned int tile_batch = (unsigned int)min(max(per_warp / 2, (int64_t)1), (int64_t)kTileBatch);  // items are fewer and longer
     const unsigned int sparse_batch = (unsigned int)min(max(per_warp, (int64_t)1), (int64_t)kSparseBatch);
     link_kernel<<<grid, kLinkBlock, 0, s>>>(sorted, N, g, cell_start, dense_list, rel, idx_s, ctrl, tile_batch,
-                                            sparse_batch);
+                                            sparse_batch, gate);
     return cudaGetLastError();
 }
 
-cudaError_t launch_write_labels(const unsigned int *rel, const int *idx_s, int *labels, int64_t N, cudaStream_t s)
+cudaError_t launch_write_labels(const unsigned int *rel, const int *idx_s, int *labels, int64_t N,
+                                const unsigned int *gate, cudaStream_t s)
 {
-    if (N > 0) write_labels_kernel<<<blocks_for(N, kBlock * 4), kBlock, 0, s>>>(rel, idx_s, labels, N);
+    const bool vec = (((uintptr_t)rel | (uintptr_t)idx_s) & 15) == 0;
+    if (N > 0) write_labels_kernel<<<blocks_for(N, kBlock * 4), kBlock, 0, s>>>(rel, idx_s, labels, N, vec, gate);
     return cudaGetLastError();
 }
 

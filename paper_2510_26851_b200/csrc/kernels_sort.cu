@@ -19,41 +19,7 @@
 
 namespace fof {
 
-// wrapped position (non-finite -> 0 and `bad`) and linear cell id of one particle
-__device__ __forceinline__ unsigned int wrap_cell(float &x, float &y, float &z, const Grid &g, bool &bad)
-{
-    if (!(isfinite(x) && isfinite(y) && isfinite(z))) { bad = true; x = y = z = 0.0f; }
-    x = wrap1(x, g.L);
-    y = wrap1(y, g.L);
-    z = wrap1(z, g.L);
-    return cell_id(cell1(x, g), cell1(y, g), cell1(z, g), g.n);
-}
-
-// Walks the particles [i0, i1) of one CTA four at a time: thread t takes the quads t, t + T, ...
-// With VEC (pos 16-byte aligned, i0 a multiple of 4) a quad is three 128-bit loads, all issued
-// before the first use, so every thread keeps 48 bytes in flight; f(x, y, z, i) is called per particle.
-template <bool VEC, typename F>
-__device__ __forceinline__ void for_each_particle(const float *__restrict__ pos, int64_t i0, int64_t i1, F f)
-{
-    for (int64_t i = i0 + 4 * (int64_t)threadIdx.x; i < i1; i += 4 * (int64_t)kPartThreads) {
-        if (VEC && i + 4 <= i1) {
-            const float4 *q = reinterpret_cast<const float4 *>(pos + 3 * i);
-            const float4 a = __ldg(q), b = __ldg(q + 1), c = __ldg(q + 2);
-            f(a.x, a.y, a.z, i);
-            f(a.w, b.x, b.y, i + 1);
-            f(b.z, b.w, c.x, i + 2);
-            f(c.y, c.z, c.w, i + 3);
-        } else {
-            const int m = (int)min((int64_t)4, i1 - i);
-            float v[12];
-#pragma unroll
-            for (int k = 0; k < 12; ++k) v[k] = (k < 3 * m) ? __ldg(pos + 3 * i + k) : 0.0f;
-#pragma unroll
-            for (int k = 0; k < 4; ++k)
-                if (k < m) f(v[3 * k], v[3 * k + 1], v[3 * k + 2], i + k);
-        }
-    }
-}
+// (wrap_cell and for_each_particle live in fof_internal.cuh: the block path uses them too)
 
 // ---------------------------------------------------------------------------------------------
 // H1 + H2 (level 1): per-CTA histogram of its chunk over the bins.
@@ -61,15 +27,17 @@ __device__ __forceinline__ void for_each_particle(const float *__restrict__ pos,
 template <bool VEC>
 __global__ void __launch_bounds__(kPartThreads) part_hist_kernel(const float *__restrict__ pos, int64_t N, Grid g,
                                                                  int shift, int bins, int64_t chunk,
-                                                                 unsigned int *__restrict__ cta_hist, Ctrl *ctrl)
+                                                                 unsigned int *__restrict__ cta_hist, Ctrl *ctrl,
+                                                                 const unsigned int *gate)
 {
     extern __shared__ unsigned int s_bin[];
+    if (gate && *gate == 0u) return;  // the block path did the work (fof_internal.cuh Ctrl::mode)
     for (int b = threadIdx.x; b < bins; b += kPartThreads) s_bin[b] = 0u;
     __syncthreads();
     const int64_t i0 = (int64_t)blockIdx.x * chunk;
     const int64_t i1 = min(N, i0 + chunk);
     bool any_bad = false;
-    for_each_particle<VEC>(pos, i0, i1, [&](float x, float y, float z, int64_t) {
+    for_each_particle<VEC, kPartThreads>(pos, i0, i1, [&](float x, float y, float z, int64_t) {
         const unsigned int c = wrap_cell(x, y, z, g, any_bad);
         atomicAdd(&s_bin[c >> shift], 1u);
     });
@@ -87,11 +55,13 @@ __global__ void __launch_bounds__(kPartThreads) part_hist_kernel(const float *__
 constexpr int kOffGroups = 8;
 
 __global__ void __launch_bounds__(32 * kOffGroups) part_offsets_kernel(unsigned int *cta_hist, int ctas, int bins,
-                                                                       unsigned int *bin_base, Ctrl *ctrl)
+                                                                       unsigned int *bin_base, Ctrl *ctrl,
+                                                                       const unsigned int *gate)
 {
     __shared__ unsigned int s_part[kOffGroups][33];
     __shared__ unsigned int s_last;
     __shared__ unsigned int s_warp[32 * kOffGroups / 32];
+    if (gate && *gate == 0u) return;  // the block path did the work (fof_internal.cuh Ctrl::mode)
     const int bx = threadIdx.x & 31, gy = threadIdx.x >> 5;
     const int b = blockIdx.x * 32 + bx;
     const int per = (ctas + kOffGroups - 1) / kOffGroups;
@@ -162,16 +132,17 @@ __global__ void __launch_bounds__(kPartThreads) part_scatter_kernel(const float 
                                                                     const unsigned int *__restrict__ cta_hist,
                                                                     const unsigned int *__restrict__ bin_base,
                                                                     float4 *__restrict__ part, int *__restrict__ labels,
-                                                                    bool labels_vec)
+                                                                    bool labels_vec, const unsigned int *gate)
 {
     extern __shared__ unsigned int s_bin[];
+    if (gate && *gate == 0u) return;  // the block path did the work (fof_internal.cuh Ctrl::mode)
     const unsigned int *src = cta_hist + (int64_t)blockIdx.x * bins;
     for (int b = threadIdx.x; b < bins; b += kPartThreads) s_bin[b] = src[b] + bin_base[b];
     __syncthreads();
     const int64_t i0 = (int64_t)blockIdx.x * chunk;
     const int64_t i1 = min(N, i0 + chunk);
     bool bad = false;
-    for_each_particle<VEC>(pos, i0, i1, [&](float x, float y, float z, int64_t i) {
+    for_each_particle<VEC, kPartThreads>(pos, i0, i1, [&](float x, float y, float z, int64_t i) {
         const unsigned int c = wrap_cell(x, y, z, g, bad);
         const unsigned int dst = atomicAdd(&s_bin[c >> shift], 1u);
         part[dst] = make_float4(x, y, z, __int_as_float((int)i));
@@ -203,11 +174,12 @@ __device__ __forceinline__ unsigned int cell_of(const float4 &v, const Grid &g)
 __global__ void __launch_bounds__(kCellSortThreads) cell_sort_kernel(
     const float4 *__restrict__ part, const unsigned int *__restrict__ bin_base, Grid g, int shift, int64_t C,
     unsigned int *__restrict__ cell_start, float4 *sorted, unsigned int *__restrict__ rel,
-    int *__restrict__ idx_s, unsigned long long *__restrict__ dense_list, Ctrl *ctrl)
+    int *__restrict__ idx_s, unsigned long long *__restrict__ dense_list, Ctrl *ctrl, const unsigned int *gate)
 {
     extern __shared__ unsigned int s_cell[];  // [2^shift]
     __shared__ unsigned long long s_warp[kCellSortThreads / 32];
     __shared__ unsigned int s_dbase;
+    if (gate && *gate == 0u) return;  // the block path did the work (fof_internal.cuh Ctrl::mode)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int cpb = 1 << shift;
     const int64_t cell0 = (int64_t)blockIdx.x << shift;
@@ -329,9 +301,11 @@ constexpr int kCoarseShift = FOF_COARSE_SHIFT;
 
 __global__ void __launch_bounds__(kPartThreads) rec_hist_kernel(const float4 *__restrict__ rec, int64_t N, Grid g,
                                                                 int shift, int bins, int64_t chunk,
-                                                                unsigned int *__restrict__ cta_hist)
+                                                                unsigned int *__restrict__ cta_hist,
+                                                                const unsigned int *gate)
 {
     extern __shared__ unsigned int s_bin[];
+    if (gate && *gate == 0u) return;  // the block path did the work (fof_internal.cuh Ctrl::mode)
     for (int b = threadIdx.x; b < bins; b += kPartThreads) s_bin[b] = 0u;
     __syncthreads();
     const int64_t i0 = (int64_t)blockIdx.x * chunk, i1 = min(N, i0 + chunk);
@@ -352,9 +326,10 @@ __global__ void __launch_bounds__(kPartThreads) rec_scatter_kernel(const float4 
                                                                    int shift, int bins, int64_t chunk,
                                                                    const unsigned int *__restrict__ cta_hist,
                                                                    const unsigned int *__restrict__ bin_base,
-                                                                   float4 *__restrict__ out)
+                                                                   float4 *__restrict__ out, const unsigned int *gate)
 {
     extern __shared__ unsigned int s_bin[];
+    if (gate && *gate == 0u) return;  // the block path did the work (fof_internal.cuh Ctrl::mode)
     const unsigned int *src = cta_hist + (int64_t)blockIdx.x * bins;
     for (int b = threadIdx.x; b < bins; b += kPartThreads) s_bin[b] = src[b] + bin_base[b];
     __syncthreads();
@@ -378,7 +353,7 @@ static inline cudaError_t set_smem(const void *fn, size_t bytes)
 cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp, int ctas, unsigned int *cta_hist,
                         unsigned int *bin_base, float4 *part, unsigned int *cell_start, float4 *sorted,
                         unsigned int *rel, int *idx_s, unsigned long long *dense_list, int *labels, Ctrl *ctrl,
-                        StageHook &hook, cudaStream_t s)
+                        const unsigned int *gate, StageHook &hook, cudaStream_t s)
 {
     if (N <= 0) return cudaSuccess;
     const size_t smem_bins = (size_t)sp.bins * sizeof(unsigned int);
@@ -395,14 +370,14 @@ cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp,
     const bool labels_vec = ((uintptr_t)labels & 15) == 0;
     if (sp.bins <= kTwoPassBins) {
         hook.begin(0, 1);
-        hist<<<ctas, kPartThreads, smem_bins, s>>>(pos, N, g, sp.shift, sp.bins, chunk, cta_hist, ctrl);
+        hist<<<ctas, kPartThreads, smem_bins, s>>>(pos, N, g, sp.shift, sp.bins, chunk, cta_hist, ctrl, gate);
         hook.end(0);
         hook.begin(1, 1);
-        part_offsets_kernel<<<(sp.bins + 31) / 32, 32 * kOffGroups, 0, s>>>(cta_hist, ctas, sp.bins, bin_base, ctrl);
+        part_offsets_kernel<<<(sp.bins + 31) / 32, 32 * kOffGroups, 0, s>>>(cta_hist, ctas, sp.bins, bin_base, ctrl, gate);
         hook.end(1);
         hook.begin(2, 1);
         scat<<<ctas, kPartThreads, smem_bins, s>>>(pos, N, g, sp.shift, sp.bins, chunk, cta_hist, bin_base, part, labels,
-                                                   labels_vec);
+                                                   labels_vec, gate);
         hook.end(2);
     } else {
         // pass 1 over bins 2^kCoarseShift times wider: pos -> `sorted` (used as scratch); pass 2: -> `part`
@@ -413,24 +388,24 @@ cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp,
         if ((e = set_smem((const void *)rec_scatter_kernel, smem_bins)) != cudaSuccess) return e;
         const size_t smem_c = (size_t)cbins * sizeof(unsigned int);
         hook.begin(0, 1);
-        hist<<<ctas, kPartThreads, smem_c, s>>>(pos, N, g, cshift, cbins, chunk, cta_hist, ctrl);
+        hist<<<ctas, kPartThreads, smem_c, s>>>(pos, N, g, cshift, cbins, chunk, cta_hist, ctrl, gate);
         hook.end(0);
         hook.begin(1, 2);
-        part_offsets_kernel<<<(cbins + 31) / 32, 32 * kOffGroups, 0, s>>>(cta_hist, ctas, cbins, cbase, ctrl);
+        part_offsets_kernel<<<(cbins + 31) / 32, 32 * kOffGroups, 0, s>>>(cta_hist, ctas, cbins, cbase, ctrl, gate);
         hook.end(1);
         hook.begin(2, 3);
         scat<<<ctas, kPartThreads, smem_c, s>>>(pos, N, g, cshift, cbins, chunk, cta_hist, cbase, sorted, labels,
-                                                labels_vec);
-        rec_hist_kernel<<<ctas, kPartThreads, smem_bins, s>>>(sorted, N, g, sp.shift, sp.bins, chunk, cta_hist);
+                                                labels_vec, gate);
+        rec_hist_kernel<<<ctas, kPartThreads, smem_bins, s>>>(sorted, N, g, sp.shift, sp.bins, chunk, cta_hist, gate);
         if ((e = cudaMemsetAsync(&ctrl->scan_ticket, 0, sizeof(unsigned int), s)) != cudaSuccess) return e;
-        part_offsets_kernel<<<(sp.bins + 31) / 32, 32 * kOffGroups, 0, s>>>(cta_hist, ctas, sp.bins, bin_base, ctrl);
+        part_offsets_kernel<<<(sp.bins + 31) / 32, 32 * kOffGroups, 0, s>>>(cta_hist, ctas, sp.bins, bin_base, ctrl, gate);
         rec_scatter_kernel<<<ctas, kPartThreads, smem_bins, s>>>(sorted, N, g, sp.shift, sp.bins, chunk, cta_hist,
-                                                                 bin_base, part);
+                                                                 bin_base, part, gate);
         hook.end(2);
     }
     hook.begin(3, 1);
     cell_sort_kernel<<<sp.bins, kCellSortThreads, smem_cells, s>>>(part, bin_base, g, sp.shift, C, cell_start, sorted,
-                                                                  rel, idx_s, dense_list, ctrl);
+                                                                  rel, idx_s, dense_list, ctrl, gate);
     hook.end(3);
     return cudaGetLastError();
 }

@@ -26,16 +26,18 @@ def B():
     return binding
 
 
-def gpu_fof(B, pos, L, b, N_min, mass=None, grid=None, particle_group=True):
+def gpu_fof(B, pos, L, b, N_min, mass=None, grid=None, particle_group=True, path="auto"):
     N = len(pos)
-    f = B.FoF(N, L, b, N_min, grid=grid)
+    f = B.FoF(N, L, b, N_min, grid=grid, path=path)
     dpos = torch.from_numpy(np.ascontiguousarray(pos, dtype=np.float32)).cuda().reshape(N, 3)
     dmass = None if mass is None else torch.from_numpy(mass).cuda()
     labels = f.link(dpos)
     status = f.status()
     E, tests, grid_pairs = f.link_stats()
+    ran = f.link_path()
     g = f.groups(dpos, labels, mass=dmass, particle_group=particle_group)
     out = dict(labels=labels.cpu().numpy(), E=E, tests=tests, grid_pairs=grid_pairs, status=status, K=g["K"], grid=f.grid,
+               ran=ran,
                group_label=g["group_label"].cpu().numpy(), group_size=g["group_size"].cpu().numpy(),
                group_mass=g["group_mass"].cpu().numpy(), group_com=g["group_com"].cpu().numpy(),
                particle_group=None if g["particle_group"] is None else g["particle_group"].cpu().numpy())
@@ -43,11 +45,20 @@ def gpu_fof(B, pos, L, b, N_min, mass=None, grid=None, particle_group=True):
     return out
 
 
-def check_against_oracle(B, pos, L, b, N_min, mass=None, grid=None, brute=False):
+def check_against_oracle(B, pos, L, b, N_min, mass=None, grid=None, brute=False, paths=("cells", "blocks")):
+    """Both implementations of H1-H5 (the block path where the plan admits it, and the cell path) against
+    the oracle; returns the results of the last path in `paths` (the default one)."""
     lab, E = (oracle.labels_brute if brute else oracle.labels_cells)(pos, L, b)
     og = oracle.groups(pos, lab, L, N_min, mass=mass)
-    got = gpu_fof(B, pos, L, b, N_min, mass=mass, grid=grid)
+    for path in paths:
+        got = _check_one(B, pos, L, b, N_min, mass, grid, path, lab, E, og)
+    return got, lab, og
+
+
+def _check_one(B, pos, L, b, N_min, mass, grid, path, lab, E, og):
+    got = gpu_fof(B, pos, L, b, N_min, mass=mass, grid=grid, path=path)
     assert got["status"] == 0
+    assert path != "cells" or got["ran"][0] == "cells"
     assert np.array_equal(got["labels"], lab), "canonical labels differ"
     assert got["E"] == E, "edge count differs"
     assert got["K"] == og["K"]
@@ -61,7 +72,7 @@ def check_against_oracle(B, pos, L, b, N_min, mass=None, grid=None, brute=False)
         d = np.abs(got["group_com"].astype(np.float64) - og["group_com"])
         d = np.minimum(d, float(np.float32(L)) - d)
         assert d.max() <= 1e-5 * L, f"centre of mass off by {d.max()}"
-    return got, lab, og
+    return got
 
 
 # --------------------------------------------------------------------------- closed forms, tiny
@@ -489,7 +500,7 @@ def test_stochastic_link_against_oracle(B, alpha, kappa):
     p = inputs.make_positions(w)
     b_link = w.b
     b_cand = float(np.float32(kappa * w.b))
-    f = B.FoF(len(p), w.L, b_cand, w.N_min)
+    f = B.FoF(len(p), w.L, b_cand, w.N_min, path="cells")
     dpos = torch.from_numpy(p).cuda()
     f.link(dpos)                                   # the binning every sample re-uses
     for sample in (0, 1, 7):
@@ -523,7 +534,7 @@ def test_stochastic_batch_equals_single_samples_and_oracle(B, S):
     p = inputs.make_positions(w)
     b_link, alpha = w.b, 4.0
     b_cand = float(np.float32(1.5 * w.b))
-    f = B.FoF(len(p), w.L, b_cand, w.N_min)
+    f = B.FoF(len(p), w.L, b_cand, w.N_min, path="cells")
     f.link(torch.from_numpy(p).cuda())
     labels, logp, grad = f.link_stochastic_batch(b_link, alpha, 99, 3, S)
     E_all, ncand, _ = f.link_stats()
@@ -551,7 +562,7 @@ def test_stochastic_link_wraps_and_needs_a_link_first(B):
     rng = np.random.default_rng(17)
     L, b = 8.0, 1.0
     p = (rng.random((3000, 3)) * L).astype(np.float32)          # n = 5 cells per axis at b_cand = 1.5: every pair wraps
-    f = B.FoF(len(p), L, 1.5, 5)
+    f = B.FoF(len(p), L, 1.5, 5, path="cells")
     with pytest.raises(B.FofError) as e:
         f.link_stochastic(b, 3.0, 1, 0)
     assert e.value.code == B.FOF_ERR_STATE
