@@ -79,16 +79,16 @@ void layout(fof_handle *h)
     h->off_cta_hist = off;    off += align256((size_t)kMaxPartCtas * h->sort.bins * sizeof(unsigned int));
     // fine bin offsets, and behind them the coarse ones of the two-pass partition (<= bins / 64 + 2 entries)
     h->off_bin_base = off;    off += align256(((size_t)h->sort.bins + 2 + (size_t)h->sort.bins / 64 + 4) * sizeof(unsigned int));
-    // `part` and `sorted` are adjacent: the block path's record array (own + ghost copies, part_cap records)
+    // `part` and `sorted` are adjacent: the block path's record array (one slice of kBlockCap records per block)
     // spans both; the cross-block equivalence pairs of the block path live in the idx_s array
-    h->part_cap = (int64_t)(N + N / 4 + 64);
-    if (h->part_cap > (int64_t)(2 * N + 1)) h->part_cap = (int64_t)(2 * N + 1);
     h->off_part = off;        off += align256((N + 1) * sizeof(float4));
     h->off_sorted = off;      off += align256((N + 1) * sizeof(float4));
-    h->off_idx = off;         off += align256((N + 1 + 2 * (N / 4 + 64)) * sizeof(int));
+    if (h->block_ok) {  // the block path's fixed slices: bins x kBlockCap records from off_part on
+        const size_t need = h->off_part + align256((size_t)h->bg.bins * kBlockCap * sizeof(float4));
+        if (need > off) off = need;
+    }
+    h->off_idx = off;         off += align256((2 * N + 2) * sizeof(int));  // also: one int2 per linked ghost record
     h->off_dense = off;       off += align256(dense_items_max(N) * sizeof(unsigned long long));
-    h->off_bin_total = off;   off += align256(((size_t)kMaxBlockBins + 2) * sizeof(unsigned int));
-    h->off_bbase = off;       off += align256(((size_t)kMaxBlockBins + 2) * sizeof(unsigned int));
     h->off_cursor = off;      off += align256(((size_t)kMaxBlockBins + 2) * sizeof(unsigned int));
     h->off_cnt = off;         off += align256((N + 1) * sizeof(int));
     h->off_acc = off;         off += align256(((size_t)h->max_groups + 1) * 4 * sizeof(double));
@@ -122,11 +122,11 @@ int cuda_fail(fof_handle *h, cudaError_t e, const char *where)
     } while (0)
 
 // Profiled stages, in execution order (fof_profile_name).
-enum Stage { kLinkClear = 0, kBlockHist, kBlockOffsets, kBlockPartition, kBlockLink, kBlockCross, kBlockFlatten,
+enum Stage { kLinkClear = 0, kBlockPartition, kBlockLink, kBlockCross, kBlockFlatten,
              kLinkHist, kLinkOffsets, kLinkPartition, kLinkCellSort, kLinkPairs, kLinkLabels,
              kGroupsClear, kGroupsCount, kGroupsCompact, kGroupsReduce, kGroupsFinish, kNumStages };
 const char *const kStageName[kNumStages] = {
-    "link.clear", "block.hist", "block.offsets", "block.partition", "block.link", "block.cross", "block.flatten",
+    "link.clear", "block.partition", "block.link", "block.cross", "block.flatten",
     "link.hist", "link.offsets", "link.partition", "link.cell_sort", "link.pairs", "link.labels",
     "groups.clear", "groups.count", "groups.compact", "groups.reduce", "groups.finish"};
 static_assert(kNumStages <= kMaxStages, "raise kMaxStages");
@@ -349,10 +349,9 @@ int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *s
     // not fit shared memory, and the cell path below, gated on that flag, then does the work.
     const bool blocks = h->block_ok && (h->path == FOF_PATH_BLOCKS || (h->path == FOF_PATH_AUTO && kAutoIsBlocks)) && has;
     if (blocks) {
-        StageHook hook{h, s, kBlockHist};
-        CK(launch_block_path(pos, h->N, h->grid, h->bg, h->part_ctas, at<unsigned int>(ws, h->off_bin_total),
-                             at<unsigned int>(ws, h->off_bbase), at<unsigned int>(ws, h->off_cursor),
-                             at<float4>(ws, h->off_part), h->part_cap, at<int2>(ws, h->off_idx), labels, ctrl, hook, s),
+        StageHook hook{h, s, kBlockPartition};
+        CK(launch_block_path(pos, h->N, h->grid, h->bg, h->part_ctas, at<unsigned int>(ws, h->off_cursor),
+                             at<float4>(ws, h->off_part), at<int2>(ws, h->off_idx), labels, ctrl, hook, s),
            "block path kernels");
     }
     const unsigned int *gate = blocks ? &ctrl->mode : nullptr;

@@ -68,8 +68,14 @@ struct BlockGeom {
     int X, Y, Z;        // local grid: 2^sx + 2, 2^sy + 2, 2^sz + 1
     int ncell;          // X * Y * Z
 };
-constexpr int kBlockCap = 4096;      // most records (own + ghost) of a block that block_link_kernel holds
-constexpr int kBlockThreads = 512;   // threads per CTA of block_link_kernel
+#ifndef FOF_BLOCK_THREADS
+#define FOF_BLOCK_THREADS 512
+#endif
+#ifndef FOF_BLOCK_CAP
+#define FOF_BLOCK_CAP 4096
+#endif
+constexpr int kBlockCap = FOF_BLOCK_CAP;      // most records (own + ghost) of a block that block_link_kernel holds
+constexpr int kBlockThreads = FOF_BLOCK_THREADS;   // threads per CTA of block_link_kernel
 constexpr int kMaxBlockBins = 16384; // most blocks (one shared-memory counter each in the partition)
 constexpr unsigned int kGhostBit = 0x80000000u;  // record.w = original index | kGhostBit for a ghost copy
 
@@ -128,8 +134,7 @@ struct fof_handle {
     fof::BlockGeom bg;      // block path geometry (valid if block_ok)
     bool block_ok;          // the plan admits the block path (>= 3 blocks per axis, <= kMaxBlockBins blocks)
     int path;               // FOF_PATH_AUTO / FOF_PATH_BLOCKS / FOF_PATH_CELLS
-    size_t off_bin_total, off_bbase, off_cursor;  // block path: records per block, exclusive offsets, write cursors
-    int64_t part_cap;       // block path: capacity of the record array (own + ghost)
+    size_t off_cursor;      // block path: records written to every block's slice so far
     size_t off_ctrl, off_cell, off_part, off_cta_hist, off_bin_base, off_sorted, off_cnt, off_acc, off_gscan_state;
     size_t off_rel, off_idx, off_dense;  // union-find (cell-sorted space), original index of each slot, work items
     size_t ws_bytes;
@@ -294,9 +299,8 @@ cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp,
 // block path (kernels_block.cu): histogram + offsets + partition into blocks (with ghost copies), one CTA per
 // block links out of shared memory, equivalence pairs across blocks, flatten.  Sets ctrl->mode = 1 (and does
 // nothing else) if a block does not fit: the gated cell path then runs instead.
-cudaError_t launch_block_path(const float *pos, int64_t N, Grid g, const BlockGeom &bg, int ctas, unsigned int *bin_total,
-                              unsigned int *bin_base, unsigned int *cursor, float4 *part, int64_t part_cap, int2 *cross,
-                              int *labels, Ctrl *ctrl, StageHook &hook, cudaStream_t s);
+cudaError_t launch_block_path(const float *pos, int64_t N, Grid g, const BlockGeom &bg, int ctas, unsigned int *cursor,
+                              float4 *part, int2 *cross, int *labels, Ctrl *ctrl, StageHook &hook, cudaStream_t s);
 cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
                         const unsigned long long *dense_list, unsigned int *rel, const int *idx_s, Ctrl *ctrl,
                         int num_sms, const unsigned int *gate, cudaStream_t s);

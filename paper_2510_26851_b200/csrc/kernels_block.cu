@@ -12,15 +12,17 @@
 // to the block(s) behind that face.  A block then owns every pair (own, own) and (own, ghost): each unordered
 // pair of particles in adjacent cells is tested by exactly one block (the backward one), and nothing that a CTA
 // needs lives outside its contiguous slice of the record array, which TMA brings in with one bulk copy.
-//   block_hist_kernel     records (own + ghost) per block                        pos -> bin_total
-//   block_offsets_kernel  exclusive scan; decides ctrl->mode (1 = a block does not fit: cell path runs)
-//   block_scatter_kernel  records to their blocks through shared cursors          pos -> part, labels[i] = i
+//   block_scatter_kernel  records to their blocks (fixed slices, shared cursors)   pos -> part, labels[i] = i;
+//                         sets ctrl->mode = 1 if a block overflows its slice (the cell path then runs)
 //   block_link_kernel     TMA load, counting sort by local cell in shared memory, half-stencil tests,
 //                         union-find in shared memory rooted at the minimum ORIGINAL index; writes
 //                         labels[own non-root] = original index of its local root, lists one equivalence
 //                         (ghost, local root) per linked ghost
 //   cross_link_kernel     unions of the listed equivalences on `labels` (global lock-free union-find)
 //   flatten_labels_kernel labels[i] = root(i)
+#include <stdio.h>
+#include <stdlib.h>
+
 #include "fof_internal.cuh"
 
 namespace fof {
@@ -28,6 +30,14 @@ namespace fof {
 namespace {
 
 constexpr unsigned int kFull = 0xffffffffu;
+#ifdef FOF_BLOCK_TIMING
+__device__ unsigned long long g_dbg[16];
+#define DBG_T(var) const long long var = clock64()
+#define DBG_ADD(k, a, b) do { if ((threadIdx.x & 31u) == 0) atomicAdd(&g_dbg[k], (unsigned long long)((b) - (a))); } while (0)
+#else
+#define DBG_T(var)
+#define DBG_ADD(k, a, b)
+#endif
 
 // ---- which blocks get a copy of a particle ---------------------------------------------------------------
 // H = forward half of the 26 block offsets: (1,0,0), (*,1,0), (*,*,1).  Block A tests (own of A) x (own of
@@ -78,107 +88,104 @@ __device__ __forceinline__ void wrap3(float &x, float &y, float &z, const Grid &
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// records per block: per-CTA histogram in shared memory, then one global atomic per (CTA, non-empty block)
+// records to their blocks.  Block b owns the fixed slice part[b cap, (b + 1) cap) (no histogram pass, no offsets:
+// the plan sizes the blocks so that a block holds about half of what fits; a block that overflows sets
+// ctrl->mode = 1 and the cell path runs instead).  A CTA takes tiles of TH x PER particles (registers); the rank
+// of a record among the tile's records of its block comes from a shared-memory counter, the tile's slots from
+// ONE global atomic per (tile, block) on the block's cursor, issued by the thread that drew rank 0: all CTAs
+// append to the same few thousand open lines, which the L2 merges before they reach DRAM (measured, 2^24 records
+// into 4096 blocks: private per-CTA streams 0.42 ms, shared cursors 0.25 ms; a scattered 16-byte store costs the
+// same ~12 ps chip-wide whatever the pattern).  Only the counters a tile touched are read and cleared again, so
+// the cost of a tile does not depend on the number of blocks.  The rare ghost copies take one global atomic each.
 // ---------------------------------------------------------------------------------------------------------
+#ifndef FOF_SCAT_THREADS
+#define FOF_SCAT_THREADS 512
+#endif
+#ifndef FOF_SCAT_PER
+#define FOF_SCAT_PER 4
+#endif
+#ifndef FOF_SCAT_MINB
+#define FOF_SCAT_MINB 3
+#endif
+#ifndef FOF_SCAT_CTAS
+#define FOF_SCAT_CTAS 3
+#endif
+constexpr int kScatThreads = FOF_SCAT_THREADS, kScatPer = FOF_SCAT_PER;
+
+#ifdef FOF_SCAT_DIRECT
+// direct variant: one global atomic per record on its block's cursor, no shared memory, no barriers
 template <bool VEC>
-__global__ void __launch_bounds__(kPartThreads) block_hist_kernel(const float *__restrict__ pos, int64_t N, Grid g,
-                                                                  BlockGeom bg, int64_t chunk,
-                                                                  unsigned int *__restrict__ bin_total, Ctrl *ctrl)
+__global__ void __launch_bounds__(256) block_scatter_kernel(const float *__restrict__ pos, int64_t N, Grid g,
+                                                            BlockGeom bg, unsigned int *cursor,
+                                                            float4 *__restrict__ part, unsigned int cap,
+                                                            int *__restrict__ labels, bool labels_vec, Ctrl *ctrl)
 {
-    extern __shared__ unsigned int s_bin[];
-    for (int b = threadIdx.x; b < bg.bins; b += kPartThreads) s_bin[b] = 0u;
-    __syncthreads();
-    const int64_t i0 = (int64_t)blockIdx.x * chunk;
-    const int64_t i1 = min(N, i0 + chunk);
-    bool bad = false;
-    for_each_particle<VEC, kPartThreads>(pos, i0, i1, [&](float x, float y, float z, int64_t) {
-        wrap3(x, y, z, g, bad);
-        const unsigned int own = classify(x, y, z, g, bg, [&](unsigned int gb) { atomicAdd(&s_bin[gb], 1u); });
-        atomicAdd(&s_bin[own], 1u);
-    });
+    bool bad = false, over = false;
+    for (int64_t i = ((int64_t)blockIdx.x * 256 + threadIdx.x) * 4; i < N; i += (int64_t)gridDim.x * 256 * 4) {
+        float4 rec[4];
+        if (VEC && i + 4 <= N) {
+            const float4 *p = reinterpret_cast<const float4 *>(pos + 3 * i);
+            const float4 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
+            rec[0] = make_float4(a.x, a.y, a.z, __int_as_float((int)i));
+            rec[1] = make_float4(a.w, b.x, b.y, __int_as_float((int)i + 1));
+            rec[2] = make_float4(b.z, b.w, c.x, __int_as_float((int)i + 2));
+            rec[3] = make_float4(c.y, c.z, c.w, __int_as_float((int)i + 3));
+        } else {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int64_t j = i + k;
+                rec[k] = j < N ? make_float4(__ldg(pos + 3 * j), __ldg(pos + 3 * j + 1), __ldg(pos + 3 * j + 2), __int_as_float((int)j))
+                               : make_float4(0.f, 0.f, 0.f, __int_as_float(-1));
+            }
+        }
+        if (labels_vec && i + 4 <= N) *reinterpret_cast<int4 *>(labels + i) = make_int4((int)i, (int)i + 1, (int)i + 2, (int)i + 3);
+        else
+            for (int k = 0; k < 4; ++k) if (i + k < N) labels[i + k] = (int)(i + k);
+        unsigned int bin[4], at[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            bin[k] = 0xffffffffu;
+            if (__float_as_int(rec[k].w) >= 0) {
+                wrap3(rec[k].x, rec[k].y, rec[k].z, g, bad);
+                const float4 r = rec[k];
+                bin[k] = classify(r.x, r.y, r.z, g, bg, [&](unsigned int gb) {
+                    const unsigned int a2 = atomicAdd(&cursor[gb], 1u);
+                    if (a2 < cap) part[(size_t)gb * cap + a2] = make_float4(r.x, r.y, r.z, __uint_as_float(__float_as_uint(r.w) | kGhostBit));
+                    else over = true;
+                });
+                at[k] = atomicAdd(&cursor[bin[k]], 1u);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            if (bin[k] != 0xffffffffu) {
+                if (at[k] < cap) part[(size_t)bin[k] * cap + at[k]] = rec[k];
+                else over = true;
+            }
+    }
     if (bad) atomicOr(&ctrl->error, 1u);
-    __syncthreads();
-    for (int b = threadIdx.x; b < bg.bins; b += kPartThreads) {
-        const unsigned int c = s_bin[b];
-        if (c) atomicAdd(&bin_total[b], c);
-    }
+    if (over) ctrl->mode = 1u;
 }
-
-// ---------------------------------------------------------------------------------------------------------
-// one CTA: exclusive scan of the block totals -> bin_base (and the write cursors), fullest block, mode
-// ---------------------------------------------------------------------------------------------------------
-constexpr int kOffThreads = 1024;
-__global__ void __launch_bounds__(kOffThreads) block_offsets_kernel(const unsigned int *__restrict__ bin_total, int bins,
-                                                                    unsigned int *__restrict__ bin_base,
-                                                                    unsigned int *__restrict__ cursor, unsigned int cap,
-                                                                    unsigned long long part_cap, Ctrl *ctrl)
-{
-    __shared__ unsigned int s_warp[kOffThreads / 32];
-    __shared__ unsigned int s_max[kOffThreads / 32];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int per = (bins + kOffThreads - 1) / kOffThreads;
-    const int b0 = tid * per, b1 = min(bins, b0 + per);
-    unsigned int sum = 0, mx = 0;
-    for (int b = b0; b < b1; ++b) { const unsigned int c = bin_total[b]; sum += c; mx = max(mx, c); }
-    unsigned int incl = sum;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const unsigned int t = __shfl_up_sync(kFull, incl, o);
-        if (lane >= o) incl += t;
-    }
-    mx = __reduce_max_sync(kFull, mx);
-    if (lane == 31) s_warp[warp] = incl;
-    if (lane == 0) s_max[warp] = mx;
-    __syncthreads();
-    unsigned int woff = 0, total = 0, gmax = 0;
-#pragma unroll
-    for (int w = 0; w < kOffThreads / 32; ++w) {
-        const unsigned int t = s_warp[w];
-        if (w < warp) woff += t;
-        total += t;
-        gmax = max(gmax, s_max[w]);
-    }
-    unsigned int run = woff + incl - sum;
-    for (int b = b0; b < b1; ++b) {
-        bin_base[b] = run;
-        cursor[b] = run;
-        run += bin_total[b];
-    }
-    if (tid == 0) {
-        bin_base[bins] = total;
-        ctrl->max_block = gmax;
-        ctrl->mode = (gmax > cap || (unsigned long long)total > part_cap) ? 1u : 0u;
-    }
-}
-
-// ---------------------------------------------------------------------------------------------------------
-// records to their blocks.  A CTA takes tiles of TH x PER particles (registers); the rank of a record among
-// the tile's records of its block comes from a shared-memory counter, the tile's slice of the block from ONE
-// global atomic per (tile, non-empty block) on the block's cursor: all CTAs append to the same few thousand
-// open lines, which the L2 merges before they reach DRAM (private per-CTA streams: 0.42 ms, shared: 0.25 ms for
-// 2^24 records into 4096 blocks).  The rare ghost copies take one global atomic each.
-// ---------------------------------------------------------------------------------------------------------
-constexpr int kScatThreads = 512, kScatPer = 8;
-
+#else
 template <bool VEC>
-__global__ void __launch_bounds__(kScatThreads) block_scatter_kernel(const float *__restrict__ pos, int64_t N, Grid g,
+__global__ void __launch_bounds__(kScatThreads, FOF_SCAT_MINB) block_scatter_kernel(const float *__restrict__ pos, int64_t N, Grid g,
                                                                      BlockGeom bg, unsigned int *cursor,
-                                                                     float4 *__restrict__ part, int *__restrict__ labels,
-                                                                     bool labels_vec, Ctrl *ctrl)
+                                                                     float4 *__restrict__ part, unsigned int cap,
+                                                                     int *__restrict__ labels, bool labels_vec, Ctrl *ctrl)
 {
-    extern __shared__ unsigned int s_cnt[];  // [bins]
+    extern __shared__ unsigned int s_cnt[];  // [bins]: records of the current tile per block, then the tile's first slot
     __shared__ unsigned int s_tile;
-    if (*(volatile unsigned int *)&ctrl->mode) return;
     constexpr int T = kScatThreads * kScatPer;
     const int64_t ntiles = (N + T - 1) / T;
     const int tid = threadIdx.x;
+    for (int b = tid; b < bg.bins; b += kScatThreads) s_cnt[b] = 0u;
+    bool bad = false, over = false;
     for (;;) {
         __syncthreads();
         if (tid == 0) s_tile = atomicAdd(&ctrl->tile_ticket2, 1u);
-        for (int b = tid; b < bg.bins; b += kScatThreads) s_cnt[b] = 0u;
         __syncthreads();
         const int64_t tile = s_tile;
-        if (tile >= ntiles) return;
+        if (tile >= ntiles) break;
         const int64_t base = tile * T;
         float4 rec[kScatPer];
         unsigned int bin[kScatPer], rank[kScatPer];
@@ -206,7 +213,6 @@ __global__ void __launch_bounds__(kScatThreads) block_scatter_kernel(const float
             else
                 for (int k = 0; k < 4; ++k) if (i + k < N) labels[i + k] = (int)(i + k);
         }
-        bool bad = false;
 #pragma unroll
         for (int k = 0; k < kScatPer; ++k) {
             bin[k] = 0xffffffffu;
@@ -214,23 +220,39 @@ __global__ void __launch_bounds__(kScatThreads) block_scatter_kernel(const float
                 wrap3(rec[k].x, rec[k].y, rec[k].z, g, bad);
                 const float4 r = rec[k];
                 bin[k] = classify(r.x, r.y, r.z, g, bg, [&](unsigned int gb) {
-                    part[atomicAdd(&cursor[gb], 1u)] =
-                        make_float4(r.x, r.y, r.z, __uint_as_float(__float_as_uint(r.w) | kGhostBit));
+                    const unsigned int at = atomicAdd(&cursor[gb], 1u);
+                    if (at < cap) part[(size_t)gb * cap + at] = make_float4(r.x, r.y, r.z, __uint_as_float(__float_as_uint(r.w) | kGhostBit));
+                    else over = true;
                 });
                 rank[k] = atomicAdd(&s_cnt[bin[k]], 1u);
             }
         }
         __syncthreads();
-        for (int b = tid; b < bg.bins; b += kScatThreads) {
-            const unsigned int c = s_cnt[b];
-            if (c) s_cnt[b] = atomicAdd(&cursor[b], c);
-        }
+#pragma unroll
+        for (int k = 0; k < kScatPer; ++k)
+            if (bin[k] != 0xffffffffu && rank[k] == 0u) {  // I drew the first rank: I fetch the tile's slots of this block
+                const unsigned int c = s_cnt[bin[k]];
+                const unsigned int at = atomicAdd(&cursor[bin[k]], c);
+                if (at + c > cap) over = true;
+                s_cnt[bin[k]] = at;
+            }
         __syncthreads();
 #pragma unroll
         for (int k = 0; k < kScatPer; ++k)
-            if (bin[k] != 0xffffffffu) part[s_cnt[bin[k]] + rank[k]] = rec[k];
+            if (bin[k] != 0xffffffffu) {
+                const unsigned int at = s_cnt[bin[k]] + rank[k];
+                if (at < cap) part[(size_t)bin[k] * cap + at] = rec[k];
+            }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < kScatPer; ++k)
+            if (bin[k] != 0xffffffffu && rank[k] == 0u) s_cnt[bin[k]] = 0u;
     }
+    if (bad) atomicOr(&ctrl->error, 1u);
+    if (over) ctrl->mode = 1u;
 }
+
+#endif
 
 // ---------------------------------------------------------------------------------------------------------
 // block_link_kernel
@@ -331,99 +353,287 @@ __device__ __forceinline__ void local_cell(const float4 &r, const Grid &g, const
 }
 
 constexpr int kRecPerThread = kBlockCap / kBlockThreads;
+constexpr int kDenseB = 8;                    // an OWN cell with >= kDenseB records is DENSE: its same-cell pairs go to the tile role
+constexpr int kMaxItems = (kBlockCap / kDenseB + 3) & ~3;  // (dense cell, tile) work items of one block
+constexpr int kWarps = kBlockThreads / 32;
+#ifndef FOF_QUEUE
+#define FOF_QUEUE 256
+#endif
+constexpr int kQueue = FOF_QUEUE;                   // pairs a warp lists before it tests them
+#ifndef FOF_LONGRUN
+#define FOF_LONGRUN (1 << 30)  // off: measured slower (1.9 vs 1.2 ms at 256^3) than letting every lane list its own runs
+#endif
+constexpr int kLongRun = FOF_LONGRUN;                   // longer candidate runs are walked by the whole warp instead
 
-// Every pair (own, own) in the same or in adjacent cells is tested by the particle whose cell sees the other
-// one in its forward half stencil (+x, then the rows (dy, dz) = (+1, 0), (-1, +1), (0, +1), (+1, +1)); a row is
-// one contiguous run of slots (x-fastest local cell ids), trimmed to the cells the home particle can reach.
-// A pair (own, ghost) belongs to this block whatever its direction, so a ghost is a home particle too, but
-// only against OWN candidates (ghost-ghost pairs belong to other blocks).
+struct BlockView {
+    float4 *rec;          // [kBlockCap] records in local-cell order (x fastest)
+    unsigned int *par;    // [kBlockCap] union-find parent (slot index)
+    unsigned int *cbeg;   // [ncell + 1] first slot of every local cell
+    unsigned int *items;  // [kMaxItems] cell | tile << 16
+    unsigned int *queue;  // [kQueue] per warp: home slot << 16 | candidate slot
+    int M;
+};
+__device__ __forceinline__ unsigned int lanemask_lt()
+{
+    unsigned int m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+
+// ---- who tests which pair (every unordered pair in the same or in adjacent cells with at least one OWN end, once)
+//   same cell, dense       the tile role: tiles of <= 32 records in registers, candidates broadcast, ballots;
+//   everything else        the chunk role: the end whose cell sees the other one in its forward half stencil (+x; rows
+//                          (dy, dz) = (+1, 0), (-1, +1), (0, +1), (+1, +1)) is the HOME of the pair and lists it.
+// A pair (own, ghost) belongs to this block whatever its direction (no half space of cell offsets is consistent
+// with the half space of block offsets), so a ghost is a home too, but lists OWN candidates only.
+
+// =========================================================================================================
+// chunk role: 32 consecutive slots, one home per lane.  Each home lists its candidate pairs into the warp's
+// queue (runs of consecutive slots: a grid row of cells is contiguous), then all 32 lanes test listed pairs:
+// a lane with forty candidates costs the others nothing.
+// =========================================================================================================
 template <bool WRAP>
-__device__ __forceinline__ void link_phase(const float4 *rec, const unsigned int *cbeg, unsigned int *par, int M,
-                                           const Grid &g, const BlockGeom &bg, const BlockOrigin &o,
-                                           unsigned int &nedges, unsigned int &ntests)
+__device__ __forceinline__ void chunk_role(const BlockView &v, int s0, const Grid &g, const BlockGeom &bg,
+                                           const BlockOrigin &o, int lane, unsigned int &nedges, unsigned int &ntests)
 {
     const float lo = g.reach, hi = 1.0f - g.reach;
     const int X = bg.X, XY = bg.X * bg.Y;
+    const float4 *rec = v.rec;
+    const unsigned int *cbeg = v.cbeg;
+    const int s = s0 + lane;
+    int b0 = 0, b1 = 0, b2 = 0, b3 = 0, b4 = 0, l0 = 0, l1 = 0, l2 = 0, l3 = 0, l4 = 0;  // run r = [b_r, b_r + l_r)
+    float4 me = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (s < v.M) {
+        me = rec[s];
+        int lx, ly, lz;
+        float fx, fy, fz;
+        local_cell(me, g, bg, o, lx, ly, lz, fx, fy, fz);
+        const int lc = lx + X * (ly + bg.Y * lz);
+        const bool xl = fx < lo, xh = fx > hi, yl = fy < lo, yh = fy > hi, zh = fz > hi;
+        // an own home meets every cell of the local grid; a ghost home meets OWN cells only (ghost-ghost pairs belong
+        // to other blocks): rows ly' in [1, ncy], lz' < ncz, cells lx' in [1, ncx]
+        const bool ghost = (__float_as_uint(me.w) & kGhostBit) != 0u;
+        const int xmin = ghost ? 1 : 0, xmax = ghost ? o.ncx : X - 1;
+        const int xa = max(lx - (xl ? 1 : 0), xmin), xb = min(lx + (xh ? 1 : 0), xmax);  // cells of a neighbour row
+        auto row = [&](int dy, int dz, int &bb, int &ll) {
+            const int yy = ly + dy, zz = lz + dz;
+            if (xa > xb || (ghost && (yy < 1 || yy > o.ncy || zz >= o.ncz))) return;
+            const int base = X * (yy + bg.Y * zz);
+            bb = (int)cbeg[base + xa];
+            ll = (int)cbeg[base + xb + 1] - bb;
+        };
+        const int c1 = (int)cbeg[lc + 1];
+        if (!ghost) {
+            // my cell after me (the tile role has the same-cell pairs of a dense cell) [+ the +x cell]
+            b0 = c1 - (int)cbeg[lc] >= kDenseB ? c1 : s + 1;
+            l0 = (xh ? (int)cbeg[lc + 2] : c1) - b0;
+        } else if (xh && lx + 1 <= xmax && ly >= 1 && ly <= o.ncy && lz < o.ncz) {
+            b0 = c1;
+            l0 = (int)cbeg[lc + 2] - c1;
+        }
+        if (yh) row(1, 0, b1, l1);
+        if (zh) {
+            if (yl) row(-1, 1, b2, l2);
+            row(0, 1, b3, l3);
+            if (yh) row(1, 1, b4, l4);
+        }
+    }
+    unsigned int *queue = v.queue;
+    int nq = 0;  // pairs waiting in the queue (warp-uniform)
+    auto drain = [&]() {
+        __syncwarp();
+        for (int q = lane; q < nq; q += 32) {  // the trip count differs by at most one between lanes
+            const unsigned int e = queue[q];
+            const int i = (int)(e >> 16), j = (int)(e & 0xffffu);
+            if (linked_b<WRAP>(rec[i], rec[j], g)) {
+                ++nedges;
+                if (((volatile unsigned int *)v.par)[i] != ((volatile unsigned int *)v.par)[j]) unite_s(v.par, rec, i, j);
+            }
+        }
+        __syncwarp();
+        nq = 0;
+    };
+    // ---- long runs (a dense neighbour cell): listed by the whole warp, 32 pairs per pass
+    if (__any_sync(kFull, max(max(max(l0, l1), max(l2, l3)), l4) >= kLongRun)) {
+        auto long_runs = [&](int b, int &l) {
+            unsigned int lng = __ballot_sync(kFull, l >= kLongRun);
+            while (lng) {
+                const int h = __ffs((int)lng) - 1;
+                lng &= lng - 1u;
+                const int bb = __shfl_sync(kFull, b, h), ll = __shfl_sync(kFull, l, h);
+                const unsigned int hs = (unsigned int)(s0 + h) << 16;
+                if (lane == 0) ntests += (unsigned int)ll;
+                for (int off = 0; off < ll; off += 32) {
+                    const int cnt = min(32, ll - off);
+                    if (nq + cnt > kQueue) drain();
+                    if (lane < cnt) queue[nq + lane] = hs | (unsigned int)(bb + off + lane);
+                    nq += cnt;
+                }
+            }
+            if (l >= kLongRun) l = 0;
+        };
+        long_runs(b0, l0); long_runs(b1, l1); long_runs(b2, l2); long_runs(b3, l3); long_runs(b4, l4);
+    }
+    // ---- short runs: each lane lists its own pairs behind what is already queued
+    const int T = l0 + l1 + l2 + l3 + l4;
+    int incl = T;
+#pragma unroll
+    for (int q = 1; q < 32; q <<= 1) {
+        const int w = __shfl_up_sync(kFull, incl, q);
+        if (lane >= q) incl += w;
+    }
+    const int total = __shfl_sync(kFull, incl, 31);
+    if (total) {
+        if (lane == 31) ntests += (unsigned int)total;
+        const unsigned int hs = (unsigned int)s << 16;
+        for (int w0 = 0; w0 < total;) {
+            if (nq + min(total - w0, 32) > kQueue) drain();
+            const int room = kQueue - nq;   // list the pairs at positions [w0, w0 + room) of the short list
+            int base = incl - T - w0;       // position of my first pair relative to the window
+            auto push = [&](int b, int l) {
+                const int k0 = max(0, -base), k1 = min(l, room - base);
+                for (int k = k0; k < k1; ++k) queue[nq + base + k] = hs | (unsigned int)(b + k);
+                base += l;
+            };
+            push(b0, l0); push(b1, l1); push(b2, l2); push(b3, l3); push(b4, l4);
+            const int n = min(room, total - w0);
+            nq += n;
+            w0 += n;
+        }
+    }
+    if (nq) drain();
+}
+
+// =========================================================================================================
+// tile role: the pairs inside one dense cell
+// =========================================================================================================
+// Returns, in lane k, the mask of tile lanes linked to the record at slot jb + k (k < cnt <= 32).
+__device__ __forceinline__ unsigned int batch_adjacency_b(const float4 &me, const float4 *rec, int jb, int cnt,
+                                                          const Grid &g, int lane)
+{
+    unsigned int adjT = 0;
+#pragma unroll 4
+    for (int k = 0; k < cnt; ++k) {
+        const unsigned int bal = __ballot_sync(kFull, linked_b<false>(me, rec[jb + k], g));  // pairs inside one cell never wrap
+        if (lane == k) adjT = bal;
+    }
+    return adjT;
+}
+
+__device__ __forceinline__ void tile_role(const BlockView &v, unsigned int item, const Grid &g, int lane,
+                                          unsigned int &nedges, unsigned int &ntests)
+{
+    const float inf = __int_as_float(0x7f800000);
+    const float4 *rec = v.rec;
+    const int c = (int)(item & 0xffffu), t = (int)(item >> 16);
+    const int d0 = (int)v.cbeg[c];
+    const int m = (int)v.cbeg[c + 1] - d0;
+    const int nt = (m + 31) >> 5, ts = (m + nt - 1) / nt;  // balanced tiles: 43 -> 22 + 21
+    const int ib = d0 + t * ts;
+    const int cntI = min(ts, m - t * ts);
+    float4 me = make_float4(inf, inf, inf, 0.0f);  // a lane without a record sits at +inf: every test fails
+    if (lane < cntI) me = rec[ib + lane];
+    const unsigned int self = 1u << lane;
+    // ---- the tile against itself
+    const unsigned int adj = batch_adjacency_b(me, rec, ib, cntI, g, lane) & ~self;
+    nedges += (unsigned int)__popc(adj & lanemask_lt());
+    if (lane == 0) ntests += (unsigned int)(cntI * (cntI - 1) / 2);
+    // components of the tile: breadth-first from the lowest unlabelled lane, one warp OR-reduction per level;
+    // head = member with the smallest original index, every other member hooks straight under it
+    unsigned int grp = self;
+    int head = lane;
+    if (__any_sync(kFull, adj != 0u)) {
+        const unsigned int my_oi = lane < cntI ? (__float_as_uint(me.w) & ~kGhostBit) : 0xffffffffu;
+        unsigned int todo = __ballot_sync(kFull, adj != 0u);
+        while (todo) {
+            const int r = __ffs((int)todo) - 1;
+            unsigned int vis = 1u << r;
+            while (true) {
+                const unsigned int nxt = vis | __reduce_or_sync(kFull, (vis & self) ? adj : 0u);
+                if (nxt == vis) break;
+                vis = nxt;
+            }
+            const bool in = (vis & self) != 0u;
+            const unsigned int mn = __reduce_min_sync(kFull, in ? my_oi : 0xffffffffu);
+            const unsigned int hb = __ballot_sync(kFull, in && my_oi == mn);
+            if (in) { grp = vis; head = __ffs((int)hb) - 1; }
+            todo &= ~vis;
+        }
+    }
+    if (head != lane && atomicCAS(v.par + ib + lane, (unsigned int)(ib + lane), (unsigned int)(ib + head)) != (unsigned int)(ib + lane))
+        unite_s(v.par, rec, ib + lane, ib + head);  // somebody hooked me first: general path
+    __syncwarp();
+    const bool leader = head == lane;
+    // ---- the earlier tiles of my cell: candidate k (lane k's slot) joins every component of the tile it is linked to
+    for (int jb = d0; jb < ib; jb += 32) {
+        const int cnt = min(32, ib - jb);
+        const unsigned int adjT = batch_adjacency_b(me, rec, jb, cnt, g, lane);
+        nedges += (unsigned int)__popc(adjT);
+        if (lane == 0) ntests += (unsigned int)(cnt * cntI);
+        const unsigned int active = __reduce_or_sync(kFull, adjT);
+        if (active) {
+            unsigned int lead = __ballot_sync(kFull, leader && (grp & active));
+            while (lead) {
+                const int gl = __ffs((int)lead) - 1;
+                lead &= lead - 1u;
+                const unsigned int members = __shfl_sync(kFull, grp, gl);
+                if (adjT & members) unite_s(v.par, rec, jb + lane, ib + gl);
+            }
+        }
+        __syncwarp();
+    }
+}
+
+template <bool WRAP>
+__device__ __forceinline__ void link_phase(const BlockView &v, unsigned int nitems, unsigned int *ticket, const Grid &g,
+                                           const BlockGeom &bg, const BlockOrigin &o, unsigned int &nedges,
+                                           unsigned int &ntests)
+{
     const int lane = (int)(threadIdx.x & 31u);
-    // One home particle per lane; its (up to five) candidate runs are walked as ONE list, all lanes of the warp
-    // in lock step (warp-uniform trip count, __syncwarp() per trip: left to themselves the lanes drift apart
-    // through the unions and never reconverge -- measured 3 of 32 lanes active).
-    for (int s0 = (int)(threadIdx.x & ~31u); s0 < M; s0 += kBlockThreads) {
-        const int s = s0 + lane;
-        int b0 = 0, b1 = 0, b2 = 0, b3 = 0, b4 = 0, e0 = 0, e1 = 0, e2 = 0, e3 = 0, e4 = 0;  // run r = [b_r, b_r + len_r); e_r = prefix ends
-        float4 me = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (s < M) {
-            me = rec[s];
-            int lx, ly, lz;
-            float fx, fy, fz;
-            local_cell(me, g, bg, o, lx, ly, lz, fx, fy, fz);
-            const int lc = lx + X * (ly + bg.Y * lz);
-            const bool xl = fx < lo, xh = fx > hi, yl = fy < lo, yh = fy > hi, zh = fz > hi;
-            const int ol = xl ? 1 : 0, oh = xh ? 1 : 0;
-            if (!(__float_as_uint(me.w) & kGhostBit)) {
-                b0 = s + 1; e0 = (int)cbeg[lc + 1 + oh] - b0;  // my cell after me [+ the +x cell]
-                if (yh) { b1 = (int)cbeg[lc + X - ol]; e1 = (int)cbeg[lc + X + 1 + oh] - b1; }
-                if (zh) {
-                    const int up = lc + XY;
-                    if (yl) { b2 = (int)cbeg[up - X - ol]; e2 = (int)cbeg[up - X + 1 + oh] - b2; }
-                    b3 = (int)cbeg[up - ol]; e3 = (int)cbeg[up + 1 + oh] - b3;
-                    if (yh) { b4 = (int)cbeg[up + X - ol]; e4 = (int)cbeg[up + X + 1 + oh] - b4; }
-                }
-            } else {
-                // a ghost meets OWN cells only: row (ly + dy, lz + dz), cells lx + xa .. lx + xb clipped to [1, ncx]
-                auto row = [&](int dy, int dz, int xa, int xb, int &bb, int &ll) {
-                    const int yy = ly + dy, zz = lz + dz;
-                    if (yy < 1 || yy > o.ncy || zz >= o.ncz) return;
-                    const int a = max(lx + xa, 1), b = min(lx + xb, o.ncx);
-                    if (a > b) return;
-                    const int base = X * (yy + bg.Y * zz);
-                    bb = (int)cbeg[base + a];
-                    ll = (int)cbeg[base + b + 1] - bb;
-                };
-                if (xh) row(0, 0, 1, 1, b0, e0);
-                if (yh) row(1, 0, -ol, oh, b1, e1);
-                if (zh) {
-                    if (yl) row(-1, 1, -ol, oh, b2, e2);
-                    row(0, 1, -ol, oh, b3, e3);
-                    if (yh) row(1, 1, -ol, oh, b4, e4);
-                }
-            }
-        }
-        // prefix ends; run r covers list positions [e_{r-1}, e_r)
-        e1 += e0; e2 += e1; e3 += e2; e4 += e3;
-        ntests += (unsigned int)e4;
-        const int trips = __reduce_max_sync(kFull, e4);
-        int ri = s;  // a slot known to be in my set (skips the union when the partner already points at it)
-        for (int k = 0; k < trips; ++k) {
-            if (k < e4) {
-                const int j = k < e0 ? b0 + k : (k < e1 ? b1 + (k - e0) : (k < e2 ? b2 + (k - e1) : (k < e3 ? b3 + (k - e2) : b4 + (k - e3))));
-                if (linked_b<WRAP>(me, rec[j], g)) {
-                    ++nedges;
-                    if ((int)((volatile unsigned int *)par)[j] != ri) ri = unite_s(par, rec, s, j);
-                }
-            }
-            __syncwarp();
-        }
+    const unsigned int nchunks = (unsigned int)((v.M + 31) >> 5);
+    while (true) {  // warps draw tiles first (the long items), then chunks
+        unsigned int it = 0;
+        if (lane == 0) it = atomicAdd(ticket, 1u);
+        it = __shfl_sync(kFull, it, 0);
+        DBG_T(t0);
+#ifdef FOF_ABL_NOTILE
+        if (it < nitems) { }
+#else
+        if (it < nitems) { tile_role(v, v.items[it], g, lane, nedges, ntests); DBG_T(t1); DBG_ADD(4, t0, t1); DBG_ADD(8, 0, 1); }
+#endif
+#ifdef FOF_ABL_NOCHUNK
+        else if (it - nitems < nchunks) { }
+#else
+        else if (it - nitems < nchunks) { chunk_role<WRAP>(v, (int)(it - nitems) * 32, g, bg, o, lane, nedges, ntests); DBG_T(t1); DBG_ADD(5, t0, t1); DBG_ADD(9, 0, 1); }
+#endif
+        else break;
     }
 }
 
 __global__ void __launch_bounds__(kBlockThreads, 2) block_link_kernel(const float4 *__restrict__ part,
-                                                                      const unsigned int *__restrict__ bin_base, Grid g,
-                                                                      BlockGeom bg, int *labels, int2 *__restrict__ cross,
-                                                                      Ctrl *ctrl)
+                                                                      const unsigned int *__restrict__ cursor,
+                                                                      unsigned int cap, Grid g, BlockGeom bg, int *labels,
+                                                                      int2 *__restrict__ cross, Ctrl *ctrl)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float4 *rec = reinterpret_cast<float4 *>(smem_raw);                                  // [kBlockCap]
-    unsigned int *par = reinterpret_cast<unsigned int *>(smem_raw + (size_t)kBlockCap * 16);  // [kBlockCap]
-    unsigned int *cbeg = par + kBlockCap;                                                // [ncell + 1]
+    BlockView v;
+    v.rec = reinterpret_cast<float4 *>(smem_raw);
+    v.par = reinterpret_cast<unsigned int *>(smem_raw + (size_t)kBlockCap * 16);
+    v.items = v.par + kBlockCap;
+    v.queue = v.items + kMaxItems + kQueue * (threadIdx.x >> 5);
+    v.cbeg = v.items + kMaxItems + kQueue * kWarps;  // [ncell + 1]
     __shared__ unsigned long long s_bar;
-    __shared__ unsigned int s_warp[kBlockThreads / 32];
-    __shared__ unsigned int s_red[2];
+    __shared__ unsigned int s_warp[kWarps];
+    __shared__ unsigned int s_red[2], s_nitems, s_ticket;
     if (*(volatile unsigned int *)&ctrl->mode) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const unsigned int p0 = bin_base[blockIdx.x];
-    const int M = (int)(bin_base[blockIdx.x + 1] - p0);
+    const size_t p0 = (size_t)blockIdx.x * cap;
+    const int M = (int)cursor[blockIdx.x];  // <= cap: an overflowing block has set ctrl->mode
     if (M == 0) return;
+    float4 *rec = v.rec;
+    unsigned int *cbeg = v.cbeg;
+    v.M = M;
+    DBG_T(tA);
 
     // ---- A: one TMA bulk copy brings the block's records in; meanwhile the cell counters are cleared
     if (tid == 0) {
@@ -431,6 +641,9 @@ __global__ void __launch_bounds__(kBlockThreads, 2) block_link_kernel(const floa
         mbar_expect_tx(&s_bar, (unsigned int)M * 16u);
         tma_load_1d(rec, part + p0, (unsigned int)M * 16u, &s_bar);
         s_red[0] = s_red[1] = 0u;
+        s_nitems = 0u;
+        s_ticket = 0u;
+        if ((unsigned int)M > *(volatile unsigned int *)&ctrl->max_block) atomicMax(&ctrl->max_block, (unsigned int)M);
     }
     const int ncell = bg.ncell;
     for (int c = tid; c <= ncell; c += kBlockThreads) cbeg[c] = 0u;
@@ -446,6 +659,8 @@ __global__ void __launch_bounds__(kBlockThreads, 2) block_link_kernel(const floa
                       o.z0 + (1 << bg.sz) >= g.n;
     __syncthreads();
     mbar_wait(&s_bar, 0);
+    DBG_T(tB);
+    DBG_ADD(0, tA, tB);
 
     // ---- B: counting sort by local cell, in place (records pass through registers)
     float4 r[kRecPerThread];
@@ -478,10 +693,22 @@ __global__ void __launch_bounds__(kBlockThreads, 2) block_link_kernel(const floa
         __syncthreads();
         unsigned int woff = 0;
 #pragma unroll
-        for (int w = 0; w < kBlockThreads / 32; ++w)
+        for (int w = 0; w < kWarps; ++w)
             if (w < warp) woff += s_warp[w];
         unsigned int run = woff + incl - sum;
-        for (int c = c0; c < c1; ++c) { const unsigned int t = cbeg[c]; cbeg[c] = run; run += t; }
+        for (int c = c0; c < c1; ++c) {
+            const unsigned int n = cbeg[c];
+            cbeg[c] = run;
+            run += n;
+            if (n >= (unsigned int)kDenseB) {  // a dense OWN cell: one work item per tile of <= 32 records
+                const int lx = c % bg.X, ly = (c / bg.X) % bg.Y, lz = c / (bg.X * bg.Y);
+                if (lx >= 1 && lx <= o.ncx && ly >= 1 && ly <= o.ncy && lz < o.ncz) {
+                    const unsigned int nt = (n + 31u) >> 5;
+                    const unsigned int at = atomicAdd(&s_nitems, nt);
+                    for (unsigned int t = 0; t < nt; ++t) v.items[at + t] = (unsigned int)c | (t << 16);
+                }
+            }
+        }
         if (tid == 0) cbeg[ncell] = (unsigned int)M;
     }
     __syncthreads();
@@ -491,16 +718,22 @@ __global__ void __launch_bounds__(kBlockThreads, 2) block_link_kernel(const floa
         if (s < M) {
             const int slot = (int)(cbeg[key[k] >> 16] + (key[k] & 0xffffu));
             rec[slot] = r[k];
-            par[slot] = (unsigned int)slot;
+            v.par[slot] = (unsigned int)slot;
         }
     }
     __syncthreads();
 
-    // ---- C: half-stencil tests + unions
+    DBG_T(tC);
+    DBG_ADD(1, tB, tC);
+    // ---- C: pair tests + unions
     unsigned int nedges = 0, ntests = 0;
-    if (wrap) link_phase<true>(rec, cbeg, par, M, g, bg, o, nedges, ntests);
-    else link_phase<false>(rec, cbeg, par, M, g, bg, o, nedges, ntests);
+    if (wrap) link_phase<true>(v, s_nitems, &s_ticket, g, bg, o, nedges, ntests);
+    else link_phase<false>(v, s_nitems, &s_ticket, g, bg, o, nedges, ntests);
+    DBG_T(tC2);
+    DBG_ADD(6, tC, tC2);
     __syncthreads();
+    DBG_T(tD);
+    DBG_ADD(2, tC, tD);
 
     // ---- D: labels of my own non-roots; one equivalence per linked ghost
     for (int s0 = warp * 32; s0 < M; s0 += kBlockThreads) {
@@ -508,7 +741,7 @@ __global__ void __launch_bounds__(kBlockThreads, 2) block_link_kernel(const floa
         bool emit = false;
         unsigned int me_o = 0, root_o = 0;
         if (s < M) {
-            const int rt = find_s(par, s);
+            const int rt = find_s(v.par, s);
             if (rt != s) {
                 const unsigned int w = __float_as_uint(rec[s].w);
                 me_o = w & ~kGhostBit;
@@ -529,6 +762,8 @@ __global__ void __launch_bounds__(kBlockThreads, 2) block_link_kernel(const floa
     ntests = __reduce_add_sync(kFull, ntests);
     if (lane == 0) { atomicAdd(&s_red[0], nedges); atomicAdd(&s_red[1], ntests); }
     __syncthreads();
+    DBG_T(tE);
+    DBG_ADD(3, tD, tE);
     if (tid == 0) {
         if (s_red[0]) atomicAdd(&ctrl->edges, (unsigned long long)s_red[0]);
         if (s_red[1]) atomicAdd(&ctrl->pair_tests, (unsigned long long)s_red[1]);
@@ -592,7 +827,7 @@ __global__ void __launch_bounds__(kBlock) flatten_labels_kernel(int *labels, int
     while (moving) {
         int p[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) p[k] = ((volatile int *)labels)[r[k]];
+        for (int k = 0; k < 4; ++k) p[k] = i0 + k < N ? ((volatile int *)labels)[r[k]] : r[k];  // nothing to chase behind the last particle
         moving = false;
 #pragma unroll
         for (int k = 0; k < 4; ++k) { moving |= p[k] != r[k]; r[k] = p[k]; }
@@ -600,6 +835,11 @@ __global__ void __launch_bounds__(kBlock) flatten_labels_kernel(int *labels, int
 #pragma unroll
     for (int k = 0; k < 4; ++k)
         if (i0 + k < N && r[k] != l[k]) labels[i0 + k] = r[k];
+}
+
+inline size_t block_link_smem(const BlockGeom &bg)
+{
+    return (size_t)kBlockCap * 20 + (size_t)kMaxItems * 4 + (size_t)kWarps * kQueue * 4 + ((size_t)bg.ncell + 1) * 4;
 }
 
 inline cudaError_t set_smem(const void *fn, size_t bytes)
@@ -610,42 +850,48 @@ inline cudaError_t set_smem(const void *fn, size_t bytes)
 
 }  // namespace
 
-cudaError_t launch_block_path(const float *pos, int64_t N, Grid g, const BlockGeom &bg, int ctas, unsigned int *bin_total,
-                              unsigned int *bin_base, unsigned int *cursor, float4 *part, int64_t part_cap, int2 *cross,
-                              int *labels, Ctrl *ctrl, StageHook &hook, cudaStream_t s)
+#ifdef FOF_BLOCK_TIMING
+extern "C" void fof_dbg_read(unsigned long long *out, int reset)
+{
+    cudaMemcpyFromSymbol(out, g_dbg, sizeof(g_dbg));
+    if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_dbg, z, sizeof(z)); }
+}
+#endif
+
+cudaError_t launch_block_path(const float *pos, int64_t N, Grid g, const BlockGeom &bg, int ctas, unsigned int *cursor,
+                              float4 *part, int2 *cross, int *labels, Ctrl *ctrl, StageHook &hook, cudaStream_t s)
 {
     if (N <= 0) return cudaSuccess;
     cudaError_t e;
     const bool vec = ((uintptr_t)pos & 15) == 0;
     const bool labels_vec = ((uintptr_t)labels & 15) == 0;
     const size_t smem_bins = (size_t)bg.bins * sizeof(unsigned int);
-    const size_t smem_link = (size_t)kBlockCap * 20 + ((size_t)bg.ncell + 1) * sizeof(unsigned int);
-    auto hist = vec ? block_hist_kernel<true> : block_hist_kernel<false>;
+    const size_t smem_link = block_link_smem(bg);
     auto scat = vec ? block_scatter_kernel<true> : block_scatter_kernel<false>;
-    if ((e = set_smem((const void *)hist, smem_bins)) != cudaSuccess) return e;
     if ((e = set_smem((const void *)scat, smem_bins)) != cudaSuccess) return e;
     if ((e = set_smem((const void *)block_link_kernel, smem_link)) != cudaSuccess) return e;
-    const int64_t chunk = ((N + ctas - 1) / ctas + 3) & ~(int64_t)3;
     hook.begin(0, 1);
-    if ((e = cudaMemsetAsync(bin_total, 0, smem_bins, s)) != cudaSuccess) return e;
-    hist<<<ctas, kPartThreads, smem_bins, s>>>(pos, N, g, bg, chunk, bin_total, ctrl);
+    if ((e = cudaMemsetAsync(cursor, 0, smem_bins, s)) != cudaSuccess) return e;
+#ifdef FOF_SCAT_DIRECT
+    scat<<<FOF_SCAT_CTAS * ctas, 256, 0, s>>>(pos, N, g, bg, cursor, part, (unsigned int)kBlockCap, labels, labels_vec, ctrl);
+#else
+    scat<<<FOF_SCAT_CTAS * ctas, kScatThreads, smem_bins, s>>>(pos, N, g, bg, cursor, part, (unsigned int)kBlockCap, labels,
+                                                              labels_vec, ctrl);
+#endif
     hook.end(0);
+    if (getenv("FOF_DEBUG_SYNC")) { e = cudaStreamSynchronize(s); fprintf(stderr, "[fof] after scatter: %s\n", cudaGetErrorString(e)); if (e != cudaSuccess) return e; }
     hook.begin(1, 1);
-    block_offsets_kernel<<<1, kOffThreads, 0, s>>>(bin_total, bg.bins, bin_base, cursor, (unsigned int)kBlockCap,
-                                                   (unsigned long long)part_cap, ctrl);
+    block_link_kernel<<<bg.bins, kBlockThreads, smem_link, s>>>(part, cursor, (unsigned int)kBlockCap, g, bg, labels, cross, ctrl);
     hook.end(1);
+    if (getenv("FOF_DEBUG_SYNC")) { e = cudaStreamSynchronize(s); Ctrl hc; cudaMemcpy(&hc, ctrl, sizeof(hc), cudaMemcpyDeviceToHost); fprintf(stderr, "[fof] after block_link: %s mode %u ncross %u max_block %u N %lld\n", cudaGetErrorString(e), hc.mode, hc.ncross, hc.max_block, (long long)N); if (e != cudaSuccess) return e; }
     hook.begin(2, 1);
-    scat<<<2 * ctas, kScatThreads, smem_bins, s>>>(pos, N, g, bg, cursor, part, labels, labels_vec, ctrl);
-    hook.end(2);
-    hook.begin(3, 1);
-    block_link_kernel<<<bg.bins, kBlockThreads, smem_link, s>>>(part, bin_base, g, bg, labels, cross, ctrl);
-    hook.end(3);
-    hook.begin(4, 1);
     cross_link_kernel<<<2 * ctas, kBlock, 0, s>>>(cross, labels, ctrl);
-    hook.end(4);
-    hook.begin(5, 1);
+    hook.end(2);
+    if (getenv("FOF_DEBUG_SYNC")) { e = cudaStreamSynchronize(s); fprintf(stderr, "[fof] after cross_link: %s\n", cudaGetErrorString(e)); if (e != cudaSuccess) return e; }
+    hook.begin(3, 1);
     flatten_labels_kernel<<<(unsigned int)((N + 4 * kBlock - 1) / (4 * kBlock)), kBlock, 0, s>>>(labels, N, labels_vec, ctrl);
-    hook.end(5);
+    hook.end(3);
+    if (getenv("FOF_DEBUG_SYNC")) { e = cudaStreamSynchronize(s); fprintf(stderr, "[fof] after flatten: %s\n", cudaGetErrorString(e)); if (e != cudaSuccess) return e; }
     return cudaGetLastError();
 }
 
