@@ -113,7 +113,10 @@ int fof_link_stats(fof_handle *h, void *ws, void *stream, uint64_t *edges_host, 
  *   particle_group  dev [N] int32 or NULL: compact id of each particle's group, -1 if dropped
  *   cap             capacity of the group_* arrays; floor(N / N_min) always suffices
  *   K_host          host: number of kept groups
- * Synchronises `stream` once to return K.  K > cap -> FOF_ERR_CAPACITY. */
+ * Synchronises `stream` once to return K.  K > cap -> FOF_ERR_CAPACITY.
+ * fof_groups works from (pos, labels) alone.  If `labels` is the very buffer the last fof_link on (h, ws)
+ * filled, the group sizes that call counted on the way (H6 is fused into its label pass) are re-used: the
+ * caller must then not have modified that buffer in between (pass a copy to have any other labels counted). */
 int fof_groups(fof_handle *h, const float *pos, const float *mass, const int32_t *labels, void *ws,
                int32_t *group_label, int32_t *group_size, float *group_mass, float *group_com,
                int32_t *particle_group, int64_t cap, int64_t *K_host, void *stream);

@@ -336,7 +336,10 @@ int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *s
     int *idx_s = at<int>(ws, h->off_idx);
     unsigned long long *dense = at<unsigned long long>(ws, h->off_dense);
     h->linked = false;
+    h->counted = false;
     const int has = h->N > 0;
+    int *cnt = at<int>(ws, h->off_cnt);
+    unsigned long long *gstate = at<unsigned long long>(ws, h->off_gscan_state);
     if (h->prof_slots) {
         h->prof_cur = (h->prof_cur + 1) % h->prof_slots;
         for (int k = 0; k < kNumStages; ++k) h->ev_valid[h->prof_cur * kMaxStages + k] = false;
@@ -351,7 +354,8 @@ int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *s
     if (blocks) {
         StageHook hook{h, s, kBlockPartition};
         CK(launch_block_path(pos, h->N, h->grid, h->bg, h->part_ctas, at<unsigned int>(ws, h->off_cursor),
-                             at<float4>(ws, h->off_part), at<int2>(ws, h->off_idx), labels, ctrl, hook, s),
+                             at<float4>(ws, h->off_part), at<int2>(ws, h->off_idx), labels, cnt, gstate, h->gscan_tiles, ctrl,
+                             hook, s),
            "block path kernels");
     }
     const unsigned int *gate = blocks ? &ctrl->mode : nullptr;
@@ -359,15 +363,20 @@ int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *s
         StageHook hook{h, s, kLinkHist};
         CK(launch_sort(pos, h->N, h->grid, h->sort, h->part_ctas, at<unsigned int>(ws, h->off_cta_hist),
                        at<unsigned int>(ws, h->off_bin_base), at<float4>(ws, h->off_part), cell, sorted, rel, idx_s,
-                       dense, labels, ctrl, gate, hook, s), "sort kernels");
+                       dense, labels, ctrl, gate, cnt, hook, s), "sort kernels");
     }
     {
         StageTimer t(h, s, kLinkPairs, has);
         CK(launch_link(sorted, h->N, h->grid, cell, dense, rel, idx_s, ctrl, h->num_sms, gate, s), "link kernels");
     }
-    { StageTimer t(h, s, kLinkLabels, has); CK(launch_write_labels(rel, idx_s, labels, h->N, gate, s), "write_labels_kernel"); }
+    {
+        StageTimer t(h, s, kLinkLabels, has);
+        CK(launch_write_labels(rel, idx_s, labels, h->N, gate, cnt, gstate, h->gscan_tiles, ctrl, s), "write_labels_kernel");
+    }
     h->linked = true;
     h->linked_ws = ws;
+    h->counted = has != 0;  // H6 rode along: fof_groups on these very labels starts at the compaction
+    h->counted_labels = labels;
     h->linked_cells = !blocks;  // the cell-sorted arrays are certainly there only if the cell path ran ungated
     return FOF_OK;
 }
@@ -408,13 +417,19 @@ int fof_groups(fof_handle *h, const float *pos, const float *mass, const int32_t
     const int has = h->N > 0;
     if (h->prof_slots)
         for (int k = kGroupsClear; k <= kGroupsFinish; ++k) h->ev_valid[h->prof_cur * kMaxStages + k] = false;
-    {
-        StageTimer t(h, s, kGroupsClear, 0);
-        CK(cudaMemsetAsync(cnt, 0, (size_t)(h->N + 1) * sizeof(int), s), "memset cnt");
-    }
-    {   // also clears the compaction's ticket, K and scan state
-        StageTimer t(h, s, kGroupsCount, 1);
-        CK(launch_group_count(labels, h->N, cnt, state, h->gscan_tiles, ctrl, s), "group_count_kernel");
+    // The sizes of the groups of `labels` are already in the workspace if these are the labels the last fof_link
+    // on (h, ws) wrote (H6 is fused into its label pass); any other labels are counted here.
+    const bool counted = h->counted && h->linked && h->linked_ws == ws && h->counted_labels == (const void *)labels;
+    h->counted = false;  // the compaction below overwrites the counters
+    if (!counted) {
+        {
+            StageTimer t(h, s, kGroupsClear, 0);
+            CK(cudaMemsetAsync(cnt, 0, (size_t)(h->N + 1) * sizeof(int), s), "memset cnt");
+        }
+        {   // also clears the compaction's ticket, K and scan state
+            StageTimer t(h, s, kGroupsCount, 1);
+            CK(launch_group_count(labels, h->N, cnt, state, h->gscan_tiles, ctrl, s), "group_count_kernel");
+        }
     }
     {
         StageTimer t(h, s, kGroupsCompact, has);
@@ -493,6 +508,7 @@ int fof_subgroups(fof_handle *h, const float *pos, const float *vel, const int32
         h->num_sms = sms;
     }
     h->linked = false;  // the member lists and their union-find re-use the link's arrays
+    h->counted = false;
     h->launches += h->N > 0 ? (K > 0 ? 6 : 3) : 0;
     CK(launch_subgroups(pos, vel, particle_group, group_size, h->N, K, h->L, sigma_x, sigma_v, ell,
                         at<unsigned int>(ws, h->off_cnt), at<unsigned int>(ws, h->off_part), at<int>(ws, h->off_idx),

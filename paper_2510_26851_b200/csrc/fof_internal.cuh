@@ -42,7 +42,8 @@ struct Ctrl {
     unsigned int ncross;            // block path: equivalence pairs listed by block_link_kernel
     unsigned int tile_ticket2;      // block path: next input tile of block_scatter_kernel
     unsigned int max_block;         // block path: records (own + ghost) of the fullest block
-    unsigned int pad1[3];
+    unsigned int part_ticket;       // cell path: next input tile of part_scatter_tiled_kernel
+    unsigned int pad1[2];
 };
 static_assert(sizeof(Ctrl) <= 256, "Ctrl must fit its 256-byte slot");
 
@@ -141,6 +142,8 @@ struct fof_handle {
     int64_t gscan_tiles, max_groups;
     int num_sms, part_ctas;
     bool linked;
+    bool counted;           // the last fof_link left the group sizes of `counted_labels` in the workspace (H6 done)
+    const void *counted_labels;
     bool linked_cells;      // the last fof_link left cell_start / sorted / idx_s / rel in the workspace for certain
     const void *linked_ws;
     char cuda_err[256];
@@ -295,18 +298,20 @@ struct StageHook {
 cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp, int ctas, unsigned int *cta_hist,
                         unsigned int *bin_base, float4 *part, unsigned int *cell_start, float4 *sorted,
                         unsigned int *rel, int *idx_s, unsigned long long *dense_list, int *labels, Ctrl *ctrl,
-                        const unsigned int *gate, StageHook &hook, cudaStream_t s);
+                        const unsigned int *gate, int *cnt, StageHook &hook, cudaStream_t s);
 // block path (kernels_block.cu): histogram + offsets + partition into blocks (with ghost copies), one CTA per
 // block links out of shared memory, equivalence pairs across blocks, flatten.  Sets ctrl->mode = 1 (and does
 // nothing else) if a block does not fit: the gated cell path then runs instead.
 cudaError_t launch_block_path(const float *pos, int64_t N, Grid g, const BlockGeom &bg, int ctas, unsigned int *cursor,
-                              float4 *part, int2 *cross, int *labels, Ctrl *ctrl, StageHook &hook, cudaStream_t s);
+                              float4 *part, int2 *cross, int *labels, int *cnt, unsigned long long *state,
+                              int64_t state_items, Ctrl *ctrl, StageHook &hook, cudaStream_t s);
 cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
                         const unsigned long long *dense_list, unsigned int *rel, const int *idx_s, Ctrl *ctrl,
                         int num_sms, const unsigned int *gate, cudaStream_t s);
 cudaError_t launch_grid_pairs(const unsigned int *cell_start, Grid g, Ctrl *ctrl, int num_sms, cudaStream_t s);
 cudaError_t launch_write_labels(const unsigned int *rel, const int *idx_s, int *labels, int64_t N,
-                                const unsigned int *gate, cudaStream_t s);
+                                const unsigned int *gate, int *cnt, unsigned long long *state, int64_t state_items,
+                                Ctrl *ctrl, cudaStream_t s);
 
 cudaError_t launch_group_count(const int *labels, int64_t N, int *cnt, unsigned long long *state,
                                int64_t state_items, Ctrl *ctrl, cudaStream_t s);

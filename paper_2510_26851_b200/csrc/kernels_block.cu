@@ -118,7 +118,8 @@ template <bool VEC>
 __global__ void __launch_bounds__(256) block_scatter_kernel(const float *__restrict__ pos, int64_t N, Grid g,
                                                             BlockGeom bg, unsigned int *cursor,
                                                             float4 *__restrict__ part, unsigned int cap,
-                                                            int *__restrict__ labels, bool labels_vec, Ctrl *ctrl)
+                                                            int *__restrict__ labels, bool labels_vec, int *__restrict__ cnt,
+                                                            Ctrl *ctrl)
 {
     bool bad = false, over = false;
     for (int64_t i = ((int64_t)blockIdx.x * 256 + threadIdx.x) * 4; i < N; i += (int64_t)gridDim.x * 256 * 4) {
@@ -141,6 +142,7 @@ __global__ void __launch_bounds__(256) block_scatter_kernel(const float *__restr
         if (labels_vec && i + 4 <= N) *reinterpret_cast<int4 *>(labels + i) = make_int4((int)i, (int)i + 1, (int)i + 2, (int)i + 3);
         else
             for (int k = 0; k < 4; ++k) if (i + k < N) labels[i + k] = (int)(i + k);
+        for (int k = 0; k < 4; ++k) if (i + k < N) cnt[i + k] = 0;
         unsigned int bin[4], at[4];
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
@@ -171,7 +173,8 @@ template <bool VEC>
 __global__ void __launch_bounds__(kScatThreads, FOF_SCAT_MINB) block_scatter_kernel(const float *__restrict__ pos, int64_t N, Grid g,
                                                                      BlockGeom bg, unsigned int *cursor,
                                                                      float4 *__restrict__ part, unsigned int cap,
-                                                                     int *__restrict__ labels, bool labels_vec, Ctrl *ctrl)
+                                                                     int *__restrict__ labels, bool labels_vec,
+                                                                     int *__restrict__ cnt, Ctrl *ctrl)
 {
     extern __shared__ unsigned int s_cnt[];  // [bins]: records of the current tile per block, then the tile's first slot
     __shared__ unsigned int s_tile;
@@ -208,10 +211,13 @@ __global__ void __launch_bounds__(kScatThreads, FOF_SCAT_MINB) block_scatter_ker
                                            : make_float4(0.f, 0.f, 0.f, __int_as_float(-1));
                 }
             }
-            // H5, first half: labels[i] = i (final for every singleton), coalesced
+            // H5, first half: labels[i] = i (final for every singleton), coalesced; the size counters of H6 start at 0
             if (labels_vec && i + 4 <= N) *reinterpret_cast<int4 *>(labels + i) = make_int4((int)i, (int)i + 1, (int)i + 2, (int)i + 3);
             else
                 for (int k = 0; k < 4; ++k) if (i + k < N) labels[i + k] = (int)(i + k);
+            if (i + 4 <= N) *reinterpret_cast<int4 *>(cnt + i) = make_int4(0, 0, 0, 0);  // workspace array: aligned
+            else
+                for (int k = 0; k < 4; ++k) if (i + k < N) cnt[i + k] = 0;
         }
 #pragma unroll
         for (int k = 0; k < kScatPer; ++k) {
@@ -803,9 +809,16 @@ __global__ void __launch_bounds__(kBlock) cross_link_kernel(const int2 *__restri
 
 // labels[i] = root(i); four particles per thread.  Only the thread that owns i writes labels[i]; what it reads
 // of other entries is the parent or an ancestor, old or new.
-__global__ void __launch_bounds__(kBlock) flatten_labels_kernel(int *labels, int64_t N, bool vec, const Ctrl *ctrl)
+__global__ void __launch_bounds__(kBlock) flatten_labels_kernel(int *labels, int64_t N, bool vec, Ctrl *ctrl,
+                                                                int *__restrict__ cnt, unsigned long long *state,
+                                                                int64_t state_items)
 {
     if (*(volatile const unsigned int *)&ctrl->mode) return;
+    {   // H6 rides along (see write_labels_kernel): clear the state of the compaction scan of fof_groups
+        const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+        if (tid == 0) { ctrl->gscan_ticket = 0u; ctrl->K = 0; }
+        for (int64_t k = tid; k < state_items; k += (int64_t)gridDim.x * kBlock) state[k] = 0ull;
+    }
     const int64_t i0 = ((int64_t)blockIdx.x * kBlock + threadIdx.x) * 4;
     if (i0 >= N) return;
     int l[4];
@@ -834,7 +847,10 @@ __global__ void __launch_bounds__(kBlock) flatten_labels_kernel(int *labels, int
     }
 #pragma unroll
     for (int k = 0; k < 4; ++k)
-        if (i0 + k < N && r[k] != l[k]) labels[i0 + k] = r[k];
+        if (i0 + k < N && r[k] != (int)(i0 + k)) {  // a non-root: one more member of r[k]'s group
+            if (r[k] != l[k]) labels[i0 + k] = r[k];
+            atomicAdd(cnt + r[k], 1);
+        }
 }
 
 inline size_t block_link_smem(const BlockGeom &bg)
@@ -859,7 +875,8 @@ extern "C" void fof_dbg_read(unsigned long long *out, int reset)
 #endif
 
 cudaError_t launch_block_path(const float *pos, int64_t N, Grid g, const BlockGeom &bg, int ctas, unsigned int *cursor,
-                              float4 *part, int2 *cross, int *labels, Ctrl *ctrl, StageHook &hook, cudaStream_t s)
+                              float4 *part, int2 *cross, int *labels, int *cnt, unsigned long long *state,
+                              int64_t state_items, Ctrl *ctrl, StageHook &hook, cudaStream_t s)
 {
     if (N <= 0) return cudaSuccess;
     cudaError_t e;
@@ -873,10 +890,10 @@ cudaError_t launch_block_path(const float *pos, int64_t N, Grid g, const BlockGe
     hook.begin(0, 1);
     if ((e = cudaMemsetAsync(cursor, 0, smem_bins, s)) != cudaSuccess) return e;
 #ifdef FOF_SCAT_DIRECT
-    scat<<<FOF_SCAT_CTAS * ctas, 256, 0, s>>>(pos, N, g, bg, cursor, part, (unsigned int)kBlockCap, labels, labels_vec, ctrl);
+    scat<<<FOF_SCAT_CTAS * ctas, 256, 0, s>>>(pos, N, g, bg, cursor, part, (unsigned int)kBlockCap, labels, labels_vec, cnt, ctrl);
 #else
     scat<<<FOF_SCAT_CTAS * ctas, kScatThreads, smem_bins, s>>>(pos, N, g, bg, cursor, part, (unsigned int)kBlockCap, labels,
-                                                              labels_vec, ctrl);
+                                                              labels_vec, cnt, ctrl);
 #endif
     hook.end(0);
     if (getenv("FOF_DEBUG_SYNC")) { e = cudaStreamSynchronize(s); fprintf(stderr, "[fof] after scatter: %s\n", cudaGetErrorString(e)); if (e != cudaSuccess) return e; }
@@ -889,7 +906,8 @@ cudaError_t launch_block_path(const float *pos, int64_t N, Grid g, const BlockGe
     hook.end(2);
     if (getenv("FOF_DEBUG_SYNC")) { e = cudaStreamSynchronize(s); fprintf(stderr, "[fof] after cross_link: %s\n", cudaGetErrorString(e)); if (e != cudaSuccess) return e; }
     hook.begin(3, 1);
-    flatten_labels_kernel<<<(unsigned int)((N + 4 * kBlock - 1) / (4 * kBlock)), kBlock, 0, s>>>(labels, N, labels_vec, ctrl);
+    flatten_labels_kernel<<<(unsigned int)((N + 4 * kBlock - 1) / (4 * kBlock)), kBlock, 0, s>>>(labels, N, labels_vec, ctrl, cnt, state,
+                                                                                                 state_items);
     hook.end(3);
     if (getenv("FOF_DEBUG_SYNC")) { e = cudaStreamSynchronize(s); fprintf(stderr, "[fof] after flatten: %s\n", cudaGetErrorString(e)); if (e != cudaSuccess) return e; }
     return cudaGetLastError();

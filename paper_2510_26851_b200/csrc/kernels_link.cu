@@ -598,8 +598,18 @@ __global__ void __launch_bounds__(kLinkBlock, FOF_LINK_MINB) link_kernel(const f
 // lock step so that the (up to four) loads of one round are in flight together; read-only chase.
 __global__ void __launch_bounds__(kBlock) write_labels_kernel(const unsigned int *__restrict__ rel,
                                                               const int *__restrict__ idx_s, int *__restrict__ labels,
-                                                              int64_t N, bool vec, const unsigned int *gate)
+                                                              int64_t N, bool vec, const unsigned int *gate,
+                                                              int *__restrict__ cnt, unsigned long long *state,
+                                                              int64_t state_items, Ctrl *ctrl)
 {
+    // cnt != nullptr: H6 rides along ("parallel histogram"): every non-root adds one to the size
+    // counter of its canonical particle (zeroed by cell_sort_kernel), and the state of the compaction scan of
+    // fof_groups is cleared, so that a fof_groups on these labels starts at H7.
+    if (cnt && !(gate && *gate == 0u)) {
+        const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+        if (tid == 0) { ctrl->gscan_ticket = 0u; ctrl->K = 0; }
+        for (int64_t k = tid; k < state_items; k += (int64_t)gridDim.x * kBlock) state[k] = 0ull;
+    }
     // vec: rel and idx_s are 16-byte aligned (the workspace arrays are; the per-sample union-find arrays of
     // fof_link_stochastic_batch, rel_s + k N, are not when N is not a multiple of 4)
     const int64_t s0 = ((int64_t)blockIdx.x * kBlock + threadIdx.x) * 4;
@@ -629,7 +639,11 @@ __global__ void __launch_bounds__(kBlock) write_labels_kernel(const unsigned int
     }
 #pragma unroll
     for (int k = 0; k < 4; ++k)
-        if (d[k]) labels[oi[k]] = __ldg(idx_s + r[k]);
+        if (d[k]) {
+            const int lab = __ldg(idx_s + r[k]);
+            labels[oi[k]] = lab;
+            if (cnt) atomicAdd(cnt + lab, 1);
+        }
 }
 
 // P_exec of DESIGN.md §7: candidate pairs the unfiltered half stencil implies on this grid,
@@ -689,10 +703,13 @@ cudaError_t launch_link(const float4 *sorted, int64_t N, Grid g, const unsigned 
 }
 
 cudaError_t launch_write_labels(const unsigned int *rel, const int *idx_s, int *labels, int64_t N,
-                                const unsigned int *gate, cudaStream_t s)
+                                const unsigned int *gate, int *cnt, unsigned long long *state, int64_t state_items,
+                                Ctrl *ctrl, cudaStream_t s)
 {
     const bool vec = (((uintptr_t)rel | (uintptr_t)idx_s) & 15) == 0;
-    if (N > 0) write_labels_kernel<<<blocks_for(N, kBlock * 4), kBlock, 0, s>>>(rel, idx_s, labels, N, vec, gate);
+    if (N > 0)
+        write_labels_kernel<<<blocks_for(N, kBlock * 4), kBlock, 0, s>>>(rel, idx_s, labels, N, vec, gate, cnt, state,
+                                                                         state_items, ctrl);
     return cudaGetLastError();
 }
 

@@ -598,7 +598,7 @@ cudaError_t launch_link_stochastic(const float4 *sorted, int64_t N, Grid g, cons
     iota_kernel<<<blocks_for(N, kBlock), kBlock, 0, s>>>(labels, N);
     link_stochastic_kernel<<<blocks_for(N, kBlock), kBlock, 0, s>>>(sorted, N, g, cell_start, idx_s, rel, sp, logp, grad,
                                                                     ctrl);
-    return launch_write_labels(rel, idx_s, labels, N, nullptr, s);
+    return launch_write_labels(rel, idx_s, labels, N, nullptr, nullptr, nullptr, 0, nullptr, s);
 }
 
 // S samples sample0 .. sample0 + S - 1 on one binning, four per pass (then one by one).
@@ -635,7 +635,7 @@ cudaError_t launch_link_stochastic_batch(const float4 *sorted, int64_t N, Grid g
     for (int k = 0; k < S; ++k) {
         int *lab = labels + (size_t)k * (size_t)N;
         iota_kernel<<<grid, kBlock, 0, s>>>(lab, N);
-        if ((e = launch_write_labels(rel_s + (size_t)k * (size_t)N, idx_s, lab, N, nullptr, s)) != cudaSuccess) return e;
+        if ((e = launch_write_labels(rel_s + (size_t)k * (size_t)N, idx_s, lab, N, nullptr, nullptr, nullptr, 0, nullptr, s)) != cudaSuccess) return e;
     }
     return cudaGetLastError();
 }
