@@ -34,9 +34,16 @@ from paper_2510_26851_b200 import inputs  # noqa: E402
 METRIC = "fof_linked_particles_per_s"
 UNIT = "particles/s"
 
-# Algorithmic bytes per particle of each profiled stage (DESIGN.md §6; the compulsory streams of
-# SURVEY.md §8d split per kernel).  Cell arrays, neighbour re-reads and scan state are
+# Algorithmic bytes per particle of each profiled stage (DESIGN.md section 6; the compulsory streams of
+# SURVEY.md section 8d split per kernel).  Cell arrays, neighbour re-reads and scan state are
 # implementation cost and are deliberately NOT counted.
+# NOTE on per-stage fractions: the byte model charges streams to the stage that SURVEY.md's reference pipeline
+# would run them in.  Where the design removed or merged a pass the per-stage figure is not a statement about
+# that kernel: link.labels is charged 24 B (flatten 8 + canonicalise 12 + write 4) although the union-find is
+# rooted at the minimum original index and needs neither a flatten nor a min pass (its "achieved" can exceed
+# the HBM peak); groups.count is charged 8 B but runs inside link.labels (its stage time is 0 when fof_groups
+# follows fof_link on the same labels); groups.clear, link.clear and link.offsets move no algorithmic bytes.
+# Only the sum (124 B per particle, `roofline.path`) is the figure north_star's 40 % target refers to.
 ALG_BYTES_PER_PARTICLE = {
     "link.clear": 0,
     "link.hist": 12,               # read pos (histogram)
@@ -51,7 +58,13 @@ ALG_BYTES_PER_PARTICLE = {
     "groups.compact": 4 + 4,       # read sizes, write id map
     "groups.reduce": 12 + 4 + 4 + 4,  # read pos, mass, labels, id
     "groups.finish": 0,
+    # block path (FOF_PATH_BLOCKS): the same 84 B of the link phase, charged to its four kernels
+    "block.partition": 12 + 12 + 16,   # one pass reads pos and writes the records (no histogram pass)
+    "block.link": 16 + 4,              # read the records once, write the local forests
+    "block.cross": 0,
+    "block.flatten": 8 + 12 + 4,       # flatten + canonicalise + labels
 }
+ALG_BYTES_TOTAL = 124  # link 84 + groups 40
 
 
 def peaks():
@@ -64,19 +77,41 @@ def peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 20 ms while the timed region runs."""
+    """SM clock and throttle reasons sampled through NVML every ~2 ms while the timed region runs (falls back to
+    `nvidia-smi -lms 5` if the NVML binding is missing)."""
 
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index: int):
-        self.rows, self.p, self.index = [], None, index
+        self.rows, self.p, self.index, self.stop, self.nv = [], None, index, False, None
+
+    def _physical_index(self):
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+        if vis:
+            try:
+                return int(vis.split(",")[self.index])
+            except Exception:
+                pass
+        return self.index
 
     def __enter__(self):
         try:
+            import pynvml as nv
+
+            nv.nvmlInit()
+            self.nv = nv
+            self.h = nv.nvmlDeviceGetHandleByIndex(self._physical_index())
+            self.mx = float(nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM))
+            self.t = threading.Thread(target=self._poll, daemon=True)
+            self.t.start()
+            return self
+        except Exception:
+            self.nv = None
+        try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "20"],
+                                       "--format=csv,noheader,nounits", "-lms", "5"],
                                       stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -84,11 +119,32 @@ class ClockSampler:
             self.p = None
         return self
 
+    def _poll(self):
+        nv = self.nv
+        bits = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20}
+        while not self.stop:
+            try:
+                sm = float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    rs = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    rs = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                self.rows.append([str(sm), str(self.mx), "0"] +
+                                 ["Active" if rs & bits[n] else "Not Active"
+                                  for n in ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")])
+            except Exception:
+                pass
+            time.sleep(0.002)
+
     def _read(self):
         for line in self.p.stdout:
             self.rows.append([c.strip() for c in line.split(",")])
 
     def __exit__(self, *a):
+        if self.nv is not None:
+            self.stop = True
+            self.t.join(timeout=2)
+            return
         if self.p is not None:
             time.sleep(0.15)
             self.p.terminate()
@@ -110,7 +166,7 @@ class ClockSampler:
             except Exception:
                 pass
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+                "reasons": sorted(reasons), "samples": len(sm), "how": "NVML, ~2 ms period" if self.nv else "nvidia-smi -lms 5"}
 
 
 def dist_env():
@@ -214,7 +270,7 @@ def run_ours(args):
     N = w.N
     hpos = torch.from_numpy(pos_np).pin_memory()
     dpos = hpos.to(dev, non_blocking=True)
-    f = B.FoF(N, w.L, w.b, w.N_min, device=dev, grid=args.grid)
+    f = B.FoF(N, w.L, w.b, w.N_min, device=dev, grid=args.grid, path=args.path)
     out = f.alloc_groups()
     labels = torch.empty(N, dtype=torch.int32, device=dev)
     stream = torch.cuda.current_stream()
@@ -401,40 +457,47 @@ def run_ours(args):
     peak, peak_src = peaks()
     alg = ALG_BYTES_PER_PARTICLE.get(top, 0) * N
     hbm_achieved = alg / (top_ms_live * 1e-3) / 1e9 if top_ms_live > 0 else 0.0
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")  # written by hand from the ncu --set full capture
+    # traffic: dram bytes per launch of that kernel from the committed ncu --set full capture (profiles/traffic.json,
+    # written by `python -m paper_2510_26851_b200.traffic_from_ncu`); null if the CUDA sources changed since
+    traffic, traffic_source = None, "no profiles/traffic.json"
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         try:
+            from paper_2510_26851_b200.traffic_from_ncu import source_hash
+
             with open(tpath) as fh:
-                traffic = json.load(fh).get(args.workload, {}).get(top)
-        except Exception:
-            traffic = None
-    total_alg = sum(ALG_BYTES_PER_PARTICLE.get(k, 0) for k in stages) * N
+                doc = json.load(fh)
+            if doc.get("source_hash") == source_hash():
+                traffic = doc.get(args.workload, {}).get(top)
+                traffic_source = f"profiles/traffic.json ({doc.get('report')}, sources {doc.get('source_hash')})"
+            else:
+                traffic_source = (f"profiles/traffic.json is stale: captured from sources {doc.get('source_hash')}, "
+                                  f"this tree is {source_hash()}")
+        except Exception as exc:  # noqa: BLE001
+            traffic_source = f"profiles/traffic.json unreadable: {exc}"
+    total_alg = ALG_BYTES_TOTAL * N
     path = {"alg_bytes_per_step": total_alg, "achieved": total_alg / (ms_step * 1e-3) / 1e9,
             "frac": total_alg / (ms_step * 1e-3) / 1e9 / peak,
             "frac_of_8000_nominal": total_alg / (ms_step * 1e-3) / 1e9 / 8000.0, "unit": "GB/s", "peak": peak}
-    if top == "link.pairs":
+    if top in ("link.pairs", "block.link"):
         # link_kernel is bound by FP32/ALU issue, not by HBM: 9 FP32 operations per
         # distance test (3 sub, 3 mul, 2 add, 1 compare; no FMA by definition of the predicate) against
-        # the issue ceiling SMs x 4 schedulers x 32 lanes x SM clock.
+        # the non-FMA FP32 issue rate measured on this device in this run.
         sms = torch.cuda.get_device_properties(dev).multi_processor_count
-        try:
-            with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
-                mhz = float(json.load(fh)["sm_max_mhz"])
-        except Exception:
-            mhz = 1965.0
-        alu_peak = sms * 4 * 32 * mhz * 1e6 / 1e9  # G lane-operations / s
+        alu_peak = B.fof_measure_fp32_issue() / 1e9  # G lane-operations / s, measured in this run (fof.h)
         alu_achieved = 9.0 * pair_tests / (top_ms_live * 1e-3) / 1e9
         roofline = {"bound": "alu", "kernel": top, "achieved": alu_achieved, "peak": alu_peak, "unit": "GOP/s",
-                    "frac": alu_achieved / alu_peak, "traffic": traffic,
-                    "peak_source": f"{sms} SMs x 4 schedulers x 32 lanes x {mhz:.0f} MHz (DESIGN.md 6)",
+                    "frac": alu_achieved / alu_peak, "traffic": traffic, "traffic_source": traffic_source,
+                    "peak_source": "measured in this run: fof_measure_fp32_issue (non-FMA FADD + FMUL stream on all "
+                                   f"{sms} SMs, best of 4 launches)",
                     "alg_ops_per_launch": 9 * pair_tests, "kernel_ms": top_ms_live,
                     "hbm": {"alg_bytes_per_launch": alg, "achieved": hbm_achieved, "peak": peak, "unit": "GB/s",
                             "frac": hbm_achieved / peak, "peak_source": peak_src},
                     "path": path}
     else:
         roofline = {"bound": "hbm", "kernel": top, "achieved": hbm_achieved, "peak": peak, "unit": "GB/s",
-                    "frac": hbm_achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                    "frac": hbm_achieved / peak, "traffic": traffic, "traffic_source": traffic_source,
+                    "peak_source": peak_src,
                     "alg_bytes_per_launch": alg, "kernel_ms": top_ms_live, "path": path}
 
     # ---- the oracle timed beside it on the host cores (a reported baseline, not the target)
@@ -447,6 +510,7 @@ def run_ours(args):
         parity = bool(np.array_equal(labels.cpu().numpy(), lab) and E == E_ref and K_groups == og["K"]
                       and np.array_equal(out["group_size"][:K_groups].cpu().numpy(), og["group_size"]))
 
+    t_pairs = stages.get("link.pairs") or stages.get("block.link")
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
@@ -456,8 +520,9 @@ def run_ours(args):
                    "parallelism": "replicas only" if world > 1 else "1 GPU",
                    "l2": "inputs + workspace per step exceed the 126 MB L2 (pos 12N + sorted 16N + labels 4N ...)"
                          if N * 32 > 126e6 else "working set fits L2 (small workload)"},
-        "pair_tests_per_s": pair_tests / (stages["link.pairs"] * 1e-3) if stages.get("link.pairs") else None,
-        "grid_pairs_per_s": grid_pairs / (stages["link.pairs"] * 1e-3) if stages.get("link.pairs") else None,
+        "pair_tests_per_s": pair_tests / (t_pairs * 1e-3) if t_pairs else None,
+        "grid_pairs_per_s": grid_pairs / (t_pairs * 1e-3) if t_pairs and grid_pairs else None,
+        "path": f.link_path()[0],
         "stage_ms": {k: round(v, 5) for k, v in stages.items()},
         "stage_ms_note": f"separate pass of {n_break} steps with events around every stage; the timed region carries "
                          f"events around {top} only (roofline.kernel_ms)",
@@ -480,6 +545,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2", choices=sorted(inputs.CONFIGS))
     ap.add_argument("--grid", type=int, default=None, help="force n cells per axis (tuning knob)")
+    ap.add_argument("--path", default="auto", choices=["auto", "cells", "blocks"],
+                    help="implementation of H1-H5 (fof_set_path); results are identical")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-next1", action="store_true", help="skip the sigma / backward timing")
     ap.add_argument("--no-next3", action="store_true", help="skip the stochastic-edge sample timing")

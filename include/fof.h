@@ -240,6 +240,19 @@ const char *fof_profile_name(const fof_handle *h, int k);
 int fof_profile_read(fof_handle *h, float *ms, int cap);
 uint64_t fof_launch_count(const fof_handle *h);
 
+/* Measured ceilings (measurement aids; they run no step of the method).
+ * fof_measure_fp32_issue: FP32 lane-operations per second of this device on a non-FMA FADD + FMUL stream (the
+ *   instruction mix of the link predicate, which forbids FMA contraction), best of four timed launches that
+ *   fill every SM; the ceiling bench.py quotes for the ALU-bound link kernel.  Allocates
+ *   (and frees) 256 bytes of device memory of its own.
+ * fof_measure_scatter: records per second of a copy of n_records 16-byte records (dev in/out, 16-byte aligned,
+ *   n_records >= 4096) in which the stores (scatter_stores != 0) or the loads are scattered inside windows of
+ *   2^log2_window records and the other side is coalesced: the floor of a reorder pass of H3.
+ * Both synchronise `stream`. */
+int fof_measure_fp32_issue(double *lane_ops_per_s_host, void *stream);
+int fof_measure_scatter(const void *in, void *out, int64_t n_records, int32_t log2_window, int32_t scatter_stores,
+                        double *records_per_s_host, void *stream);
+
 /* Static string for an error code. */
 const char *fof_error_string(int code);
 

@@ -101,6 +101,10 @@ def lib():
         L.fof_profile_read.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.c_int]
         L.fof_launch_count.restype = ctypes.c_uint64
         L.fof_launch_count.argtypes = [vp]
+        L.fof_measure_fp32_issue.restype = ctypes.c_int
+        L.fof_measure_fp32_issue.argtypes = [ctypes.POINTER(ctypes.c_double), vp]
+        L.fof_measure_scatter.restype = ctypes.c_int
+        L.fof_measure_scatter.argtypes = [vp, vp, i64, i32, i32, ctypes.POINTER(ctypes.c_double), vp]
         L.fof_error_string.restype = ctypes.c_char_p
         L.fof_error_string.argtypes = [ctypes.c_int]
         L.fof_last_cuda_error.restype = ctypes.c_char_p
@@ -287,6 +291,22 @@ def fof_profile_read(h):
     buf = (ctypes.c_float * n)()
     _check(lib().fof_profile_read(h, buf, n), h)
     return {lib().fof_profile_name(h, k).decode(): float(buf[k]) for k in range(n)}
+
+
+def fof_measure_fp32_issue(stream=None) -> float:
+    """FP32 lane-operations per second on a non-FMA FADD + FMUL stream (measured ceiling of the link predicate)."""
+    v = ctypes.c_double()
+    _check(lib().fof_measure_fp32_issue(ctypes.byref(v), _stream_ptr(stream)))
+    return float(v.value)
+
+
+def fof_measure_scatter(src, dst, log2_window: int, scatter_stores: bool, stream=None) -> float:
+    """records/s of a copy of 16-byte records whose stores (or loads) are scattered inside 2^k-record windows."""
+    v = ctypes.c_double()
+    n = src.numel() * src.element_size() // 16
+    _check(lib().fof_measure_scatter(_ptr(src), _ptr(dst), int(n), int(log2_window), int(bool(scatter_stores)),
+                                     ctypes.byref(v), _stream_ptr(stream)))
+    return float(v.value)
 
 
 def fof_launch_count(h) -> int:

@@ -42,8 +42,7 @@ struct Ctrl {
     unsigned int ncross;            // block path: equivalence pairs listed by block_link_kernel
     unsigned int tile_ticket2;      // block path: next input tile of block_scatter_kernel
     unsigned int max_block;         // block path: records (own + ghost) of the fullest block
-    unsigned int part_ticket;       // cell path: next input tile of part_scatter_tiled_kernel
-    unsigned int pad1[2];
+    unsigned int pad1[3];
 };
 static_assert(sizeof(Ctrl) <= 256, "Ctrl must fit its 256-byte slot");
 

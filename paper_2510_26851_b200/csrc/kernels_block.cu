@@ -860,7 +860,7 @@ inline size_t block_link_smem(const BlockGeom &bg)
 
 inline cudaError_t set_smem(const void *fn, size_t bytes)
 {
-    if (bytes <= 48 * 1024) return cudaSuccess;
+    if (bytes <= 40 * 1024) return cudaSuccess;  // static shared memory counts against the 48 KB default too
     return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 

@@ -28,10 +28,8 @@ template <bool VEC>
 __global__ void __launch_bounds__(kPartThreads) part_hist_kernel(const float *__restrict__ pos, int64_t N, Grid g,
                                                                  int shift, int bins, int64_t chunk,
                                                                  unsigned int *__restrict__ cta_hist, Ctrl *ctrl,
-                                                                 const unsigned int *gate, unsigned int *bin_total)
+                                                                 const unsigned int *gate)
 {
-    // bin_total != nullptr: only the totals per bin are needed (shared-cursor partition below): one global atomic
-    // per (CTA, non-empty bin) instead of the [CTA][bin] matrix
     extern __shared__ unsigned int s_bin[];
     if (gate && *gate == 0u) return;  // the block path did the work (fof_internal.cuh Ctrl::mode)
     for (int b = threadIdx.x; b < bins; b += kPartThreads) s_bin[b] = 0u;
@@ -45,154 +43,12 @@ __global__ void __launch_bounds__(kPartThreads) part_hist_kernel(const float *__
     });
     if (any_bad) atomicOr(&ctrl->error, 1u);
     __syncthreads();
-    if (bin_total) {
-        for (int b = threadIdx.x; b < bins; b += kPartThreads) {
-            const unsigned int c = s_bin[b];
-            if (c) atomicAdd(bin_total + b, c);
-        }
-        return;
-    }
     unsigned int *dst = cta_hist + (int64_t)blockIdx.x * bins;
     for (int b = threadIdx.x; b < bins; b += kPartThreads) dst[b] = s_bin[b];
 }
 
 // ---------------------------------------------------------------------------------------------
-// Shared-cursor partition (one pass: bins <= kTwoPassBins).  bin_scan_kernel: one CTA scans the bin totals into
-// bin_base[] and the write cursors.  part_scatter_tiled_kernel: a CTA takes tiles of kTileThreads x kTilePer
-// particles (registers); the rank of a record among the tile's records of its bin comes from a shared-memory
-// counter, the tile's slots from ONE global atomic per (tile, bin) on the bin's cursor, issued by the thread that
-// drew rank 0.  All CTAs append to the same few thousand open lines, which the L2 merges before they reach DRAM;
-// with a private output run per (CTA, bin) -- part_scatter_kernel below -- 148 x 4096 lines are open at once and
-// are evicted half written (measured on 2^24 records into 4096 bins: 0.42 ms private, 0.25 ms shared; a scattered
-// 16-byte store costs ~12 ps chip-wide whatever the pattern, 80 G records/s, so ~0.21 ms is the floor of any
-// 16-byte scatter pass at this size).  The order of the records inside a bin now depends on the run; the cell
-// sort and the union-find do not care (labels are canonical).
-// ---------------------------------------------------------------------------------------------
-constexpr int kScanThreads = 1024;
-__global__ void __launch_bounds__(kScanThreads) bin_scan_kernel(const unsigned int *__restrict__ bin_total, int bins,
-                                                                unsigned int *__restrict__ bin_base,
-                                                                unsigned int *__restrict__ cursor, const unsigned int *gate)
-{
-    __shared__ unsigned int s_warp[kScanThreads / 32];
-    if (gate && *gate == 0u) return;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int per = (bins + kScanThreads - 1) / kScanThreads;
-    const int b0 = min(tid * per, bins), b1 = min(bins, b0 + per);
-    unsigned int sum = 0;
-    for (int b = b0; b < b1; ++b) sum += bin_total[b];
-    unsigned int incl = sum;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const unsigned int t = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += t;
-    }
-    if (lane == 31) s_warp[warp] = incl;
-    __syncthreads();
-    unsigned int woff = 0, total = 0;
-#pragma unroll
-    for (int w = 0; w < kScanThreads / 32; ++w) {
-        const unsigned int t = s_warp[w];
-        if (w < warp) woff += t;
-        total += t;
-    }
-    unsigned int run = woff + incl - sum;
-    for (int b = b0; b < b1; ++b) {
-        bin_base[b] = run;
-        cursor[b] = run;
-        run += bin_total[b];
-    }
-    if (tid == 0) bin_base[bins] = total;
-}
-
-#ifndef FOF_TILE_THREADS
-#define FOF_TILE_THREADS 512
-#endif
-#ifndef FOF_TILE_PER
-#define FOF_TILE_PER 4
-#endif
-#ifndef FOF_TILE_MINB
-#define FOF_TILE_MINB 3
-#endif
-constexpr int kTileThreads = FOF_TILE_THREADS, kTilePer = FOF_TILE_PER;
-constexpr int64_t kTiledMinN = (int64_t)1 << 22;  // the shared-cursor partition pays from about four million particles
-
-template <bool VEC>
-__global__ void __launch_bounds__(kTileThreads, FOF_TILE_MINB) part_scatter_tiled_kernel(
-    const float *__restrict__ pos, int64_t N, Grid g, int shift, int bins, unsigned int *cursor, float4 *__restrict__ part,
-    int *__restrict__ labels, bool labels_vec, const unsigned int *gate, int *__restrict__ cnt, Ctrl *ctrl)
-{
-    extern __shared__ unsigned int s_cnt[];  // [bins]: records of the current tile per bin, then the tile's first slot
-    __shared__ unsigned int s_tile;
-    if (gate && *gate == 0u) return;
-    constexpr int T = kTileThreads * kTilePer;
-    const int64_t ntiles = (N + T - 1) / T;
-    const int tid = threadIdx.x;
-    for (int b = tid; b < bins; b += kTileThreads) s_cnt[b] = 0u;
-    for (;;) {
-        __syncthreads();
-        if (tid == 0) s_tile = atomicAdd(&ctrl->part_ticket, 1u);
-        __syncthreads();
-        const int64_t tile = s_tile;
-        if (tile >= ntiles) break;
-        const int64_t base = tile * T;
-        float4 rec[kTilePer];
-        unsigned int bin[kTilePer], rank[kTilePer];
-#pragma unroll
-        for (int q = 0; q < kTilePer / 4; ++q) {
-            const int64_t i = base + ((int64_t)q * kTileThreads + tid) * 4;
-            if (VEC && i + 4 <= N) {
-                const float4 *p = reinterpret_cast<const float4 *>(pos + 3 * i);
-                const float4 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
-                rec[4 * q] = make_float4(a.x, a.y, a.z, __int_as_float((int)i));
-                rec[4 * q + 1] = make_float4(a.w, b.x, b.y, __int_as_float((int)i + 1));
-                rec[4 * q + 2] = make_float4(b.z, b.w, c.x, __int_as_float((int)i + 2));
-                rec[4 * q + 3] = make_float4(c.y, c.z, c.w, __int_as_float((int)i + 3));
-            } else {
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    const int64_t j = i + k;
-                    rec[4 * q + k] = j < N ? make_float4(__ldg(pos + 3 * j), __ldg(pos + 3 * j + 1), __ldg(pos + 3 * j + 2),
-                                                         __int_as_float((int)j))
-                                           : make_float4(0.f, 0.f, 0.f, __int_as_float(-1));
-                }
-            }
-            // H5, first half: labels[i] = i (final for every root); the size counters of H6 start at 0
-            if (labels_vec && i + 4 <= N) *reinterpret_cast<int4 *>(labels + i) = make_int4((int)i, (int)i + 1, (int)i + 2, (int)i + 3);
-            else
-                for (int k = 0; k < 4; ++k) if (i + k < N) labels[i + k] = (int)(i + k);
-            if (i + 4 <= N) *reinterpret_cast<int4 *>(cnt + i) = make_int4(0, 0, 0, 0);  // workspace array: aligned
-            else
-                for (int k = 0; k < 4; ++k) if (i + k < N) cnt[i + k] = 0;
-        }
-        bool bad = false;  // the histogram pass has already flagged non-finite positions
-#pragma unroll
-        for (int k = 0; k < kTilePer; ++k) {
-            bin[k] = 0xffffffffu;
-            if (__float_as_int(rec[k].w) >= 0) {
-                bin[k] = wrap_cell(rec[k].x, rec[k].y, rec[k].z, g, bad) >> shift;
-                rank[k] = atomicAdd(&s_cnt[bin[k]], 1u);
-            }
-        }
-        __syncthreads();
-#pragma unroll
-        for (int k = 0; k < kTilePer; ++k)
-            if (bin[k] != 0xffffffffu && rank[k] == 0u) {  // I drew the first rank: I fetch the tile's slots of this bin
-                const unsigned int c = s_cnt[bin[k]];
-                s_cnt[bin[k]] = atomicAdd(&cursor[bin[k]], c);
-            }
-        __syncthreads();
-#pragma unroll
-        for (int k = 0; k < kTilePer; ++k)
-            if (bin[k] != 0xffffffffu) part[s_cnt[bin[k]] + rank[k]] = rec[k];
-        __syncthreads();
-#pragma unroll
-        for (int k = 0; k < kTilePer; ++k)
-            if (bin[k] != 0xffffffffu && rank[k] == 0u) s_cnt[bin[k]] = 0u;
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// (two-pass partition only) cta_hist[k][b] <- sum over k' < k of cta_hist[k'][b] (in place), bin_base[b] <- sum over b' < b
+// cta_hist[k][b] <- sum over k' < k of cta_hist[k'][b] (in place), bin_base[b] <- sum over b' < b
 // of the bin totals, bin_base[bins] = N.  Block = 32 bins x 8 groups of CTAs; the last block to
 // finish scans the bin totals.
 // ---------------------------------------------------------------------------------------------
@@ -495,7 +351,7 @@ __global__ void __launch_bounds__(kPartThreads) rec_scatter_kernel(const float4 
 
 static inline cudaError_t set_smem(const void *fn, size_t bytes)
 {
-    if (bytes <= 48 * 1024) return cudaSuccess;
+    if (bytes <= 40 * 1024) return cudaSuccess;  // static shared memory counts against the 48 KB default too
     return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
@@ -517,11 +373,9 @@ cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp,
     const int64_t chunk = ((N + ctas - 1) / ctas + 3) & ~(int64_t)3;  // a multiple of 4: quads stay aligned
     const int64_t C = (int64_t)g.n * g.n * g.n;
     const bool labels_vec = ((uintptr_t)labels & 15) == 0;
-    if (sp.bins <= kTwoPassBins && N < kTiledMinN) {
-        // small inputs: a private output run per (CTA, bin); the tiles of the shared-cursor variant would spend their
-        // time in barriers and in the latency of the global atomics (128^3: 0.023 vs 0.068 ms)
+    if (sp.bins <= kTwoPassBins) {
         hook.begin(0, 1);
-        hist<<<ctas, kPartThreads, smem_bins, s>>>(pos, N, g, sp.shift, sp.bins, chunk, cta_hist, ctrl, gate, nullptr);
+        hist<<<ctas, kPartThreads, smem_bins, s>>>(pos, N, g, sp.shift, sp.bins, chunk, cta_hist, ctrl, gate);
         hook.end(0);
         hook.begin(1, 1);
         part_offsets_kernel<<<(sp.bins + 31) / 32, 32 * kOffGroups, 0, s>>>(cta_hist, ctas, sp.bins, bin_base, ctrl, gate);
@@ -529,22 +383,6 @@ cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp,
         hook.begin(2, 1);
         scat<<<ctas, kPartThreads, smem_bins, s>>>(pos, N, g, sp.shift, sp.bins, chunk, cta_hist, bin_base, part, labels,
                                                    labels_vec, gate, cnt);
-        hook.end(2);
-    } else if (sp.bins <= kTwoPassBins) {
-        // shared-cursor partition: cta_hist holds the bin totals and, behind them, the write cursors
-        unsigned int *bin_total = cta_hist, *cursor = cta_hist + sp.bins;
-        auto tiled = vec ? part_scatter_tiled_kernel<true> : part_scatter_tiled_kernel<false>;
-        if ((e = set_smem((const void *)tiled, smem_bins)) != cudaSuccess) return e;
-        hook.begin(0, 1);
-        if ((e = cudaMemsetAsync(bin_total, 0, smem_bins, s)) != cudaSuccess) return e;
-        hist<<<ctas, kPartThreads, smem_bins, s>>>(pos, N, g, sp.shift, sp.bins, chunk, cta_hist, ctrl, gate, bin_total);
-        hook.end(0);
-        hook.begin(1, 1);
-        bin_scan_kernel<<<1, kScanThreads, 0, s>>>(bin_total, sp.bins, bin_base, cursor, gate);
-        hook.end(1);
-        hook.begin(2, 1);
-        tiled<<<FOF_TILE_MINB * ctas, kTileThreads, smem_bins, s>>>(pos, N, g, sp.shift, sp.bins, cursor, part, labels,
-                                                                    labels_vec, gate, cnt, ctrl);
         hook.end(2);
     } else {
         // pass 1 over bins 2^kCoarseShift times wider: pos -> `sorted` (used as scratch); pass 2: -> `part`
@@ -555,7 +393,7 @@ cudaError_t launch_sort(const float *pos, int64_t N, Grid g, const SortPlan &sp,
         if ((e = set_smem((const void *)rec_scatter_kernel, smem_bins)) != cudaSuccess) return e;
         const size_t smem_c = (size_t)cbins * sizeof(unsigned int);
         hook.begin(0, 1);
-        hist<<<ctas, kPartThreads, smem_c, s>>>(pos, N, g, cshift, cbins, chunk, cta_hist, ctrl, gate, nullptr);
+        hist<<<ctas, kPartThreads, smem_c, s>>>(pos, N, g, cshift, cbins, chunk, cta_hist, ctrl, gate);
         hook.end(0);
         hook.begin(1, 2);
         part_offsets_kernel<<<(cbins + 31) / 32, 32 * kOffGroups, 0, s>>>(cta_hist, ctas, cbins, cbase, ctrl, gate);
