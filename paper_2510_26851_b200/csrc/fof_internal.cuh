@@ -12,7 +12,7 @@ namespace fof {
 
 constexpr int kBlock = 256;           // threads per CTA for the streaming kernels
 #ifndef FOF_SCAN_ITEMS
-#define FOF_SCAN_ITEMS 16
+#define FOF_SCAN_ITEMS 32
 #endif
 constexpr int kScanItems = FOF_SCAN_ITEMS;  // items per thread in the single-pass scan (multiple of 4)
 constexpr int kScanTile = kBlock * kScanItems;
