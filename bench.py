@@ -8,8 +8,10 @@ particles, the configuration north_star's 40 %-of-roofline target is quoted on).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2] [--impl ours|reference]
 
-N > 1 (under torchrun): the path does not shard in this build ("replicas only"):
-every rank runs an independent particle set (seed + rank); value = all ranks' particles / max time.
+N > 1 (under torchrun): replicas by default (north_star fixes one GPU): every rank runs an
+independent particle set (seed + rank); value = all ranks' particles / max time, "scaling": "weak".
+`--mode slab` times the SHARDED path instead (section 2.3): the one particle set of the
+workload cut into z slabs, ghost exchange + local fof_link + label merge + cross-rank groups; "scaling": "strong".
 `--impl reference` times the CPU oracle (oracle/, as it stands) on rank 0 only.
 Prints ONE JSON line on rank 0.
 """
@@ -243,6 +245,72 @@ def run_reference(args):
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+def run_slab(args):
+    """--mode slab (N >= 2 ranks): the sharded path of PAPER.md section 2.3 on ONE particle set (strong scaling).
+    Every rank generates the seeded set, keeps its z slab, and a step is slab_fof_groups: ghost layer to the rank
+    below (ring send/recv), fof_link on own + ghost particles, equivalence pairs all-gathered, sparse merge, then
+    the cross-rank group construction (four small all-gathers).  Timed on the device, max over ranks."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_2510_26851_b200 import binding as B, slab
+
+    rank, local_rank, world = dist_env()
+    one_gpu = os.environ.get("FOF_BENCH_ONE_GPU") == "1"   # functional check only: all ranks on cuda:0 over gloo
+    if world < 2:
+        raise SystemExit("--mode slab needs at least two ranks (torchrun); one rank is the monolithic path")
+    B.lib()
+    dev = torch.device("cuda", 0 if one_gpu else local_rank)
+    torch.cuda.set_device(dev)
+    if not one_gpu:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")  # the driver counts the ranks in the NCCL log
+        dist.init_process_group("nccl", device_id=dev)
+    else:
+        dist.init_process_group("gloo")
+    w = inputs.CONFIGS[args.workload]
+    pos_np = inputs.make_positions(w)
+    N = w.N
+    own = slab.split_into_slabs(pos_np, w.L, world)[rank]
+    dpos = torch.from_numpy(pos_np[own]).to(dev)
+    dids = torch.from_numpy(own.astype(np.int32)).to(dev)
+    del pos_np
+
+    def step():
+        return slab.slab_fof_groups(dpos, dids, w.L, w.b, N, N_min=w.N_min)
+
+    for _ in range(max(args.warmup, 3)):
+        labels, cat = step()
+    stream = torch.cuda.current_stream()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    dist.barrier()
+    torch.cuda.synchronize()
+    with ClockSampler(dev.index) as clk:
+        e0.record(stream)
+        for _ in range(args.steps):
+            labels, cat = step()
+        e1.record(stream)
+        torch.cuda.synchronize()
+    dist.barrier()
+    ms_step = max_over_ranks_ms(e0.elapsed_time(e1), world, dev if not one_gpu else "cpu") / args.steps
+    k = torch.tensor([cat["K"], int(dpos.shape[0])], dtype=torch.int64, device=dev if not one_gpu else "cpu")
+    dist.all_reduce(k)
+    if rank == 0:
+        line = {"metric": METRIC, "value": N / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": w.name, "N": N, "L": w.L, "b": w.b, "N_min": w.N_min, "mode": "slab",
+                           "parallelism": f"{world} z slabs, ghost layer 1.001 b, ring exchange + 5 all-gathers",
+                           "groups_kept": int(k[0].item()), "particles_owned_total": int(k[1].item()),
+                           "l2": "per-rank inputs + workspace exceed the 126 MB L2" if N * 32 / world > 126e6 else "fits L2"},
+                "roofline": None, "cpu_baseline": None,
+                "e2e": None, "gpu_launches": None, "clocks": clk.summary(),
+                "note": "step = slab_fof_groups (exchange included); host-side index building (torch sort / unique) is "
+                        "inside the timed region"}
+        print(json.dumps(line), flush=True)
+    dist.destroy_process_group()
 
 
 # ------------------------------------------------------------------------------------------------
@@ -545,6 +613,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2", choices=sorted(inputs.CONFIGS))
     ap.add_argument("--grid", type=int, default=None, help="force n cells per axis (tuning knob)")
+    ap.add_argument("--mode", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent replicas (default, weak scaling) or the z-slab sharded path (strong scaling)")
     ap.add_argument("--path", default="auto", choices=["auto", "cells", "blocks"],
                     help="implementation of H1-H5 (fof_set_path); results are identical")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
@@ -554,6 +624,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.mode == "slab":
+        run_slab(args)
     else:
         run_ours(args)
 

@@ -182,6 +182,21 @@ int fof_layer_select(const float *pos, int64_t N, float L, int32_t axis, float l
 int fof_component_min(const int32_t *labels, const int32_t *ids, int64_t N, int32_t *tmp, int32_t *out, void *stream);
 int fof_merge_labels(const int32_t *pairs, int64_t P, int32_t *parent, int64_t G, int32_t *labels, int64_t N,
                      void *stream);
+/* fof_merge_labels_sparse: the same merge with a union-find over the U DISTINCT labels that occur in the pairs
+ *   (uniq: dev [U], ascending; parent: dev scratch [U]) instead of one entry per global id (the
+ *   cost of the union step is what made the paper's slab run slow).  Labels that no pair mentions are untouched.
+ * fof_combine_groups: cross-rank group construction.  Every rank has run fof_groups on its own particles plus
+ *   one massless proxy per canonical particle that lives on another rank, and the partial records of the groups
+ *   that touch a ghost layer have been gathered: part_label [P] ASCENDING (dev), part_size [P] members (proxies
+ *   not counted), part_mass [P], part_com [P,3].  For each of the W groups `want` [W] whose canonical particle
+ *   this rank owns (ref [W,3] = its position) the records with that label are combined into out_size [W],
+ *   out_mass [W], out_com [W,3]: mass-weighted mean of the minimum-image displacements from the canonical
+ *   particle, re-wrapped (R11), float64.  All asynchronous on `stream`. */
+int fof_merge_labels_sparse(const int32_t *pairs, int64_t P, const int32_t *uniq, int64_t U, int32_t *parent,
+                            int32_t *labels, int64_t N, void *stream);
+int fof_combine_groups(const int32_t *want, int64_t W, const float *ref, float L, const int32_t *part_label, int64_t P,
+                       const int32_t *part_size, const float *part_mass, const float *part_com, int32_t *out_size,
+                       float *out_mass, float *out_com, void *stream);
 
 /* Halo decoration (section 3.1.1 "Decorated Frozen Assignment": "particle standard deviation
  * (sigma)" as the surrogate of halo mass; R23):

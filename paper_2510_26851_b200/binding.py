@@ -79,6 +79,10 @@ def lib():
         L.fof_component_min.argtypes = [vp, vp, i64, vp, vp, vp]
         L.fof_merge_labels.restype = ctypes.c_int
         L.fof_merge_labels.argtypes = [vp, i64, vp, i64, vp, i64, vp]
+        L.fof_merge_labels_sparse.restype = ctypes.c_int
+        L.fof_merge_labels_sparse.argtypes = [vp, i64, vp, i64, vp, vp, i64, vp]
+        L.fof_combine_groups.restype = ctypes.c_int
+        L.fof_combine_groups.argtypes = [vp, i64, vp, f32, vp, i64, vp, vp, vp, vp, vp, vp, vp]
         L.fof_group_sigma.restype = ctypes.c_int
         L.fof_group_sigma.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp]
         L.fof_groups_backward.restype = ctypes.c_int
@@ -237,6 +241,18 @@ def fof_component_min(labels, ids, tmp, out, stream=None):
 def fof_merge_labels(pairs, parent, labels, stream=None):
     _check(lib().fof_merge_labels(_ptr(pairs), int(pairs.shape[0]), _ptr(parent), int(parent.shape[0]), _ptr(labels),
                                   int(labels.shape[0]), _stream_ptr(stream)))
+
+
+def fof_merge_labels_sparse(pairs, uniq, parent, labels, stream=None):
+    """pairs: cuda int32 [P,2]; uniq: cuda int32 [U] ascending distinct labels of the pairs; parent: scratch [U]."""
+    _check(lib().fof_merge_labels_sparse(_ptr(pairs), int(pairs.shape[0]), _ptr(uniq), int(uniq.shape[0]), _ptr(parent),
+                                         _ptr(labels), int(labels.shape[0]), _stream_ptr(stream)))
+
+
+def fof_combine_groups(want, ref, L, part_label, part_size, part_mass, part_com, out_size, out_mass, out_com, stream=None):
+    _check(lib().fof_combine_groups(_ptr(want), int(want.shape[0]), _ptr(ref), _f(L), _ptr(part_label),
+                                    int(part_label.shape[0]), _ptr(part_size), _ptr(part_mass), _ptr(part_com),
+                                    _ptr(out_size), _ptr(out_mass), _ptr(out_com), _stream_ptr(stream)))
 
 
 def fof_group_sigma(h, pos, mass, particle_group, group_mass, group_com, K, ws, group_sigma, stream=None):

@@ -541,6 +541,27 @@ int fof_merge_labels(const int32_t *pairs, int64_t P, int32_t *parent, int64_t G
                                                                                                     : FOF_ERR_CUDA;
 }
 
+int fof_merge_labels_sparse(const int32_t *pairs, int64_t P, const int32_t *uniq, int64_t U, int32_t *parent,
+                            int32_t *labels, int64_t N, void *stream)
+{
+    if (P < 0 || U < 0 || N < 0 || U > 2147483647LL || (U > 0 && (!parent || !uniq)) || (P > 0 && !pairs) ||
+        (N > 0 && !labels))
+        return FOF_ERR_INVALID_ARG;
+    return launch_merge_labels_sparse(pairs, P, uniq, U, parent, labels, N, (cudaStream_t)stream) == cudaSuccess
+               ? FOF_OK : FOF_ERR_CUDA;
+}
+
+int fof_combine_groups(const int32_t *want, int64_t W, const float *ref, float L, const int32_t *part_label, int64_t P,
+                       const int32_t *part_size, const float *part_mass, const float *part_com, int32_t *out_size,
+                       float *out_mass, float *out_com, void *stream)
+{
+    if (W < 0 || P < 0 || P > 2147483647LL || !(L > 0.0f)) return FOF_ERR_INVALID_ARG;
+    if (W > 0 && (!want || !ref || !out_size || !out_mass || !out_com)) return FOF_ERR_INVALID_ARG;
+    if (P > 0 && (!part_label || !part_size || !part_mass || !part_com)) return FOF_ERR_INVALID_ARG;
+    return launch_combine_groups(want, W, ref, L, part_label, P, part_size, part_mass, part_com, out_size, out_mass,
+                                 out_com, (cudaStream_t)stream) == cudaSuccess ? FOF_OK : FOF_ERR_CUDA;
+}
+
 int fof_group_sigma(fof_handle *h, const float *pos, const float *mass, const int32_t *particle_group,
                     const float *group_mass, const float *group_com, int64_t K, void *ws, float *group_sigma,
                     void *stream)

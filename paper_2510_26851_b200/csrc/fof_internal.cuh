@@ -352,5 +352,10 @@ cudaError_t launch_layer_select(const float *pos, int64_t N, float L, int axis, 
 cudaError_t launch_component_min(const int *labels, const int *ids, int64_t N, int *tmp, int *out, cudaStream_t s);
 cudaError_t launch_merge_labels(const int *pairs, int64_t P, int *parent, int64_t G, int *labels, int64_t N,
                                 cudaStream_t s);
+cudaError_t launch_merge_labels_sparse(const int *pairs, int64_t P, const int *uniq, int64_t U, int *parent, int *labels,
+                                       int64_t N, cudaStream_t s);
+cudaError_t launch_combine_groups(const int *want, int64_t W, const float *ref, float L, const int *part_label, int64_t P,
+                                  const int *part_size, const float *part_mass, const float *part_com, int *out_size,
+                                  float *out_mass, float *out_com, cudaStream_t s);
 
 }  // namespace fof

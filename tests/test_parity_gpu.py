@@ -746,6 +746,51 @@ def test_slab_fof_equals_monolithic(B, world):
     assert crossing > nz // 2          # many particles whose canonical particle lives on another rank
 
 
+@pytest.mark.parametrize("world,weighted", [(2, False), (3, True), (4, True)])
+def test_slab_groups_against_oracle(B, world, weighted):
+    """Cross-rank group construction ("identical to a monolithic run" PAPER.md:180): the union of
+    the per-rank catalogues of a 2 / 3 / 4-slab run (all ranks played in turn on this GPU) is the oracle's
+    catalogue of the whole box: labels and sizes exact, masses 1e-5 relative, centres of mass 1e-5 L.  The set
+    holds groups inside one slab, groups across a slab face, across the box face in z, and a chain through every
+    slab whose canonical particle lives on one rank only."""
+    from paper_2510_26851_b200 import slab
+
+    w = inputs.scaled(inputs.CONFIGS["cfg1"], 48)
+    p = inputs.make_positions(w)
+    rng = np.random.default_rng(7 + world)
+    nz = int(w.L / (0.8 * w.b))
+    chain = np.stack([np.full(nz, 0.37 * w.L), np.full(nz, 0.61 * w.L), (np.arange(nz) + 0.5) * (w.L / nz)], 1)
+    p = np.concatenate([p, chain.astype(np.float32)])
+    p = p[rng.permutation(len(p))]
+    N = len(p)
+    mass = rng.uniform(0.5, 1.5, N).astype(np.float32) if weighted else None
+    N_min = 5
+    lab, _ = oracle.labels_cells(p, w.L, w.b)
+    og = oracle.groups(p, lab, w.L, N_min, mass=mass)
+    own = slab.split_into_slabs(p, w.L, world)
+    parts = [(torch.from_numpy(p[o]).cuda(), torch.from_numpy(o.astype(np.int32)).cuda()) for o in own]
+    masses = None if mass is None else [torch.from_numpy(mass[o]).cuda() for o in own]
+    labels, cats = slab.slab_fof_emulated(parts, w.L, w.b, N, N_min=N_min, masses=masses)
+    for o, l in zip(own, labels):
+        assert np.array_equal(l.cpu().numpy(), lab[o])
+    glab = np.concatenate([c["group_label"].cpu().numpy() for c in cats])
+    order = np.argsort(glab)
+    assert sum(c["K"] for c in cats) == og["K"]
+    assert np.array_equal(glab[order], og["group_label"]), "the ranks' catalogues do not add up to the oracle's"
+    for c, o in zip(cats, own):
+        assert np.isin(c["group_label"].cpu().numpy(), o).all(), "a rank lists a group whose canonical particle it does not own"
+    size = np.concatenate([c["group_size"].cpu().numpy() for c in cats])[order]
+    gm = np.concatenate([c["group_mass"].cpu().numpy() for c in cats])[order]
+    com = np.concatenate([c["group_com"].cpu().numpy() for c in cats])[order]
+    assert np.array_equal(size, og["group_size"])
+    assert np.all(np.abs(gm - og["group_mass"]) <= 1e-5 * og["group_mass"])
+    d = np.abs(com.astype(np.float64) - og["group_com"])
+    d = np.minimum(d, float(np.float32(w.L)) - d)
+    assert d.max() <= 1e-5 * w.L, f"centre of mass off by {d.max()}"
+    spanning = sum(int((~np.isin(lab[o], o)).any()) for o in own)
+    assert og["group_size"].max() >= nz and spanning >= world - 1   # the chain is one group over all slabs
+
+
 @pytest.mark.parametrize("grid", [3, 4, 5, 6, 7])
 def test_tiny_grids_wrap_everywhere(B, grid):
     """n = 3 .. 5 cells per axis: every stencil wraps and the minimum-image selects are live in both roles
