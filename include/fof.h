@@ -14,7 +14,8 @@
  *  - Every call returns FOF_OK (0) or a negative FOF_ERR_* code; no exceptions, no abort, no
  *    output on stdout/stderr.
  *  - Particle index type is int32 (N < 2^31).  Positions are float32, row-major [N,3]
- *    (PAPER.md:121, 189), any finite value (they are wrapped into [0,L)).
+ *    (PAPER.md:121, 189), any finite value (they are wrapped into [0,L); a coordinate beyond about
+ *    2^24 L in magnitude, where float32 can no longer resolve L, wraps to 0).
  *  - There is NO CPU fallback.  Without a CUDA device the compute calls return FOF_ERR_CUDA.
  */
 #ifndef FOF_B200_H
@@ -144,7 +145,8 @@ int fof_link_stochastic(fof_handle *h, float b_link, float alpha, uint64_t seed,
  * p_ij are evaluated once for four samples at a time; sample k gives exactly the labels, log p and
  * (to float32 summation order) the score function that fof_link_stochastic(sample + k) gives.
  *   S        1 .. 1024 samples; labels dev [S][N]; logp dev double [S]; grad_pos dev [S][N][3] or NULL.
- *   scratch  dev, fof_stochastic_scratch_bytes(h, S) bytes (one union-find array per sample), 4-B aligned.
+ *   scratch  dev, fof_stochastic_scratch_bytes(h, S) bytes (one union-find array of N entries per sample), 4-byte
+ *            aligned (16-byte alignment and N % 4 == 0 let the label pass use 128-bit loads; neither is required).
  * After the call fof_link_stats reports the potential edges (the same for every sample) as pair tests
  * and the sampled edges summed over the S samples as E.  Same call order rules as fof_link_stochastic.
  * Asynchronous on `stream`. */

@@ -45,7 +45,7 @@ float oracle_wrap1(float x, float L)
     float p = L * f;          /* rounded product: no FMA (-ffp-contract=off) */
     float w = x - p;
     if (w < 0.0f) w = w + L;
-    if (w >= L) w = 0.0f;
+    if (!(w >= 0.0f) || w >= L) w = 0.0f;  /* R6: |x| beyond ~2^24 L, where x - L floor(x/L) is off by whole ulps of x */
     return w;
 }
 

@@ -229,8 +229,20 @@ int fof_profile_enable(fof_handle *h, int slots)
         const int n = slots * kMaxStages * 2;
         h->ev = new (std::nothrow) cudaEvent_t[n];
         h->ev_valid = new (std::nothrow) bool[slots * kMaxStages]();
-        if (!h->ev || !h->ev_valid) return FOF_ERR_INVALID_ARG;
-        for (int k = 0; k < n; ++k) CK(cudaEventCreate(&h->ev[k]), "cudaEventCreate");
+        if (!h->ev || !h->ev_valid) {
+            delete[] h->ev; delete[] h->ev_valid;
+            h->ev = nullptr; h->ev_valid = nullptr;
+            return FOF_ERR_INVALID_ARG;
+        }
+        for (int k = 0; k < n; ++k) {
+            const cudaError_t e = cudaEventCreate(&h->ev[k]);
+            if (e != cudaSuccess) {  // give back what was created
+                for (int j = 0; j < k; ++j) (void)cudaEventDestroy(h->ev[j]);
+                delete[] h->ev; delete[] h->ev_valid;
+                h->ev = nullptr; h->ev_valid = nullptr;
+                return cuda_fail(h, e, "cudaEventCreate");
+            }
+        }
         h->prof_cur = slots - 1;
         h->prof_slots = slots;
     }
@@ -614,6 +626,8 @@ int fof_run_host(fof_handle *h, const float *pos_host, const float *mass_host, i
 {
     if (!h || !dev_buf || ((uintptr_t)dev_buf & 255) || !K_host || cap < 0) return FOF_ERR_INVALID_ARG;
     if (h->N > 0 && (!pos_host || !labels_host)) return FOF_ERR_INVALID_ARG;
+    if (cap > 0 && (!group_label_host || !group_size_host || !group_mass_host || !group_com_host))
+        return FOF_ERR_INVALID_ARG;
     cudaStream_t s = (cudaStream_t)stream;
     const size_t N = (size_t)h->N;
     char *p = static_cast<char *>(dev_buf);
@@ -630,36 +644,48 @@ int fof_run_host(fof_handle *h, const float *pos_host, const float *mass_host, i
     if (N && mass_host) CK(cudaMemcpyAsync(mass, mass_host, N * sizeof(float), cudaMemcpyHostToDevice, s), "H2D mass");
     int rc = fof_link(h, pos, labels, ws, s);
     if (rc != FOF_OK) return rc;
+    // From here on a copy into the caller's labels buffer may be in flight on copy_stream: every return goes
+    // through `done`, which waits for it.
+    bool copying = false;
+    auto done = [&](int code) {
+        if (copying) (void)cudaStreamSynchronize(h->copy_stream);
+        return code;
+    };
+#define CKD(call, where)                                          \
+    do {                                                          \
+        cudaError_t e__ = (call);                                 \
+        if (e__ != cudaSuccess) return done(cuda_fail(h, e__, where)); \
+    } while (0)
     if (N) {  // the labels travel while the groups are built (fof_groups only reads them)
         if (!h->copy_stream) {
-            CK(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking), "cudaStreamCreate");
-            CK(cudaEventCreateWithFlags(&h->ev_linked, cudaEventDisableTiming), "cudaEventCreate");
+            CKD(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking), "cudaStreamCreate");
+            CKD(cudaEventCreateWithFlags(&h->ev_linked, cudaEventDisableTiming), "cudaEventCreate");
         }
-        CK(cudaEventRecord(h->ev_linked, s), "cudaEventRecord");
-        CK(cudaStreamWaitEvent(h->copy_stream, h->ev_linked, 0), "cudaStreamWaitEvent");
-        CK(cudaMemcpyAsync(labels_host, labels, N * sizeof(int), cudaMemcpyDeviceToHost, h->copy_stream), "D2H labels");
+        CKD(cudaEventRecord(h->ev_linked, s), "cudaEventRecord");
+        CKD(cudaStreamWaitEvent(h->copy_stream, h->ev_linked, 0), "cudaStreamWaitEvent");
+        copying = true;
+        CKD(cudaMemcpyAsync(labels_host, labels, N * sizeof(int), cudaMemcpyDeviceToHost, h->copy_stream), "D2H labels");
     }
     rc = fof_groups(h, pos, mass_host ? mass : nullptr, labels, ws, glabel, gsize, gmass, gcom,
                     particle_group_host ? pgroup : nullptr, cap, K_host, s);
-    if (rc != FOF_OK) {
-        if (N) (void)cudaStreamSynchronize(h->copy_stream);  // no copy into the caller's buffer after the return
-        return rc;
-    }
+    if (rc != FOF_OK) return done(rc);
     const size_t K = (size_t)*K_host;
     if (K) {
-        CK(cudaMemcpyAsync(group_label_host, glabel, K * sizeof(int), cudaMemcpyDeviceToHost, s), "D2H group_label");
-        CK(cudaMemcpyAsync(group_size_host, gsize, K * sizeof(int), cudaMemcpyDeviceToHost, s), "D2H group_size");
-        CK(cudaMemcpyAsync(group_mass_host, gmass, K * sizeof(float), cudaMemcpyDeviceToHost, s), "D2H group_mass");
-        CK(cudaMemcpyAsync(group_com_host, gcom, K * 3 * sizeof(float), cudaMemcpyDeviceToHost, s), "D2H group_com");
+        CKD(cudaMemcpyAsync(group_label_host, glabel, K * sizeof(int), cudaMemcpyDeviceToHost, s), "D2H group_label");
+        CKD(cudaMemcpyAsync(group_size_host, gsize, K * sizeof(int), cudaMemcpyDeviceToHost, s), "D2H group_size");
+        CKD(cudaMemcpyAsync(group_mass_host, gmass, K * sizeof(float), cudaMemcpyDeviceToHost, s), "D2H group_mass");
+        CKD(cudaMemcpyAsync(group_com_host, gcom, K * 3 * sizeof(float), cudaMemcpyDeviceToHost, s), "D2H group_com");
     }
     if (N && particle_group_host)
-        CK(cudaMemcpyAsync(particle_group_host, pgroup, N * sizeof(int), cudaMemcpyDeviceToHost, s), "D2H particle_group");
-    CK(cudaStreamSynchronize(s), "sync");
-    if (N) CK(cudaStreamSynchronize(h->copy_stream), "sync labels copy");
+        CKD(cudaMemcpyAsync(particle_group_host, pgroup, N * sizeof(int), cudaMemcpyDeviceToHost, s), "D2H particle_group");
+    CKD(cudaStreamSynchronize(s), "sync");
+    if (copying) CKD(cudaStreamSynchronize(h->copy_stream), "sync labels copy");
+    copying = false;
     Ctrl c;
     CK(cudaMemcpy(&c, at<Ctrl>(ws, h->off_ctrl), sizeof(Ctrl), cudaMemcpyDeviceToHost), "copy ctrl");
     if (c.error & 1u) return FOF_ERR_NONFINITE;
     return FOF_OK;
+#undef CKD
 }
 
 int fof_status(fof_handle *h, void *ws, void *stream)

@@ -168,7 +168,7 @@ __device__ __forceinline__ float wrap1(float x, float L)
     float t = __fdiv_rn(x, L);
     float w = __fsub_rn(x, __fmul_rn(L, floorf(t)));
     if (w < 0.0f) w = __fadd_rn(w, L);
-    if (w >= L) w = 0.0f;
+    if (!(w >= 0.0f) || w >= L) w = 0.0f;  // |x| beyond ~2^24 L: x - L floor(x / L) is off by whole ulps of x (R6)
     return w;
 }
 

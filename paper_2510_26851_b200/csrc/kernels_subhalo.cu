@@ -172,8 +172,11 @@ __device__ __forceinline__ SubBox sub_box(const float *p, bool valid)
     SubBox bx;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        bx.lo[a] = __reduce_min_sync(0xffffffffu, valid ? __float_as_uint(p[a]) : 0xffffffffu);
-        bx.hi[a] = __reduce_max_sync(0xffffffffu, valid ? __float_as_uint(p[a]) : 0u);
+        // wrapped coordinates are >= 0, so their bit patterns order like the values -- except -0.0f (wrap1 returns it
+        // unchanged), which + 0.0f turns into +0.0f
+        const unsigned int bits = __float_as_uint(__fadd_rn(p[a], 0.0f));
+        bx.lo[a] = __reduce_min_sync(0xffffffffu, valid ? bits : 0xffffffffu);
+        bx.hi[a] = __reduce_max_sync(0xffffffffu, valid ? bits : 0u);
     }
     return bx;
 }

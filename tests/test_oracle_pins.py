@@ -54,6 +54,20 @@ def test_wrap_identity_and_edges():
     assert d.max() < 1e-4                           # x mod L up to float32 rounding of x/L
 
 
+def test_wrap_of_huge_coordinates_lands_in_the_box():
+    """R6: beyond |x| ~ 2^24 L float32 cannot resolve L any more (x - L floor(x / L) is off by whole ulps of x); the
+    result must still be a coordinate in [0, L), whatever it is (0 where even the +L fix-up does not reach)."""
+    L = np.float32(3.7)
+    x = np.array([-3e9, 3e9, -1e12, 1e12, -2.5e8, 7e10, -3.4e38, 3.4e38, -6.2e7, 6.2e7], dtype=np.float32)
+    w = oracle.wrap(np.stack([x, x, x], 1), float(L))[:, 0]
+    assert (w >= 0).all() and (w < L).all()
+    # where float32 still resolves the box (|x| < 2^24 L = 6.2e7), the result is x mod L to rounding
+    xs = np.array([-6.1e6, 6.1e6, -123456.7, 98765.4], dtype=np.float32)
+    ws = oracle.wrap(np.stack([xs, xs, xs], 1), float(L))[:, 0]
+    d = np.abs(ws - np.mod(xs.astype(np.float64), float(L)))
+    assert np.minimum(d, float(L) - d).max() < 1.0    # off by at most an ulp of x (0.5 at 6e6)
+
+
 def test_wrap_nonfinite_is_an_error():
     p = np.zeros((4, 3), np.float32)
     p[2, 1] = np.nan

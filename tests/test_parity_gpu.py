@@ -123,6 +123,7 @@ def test_against_brute_force(B, case):
     else:  # positions far outside [0, L): the wrap is part of the path
         L, b = 3.7, 0.2
         p = (rng.standard_normal((3000, 3)) * 9).astype(np.float32)
+        p[:40] *= np.float32(1e9)   # and some beyond 2^24 L, where float32 no longer resolves the box (R6)
     for grid in (None, 3, "max"):
         if grid == "max":
             grid = int(np.floor(L / (float(np.float32(b)) * 1.001)))
