@@ -407,8 +407,9 @@ int fof_link_stats(fof_handle *h, void *ws, void *stream, uint64_t *edges_host, 
     }
     CK(cudaMemcpyAsync(&c, ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, s), "copy ctrl");
     CK(cudaStreamSynchronize(s), "sync");
-    if (edges_host) *edges_host = c.edges;
-    if (pair_tests_host) *pair_tests_host = c.pair_tests;
+    const bool blocks = !h->linked_cells && c.mode == 0u;  // the block path did the work: its counters count
+    if (edges_host) *edges_host = blocks ? c.edges_b : c.edges;
+    if (pair_tests_host) *pair_tests_host = blocks ? c.pair_tests_b : c.pair_tests;
     if (grid_pairs_host) *grid_pairs_host = c.grid_pairs;
     return FOF_OK;
 }

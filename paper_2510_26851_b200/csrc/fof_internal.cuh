@@ -43,6 +43,8 @@ struct Ctrl {
     unsigned int tile_ticket2;      // block path: next input tile of block_scatter_kernel
     unsigned int max_block;         // block path: records (own + ghost) of the fullest block
     unsigned int pad1[3];
+    unsigned long long edges_b;      // block path: true edges / distance tests of block_link_kernel (kept apart from the
+    unsigned long long pair_tests_b; // cell path's: after a late fall-back both kernels have counted)
 };
 static_assert(sizeof(Ctrl) <= 256, "Ctrl must fit its 256-byte slot");
 

@@ -619,7 +619,8 @@ __device__ __forceinline__ void link_phase(const BlockView &v, unsigned int nite
 __global__ void __launch_bounds__(kBlockThreads, 2) block_link_kernel(const float4 *__restrict__ part,
                                                                       const unsigned int *__restrict__ cursor,
                                                                       unsigned int cap, Grid g, BlockGeom bg, int *labels,
-                                                                      int2 *__restrict__ cross, Ctrl *ctrl)
+                                                                      int2 *__restrict__ cross, unsigned int cross_cap,
+                                                                      Ctrl *ctrl)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     BlockView v;
@@ -761,7 +762,12 @@ __global__ void __launch_bounds__(kBlockThreads, 2) block_link_kernel(const floa
             unsigned int at = 0;
             if (lane == 0) at = atomicAdd(&ctrl->ncross, (unsigned int)__popc(bal));
             at = __shfl_sync(kFull, at, 0);
-            if (emit) cross[at + __popc(bal & ((1u << lane) - 1u))] = make_int2((int)me_o, (int)root_o);
+            if (emit) {
+                const unsigned int k = at + (unsigned int)__popc(bal & ((1u << lane) - 1u));
+                if (k < cross_cap) cross[k] = make_int2((int)me_o, (int)root_o);
+                else ctrl->mode = 1u;  // more linked ghosts than the list holds (tiny blocks): the cell path takes over --
+                                       // it rewrites labels and counters from scratch, so what this kernel wrote is moot
+            }
         }
     }
     nedges = __reduce_add_sync(kFull, nedges);
@@ -771,8 +777,8 @@ __global__ void __launch_bounds__(kBlockThreads, 2) block_link_kernel(const floa
     DBG_T(tE);
     DBG_ADD(3, tD, tE);
     if (tid == 0) {
-        if (s_red[0]) atomicAdd(&ctrl->edges, (unsigned long long)s_red[0]);
-        if (s_red[1]) atomicAdd(&ctrl->pair_tests, (unsigned long long)s_red[1]);
+        if (s_red[0]) atomicAdd(&ctrl->edges_b, (unsigned long long)s_red[0]);
+        if (s_red[1]) atomicAdd(&ctrl->pair_tests_b, (unsigned long long)s_red[1]);
     }
 }
 
@@ -794,7 +800,7 @@ __device__ __forceinline__ int find_g(int *lab, int x)
 __global__ void __launch_bounds__(kBlock) cross_link_kernel(const int2 *__restrict__ cross, int *labels, Ctrl *ctrl)
 {
     if (*(volatile unsigned int *)&ctrl->mode) return;
-    const unsigned int n = *(volatile unsigned int *)&ctrl->ncross;
+    const unsigned int n = *(volatile unsigned int *)&ctrl->ncross;  // <= the list's capacity, or mode is set
     for (unsigned int k = blockIdx.x * kBlock + threadIdx.x; k < n; k += gridDim.x * kBlock) {
         const int2 e = cross[k];
         int ra = find_g(labels, e.x), rb = find_g(labels, e.y);
@@ -898,7 +904,8 @@ cudaError_t launch_block_path(const float *pos, int64_t N, Grid g, const BlockGe
     hook.end(0);
     if (getenv("FOF_DEBUG_SYNC")) { e = cudaStreamSynchronize(s); fprintf(stderr, "[fof] after scatter: %s\n", cudaGetErrorString(e)); if (e != cudaSuccess) return e; }
     hook.begin(1, 1);
-    block_link_kernel<<<bg.bins, kBlockThreads, smem_link, s>>>(part, cursor, (unsigned int)kBlockCap, g, bg, labels, cross, ctrl);
+    block_link_kernel<<<bg.bins, kBlockThreads, smem_link, s>>>(part, cursor, (unsigned int)kBlockCap, g, bg, labels, cross,
+                                                                (unsigned int)(N + 1), ctrl);
     hook.end(1);
     if (getenv("FOF_DEBUG_SYNC")) { e = cudaStreamSynchronize(s); Ctrl hc; cudaMemcpy(&hc, ctrl, sizeof(hc), cudaMemcpyDeviceToHost); fprintf(stderr, "[fof] after block_link: %s mode %u ncross %u max_block %u N %lld\n", cudaGetErrorString(e), hc.mode, hc.ncross, hc.max_block, (long long)N); if (e != cudaSuccess) return e; }
     hook.begin(2, 1);

@@ -267,6 +267,22 @@ def test_one_dense_clump_many_per_cell(B):
     check_against_oracle(B, p, L, b, 20)
 
 
+def test_block_path_falls_back_in_the_same_call(B):
+    """The two ways the block path gives up, both decided on the device inside fof_link: (1) a block holds more
+    records than a CTA keeps in shared memory (one clump of 20 000 in a few cells); (2) more linked ghosts than the
+    equivalence list holds (blocks of 2 cells with b ~ the cell side: nearly every particle is a ghost of seven
+    blocks).  Either way the cell path runs in the same call and the results are the oracle's."""
+    rng = np.random.default_rng(35)
+    clump = rng.standard_normal((20000, 3)) * 1.5 + 50.0
+    bg = rng.random((20000, 3)) * 100.0
+    p1 = (np.concatenate([bg, clump]) % 100.0).astype(np.float32)
+    p2 = (rng.random((20000, 3)) * 10.0).astype(np.float32)
+    for p, L, b in ((p1, 100.0, 1.0), (p2, 10.0, 1.0)):
+        got, lab, og = check_against_oracle(B, p, L, b, 20, paths=("blocks",))
+        assert got["ran"][1] > 0, "the plan should admit the block path"
+        assert got["ran"][0] == "cells", "expected the fallback to the cell path"
+
+
 # --------------------------------------------------------------------------- invariants
 def test_permutation_invariance_on_gpu(B):
     w = inputs.scaled(inputs.CONFIGS["cfg1"], 40)
