@@ -106,6 +106,7 @@ void layout(fof_handle *h)
                                        (double)h->n * 9.5367431640625e-07), 2.0f);
     h->linked = false;
     h->linked_ws = nullptr;
+    h->counted = false;
 }
 
 int cuda_fail(fof_handle *h, cudaError_t e, const char *where)
@@ -476,6 +477,7 @@ int fof_link_stochastic(fof_handle *h, float b_link, float alpha, uint64_t seed,
     if (h->N > 0 && !labels) return FOF_ERR_INVALID_ARG;
     if (!h->linked || h->linked_ws != ws || !h->linked_cells) return FOF_ERR_STATE;  // needs the cell sort of a fof_link on (h, ws)
     cudaStream_t s = (cudaStream_t)stream;
+    h->counted = false;  // the caller may be overwriting the labels buffer whose group sizes were counted
     h->launches += h->N > 0 ? 3 : 0;
     CK(launch_link_stochastic(at<float4>(ws, h->off_sorted), h->N, h->grid, at<unsigned int>(ws, h->off_cell),
                               at<int>(ws, h->off_idx), at<unsigned int>(ws, h->off_rel), b_link, alpha, seed, sample,
@@ -497,6 +499,7 @@ int fof_link_stochastic_batch(fof_handle *h, float b_link, float alpha, uint64_t
     if (h->N > 0 && (!labels || !scratch || ((uintptr_t)scratch & 3))) return FOF_ERR_INVALID_ARG;
     if (!h->linked || h->linked_ws != ws || !h->linked_cells) return FOF_ERR_STATE;  // needs the cell sort of a fof_link on (h, ws)
     cudaStream_t s = (cudaStream_t)stream;
+    h->counted = false;
     h->launches += h->N > 0 ? (unsigned long long)(S / 4 + S % 4 + 2 * S) : 0;
     CK(launch_link_stochastic_batch(at<float4>(ws, h->off_sorted), h->N, h->grid, at<unsigned int>(ws, h->off_cell),
                                     at<int>(ws, h->off_idx), static_cast<unsigned int *>(scratch), b_link, alpha, seed,

@@ -607,6 +607,25 @@ def test_stochastic_batch_equals_single_samples_and_oracle(B, S, drop):
     f.close()
 
 
+def test_groups_recounts_after_the_labels_buffer_was_reused(B):
+    """fof_groups re-uses the sizes fof_link counted only for the labels fof_link wrote: once a stochastic sample has
+    been written into the same buffer, the groups are those of the sample (counted afresh)."""
+    w = inputs.scaled(inputs.CONFIGS["cfg1"], 32)
+    p = inputs.make_positions(w)
+    f = B.FoF(len(p), w.L, w.b, w.N_min, path="cells")
+    dpos = torch.from_numpy(p).cuda()
+    labels = f.link(dpos)
+    logp = torch.zeros(1, dtype=torch.float64, device="cuda")
+    B.fof_link_stochastic(f.h, w.b, 0.5, 11, 0, labels, logp, None, f.ws)      # overwrites `labels`
+    g = f.groups(dpos, labels)
+    lab = labels.cpu().numpy()
+    og = oracle.groups(p, lab, w.L, w.N_min)
+    det, _ = oracle.labels_cells(p, w.L, w.b)
+    assert not np.array_equal(lab, det), "alpha = 0.5 should drop edges"
+    assert g["K"] == og["K"] and np.array_equal(g["group_size"].cpu().numpy(), og["group_size"])
+    f.close()
+
+
 def test_stochastic_link_wraps_and_needs_a_link_first(B):
     rng = np.random.default_rng(17)
     L, b = 8.0, 1.0
