@@ -20,9 +20,6 @@
 //                         (ghost, local root) per linked ghost
 //   cross_link_kernel     unions of the listed equivalences on `labels` (global lock-free union-find)
 //   flatten_labels_kernel labels[i] = root(i)
-#include <stdio.h>
-#include <stdlib.h>
-
 #include "fof_internal.cuh"
 
 namespace fof {
@@ -112,63 +109,6 @@ __device__ __forceinline__ void wrap3(float &x, float &y, float &z, const Grid &
 #endif
 constexpr int kScatThreads = FOF_SCAT_THREADS, kScatPer = FOF_SCAT_PER;
 
-#ifdef FOF_SCAT_DIRECT
-// direct variant: one global atomic per record on its block's cursor, no shared memory, no barriers
-template <bool VEC>
-__global__ void __launch_bounds__(256) block_scatter_kernel(const float *__restrict__ pos, int64_t N, Grid g,
-                                                            BlockGeom bg, unsigned int *cursor,
-                                                            float4 *__restrict__ part, unsigned int cap,
-                                                            int *__restrict__ labels, bool labels_vec, int *__restrict__ cnt,
-                                                            Ctrl *ctrl)
-{
-    bool bad = false, over = false;
-    for (int64_t i = ((int64_t)blockIdx.x * 256 + threadIdx.x) * 4; i < N; i += (int64_t)gridDim.x * 256 * 4) {
-        float4 rec[4];
-        if (VEC && i + 4 <= N) {
-            const float4 *p = reinterpret_cast<const float4 *>(pos + 3 * i);
-            const float4 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
-            rec[0] = make_float4(a.x, a.y, a.z, __int_as_float((int)i));
-            rec[1] = make_float4(a.w, b.x, b.y, __int_as_float((int)i + 1));
-            rec[2] = make_float4(b.z, b.w, c.x, __int_as_float((int)i + 2));
-            rec[3] = make_float4(c.y, c.z, c.w, __int_as_float((int)i + 3));
-        } else {
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const int64_t j = i + k;
-                rec[k] = j < N ? make_float4(__ldg(pos + 3 * j), __ldg(pos + 3 * j + 1), __ldg(pos + 3 * j + 2), __int_as_float((int)j))
-                               : make_float4(0.f, 0.f, 0.f, __int_as_float(-1));
-            }
-        }
-        if (labels_vec && i + 4 <= N) *reinterpret_cast<int4 *>(labels + i) = make_int4((int)i, (int)i + 1, (int)i + 2, (int)i + 3);
-        else
-            for (int k = 0; k < 4; ++k) if (i + k < N) labels[i + k] = (int)(i + k);
-        for (int k = 0; k < 4; ++k) if (i + k < N) cnt[i + k] = 0;
-        unsigned int bin[4], at[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            bin[k] = 0xffffffffu;
-            if (__float_as_int(rec[k].w) >= 0) {
-                wrap3(rec[k].x, rec[k].y, rec[k].z, g, bad);
-                const float4 r = rec[k];
-                bin[k] = classify(r.x, r.y, r.z, g, bg, [&](unsigned int gb) {
-                    const unsigned int a2 = atomicAdd(&cursor[gb], 1u);
-                    if (a2 < cap) part[(size_t)gb * cap + a2] = make_float4(r.x, r.y, r.z, __uint_as_float(__float_as_uint(r.w) | kGhostBit));
-                    else over = true;
-                });
-                at[k] = atomicAdd(&cursor[bin[k]], 1u);
-            }
-        }
-#pragma unroll
-        for (int k = 0; k < 4; ++k)
-            if (bin[k] != 0xffffffffu) {
-                if (at[k] < cap) part[(size_t)bin[k] * cap + at[k]] = rec[k];
-                else over = true;
-            }
-    }
-    if (bad) atomicOr(&ctrl->error, 1u);
-    if (over) ctrl->mode = 1u;
-}
-#else
 template <bool VEC>
 __global__ void __launch_bounds__(kScatThreads, FOF_SCAT_MINB) block_scatter_kernel(const float *__restrict__ pos, int64_t N, Grid g,
                                                                      BlockGeom bg, unsigned int *cursor,
@@ -257,8 +197,6 @@ __global__ void __launch_bounds__(kScatThreads, FOF_SCAT_MINB) block_scatter_ker
     if (bad) atomicOr(&ctrl->error, 1u);
     if (over) ctrl->mode = 1u;
 }
-
-#endif
 
 // ---------------------------------------------------------------------------------------------------------
 // block_link_kernel
@@ -403,7 +341,7 @@ __device__ __forceinline__ void chunk_role(const BlockView &v, int s0, const Gri
                                            const BlockOrigin &o, int lane, unsigned int &nedges, unsigned int &ntests)
 {
     const float lo = g.reach, hi = 1.0f - g.reach;
-    const int X = bg.X, XY = bg.X * bg.Y;
+    const int X = bg.X;
     const float4 *rec = v.rec;
     const unsigned int *cbeg = v.cbeg;
     const int s = s0 + lane;
@@ -895,28 +833,20 @@ cudaError_t launch_block_path(const float *pos, int64_t N, Grid g, const BlockGe
     if ((e = set_smem((const void *)block_link_kernel, smem_link)) != cudaSuccess) return e;
     hook.begin(0, 1);
     if ((e = cudaMemsetAsync(cursor, 0, smem_bins, s)) != cudaSuccess) return e;
-#ifdef FOF_SCAT_DIRECT
-    scat<<<FOF_SCAT_CTAS * ctas, 256, 0, s>>>(pos, N, g, bg, cursor, part, (unsigned int)kBlockCap, labels, labels_vec, cnt, ctrl);
-#else
     scat<<<FOF_SCAT_CTAS * ctas, kScatThreads, smem_bins, s>>>(pos, N, g, bg, cursor, part, (unsigned int)kBlockCap, labels,
                                                               labels_vec, cnt, ctrl);
-#endif
     hook.end(0);
-    if (getenv("FOF_DEBUG_SYNC")) { e = cudaStreamSynchronize(s); fprintf(stderr, "[fof] after scatter: %s\n", cudaGetErrorString(e)); if (e != cudaSuccess) return e; }
     hook.begin(1, 1);
     block_link_kernel<<<bg.bins, kBlockThreads, smem_link, s>>>(part, cursor, (unsigned int)kBlockCap, g, bg, labels, cross,
                                                                 (unsigned int)(N + 1), ctrl);
     hook.end(1);
-    if (getenv("FOF_DEBUG_SYNC")) { e = cudaStreamSynchronize(s); Ctrl hc; cudaMemcpy(&hc, ctrl, sizeof(hc), cudaMemcpyDeviceToHost); fprintf(stderr, "[fof] after block_link: %s mode %u ncross %u max_block %u N %lld\n", cudaGetErrorString(e), hc.mode, hc.ncross, hc.max_block, (long long)N); if (e != cudaSuccess) return e; }
     hook.begin(2, 1);
     cross_link_kernel<<<2 * ctas, kBlock, 0, s>>>(cross, labels, ctrl);
     hook.end(2);
-    if (getenv("FOF_DEBUG_SYNC")) { e = cudaStreamSynchronize(s); fprintf(stderr, "[fof] after cross_link: %s\n", cudaGetErrorString(e)); if (e != cudaSuccess) return e; }
     hook.begin(3, 1);
     flatten_labels_kernel<<<(unsigned int)((N + 4 * kBlock - 1) / (4 * kBlock)), kBlock, 0, s>>>(labels, N, labels_vec, ctrl, cnt, state,
                                                                                                  state_items);
     hook.end(3);
-    if (getenv("FOF_DEBUG_SYNC")) { e = cudaStreamSynchronize(s); fprintf(stderr, "[fof] after flatten: %s\n", cudaGetErrorString(e)); if (e != cudaSuccess) return e; }
     return cudaGetLastError();
 }
 
