@@ -577,6 +577,17 @@ def run_ours(args):
                "sample": f"full workload {w.name} (N={N}), 1 pass, {t_cpu:.2f} s, host has {os.cpu_count()} cores"}
         parity = bool(np.array_equal(labels.cpu().numpy(), lab) and E == E_ref and K_groups == og["K"]
                       and np.array_equal(out["group_size"][:K_groups].cpu().numpy(), og["group_size"]))
+        # second CPU figure: the same oracle with its pair search on all host cores (per-slab edge
+        # buffers, serial union); labels must equal the single-thread pass
+        import oracle
+
+        cores = os.cpu_count() or 1
+        t0 = time.perf_counter()
+        lab_mt, E_mt = oracle.labels_cells_threads(pos_np, w.L, w.b, cores)
+        oracle.groups(pos_np, lab_mt, w.L, w.N_min)
+        t_mt = time.perf_counter() - t0
+        cpu["all_cores"] = {"value": N / t_mt, "unit": UNIT, "cores": cores, "kind": "oracle, pair search on all cores + serial union",
+                            "seconds": round(t_mt, 3), "labels_equal_single_thread": bool(np.array_equal(lab_mt, lab) and E_mt == E_ref)}
 
     t_pairs = stages.get("link.pairs") or stages.get("block.link")
     line = {

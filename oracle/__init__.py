@@ -20,7 +20,7 @@ _SRC2 = os.path.join(_HERE, "fof_oracle_stochastic.c")  # NEXT-3: stochastic-edg
 _SRC3 = os.path.join(_HERE, "fof_oracle_subhalo.c")     # NEXT-4: six-dimensional sub-halo pass
 _LIB = os.path.join(_HERE, "libfof_oracle.so")
 # -ffp-contract=off: the float32 link predicate must not be contracted into FMAs.
-CFLAGS = ["-O2", "-std=c99", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC"]
+CFLAGS = ["-O2", "-std=c99", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC"]
 
 _lib = None
 
@@ -52,6 +52,9 @@ def _load():
         for fn in (lib.oracle_labels_brute, lib.oracle_labels_cells):
             fn.restype = ctypes.c_int
             fn.argtypes = [f32p, ctypes.c_int64, ctypes.c_float, ctypes.c_float, i32p, u64p]
+        lib.oracle_labels_cells_threads.restype = ctypes.c_int
+        lib.oracle_labels_cells_threads.argtypes = [f32p, ctypes.c_int64, ctypes.c_float, ctypes.c_float, i32p, u64p,
+                                                    ctypes.c_int32]
         lib.oracle_groups.restype = ctypes.c_int64
         lib.oracle_groups.argtypes = [f32p, f32p, i32p, ctypes.c_int64, ctypes.c_float, ctypes.c_int32,
                                       ctypes.c_int64, i32p, i32p, f64p, f64p, i32p]
@@ -146,6 +149,18 @@ def labels_brute(pos, L: float, b: float):
 def labels_cells(pos, L: float, b: float):
     """(labels int32 [N], E) by cell list + sequential union-find."""
     return _labels(_load().oracle_labels_cells, pos, L, b)
+
+
+def labels_cells_threads(pos, L: float, b: float, threads: int):
+    """(labels, E) like labels_cells, the pair search on `threads` host threads (serial union step): only for the
+    all-cores CPU figure of bench.py; parity uses labels_cells."""
+    pos, p = _pos(pos)
+    N = pos.shape[0]
+    labels = np.empty(N, dtype=np.int32)
+    E = ctypes.c_uint64(0)
+    fn = _load().oracle_labels_cells_threads
+    _check(fn(p, N, _f(L), _f(b), labels.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), ctypes.byref(E), int(threads)))
+    return labels, int(E.value)
 
 
 def groups(pos, labels, L: float, N_min: int, mass=None):

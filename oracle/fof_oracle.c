@@ -220,6 +220,105 @@ int oracle_labels_cells(const float *pos, int64_t N, float L, float b, int32_t *
     return ORACLE_OK;
 }
 
+/* ---- the same linker with the PAIR SEARCH on several host threads ("a second figure with the
+ * pair search OpenMP-parallel over cell slabs (per-thread edge buffers, serial union) on all host cores, labels
+ * required identical to the single-thread oracle").  Same grid, same stencil, same predicate, same union-find;
+ * only the order in which the edges reach the union-find differs, and the root of a set is its minimum index
+ * whatever that order is.  It exists for the all-cores CPU figure of bench.py; parity uses oracle_labels_cells. */
+typedef struct { int32_t i, j; } edge_t;
+
+int oracle_labels_cells_threads(const float *pos, int64_t N, float L, float b, int32_t *labels, uint64_t *E_out,
+                                int32_t threads)
+{
+    if (N < 0 || N > 2147483647LL || !(L > 0.0f) || !(b > 0.0f) || threads < 1) return ORACLE_ERR_ARG;
+    int64_t n = oracle_grid_n(N, L, b);
+    if (n < 3) return oracle_labels_cells(pos, N, L, b, labels, E_out);
+    float *w = (float *)malloc(sizeof(float) * 3 * (size_t)(N > 0 ? N : 1));
+    if (!w) return ORACLE_ERR_NOMEM;
+    int rc = oracle_wrap(pos, N, L, w);
+    if (rc) { free(w); return rc; }
+    for (int64_t i = 0; i < N; ++i) labels[i] = (int32_t)i;
+    int64_t C = n * n * n;
+    int32_t *cell = (int32_t *)malloc(sizeof(int32_t) * (size_t)(N > 0 ? N : 1));
+    int32_t *start = (int32_t *)calloc((size_t)C + 1, sizeof(int32_t));
+    int32_t *order = (int32_t *)malloc(sizeof(int32_t) * (size_t)(N > 0 ? N : 1));
+    int32_t *fill = (int32_t *)malloc(sizeof(int32_t) * (size_t)C);
+    edge_t **ebuf = (edge_t **)calloc((size_t)n, sizeof(edge_t *));   /* one edge buffer per z slab of cells */
+    int64_t *ecnt = (int64_t *)calloc((size_t)n, sizeof(int64_t));
+    if (!cell || !start || !order || !fill || !ebuf || !ecnt) {
+        free(w); free(cell); free(start); free(order); free(fill); free(ebuf); free(ecnt);
+        return ORACLE_ERR_NOMEM;
+    }
+    double s = (double)n / (double)L;
+    for (int64_t i = 0; i < N; ++i) {
+        int64_t c3[3];
+        for (int k = 0; k < 3; ++k) {
+            int64_t c = (int64_t)floor((double)w[3 * i + k] * s);
+            if (c < 0) c = 0;
+            if (c > n - 1) c = n - 1;
+            c3[k] = c;
+        }
+        cell[i] = (int32_t)(c3[0] + n * (c3[1] + n * c3[2]));
+        start[cell[i] + 1]++;
+    }
+    for (int64_t c = 0; c < C; ++c) start[c + 1] += start[c];
+    memcpy(fill, start, sizeof(int32_t) * (size_t)C);
+    for (int64_t i = 0; i < N; ++i) order[fill[cell[i]]++] = (int32_t)i;
+    free(fill);
+    int failed = 0;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(dynamic, 1) num_threads(threads)
+#endif
+    for (int64_t cz = 0; cz < n; ++cz) {
+        int64_t capz = 1024, cnt = 0;
+        edge_t *buf = (edge_t *)malloc(sizeof(edge_t) * (size_t)capz);
+        for (int64_t cy = 0; cy < n && buf; ++cy)
+        for (int64_t cx = 0; cx < n && buf; ++cx) {
+            int64_t c = cx + n * (cy + n * cz);
+            if (start[c] == start[c + 1]) continue;
+            for (int dz = -1; dz <= 1; ++dz)
+            for (int dy = -1; dy <= 1; ++dy)
+            for (int dx = -1; dx <= 1; ++dx) {
+                int64_t mx = (cx + dx + n) % n, my = (cy + dy + n) % n, mz = (cz + dz + n) % n;
+                int64_t m = mx + n * (my + n * mz);
+                for (int32_t p = start[c]; p < start[c + 1] && buf; ++p) {
+                    int32_t i = order[p];
+                    for (int32_t q = start[m]; q < start[m + 1]; ++q) {
+                        int32_t j = order[q];
+                        if (i < j && oracle_link(w + 3 * (int64_t)i, w + 3 * (int64_t)j, L, b)) {
+                            if (cnt == capz) {
+                                capz *= 2;
+                                edge_t *nb = (edge_t *)realloc(buf, sizeof(edge_t) * (size_t)capz);
+                                if (!nb) { free(buf); buf = NULL; break; }
+                                buf = nb;
+                            }
+                            buf[cnt].i = i; buf[cnt].j = j; ++cnt;
+                        }
+                    }
+                }
+            }
+        }
+        if (!buf) {
+#ifdef _OPENMP
+#pragma omp atomic write
+#endif
+            failed = 1;
+        }
+        ebuf[cz] = buf;
+        ecnt[cz] = buf ? cnt : 0;
+    }
+    uint64_t E = 0;
+    for (int64_t cz = 0; cz < n; ++cz) {          /* the serial union step */
+        for (int64_t k = 0; k < ecnt[cz]; ++k) uf_union(labels, ebuf[cz][k].i, ebuf[cz][k].j);
+        E += (uint64_t)ecnt[cz];
+        free(ebuf[cz]);
+    }
+    for (int64_t i = 0; i < N; ++i) labels[i] = uf_find(labels, (int32_t)i);
+    if (E_out) *E_out = E;
+    free(w); free(cell); free(start); free(order); free(ebuf); free(ecnt);
+    return failed ? ORACLE_ERR_NOMEM : ORACLE_OK;
+}
+
 /* ---- groups (Eq. 4 PAPER.md:259 made periodic, R9-R13) ----------
  * distinct labels ascending; size = member count; keep size >= N_min; kept groups numbered 0..K-1
  * by ascending canonical label.  mass = sum m_i in float64.  centre of mass: r = w[label];

@@ -68,6 +68,22 @@ def test_wrap_of_huge_coordinates_lands_in_the_box():
     assert np.minimum(d, float(L) - d).max() < 1.0    # off by at most an ulp of x (0.5 at 6e6)
 
 
+def test_threaded_pair_search_equals_the_single_thread_oracle():
+    """oracle.labels_cells_threads (the all-cores figure of bench.py) only changes the order in which edges reach the
+    union-find: labels and E must be those of labels_cells, on clustered, uniform, tiny-grid and empty inputs."""
+    rng = np.random.default_rng(12)
+    w = inputs.scaled(inputs.CONFIGS["cfg1"], 24)
+    cases = [(inputs.make_positions(w), w.L, w.b),
+             ((rng.random((5000, 3)) * 10).astype(np.float32), 10.0, 0.35),
+             ((rng.random((300, 3)) * 4).astype(np.float32), 4.0, 1.2),      # n = 3: every stencil wraps
+             (np.zeros((0, 3), np.float32), 1.0, 0.1)]
+    for p, L, b in cases:
+        ref, E = oracle.labels_cells(p, L, b)
+        for t in (1, 3, 8):
+            got, Et = oracle.labels_cells_threads(p, L, b, t)
+            assert np.array_equal(got, ref) and Et == E
+
+
 def test_wrap_nonfinite_is_an_error():
     p = np.zeros((4, 3), np.float32)
     p[2, 1] = np.nan
