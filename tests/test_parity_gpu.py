@@ -283,6 +283,39 @@ def test_block_path_falls_back_in_the_same_call(B):
         assert got["ran"][0] == "cells", "expected the fallback to the cell path"
 
 
+@pytest.mark.parametrize("seed", range(24))
+def test_random_small_boxes_both_paths(B, seed):
+    """Differential test over random geometries: box side, linking length (so grids of 6 .. 45 cells per axis and
+    block plans with 3 .. 12 blocks per axis, partial last blocks included), particle count NOT a multiple of 4,
+    a mixture of uniform points, Gaussian clumps (some across the box faces), points exactly on cell faces and
+    points outside [0, L).  Both implementations of H1-H5 against the oracle (brute force where it is cheap)."""
+    rng = np.random.default_rng(1000 + seed)
+    L = float(rng.choice([1.0, 7.3, 64.0, 1000.0]))
+    n_cells = int(rng.integers(6, 46))
+    b = float(np.float32(L / (n_cells + rng.uniform(0.05, 0.95)) / 1.001))
+    N = int(rng.integers(300, 6000)) | 1
+    n_cl = int(rng.integers(0, 6))
+    parts = [rng.random((N, 3)) * L]
+    for _ in range(n_cl):
+        c = rng.random(3) * L
+        if rng.random() < 0.5:
+            c[rng.integers(0, 3)] = 0.0                       # a clump across a box face
+        parts.append(c + rng.standard_normal((int(rng.integers(20, 400)), 3)) * b * rng.uniform(0.3, 2.0))
+    faces = (rng.integers(0, n_cells, (60, 3)) * (L / n_cells)).astype(np.float64)   # on (or an ulp off) cell faces
+    parts.append(faces + rng.choice([0.0, 1e-7 * L, -1e-7 * L], (60, 3)))
+    p = np.concatenate(parts)
+    p[:25] += L * rng.integers(-3, 4, (25, 3))                # outside the box: the wrap is part of the path
+    p = p.astype(np.float32)
+    p = p[rng.permutation(len(p))]
+    mass = rng.uniform(0.5, 1.5, len(p)).astype(np.float32) if seed % 2 else None
+    N_min = int(rng.choice([1, 2, 5, 20]))
+    got, lab, og = check_against_oracle(B, p, L, b, N_min, mass=mass, brute=len(p) <= 2500)
+    if seed % 3 == 0:                                         # and on a coarser grid than the plan's default
+        check_against_oracle(B, p, L, b, N_min, mass=mass, grid=max(6, got["grid"][0] // 2))
+    if seed % 3 == 1:                                         # and on the finest admissible grid (cell side ~ b)
+        check_against_oracle(B, p, L, b, N_min, mass=mass, grid=got["grid"][2])
+
+
 # --------------------------------------------------------------------------- invariants
 def test_permutation_invariance_on_gpu(B):
     w = inputs.scaled(inputs.CONFIGS["cfg1"], 40)
