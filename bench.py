@@ -512,9 +512,49 @@ def run_ours(args):
     torch.cuda.synchronize()
     barrier()
     e2e_ms = max_over_ranks_ms(e0.elapsed_time(e1), world, dev) / e2e_steps
-    B.fof_destroy(h2)
     assert Kh == K_groups, (Kh, K_groups)
     assert torch.equal(hl.to(dev), labels), "host-path labels differ from device-path labels"
+
+    # ---- the same call split in two (fof_host_submit / fof_host_wait): two inputs in flight, so the copy of input
+    # k+1 and of result k-1 overlap the linking of input k.  The library's streams are its own: host clock around
+    # the loop, device idle on both sides.
+    dev_buf2 = torch.empty_like(dev_buf)
+    bufs = (dev_buf, dev_buf2)
+    outs = ((hl, gl, gs, gm, gc), (pin(N), pin(cap), pin(cap), pin(cap, dt=torch.float32), pin((cap, 3), dt=torch.float32)))
+    pipe_steps = 2 * e2e_steps
+
+    def pipe(n):
+        Ks = []
+        B.fof_host_submit(h2, 0, hpos, None, *outs[0], None, cap, bufs[0])
+        for k in range(1, n):
+            B.fof_host_submit(h2, k % 2, hpos, None, *outs[k % 2], None, cap, bufs[k % 2])
+            Ks.append(B.fof_host_wait(h2, (k - 1) % 2))
+        Ks.append(B.fof_host_wait(h2, (n - 1) % 2))
+        return Ks
+
+    pipe(3)
+    for o in outs:
+        o[0].fill_(-1)
+    barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    Ks = pipe(pipe_steps)
+    torch.cuda.synchronize()
+    pipe_ms = max_over_ranks_ms((time.perf_counter() - t0) * 1e3, world, dev) / pipe_steps
+    barrier()
+    assert all(k == K_groups for k in Ks), Ks
+    for o in outs:
+        assert torch.equal(o[0].to(dev), labels), "pipelined host-path labels differ from device-path labels"
+    # what the two big copies cost on their own (one after the other, nothing else running)
+    e0.record(stream)
+    for _ in range(3):
+        dev_buf[: hpos.numel() * 4].view(torch.float32).copy_(hpos.view(-1), non_blocking=True)
+        hl.copy_(labels, non_blocking=True)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    copies_ms = e0.elapsed_time(e1) / 3
+    B.fof_destroy(h2)
+    del dev_buf2
 
     if rank != 0:
         if world > 1:
@@ -606,9 +646,17 @@ def run_ours(args):
         "stage_ms_note": f"separate pass of {n_break} steps with events around every stage; the timed region carries "
                          f"events around {top} only (roofline.kernel_ms)",
         "roofline": roofline, "cpu_baseline": cpu, "parity_vs_oracle_in_this_run": parity,
-        "e2e": {"value": whole_job_value(world, N, e2e_ms), "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
+        "e2e": {"value": whole_job_value(world, N, pipe_ms), "unit": UNIT, "ms_per_step": pipe_ms, "steps": pipe_steps,
                 "h2d_bytes_per_step": int(hpos.numel() * 4),
-                "d2h_bytes_per_step": int(N * 4 + Kh * (4 + 4 + 4 + 12) + 8)},
+                "d2h_bytes_per_step": int(N * 4 + Kh * (4 + 4 + 4 + 12) + 8),
+                "call": "fof_host_submit / fof_host_wait, two inputs in flight (every step: pinned pos host -> device, "
+                        "fof_link + fof_groups, labels + group records device -> host); host clock around the loop",
+                "single_call": {"call": "fof_run_host (one blocking call per step, CUDA events)",
+                                "value": whole_job_value(world, N, e2e_ms), "ms_per_step": e2e_ms,
+                                "steps": e2e_steps},
+                "copies_only_ms": copies_ms,
+                "copies_only_note": "pos host -> device then labels device -> host, back to back with nothing else "
+                                    "running: the floor of the single call without its kernels"},
         "gpu_launches": int(launches), "clocks": clk.summary(), "next1": next1, "next3": next3, "next4": next4,
     }
     print(json.dumps(line), flush=True)

@@ -235,6 +235,26 @@ int fof_run_host(fof_handle *h, const float *pos_host, const float *mass_host, i
                  float *group_com_host, int32_t *particle_group_host, int64_t cap, int64_t *K_host,
                  void *dev_buf, void *stream);
 
+/* The same work as fof_run_host, split into an enqueue half and a completion half so that a SEQUENCE of inputs
+ * (the "simulation analysis" use of PAPER.md:14 with the snapshots on the host: one catalogue per snapshot) keeps the PCIe link busy in
+ * both directions: while input k is linked, input k+1 travels host -> device and result k-1 device -> host.
+ * Three internal streams (in, run, out) order the work; the caller's streams are not involved.
+ *   slot      0 or 1.  At most one submit is outstanding per slot (else FOF_ERR_STATE); each slot has its own
+ *             dev_buf of fof_host_device_bytes(h, cap) bytes (256-B aligned), owned by the caller, which must not
+ *             touch it between the submit and the wait.
+ *   *_host    as in fof_run_host; pinned memory is REQUIRED for the overlap (pageable copies serialise).  They
+ *             must stay valid, and the outputs unread, until fof_host_wait(h, slot) returns.
+ * fof_host_submit returns once the copies and kernels are enqueued (it does not block on the device; inputs of
+ * consecutive submits are processed in submit order).  fof_host_wait blocks until the slot's labels, K group
+ * records and particle_group are in the host buffers, writes *K_host, frees the slot and returns the deferred
+ * status: FOF_OK, FOF_ERR_NONFINITE, FOF_ERR_CAPACITY (K > cap: *K_host is set, no group record is copied), or
+ * FOF_ERR_STATE if the slot has no submit outstanding or its submit had failed.  fof_destroy waits for whatever
+ * is still in flight.  Results are those of fof_run_host bit for bit. */
+int fof_host_submit(fof_handle *h, int32_t slot, const float *pos_host, const float *mass_host, int32_t *labels_host,
+                    int32_t *group_label_host, int32_t *group_size_host, float *group_mass_host,
+                    float *group_com_host, int32_t *particle_group_host, int64_t cap, void *dev_buf);
+int fof_host_wait(fof_handle *h, int32_t slot, int64_t *K_host);
+
 /* Synchronises `stream` and returns the deferred device-side status of the last fof_link /
  * fof_groups on (h, ws): FOF_OK or FOF_ERR_NONFINITE. */
 int fof_status(fof_handle *h, void *ws, void *stream);

@@ -89,6 +89,10 @@ def lib():
         L.fof_groups_backward.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, vp, vp]
         L.fof_host_device_bytes.restype = ctypes.c_size_t
         L.fof_host_device_bytes.argtypes = [vp, i64]
+        L.fof_host_submit.restype = ctypes.c_int
+        L.fof_host_submit.argtypes = [vp, ctypes.c_int32, vp, vp, vp, vp, vp, vp, vp, vp, i64, vp]
+        L.fof_host_wait.restype = ctypes.c_int
+        L.fof_host_wait.argtypes = [vp, ctypes.c_int32, ctypes.POINTER(i64)]
         L.fof_run_host.restype = ctypes.c_int
         L.fof_run_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, ctypes.POINTER(i64), vp, vp]
         L.fof_status.restype = ctypes.c_int
@@ -279,6 +283,21 @@ def fof_run_host(h, pos_host, mass_host, labels_host, group_label_host, group_si
                               _ptr(group_size_host), _ptr(group_mass_host), _ptr(group_com_host),
                               _ptr(particle_group_host), int(cap), ctypes.byref(K), _ptr(dev_buf),
                               _stream_ptr(stream)), h)
+    return int(K.value)
+
+
+def fof_host_submit(h, slot, pos_host, mass_host, labels_host, group_label_host, group_size_host, group_mass_host,
+                    group_com_host, particle_group_host, cap, dev_buf):
+    """Enqueue half of fof_run_host (slot 0 or 1, each with its own dev_buf); pinned host tensors."""
+    _check(lib().fof_host_submit(h, int(slot), _ptr(pos_host), _ptr(mass_host), _ptr(labels_host),
+                                 _ptr(group_label_host), _ptr(group_size_host), _ptr(group_mass_host),
+                                 _ptr(group_com_host), _ptr(particle_group_host), int(cap), _ptr(dev_buf)), h)
+
+
+def fof_host_wait(h, slot) -> int:
+    """Completion half: blocks until the slot's results are in the host buffers; returns K."""
+    K = ctypes.c_int64()
+    _check(lib().fof_host_wait(h, int(slot), ctypes.byref(K)), h)
     return int(K.value)
 
 

@@ -213,6 +213,19 @@ void fof_destroy(fof_handle *h)
         (void)cudaStreamDestroy(h->copy_stream);
         (void)cudaEventDestroy(h->ev_linked);
     }
+    if (h->in_stream) {
+        (void)cudaDeviceSynchronize();  // a submitted input may still be in flight
+        for (auto &sl : h->slot) {
+            (void)cudaStreamDestroy(sl.out);
+            (void)cudaEventDestroy(sl.ev_in);
+            (void)cudaEventDestroy(sl.ev_linked);
+            (void)cudaEventDestroy(sl.ev_groups);
+            (void)cudaEventDestroy(sl.ev_ctrl);
+            (void)cudaFreeHost(sl.ctrl_pin);
+        }
+        (void)cudaStreamDestroy(h->in_stream);
+        (void)cudaStreamDestroy(h->run_stream);
+    }
     delete h;
 }
 
@@ -415,19 +428,18 @@ int fof_link_stats(fof_handle *h, void *ws, void *stream, uint64_t *edges_host, 
     return FOF_OK;
 }
 
-int fof_groups(fof_handle *h, const float *pos, const float *mass, const int32_t *labels, void *ws,
-               int32_t *group_label, int32_t *group_size, float *group_mass, float *group_com,
-               int32_t *particle_group, int64_t cap, int64_t *K_host, void *stream)
+}  // extern "C"
+
+// The kernels of fof_groups, enqueued on `s` without waiting for them (fof_groups and fof_host_submit share it):
+// K is left in the workspace's Ctrl.
+static int groups_enqueue(fof_handle *h, const float *pos, const float *mass, const int32_t *labels, void *ws,
+                          int32_t *group_label, int32_t *group_size, float *group_mass, float *group_com,
+                          int32_t *particle_group, int64_t cap, cudaStream_t s)
 {
-    if (!h || !ws || ((uintptr_t)ws & 255) || !K_host || cap < 0) return FOF_ERR_INVALID_ARG;
-    if (h->N > 0 && (!pos || !labels)) return FOF_ERR_INVALID_ARG;
-    if (cap > 0 && (!group_label || !group_size || !group_mass || !group_com)) return FOF_ERR_INVALID_ARG;
-    cudaStream_t s = (cudaStream_t)stream;
     Ctrl *ctrl = at<Ctrl>(ws, h->off_ctrl);
     int *cnt = at<int>(ws, h->off_cnt);
     double *acc = at<double>(ws, h->off_acc);
     unsigned long long *state = at<unsigned long long>(ws, h->off_gscan_state);
-    *K_host = 0;
     const int has = h->N > 0;
     if (h->prof_slots)
         for (int k = kGroupsClear; k <= kGroupsFinish; ++k) h->ev_valid[h->prof_cur * kMaxStages + k] = false;
@@ -461,8 +473,25 @@ int fof_groups(fof_handle *h, const float *pos, const float *mass, const int32_t
         CK(launch_group_finish(pos, group_label, group_size, acc, mass != nullptr, h->grid, fin, ctrl, group_mass,
                                group_com, s), "group_finish_kernel");
     }
+    return FOF_OK;
+}
+
+extern "C" {
+
+int fof_groups(fof_handle *h, const float *pos, const float *mass, const int32_t *labels, void *ws,
+               int32_t *group_label, int32_t *group_size, float *group_mass, float *group_com,
+               int32_t *particle_group, int64_t cap, int64_t *K_host, void *stream)
+{
+    if (!h || !ws || ((uintptr_t)ws & 255) || !K_host || cap < 0) return FOF_ERR_INVALID_ARG;
+    if (h->N > 0 && (!pos || !labels)) return FOF_ERR_INVALID_ARG;
+    if (cap > 0 && (!group_label || !group_size || !group_mass || !group_com)) return FOF_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    *K_host = 0;
+    const int rc = groups_enqueue(h, pos, mass, labels, ws, group_label, group_size, group_mass, group_com,
+                                  particle_group, cap, s);
+    if (rc != FOF_OK) return rc;
     long long K = 0;
-    CK(cudaMemcpyAsync(&K, &ctrl->K, sizeof(K), cudaMemcpyDeviceToHost, s), "copy K");
+    CK(cudaMemcpyAsync(&K, &at<Ctrl>(ws, h->off_ctrl)->K, sizeof(K), cudaMemcpyDeviceToHost, s), "copy K");
     CK(cudaStreamSynchronize(s), "sync");
     *K_host = (int64_t)K;
     if (K > cap) return FOF_ERR_CAPACITY;
@@ -690,6 +719,121 @@ int fof_run_host(fof_handle *h, const float *pos_host, const float *mass_host, i
     if (c.error & 1u) return FOF_ERR_NONFINITE;
     return FOF_OK;
 #undef CKD
+}
+
+static int host_streams(fof_handle *h)
+{
+    if (h->in_stream) return FOF_OK;
+    cudaStream_t in = nullptr, run = nullptr;
+    CK(cudaStreamCreateWithFlags(&in, cudaStreamNonBlocking), "cudaStreamCreate");
+    CK(cudaStreamCreateWithFlags(&run, cudaStreamNonBlocking), "cudaStreamCreate");
+    for (auto &sl : h->slot) {
+        CK(cudaStreamCreateWithFlags(&sl.out, cudaStreamNonBlocking), "cudaStreamCreate");
+        CK(cudaEventCreateWithFlags(&sl.ev_in, cudaEventDisableTiming), "cudaEventCreate");
+        CK(cudaEventCreateWithFlags(&sl.ev_linked, cudaEventDisableTiming), "cudaEventCreate");
+        CK(cudaEventCreateWithFlags(&sl.ev_groups, cudaEventDisableTiming), "cudaEventCreate");
+        CK(cudaEventCreateWithFlags(&sl.ev_ctrl, cudaEventDisableTiming), "cudaEventCreate");
+        CK(cudaHostAlloc((void **)&sl.ctrl_pin, sizeof(Ctrl), cudaHostAllocDefault), "cudaHostAlloc");
+        sl.busy = false;
+    }
+    h->run_stream = run;
+    h->in_stream = in;  // set last: fof_destroy takes it as "all of the above exist"
+    return FOF_OK;
+}
+
+int fof_host_submit(fof_handle *h, int32_t slot, const float *pos_host, const float *mass_host, int32_t *labels_host,
+                    int32_t *group_label_host, int32_t *group_size_host, float *group_mass_host,
+                    float *group_com_host, int32_t *particle_group_host, int64_t cap, void *dev_buf)
+{
+    if (!h || slot < 0 || slot > 1 || !dev_buf || ((uintptr_t)dev_buf & 255) || cap < 0) return FOF_ERR_INVALID_ARG;
+    if (h->N > 0 && (!pos_host || !labels_host)) return FOF_ERR_INVALID_ARG;
+    if (cap > 0 && (!group_label_host || !group_size_host || !group_mass_host || !group_com_host))
+        return FOF_ERR_INVALID_ARG;
+    {
+        const int rc = host_streams(h);
+        if (rc != FOF_OK) return rc;
+    }
+    fof_handle::HostSlot &sl = h->slot[slot];
+    if (sl.busy) return FOF_ERR_STATE;
+    const size_t N = (size_t)h->N;
+    char *p = static_cast<char *>(dev_buf);
+    float *pos = (float *)p;      p += align256((N + 1) * 3 * sizeof(float));
+    float *mass = (float *)p;     p += align256((N + 1) * sizeof(float));
+    int *labels = (int *)p;       p += align256((N + 1) * sizeof(int));
+    int *pgroup = (int *)p;       p += align256((N + 1) * sizeof(int));
+    int *glabel = (int *)p;       p += align256(((size_t)cap + 1) * sizeof(int));
+    int *gsize = (int *)p;        p += align256(((size_t)cap + 1) * sizeof(int));
+    float *gmass = (float *)p;    p += align256(((size_t)cap + 1) * sizeof(float));
+    float *gcom = (float *)p;     p += align256(((size_t)cap + 1) * 3 * sizeof(float));
+    void *ws = p;
+    cudaStream_t in = h->in_stream, run = h->run_stream;
+    // Anything enqueued below is waited for by fof_host_wait, also after an error in the middle: the slot is
+    // busy from the first copy on.
+    sl.busy = true;
+    sl.cap = -1;  // "the groups were not enqueued"
+    if (N) CK(cudaMemcpyAsync(pos, pos_host, N * 3 * sizeof(float), cudaMemcpyHostToDevice, in), "H2D pos");
+    if (N && mass_host) CK(cudaMemcpyAsync(mass, mass_host, N * sizeof(float), cudaMemcpyHostToDevice, in), "H2D mass");
+    CK(cudaEventRecord(sl.ev_in, in), "cudaEventRecord");
+    CK(cudaStreamWaitEvent(run, sl.ev_in, 0), "cudaStreamWaitEvent");
+    int rc = fof_link(h, pos, labels, ws, run);
+    if (rc != FOF_OK) return rc;
+    CK(cudaEventRecord(sl.ev_linked, run), "cudaEventRecord");
+    CK(cudaStreamWaitEvent(sl.out, sl.ev_linked, 0), "cudaStreamWaitEvent");
+    if (N) CK(cudaMemcpyAsync(labels_host, labels, N * sizeof(int), cudaMemcpyDeviceToHost, sl.out), "D2H labels");
+    rc = groups_enqueue(h, pos, mass_host ? mass : nullptr, labels, ws, glabel, gsize, gmass, gcom,
+                        particle_group_host ? pgroup : nullptr, cap, run);
+    if (rc != FOF_OK) return rc;
+    // K and the error bits follow the labels on the slot's own copy stream: `run` never waits for a copy
+    CK(cudaEventRecord(sl.ev_groups, run), "cudaEventRecord");
+    CK(cudaStreamWaitEvent(sl.out, sl.ev_groups, 0), "cudaStreamWaitEvent");
+    CK(cudaMemcpyAsync(sl.ctrl_pin, at<Ctrl>(ws, h->off_ctrl), sizeof(Ctrl), cudaMemcpyDeviceToHost, sl.out), "copy ctrl");
+    CK(cudaEventRecord(sl.ev_ctrl, sl.out), "cudaEventRecord");
+    if (N && particle_group_host)
+        CK(cudaMemcpyAsync(particle_group_host, pgroup, N * sizeof(int), cudaMemcpyDeviceToHost, sl.out),
+           "D2H particle_group");
+    sl.cap = cap;
+    sl.group_label_host = group_label_host; sl.group_size_host = group_size_host;
+    sl.group_mass_host = group_mass_host;   sl.group_com_host = group_com_host;
+    sl.glabel = glabel; sl.gsize = gsize; sl.gmass = gmass; sl.gcom = gcom;
+    return FOF_OK;
+}
+
+int fof_host_wait(fof_handle *h, int32_t slot, int64_t *K_host)
+{
+    if (!h || slot < 0 || slot > 1 || !K_host) return FOF_ERR_INVALID_ARG;
+    if (!h->in_stream || !h->slot[slot].busy) return FOF_ERR_STATE;
+    fof_handle::HostSlot &sl = h->slot[slot];
+    *K_host = 0;
+    sl.busy = false;
+    if (sl.cap < 0) {  // the submit failed half way: drain what it enqueued
+        (void)cudaStreamSynchronize(h->in_stream);
+        (void)cudaStreamSynchronize(h->run_stream);
+        (void)cudaStreamSynchronize(sl.out);
+        return FOF_ERR_STATE;
+    }
+    int rc = FOF_OK;
+    cudaError_t e = cudaEventSynchronize(sl.ev_ctrl);  // K and the error bits are in ctrl_pin now
+    if (e == cudaSuccess) {
+        const long long K = sl.ctrl_pin->K;
+        *K_host = (int64_t)K;
+        if (K > sl.cap) rc = FOF_ERR_CAPACITY;
+        else if (K > 0) {
+            const size_t k = (size_t)K;
+            e = cudaMemcpyAsync(sl.group_label_host, sl.glabel, k * sizeof(int), cudaMemcpyDeviceToHost, sl.out);
+            if (e == cudaSuccess)
+                e = cudaMemcpyAsync(sl.group_size_host, sl.gsize, k * sizeof(int), cudaMemcpyDeviceToHost, sl.out);
+            if (e == cudaSuccess)
+                e = cudaMemcpyAsync(sl.group_mass_host, sl.gmass, k * sizeof(float), cudaMemcpyDeviceToHost, sl.out);
+            if (e == cudaSuccess)
+                e = cudaMemcpyAsync(sl.group_com_host, sl.gcom, k * 3 * sizeof(float), cudaMemcpyDeviceToHost, sl.out);
+        }
+    }
+    const cudaError_t e2 = cudaStreamSynchronize(sl.out);  // always: the caller's buffers are free after this call
+    if (e != cudaSuccess) return cuda_fail(h, e, "fof_host_wait");
+    if (e2 != cudaSuccess) return cuda_fail(h, e2, "fof_host_wait");
+    if (rc != FOF_OK) return rc;
+    if (sl.ctrl_pin->error & 1u) return FOF_ERR_NONFINITE;
+    return FOF_OK;
 }
 
 int fof_status(fof_handle *h, void *ws, void *stream)

@@ -158,6 +158,19 @@ struct fof_handle {
     // fof_run_host: the labels go back to the host on a stream of their own while the groups are built
     cudaStream_t copy_stream;
     cudaEvent_t ev_linked;
+    // fof_host_submit / fof_host_wait: two inputs in flight, host -> device, compute and device -> host streams
+    struct HostSlot {
+        bool busy;
+        cudaStream_t out;            // this slot's device -> host copies
+        cudaEvent_t ev_in, ev_linked, ev_groups, ev_ctrl;
+        fof::Ctrl *ctrl_pin;         // pinned copy of the workspace's Ctrl (K, error bits) taken after the groups
+        int64_t cap;
+        int32_t *group_label_host, *group_size_host;
+        float *group_mass_host, *group_com_host;
+        const int *glabel, *gsize;   // device side of the group records (in the slot's dev_buf)
+        const float *gmass, *gcom;
+    } slot[2];
+    cudaStream_t in_stream, run_stream;
 };
 
 namespace fof {

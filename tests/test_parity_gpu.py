@@ -448,6 +448,113 @@ def test_run_host_path(B):
     B.fof_destroy(h)
 
 
+def test_host_pipeline_against_oracle(B):
+    """fof_host_submit / fof_host_wait: six different inputs through the two slots, two in flight all the time;
+    every result equals the oracle's for ITS input (a mixed-up slot, a copy that overtakes its kernel or a result
+    read before its copy landed would show), for both link paths."""
+    import dataclasses
+    base = inputs.scaled(inputs.CONFIGS["cfg1"], 40)
+    ws = [dataclasses.replace(base, seed=base.seed + 100 * k) for k in range(6)]
+    ps = [inputs.make_positions(w) for w in ws]
+    N = len(ps[0])
+    assert all(len(p) == N for p in ps)
+    ms = [inputs.make_masses(w) for w in ws]
+    want = []
+    for p, m in zip(ps, ms):
+        lab, _ = oracle.labels_cells(p, base.L, base.b)
+        want.append((lab, oracle.groups(p, lab, base.L, base.N_min, mass=m)))
+    assert len({o["K"] for _, o in want}) > 1  # the inputs really differ
+    cap = N // base.N_min
+    pin = lambda *s, dt=torch.int32: torch.empty(*s, dtype=dt).pin_memory()  # noqa: E731
+    for path in ("cells", "blocks"):
+        h = B.fof_create(N, base.L, base.b, base.N_min)
+        B.fof_set_path(h, {"cells": B.FOF_PATH_CELLS, "blocks": B.FOF_PATH_BLOCKS}[path])
+        nbytes = B.fof_host_device_bytes(h, cap) + 256
+        dev = [torch.empty(nbytes, dtype=torch.uint8, device="cuda") for _ in range(2)]
+        hp = [torch.from_numpy(p).pin_memory() for p in ps]
+        hm = [torch.from_numpy(m).pin_memory() for m in ms]
+        outs = [dict(hl=pin(N), gl=pin(cap), gs=pin(cap), gm=pin(cap, dt=torch.float32),
+                     gc=pin((cap, 3), dt=torch.float32), pg=pin(N)) for _ in range(2)]
+
+        def submit(k):
+            o = outs[k % 2]
+            for t in o.values():
+                t.fill_(-7)
+            B.fof_host_submit(h, k % 2, hp[k], hm[k], o["hl"], o["gl"], o["gs"], o["gm"], o["gc"], o["pg"], cap,
+                              dev[k % 2])
+
+        def collect(k):
+            o = outs[k % 2]
+            K = B.fof_host_wait(h, k % 2)
+            lab, og = want[k]
+            assert K == og["K"], (path, k)
+            assert np.array_equal(o["hl"].numpy(), lab), (path, k)
+            assert np.array_equal(o["gs"].numpy()[:K], og["group_size"])
+            assert np.array_equal(o["gl"].numpy()[:K], og["group_label"])
+            assert np.array_equal(o["pg"].numpy(), og["particle_group"])
+            assert np.all(np.abs(o["gm"].numpy()[:K] - og["group_mass"]) <= 1e-5 * og["group_mass"])
+            d = np.abs(o["gc"].numpy()[:K].astype(np.float64) - og["group_com"])
+            assert np.minimum(d, base.L - d).max() <= 1e-5 * base.L
+
+        submit(0)
+        for k in range(1, len(ps)):
+            submit(k)
+            collect(k - 1)
+        collect(len(ps) - 1)
+        B.fof_destroy(h)
+
+
+def test_host_pipeline_errors(B):
+    """Call-order and deferred errors of the pipelined host path."""
+    w = inputs.scaled(inputs.CONFIGS["cfg1"], 24)
+    p = inputs.make_positions(w)
+    N = len(p)
+    lab, _ = oracle.labels_cells(p, w.L, w.b)
+    og = oracle.groups(p, lab, w.L, w.N_min)
+    assert og["K"] >= 2
+    h = B.fof_create(N, w.L, w.b, w.N_min)
+    cap = N // w.N_min
+    dev = torch.empty(B.fof_host_device_bytes(h, cap) + 256, dtype=torch.uint8, device="cuda")
+    pin = lambda *s, dt=torch.int32: torch.empty(*s, dtype=dt).pin_memory()  # noqa: E731
+    hp, hl = torch.from_numpy(p).pin_memory(), pin(N)
+    gl, gs, gm, gc = pin(cap), pin(cap), pin(cap, dt=torch.float32), pin((cap, 3), dt=torch.float32)
+    with pytest.raises(B.FofError) as e:
+        B.fof_host_wait(h, 0)  # nothing submitted
+    assert e.value.code == B.FOF_ERR_STATE
+    with pytest.raises(B.FofError) as e:
+        B.fof_host_submit(h, 2, hp, None, hl, gl, gs, gm, gc, None, cap, dev)
+    assert e.value.code == B.FOF_ERR_INVALID_ARG
+    B.fof_host_submit(h, 0, hp, None, hl, gl, gs, gm, gc, None, cap, dev)
+    with pytest.raises(B.FofError) as e:
+        B.fof_host_submit(h, 0, hp, None, hl, gl, gs, gm, gc, None, cap, dev)  # slot busy
+    assert e.value.code == B.FOF_ERR_STATE
+    assert B.fof_host_wait(h, 0) == og["K"]
+    assert np.array_equal(hl.numpy(), lab)
+    with pytest.raises(B.FofError) as e:
+        B.fof_host_wait(h, 0)  # already collected
+    assert e.value.code == B.FOF_ERR_STATE
+    # more groups than capacity: K is reported, the labels still arrive
+    small = og["K"] - 1
+    dev2 = torch.empty(B.fof_host_device_bytes(h, small) + 256, dtype=torch.uint8, device="cuda")
+    hl.fill_(-1)
+    B.fof_host_submit(h, 1, hp, None, hl, gl, gs, gm, gc, None, small, dev2)
+    with pytest.raises(B.FofError) as e:
+        B.fof_host_wait(h, 1)
+    assert e.value.code == B.FOF_ERR_CAPACITY
+    assert np.array_equal(hl.numpy(), lab)
+    # a non-finite coordinate is reported by the wait
+    bad = torch.from_numpy(p.copy()).pin_memory()
+    bad[5, 1] = float("nan")
+    B.fof_host_submit(h, 0, bad, None, hl, gl, gs, gm, gc, None, cap, dev)
+    with pytest.raises(B.FofError) as e:
+        B.fof_host_wait(h, 0)
+    assert e.value.code == B.FOF_ERR_NONFINITE
+    # the slot is usable again, and destroying the handle with a submit in flight is safe
+    B.fof_host_submit(h, 0, hp, None, hl, gl, gs, gm, gc, None, cap, dev)
+    B.fof_destroy(h)
+    torch.cuda.synchronize()
+
+
 @pytest.mark.parametrize("n_particles", [4099, 65537])
 def test_unaligned_caller_pointers(B, n_particles):
     """pos / labels / particle_group that are only 4-byte aligned (views one element into a buffer) and
