@@ -454,9 +454,34 @@ def run_ours(args):
         torch.cuda.synchronize()
         t_batch = ev[0].elapsed_time(ev[1]) / S
         same = bool(torch.equal(labS[S - 1], lab3))   # the last single sample was sample S - 1
-        del labS, gS, scr
+        # the same S samples from the potential-edge list: built once per link (two calls: the first sizes the
+        # buffer), then every sample is a stream over it
+        f3.stochastic_list(w.b, 5.0)
+        torch.cuda.synchronize()
+        ev[0].record(stream)
+        slist, records = f3.stochastic_list(w.b, 5.0)
+        ev[1].record(stream)
+        labL = torch.empty((S, N), dtype=torch.int32, device=dev)
+        gL = torch.empty((S, N, 3), dtype=torch.float32, device=dev)
+        B.fof_link_stochastic_list(f3.h, slist, 2024, 0, S, labL, lpS, gL, scr, f3.ws)
+        torch.cuda.synchronize()
+        t_build = ev[0].elapsed_time(ev[1])
+        ev[0].record(stream)
+        B.fof_link_stochastic_list(f3.h, slist, 2024, 0, S, labL, lpS, gL, scr, f3.ws)
+        ev[1].record(stream)
+        torch.cuda.synchronize()
+        t_list = ev[0].elapsed_time(ev[1]) / S
+        same_list = bool(torch.equal(labL, labS))
+        gmax = float(gS.abs().max().item())
+        grad_diff = float((gL - gS).abs().max().item()) / gmax if gmax > 0 else 0.0
+        del labS, gS, labL, gL, slist, scr
         next3 = {"samples": S, "binning_ms": t_bin, "ms_per_sample": t_smp, "batched_ms_per_sample": t_batch,
                  "batched_labels_equal_single": same,
+                 "list": {"build_ms": t_build, "records": records, "bytes": int(B.fof_stochastic_list_bytes(f3.h, records)),
+                          "ms_per_sample": t_list, "ms_per_sample_with_build": t_list + t_build / S,
+                          "labels_equal_batched": same_list, "score_max_rel_diff_vs_batched": grad_diff,
+                          "what": "fof_stochastic_list_build once per link (count + fill, both calls timed), then "
+                                  "fof_link_stochastic_list: every sample streams the 32-byte records"},
                  "potential_edges": cand3, "sampled_edges_last": e3,
                  "potential_edges_per_s": cand3 / (t_smp * 1e-3), "particles_per_s_per_sample": N / (t_smp * 1e-3),
                  "config": "b_cand = 1.5 b, alpha = 5, log p(y) and score function on"}

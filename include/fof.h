@@ -154,6 +154,37 @@ size_t fof_stochastic_scratch_bytes(const fof_handle *h, int32_t S);
 int fof_link_stochastic_batch(fof_handle *h, float b_link, float alpha, uint64_t seed, uint32_t sample, int32_t S,
                               int32_t *labels, double *logp, float *grad_pos, void *scratch, void *ws, void *stream);
 
+/* The same S samples from a potential-edge LIST ("we do not rebuild the neighbor list"; section 3.2,
+ * S = 16 samples per optimisation step share the neighbour structure).  Which pairs are potential
+ * edges, their p_ij, t_ij = alpha (b_link^2 - d^2) / b_link^2 and their displacement do not depend on the sample:
+ * fof_stochastic_list_build writes them down once per fof_link, and every sample is then one stream over that list
+ * (draw, log term, score-function term, hook) instead of a new neighbour search.
+ *
+ * fof_stochastic_list_build(h, b_link, alpha, list, list_bytes, records_host, ws, stream)
+ *   Must follow a fof_link on (h, ws) (FOF_ERR_STATE otherwise; cell path, as fof_link_stochastic).  Counts the
+ *   records, synchronises `stream` once to report them in *records_host (every potential edge is recorded under both
+ *   of its particles: records = 2 x potential edges), and, if `list` (dev, 256-B aligned, owned by the caller) holds
+ *   fof_stochastic_list_bytes(h, *records_host) bytes, fills it (asynchronous on `stream`).  A smaller buffer --
+ *   at least fof_stochastic_list_bytes(h, 0), which holds the per-particle offsets -- gives FOF_ERR_CAPACITY with
+ *   *records_host set: allocate and call again (the per-particle counts stay in the workspace until the next
+ *   fof_link / fof_groups / fof_subgroups on it, so the second call does not search again; they take the place of the
+ *   group sizes fof_link left there: a later fof_groups counts its labels afresh).  More than 2^32 - 1 records:
+ *   FOF_ERR_CAPACITY as well.
+ *   32 bytes per record; at cfg2 (N = 2^24, b = 0.2 spacings as the candidate radius) 2.5e8 records, 8 GB.
+ * fof_link_stochastic_list(h, list, seed, sample, S, labels, logp, grad_pos, scratch, ws, stream)
+ *   labels / logp / grad_pos / scratch as in fof_link_stochastic_batch, with b_link and alpha those of the build;
+ *   sample k gives exactly the labels, and to float32 summation order the log p and score function, of
+ *   fof_link_stochastic(sample + k).
+ *   `list` must be the buffer of the last fof_stochastic_list_build on h, and no fof_link may have run on h since
+ *   (FOF_ERR_STATE): the list describes the positions of the link it was built after.  `ws`: that link's workspace
+ *   (only the counters of fof_link_stats are written: pair tests = potential edges, E = sampled edges summed over the
+ *   S samples).  Asynchronous on `stream`. */
+size_t fof_stochastic_list_bytes(const fof_handle *h, uint64_t records);
+int fof_stochastic_list_build(fof_handle *h, float b_link, float alpha, void *list, size_t list_bytes,
+                              uint64_t *records_host, void *ws, void *stream);
+int fof_link_stochastic_list(fof_handle *h, const void *list, uint64_t seed, uint32_t sample, int32_t S,
+                             int32_t *labels, double *logp, float *grad_pos, void *scratch, void *ws, void *stream);
+
 /* Six-dimensional sub-halo pass (section 2.1.1, Eq. 3; R29-R31): inside every
  * kept halo a second FoF in phase space, two members linked iff
  *     (x_i - x_j)^2 / sigma_x + (v_i - v_j)^2 / sigma_v <= ell^2

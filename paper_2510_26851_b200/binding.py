@@ -71,6 +71,13 @@ def lib():
         L.fof_link_stochastic_batch.restype = ctypes.c_int
         L.fof_link_stochastic_batch.argtypes = [vp, f32, f32, ctypes.c_uint64, ctypes.c_uint32, ctypes.c_int32, vp, vp, vp,
                                                 vp, vp, vp]
+        L.fof_stochastic_list_bytes.restype = ctypes.c_size_t
+        L.fof_stochastic_list_bytes.argtypes = [vp, ctypes.c_uint64]
+        L.fof_stochastic_list_build.restype = ctypes.c_int
+        L.fof_stochastic_list_build.argtypes = [vp, f32, f32, vp, ctypes.c_size_t, ctypes.POINTER(ctypes.c_uint64), vp, vp]
+        L.fof_link_stochastic_list.restype = ctypes.c_int
+        L.fof_link_stochastic_list.argtypes = [vp, vp, ctypes.c_uint64, ctypes.c_uint32, ctypes.c_int32, vp, vp, vp, vp,
+                                               vp, vp]
         L.fof_subgroups.restype = ctypes.c_int
         L.fof_subgroups.argtypes = [vp, vp, vp, vp, vp, i64, f32, f32, f32, vp, vp, vp]
         L.fof_layer_select.restype = ctypes.c_int
@@ -225,6 +232,27 @@ def fof_link_stochastic_batch(h, b_link, alpha, seed, sample, S, labels, logp, g
     """labels: cuda int32 [S,N]; logp: cuda float64 [S]; grad_pos: cuda float32 [S,N,3] or None; scratch: cuda bytes."""
     _check(lib().fof_link_stochastic_batch(h, _f(b_link), _f(alpha), int(seed), int(sample), int(S), _ptr(labels),
                                            _ptr(logp), _ptr(grad_pos), _ptr(scratch), _ptr(ws), _stream_ptr(stream)), h)
+
+
+def fof_stochastic_list_bytes(h, records: int) -> int:
+    return int(lib().fof_stochastic_list_bytes(h, int(records)))
+
+
+def fof_stochastic_list_build(h, b_link, alpha, list_buf, ws, stream=None):
+    """list_buf: cuda uint8 tensor.  Returns (records, filled): filled is False if list_buf was too small for them."""
+    R = ctypes.c_uint64()
+    rc = lib().fof_stochastic_list_build(h, _f(b_link), _f(alpha), _ptr(list_buf), int(list_buf.numel()),
+                                         ctypes.byref(R), _ptr(ws), _stream_ptr(stream))
+    if rc == FOF_ERR_CAPACITY and R.value <= 0xFFFFFFFF:
+        return int(R.value), False
+    _check(rc, h)
+    return int(R.value), True
+
+
+def fof_link_stochastic_list(h, list_buf, seed, sample, S, labels, logp, grad_pos, scratch, ws, stream=None):
+    """labels: cuda int32 [S,N]; logp: cuda float64 [S]; grad_pos: cuda float32 [S,N,3] or None; scratch: cuda bytes."""
+    _check(lib().fof_link_stochastic_list(h, _ptr(list_buf), int(seed), int(sample), int(S), _ptr(labels), _ptr(logp),
+                                          _ptr(grad_pos), _ptr(scratch), _ptr(ws), _stream_ptr(stream)), h)
 
 
 def fof_subgroups(h, pos, vel, particle_group, group_size, K, sigma_x, sigma_v, ell, sub_labels, ws, stream=None):
@@ -443,6 +471,36 @@ class FoF:
         scratch = torch.empty(max(fof_stochastic_scratch_bytes(self.h, S), 4), dtype=torch.uint8, device=d)
         with torch.cuda.device(d):
             fof_link_stochastic_batch(self.h, b_link, alpha, seed, sample, S, labels, logp, grad, scratch, self.ws, stream)
+        return labels, logp, grad
+
+    def stochastic_list(self, b_link, alpha, stream=None):
+        """The potential-edge list of the last link() (a cuda byte tensor to pass to link_stochastic_list) and its
+        number of records; two calls of the build: the first one sizes the buffer."""
+        import torch
+
+        d = self.device
+        with torch.cuda.device(d):
+            buf = torch.empty(fof_stochastic_list_bytes(self.h, 0), dtype=torch.uint8, device=d)
+            records, filled = fof_stochastic_list_build(self.h, b_link, alpha, buf, self.ws, stream)
+            if not filled:
+                del buf
+                buf = torch.empty(fof_stochastic_list_bytes(self.h, records), dtype=torch.uint8, device=d)
+                records, filled = fof_stochastic_list_build(self.h, b_link, alpha, buf, self.ws, stream)
+                assert filled
+        assert buf.data_ptr() % 256 == 0
+        return buf, records
+
+    def link_stochastic_list(self, slist, seed, sample, S, want_grad=True, stream=None):
+        """S samples over the list of stochastic_list(): (labels [S,N], logp [S], grad [S,N,3] or None)."""
+        import torch
+
+        d = self.device
+        labels = torch.empty((S, self.N), dtype=torch.int32, device=d)
+        logp = torch.zeros(S, dtype=torch.float64, device=d)
+        grad = torch.empty((S, self.N, 3), dtype=torch.float32, device=d) if want_grad else None
+        scratch = torch.empty(max(fof_stochastic_scratch_bytes(self.h, S), 4), dtype=torch.uint8, device=d)
+        with torch.cuda.device(d):
+            fof_link_stochastic_list(self.h, slist, seed, sample, S, labels, logp, grad, scratch, self.ws, stream)
         return labels, logp, grad
 
     def subgroups(self, pos, vel, g, sigma_x, sigma_v, ell, stream=None):

@@ -401,6 +401,8 @@ int fof_link(fof_handle *h, const float *pos, int32_t *labels, void *ws, void *s
     }
     h->linked = true;
     h->linked_ws = ws;
+    h->slist = nullptr;  // a potential-edge list describes the positions of the link it was built after
+    h->slist_counts_ws = nullptr;
     h->counted = has != 0;  // H6 rode along: fof_groups on these very labels starts at the compaction
     h->counted_labels = labels;
     h->linked_cells = !blocks;  // the cell-sorted arrays are certainly there only if the cell path ran ungated
@@ -447,6 +449,7 @@ static int groups_enqueue(fof_handle *h, const float *pos, const float *mass, co
     // on (h, ws) wrote (H6 is fused into its label pass); any other labels are counted here.
     const bool counted = h->counted && h->linked && h->linked_ws == ws && h->counted_labels == (const void *)labels;
     h->counted = false;  // the compaction below overwrites the counters
+    h->slist_counts_ws = nullptr;
     if (!counted) {
         {
             StageTimer t(h, s, kGroupsClear, 0);
@@ -537,6 +540,66 @@ int fof_link_stochastic_batch(fof_handle *h, float b_link, float alpha, uint64_t
     return FOF_OK;
 }
 
+size_t fof_stochastic_list_bytes(const fof_handle *h, uint64_t records)
+{
+    if (!h) return 0;
+    return stoch_list_fixed_bytes(h->N) + (size_t)records * 32;
+}
+
+int fof_stochastic_list_build(fof_handle *h, float b_link, float alpha, void *list, size_t list_bytes,
+                              uint64_t *records_host, void *ws, void *stream)
+{
+    if (!h || !ws || ((uintptr_t)ws & 255) || !list || ((uintptr_t)list & 255) || !records_host) return FOF_ERR_INVALID_ARG;
+    if (!(b_link > 0.0f) || !(b_link <= h->b) || !isfinite(alpha)) return FOF_ERR_INVALID_ARG;
+    if (list_bytes < stoch_list_fixed_bytes(h->N)) return FOF_ERR_INVALID_ARG;
+    if (!h->linked || h->linked_ws != ws || !h->linked_cells) return FOF_ERR_STATE;  // needs the cell sort of a fof_link on (h, ws)
+    cudaStream_t s = (cudaStream_t)stream;
+    const StochList v = stoch_list_views(list, h->N);
+    h->slist = nullptr;
+    *records_host = 0;
+    // The record counts of every particle go to the workspace (the group-size counters, free between fof_link and
+    // fof_groups) and stay valid until one of those runs: the call that sizes the buffer pays for the search, the
+    // call that fills it does not search again.
+    unsigned int *counts = reinterpret_cast<unsigned int *>(at<int>(ws, h->off_cnt));
+    h->counted = false;
+    if (h->slist_counts_ws != ws) {
+        h->launches += h->N > 0 ? 1 : 0;
+        CK(launch_stoch_list_count(at<float4>(ws, h->off_sorted), h->N, h->grid, at<unsigned int>(ws, h->off_cell),
+                                   at<int>(ws, h->off_idx), counts, s), "stochastic list: count");
+        h->slist_counts_ws = ws;
+    }
+    h->launches += 3;
+    CK(launch_stoch_list_offsets(counts, h->N, v, s), "stochastic list: offsets");
+    StochListHead head;
+    CK(cudaMemcpyAsync(&head, v.head, sizeof(head), cudaMemcpyDeviceToHost, s), "copy list head");
+    CK(cudaStreamSynchronize(s), "sync");
+    *records_host = (uint64_t)head.records;
+    if (head.records > 0xffffffffull || list_bytes < fof_stochastic_list_bytes(h, head.records)) return FOF_ERR_CAPACITY;
+    h->launches += h->N > 0 ? 1 : 0;
+    CK(launch_stoch_list_fill(at<float4>(ws, h->off_sorted), h->N, h->grid, at<unsigned int>(ws, h->off_cell),
+                              at<int>(ws, h->off_idx), b_link, alpha, v, s), "stochastic list: fill");
+    h->slist = list;
+    h->slist_b_link = b_link;
+    h->slist_alpha = alpha;
+    return FOF_OK;
+}
+
+int fof_link_stochastic_list(fof_handle *h, const void *list, uint64_t seed, uint32_t sample0, int32_t S,
+                             int32_t *labels, double *logp, float *grad_pos, void *scratch, void *ws, void *stream)
+{
+    if (!h || !ws || ((uintptr_t)ws & 255) || !list || !logp || S <= 0 || S > 1024) return FOF_ERR_INVALID_ARG;
+    if (h->N > 0 && (!labels || !scratch || ((uintptr_t)scratch & 3))) return FOF_ERR_INVALID_ARG;
+    if (!h->slist || h->slist != list) return FOF_ERR_STATE;  // not the list of the last fof_stochastic_list_build
+    cudaStream_t s = (cudaStream_t)stream;
+    h->counted = false;  // the caller may be overwriting the labels buffer whose group sizes were counted
+    h->launches += h->N > 0 ? (unsigned long long)(S / 4 + S % 4 + 2 * S) : 0;
+    CK(launch_link_stochastic_list(stoch_list_views(const_cast<void *>(list), h->N), h->N, h->slist_b_link,
+                                   h->slist_alpha, seed, sample0, S, static_cast<unsigned int *>(scratch), labels, logp,
+                                   grad_pos, at<Ctrl>(ws, h->off_ctrl), s),
+       "stochastic link kernels (list)");
+    return FOF_OK;
+}
+
 int fof_subgroups(fof_handle *h, const float *pos, const float *vel, const int32_t *particle_group,
                   const int32_t *group_size, int64_t K, float sigma_x, float sigma_v, float ell, int32_t *sub_labels,
                   void *ws, void *stream)
@@ -554,6 +617,7 @@ int fof_subgroups(fof_handle *h, const float *pos, const float *vel, const int32
     }
     h->linked = false;  // the member lists and their union-find re-use the link's arrays
     h->counted = false;
+    h->slist_counts_ws = nullptr;
     h->launches += h->N > 0 ? (K > 0 ? 6 : 3) : 0;
     CK(launch_subgroups(pos, vel, particle_group, group_size, h->N, K, h->L, sigma_x, sigma_v, ell,
                         at<unsigned int>(ws, h->off_cnt), at<unsigned int>(ws, h->off_part), at<int>(ws, h->off_idx),

@@ -171,6 +171,10 @@ struct fof_handle {
         const float *gmass, *gcom;
     } slot[2];
     cudaStream_t in_stream, run_stream;
+    // the potential-edge list the last fof_stochastic_list_build on this handle filled (nullptr: none is valid)
+    const void *slist;
+    float slist_b_link, slist_alpha;
+    const void *slist_counts_ws;  // the workspace whose group-size counters hold the record counts of the current link
 };
 
 namespace fof {
@@ -356,6 +360,47 @@ cudaError_t launch_link_stochastic_batch(const float4 *sorted, int64_t N, Grid g
                                          const int *idx_s, unsigned int *rel_s, float b_link, float alpha,
                                          unsigned long long seed, unsigned int sample0, int S, int *labels,
                                          double *logp, float *grad, Ctrl *ctrl, cudaStream_t s);
+
+// The potential-edge list of the stochastic path (fof_stochastic_list_build): views into the caller's buffer.
+struct StochListHead {
+    unsigned long long records;    // directed records (every potential edge appears under both of its particles)
+    unsigned long long potential;  // potential edges (owned records)
+    double logp0;                  // log p(y = 0): sum over the potential edges of log(1 - p)
+};
+constexpr int kListScanTile = 4096;  // entries per CTA of the offset scan
+struct StochList {
+    StochListHead *head;
+    unsigned long long *bsum;  // per scan tile: entries before it
+    unsigned int *roff;        // [N + 1] first record of every home particle (cell-sorted slot order)
+    int *home_orig;            // [N] original index of the home particle
+    uint4 *rec;                // two uint4 per record
+};
+inline size_t stoch_list_align(size_t x) { return (x + 255) & ~(size_t)255; }
+inline size_t stoch_list_fixed_bytes(int64_t N)
+{
+    const size_t tiles = (size_t)((N + kListScanTile) / kListScanTile) + 1;
+    return 256 + stoch_list_align(tiles * 8) + stoch_list_align(((size_t)N + 1) * 4) + stoch_list_align((size_t)N * 4 + 4);
+}
+inline StochList stoch_list_views(void *list, int64_t N)
+{
+    const size_t tiles = (size_t)((N + kListScanTile) / kListScanTile) + 1;
+    char *p = static_cast<char *>(list);
+    StochList v;
+    v.head = (StochListHead *)p;          p += 256;
+    v.bsum = (unsigned long long *)p;     p += stoch_list_align(tiles * 8);
+    v.roff = (unsigned int *)p;           p += stoch_list_align(((size_t)N + 1) * 4);
+    v.home_orig = (int *)p;               p += stoch_list_align((size_t)N * 4 + 4);
+    v.rec = (uint4 *)p;
+    return v;
+}
+cudaError_t launch_stoch_list_count(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
+                                    const int *idx_s, unsigned int *counts, cudaStream_t s);
+cudaError_t launch_stoch_list_offsets(const unsigned int *counts, int64_t N, StochList list, cudaStream_t s);
+cudaError_t launch_stoch_list_fill(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
+                                   const int *idx_s, float b_link, float alpha, StochList list, cudaStream_t s);
+cudaError_t launch_link_stochastic_list(StochList list, int64_t N, float b_link, float alpha, unsigned long long seed,
+                                        unsigned int sample0, int S, unsigned int *rel_s, int *labels, double *logp,
+                                        float *grad, Ctrl *ctrl, cudaStream_t s);
 
 cudaError_t launch_subgroups(const float *pos, const float *vel, const int *particle_group, const int *group_size,
                              int64_t N, int64_t K, float L, float sigma_x, float sigma_v, float ell,

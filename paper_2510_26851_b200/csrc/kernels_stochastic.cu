@@ -569,6 +569,331 @@ __global__ void __launch_bounds__(kBlock, 4) link_stochastic_multi_kernel(const 
     }
 }
 
+// =============================================================================================
+// The potential-edge list ("we do not rebuild the neighbor list"; section 3.2: the S samples of a
+// REINFORCE step share the neighbour structure).  Which pairs are potential edges, their p_ij, t_ij and
+// displacement do not depend on the sample: fof_stochastic_list_build writes them down once, home particle by home
+// particle in cell-sorted slot order (every potential edge under both of its particles, so that a particle's
+// score-function terms are its own records: no atomics, fixed summation order), and a sample is one coalesced stream
+// over the list: draw, log term, gradient term, hook.  A record is two 16-byte halves in two arrays (recA = rec,
+// recB = rec + records):
+//   A: cand   original index of the other particle; bit 31: this side OWNS the pair (its cell-sorted slot is the
+//             smaller one): it counts the edge, adds its log term and hooks
+//      p      p_ij (the bits the single-sample kernel compares the draw with)
+//      slot   cell-sorted slot of the other particle
+//      home   cell-sorted slot of the home particle
+//   B: dx, dy, dz  minimum-image displacement home - other, or 0 where t was clamped (no gradient there)
+//      t      t_ij clamped to [-30, 30]: log p - log(1 - p)
+// =============================================================================================
+struct BatchCount {
+    const Grid &g;
+    unsigned int &count;
+    __device__ __forceinline__ void operator()(StochSmem &sm, int cnt, bool wrap, const float4 &mine, int myslot, int s0,
+                                               int lane) const
+    {
+        count += (unsigned int)__popc(stoch_batch_adjacency(sm, cnt, wrap, mine, s0, g, lane));
+    }
+};
+
+struct BatchFill {
+    const Grid &g;
+    const StochParams &sp;
+    const int *__restrict__ idx_s;
+    uint4 *recA, *recB;
+    unsigned int &wr;     // this lane's next record
+    double &lp0;          // sum over the pairs this lane owns of log(1 - p) = log p - t: float32 log p and t as the
+                          // sample kernels, their difference and the sum in float64 (the sample pass adds t back for
+                          // every sampled edge: that cancellation must be exact)
+    unsigned int &ncand;  // pairs this lane owns
+    __device__ __forceinline__ void operator()(StochSmem &sm, int cnt, bool wrap, const float4 &mine, int myslot, int s0,
+                                               int lane) const
+    {
+        unsigned int m = stoch_batch_adjacency(sm, cnt, wrap, mine, s0, g, lane);
+        const float4 ph = sm.home[lane];
+        while (__any_sync(0xffffffffu, m != 0u)) {
+            if (m) {
+                const float4 pj = sm.cand[__ffs((int)m) - 1];
+                m &= m - 1u;
+                const int j = __float_as_int(pj.w);
+                const bool owned = j > myslot;
+                const float ddx = min_image(__fsub_rn(ph.x, pj.x), g.L, g.h);
+                const float ddy = min_image(__fsub_rn(ph.y, pj.y), g.L, g.h);
+                const float ddz = min_image(__fsub_rn(ph.z, pj.z), g.L, g.h);
+                const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(ddx, ddx), __fmul_rn(ddy, ddy)), __fmul_rn(ddz, ddz));
+                const float tt = __fmul_rn(sp.c, __fsub_rn(sp.b2, d2));
+                float e;
+                const float pr = sigmoid_fixed(tt, e);
+                const float tc = fminf(fmaxf(tt, -30.0f), 30.0f);
+                const unsigned int oj = (unsigned int)__ldg(idx_s + j);
+                if (owned) {
+                    ++ncand;
+                    lp0 += (double)(-__logf(__fadd_rn(1.0f, e))) - (double)tc;
+                }
+                const bool gon = tt == tc;
+                uint4 a, b;
+                a.x = oj | (owned ? 0x80000000u : 0u);
+                a.y = (unsigned int)__float_as_int(pr);
+                a.z = (unsigned int)j;
+                a.w = (unsigned int)myslot;
+                b.x = (unsigned int)__float_as_int(gon ? ddx : 0.0f);
+                b.y = (unsigned int)__float_as_int(gon ? ddy : 0.0f);
+                b.z = (unsigned int)__float_as_int(gon ? ddz : 0.0f);
+                b.w = (unsigned int)__float_as_int(tc);
+                __stcs(recA + wr, a);
+                __stcs(recB + wr, b);
+                ++wr;
+            }
+        }
+    }
+};
+
+// FILL = false: counts[slot] = number of records of the home particle in `slot`;
+// FILL = true: the records, from roff[slot] on (the scanned counts), and home_orig[slot] = its original index.
+template <bool FILL>
+__global__ void __launch_bounds__(kBlock, FOF_STOCH_MINB) stoch_list_kernel(const float4 *__restrict__ sorted, int64_t N, Grid g,
+                                                            const unsigned int *__restrict__ cs,
+                                                            const int *__restrict__ idx_s, StochParams sp,
+                                                            StochList list, unsigned int *counts)
+{
+    constexpr unsigned int kAll = 0xffffffffu;
+    __shared__ StochSmem s_all[kStochWarps];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    StochSmem &sm = s_all[wib];
+    const int64_t s64 = ((int64_t)blockIdx.x * kStochWarps + wib) * 32 + lane;
+    const bool valid = s64 < N;
+    const int myslot = (int)min(s64, N - 1);
+    const float4 me = __ldg(sorted + myslot);
+    const unsigned int oi = (unsigned int)__ldg(idx_s + myslot);
+    const int cx = min(__float2int_rd(__fmul_rn(me.x, g.inv_cell)), g.n_minus_1),
+              cy = min(__float2int_rd(__fmul_rn(me.y, g.inv_cell)), g.n_minus_1),
+              cz = min(__float2int_rd(__fmul_rn(me.z, g.inv_cell)), g.n_minus_1);
+    if (!FILL) {
+        unsigned int count = 0;
+        const BatchCount batch = {g, count};
+        stoch_tile_warp(sorted, g, cs, sm, me, myslot, oi, valid, cx, cy, cz, lane, batch);
+        if (valid) counts[myslot] = count;
+    } else {
+        if (valid) list.home_orig[myslot] = (int)oi;
+        unsigned int wr = valid ? list.roff[myslot] : 0u, ncand = 0;
+        double lp0 = 0.0;
+        const BatchFill batch = {g, sp, idx_s, list.rec, list.rec + list.roff[N], wr, lp0, ncand};
+        stoch_tile_warp(sorted, g, cs, sm, me, myslot, oi, valid, cx, cy, cz, lane, batch);
+        __syncwarp();
+        double lpd = lp0;
+        for (int o = 16; o > 0; o >>= 1) {
+            lpd += __shfl_xor_sync(kAll, lpd, o);
+            ncand += __shfl_xor_sync(kAll, ncand, o);
+        }
+        if (lane == 0 && ncand) {
+            atomicAdd(&list.head->logp0, lpd);
+            atomicAdd(&list.head->potential, (unsigned long long)ncand);
+        }
+    }
+}
+
+// ---- exclusive scan of roff[0 .. N) in place, roff[N] = total (three small kernels: tile sums, their scan, apply)
+constexpr int kListScanThreads = 512, kListScanPer = kListScanTile / kListScanThreads;
+
+__device__ __forceinline__ unsigned long long block_exclusive_u64(unsigned long long v, unsigned long long *s_w,
+                                                                  unsigned long long &total)
+{
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    unsigned long long incl = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned long long t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    __syncthreads();  // s_w may still be read from a previous call
+    if (lane == 31) s_w[w] = incl;
+    __syncthreads();
+    unsigned long long before = 0, all = 0;
+    for (int k = 0; k < nw; ++k) {
+        const unsigned long long t = s_w[k];
+        if (k < w) before += t;
+        all += t;
+    }
+    total = all;
+    return before + incl - v;
+}
+
+__global__ void __launch_bounds__(kListScanThreads) list_scan_sums_kernel(const unsigned int *__restrict__ v, int64_t n,
+                                                                          unsigned long long *bsum)
+{
+    __shared__ unsigned long long s_w[kListScanThreads / 32];
+    const int64_t i0 = (int64_t)blockIdx.x * kListScanTile + (int64_t)threadIdx.x * kListScanPer;
+    unsigned long long sum = 0;
+#pragma unroll
+    for (int k = 0; k < kListScanPer; ++k)
+        if (i0 + k < n) sum += v[i0 + k];
+    unsigned long long total;
+    (void)block_exclusive_u64(sum, s_w, total);
+    if (threadIdx.x == 0) bsum[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(1024) list_scan_top_kernel(unsigned long long *bsum, int nb, StochListHead *head)
+{
+    __shared__ unsigned long long s_w[32];
+    unsigned long long carry = 0;
+    for (int base = 0; base < nb; base += 1024) {
+        const int i = base + (int)threadIdx.x;
+        const unsigned long long v = i < nb ? bsum[i] : 0ull;
+        unsigned long long total;
+        const unsigned long long ex = block_exclusive_u64(v, s_w, total);
+        if (i < nb) bsum[i] = carry + ex;
+        carry += total;
+    }
+    if (threadIdx.x == 0) {
+        head->records = carry;
+        head->potential = 0ull;
+        head->logp0 = 0.0;
+    }
+}
+
+__global__ void __launch_bounds__(kListScanThreads) list_scan_apply_kernel(unsigned int *v, int64_t n,
+                                                                           const unsigned long long *__restrict__ bsum,
+                                                                           const StochListHead *head)
+{
+    __shared__ unsigned long long s_w[kListScanThreads / 32];
+    const int64_t i0 = (int64_t)blockIdx.x * kListScanTile + (int64_t)threadIdx.x * kListScanPer;
+    unsigned int x[kListScanPer];
+    unsigned long long sum = 0;
+#pragma unroll
+    for (int k = 0; k < kListScanPer; ++k) {
+        x[k] = i0 + k < n ? v[i0 + k] : 0u;
+        sum += x[k];
+    }
+    unsigned long long total;
+    unsigned long long run = bsum[blockIdx.x] + block_exclusive_u64(sum, s_w, total);
+#pragma unroll
+    for (int k = 0; k < kListScanPer; ++k) {
+        if (i0 + k < n) v[i0 + k] = (unsigned int)run;
+        run += x[k];
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) v[n] = (unsigned int)head->records;
+}
+
+// SB samples over the list.  One warp per 32 consecutive home particles = one contiguous run of records, read 32 at
+// a time (coalesced 128-bit loads), every lane one record.  The gradient terms of a home particle are consecutive
+// lanes: a segmented warp scan sums them (the segment structure is shared by the SB samples), a run that continues
+// in the next 32 records is carried over in registers, and the lane that holds a particle's last record stores its
+// total: every particle's sum is formed by this warp alone, in record order.
+// The union-find of sample k is rel + k N, in cell-sorted slot space as in fof_link (neighbours in space are
+// neighbours in memory), ordered by list.home_orig, which is idx_s.
+#ifndef FOF_STREAM_BLOCK
+#define FOF_STREAM_BLOCK 64   // small CTAs: the runs of neighbouring tiles differ a lot in length (a halo next to background)
+#endif
+#ifndef FOF_STREAM_MINB
+#define FOF_STREAM_MINB 16
+#endif
+constexpr int kStreamBlock = FOF_STREAM_BLOCK;
+template <int SB>
+__global__ void __launch_bounds__(kStreamBlock, FOF_STREAM_MINB) stoch_stream_kernel(StochList list, int64_t N, StochKeys keys, float gscale,
+                                                              unsigned int *rel, double *logp, float *grad, Ctrl *ctrl)
+{
+    constexpr unsigned int kAll = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const int64_t tile = ((int64_t)blockIdx.x * kStreamBlock + threadIdx.x) >> 5;  // 32 homes
+    const int64_t h0 = tile * 32;
+    if (h0 >= N) return;  // whole warps only
+    const unsigned int rb = list.roff[h0], re = list.roff[min(h0 + 32, N)];
+    const uint4 *__restrict__ recA = list.rec;
+    const uint4 *__restrict__ recB = list.rec + list.roff[N];
+    const bool want_grad = grad != nullptr;
+    double lp[SB];  // sum of t over the sampled edges: cancels against the t inside list.head->logp0, hence float64
+    float carry[SB][3];
+    unsigned int nedge[SB];
+#pragma unroll
+    for (int k = 0; k < SB; ++k) { lp[k] = 0.0; nedge[k] = 0u; carry[k][0] = carry[k][1] = carry[k][2] = 0.0f; }
+    const unsigned int tile_orig = (unsigned int)__ldg(list.home_orig + min(h0 + lane, N - 1));  // lane l: original index of home h0 + l
+    int prev_home = -1;  // home of the record before this batch
+    for (unsigned int r0 = rb; r0 < re; r0 += 32) {
+        const unsigned int r = r0 + lane;
+        const bool has = r < re;
+        uint4 a = make_uint4(0u, 0u, 0u, 0u), b = make_uint4(0u, 0u, 0u, 0u);
+        if (has) {
+            a = __ldcs(recA + r);
+            b = __ldcs(recB + r);
+        }
+        const int home = has ? (int)a.w : -2 - lane;
+        const bool owned = (a.x >> 31) != 0u;
+        const unsigned int oj = a.x & 0x7fffffffu;
+        const float pr = __int_as_float((int)a.y), tc = __int_as_float((int)b.w);
+        const float ddx = __int_as_float((int)b.x), ddy = __int_as_float((int)b.y), ddz = __int_as_float((int)b.z);
+        const int j = (int)a.z;
+        const unsigned int ooi = __shfl_sync(kAll, tile_orig, (int)a.w - (int)h0);  // every home of the run is in my tile
+        const unsigned int klo = min(ooi, oj), khi = max(ooi, oj);
+        // segments of equal home: `first` = lane of my segment's first record in this batch; the last record of a
+        // particle is where the next record (the next batch's first one for lane 31) has another home
+        const int left = __shfl_up_sync(kAll, home, 1);
+        const unsigned int heads = __ballot_sync(kAll, lane == 0 || left != home);
+        const int first = 31 - __clz((int)(heads & (0xffffffffu >> (31 - lane))));
+        int right = __shfl_down_sync(kAll, home, 1);
+        if (lane == 31) right = (r + 1 < re) ? (int)__ldg(&recA[r + 1].w) : -1;
+        const bool tail = has && right != home;
+        const bool cont = lane == first && first == 0 && home == prev_home;  // lane 0 continues the previous batch's run
+        prev_home = __shfl_sync(kAll, home, 31);
+        bool hook[SB];
+#pragma unroll
+        for (int k = 0; k < SB; ++k) {
+            const float u = __fmul_rn((float)rng_u24(keys.k[k], klo, khi), 5.9604644775390625e-8f);
+            const bool y = has && u < pr;
+            hook[k] = owned && y;
+            if (want_grad) {
+                const float cgr = ((y ? 1.0f : 0.0f) - pr) * gscale;
+                float gx = cgr * ddx, gy = cgr * ddy, gz = cgr * ddz;
+                if (cont) { gx += carry[k][0]; gy += carry[k][1]; gz += carry[k][2]; }
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const float vx = __shfl_up_sync(kAll, gx, o), vy = __shfl_up_sync(kAll, gy, o),
+                                vz = __shfl_up_sync(kAll, gz, o);
+                    if (lane - o >= first) { gx += vx; gy += vy; gz += vz; }
+                }
+                if (tail) {
+                    float *gk = grad + (int64_t)k * 3 * N + 3 * (int64_t)ooi;
+                    gk[0] = gx;
+                    gk[1] = gy;
+                    gk[2] = gz;
+                }
+                carry[k][0] = __shfl_sync(kAll, gx, 31);
+                carry[k][1] = __shfl_sync(kAll, gy, 31);
+                carry[k][2] = __shfl_sync(kAll, gz, 31);
+            }
+            if (hook[k]) {
+                lp[k] += (double)tc;
+                ++nedge[k];
+            }
+        }
+        // the hooks of the SB samples: first every parent load (independent, all in flight together), then the
+        // unions that are not already inside one set
+        int pa[SB], pb[SB];
+#pragma unroll
+        for (int k = 0; k < SB; ++k) {
+            const unsigned int *rk = rel + (int64_t)k * N;
+            pa[k] = pb[k] = 0;
+            if (hook[k]) {
+                pa[k] = home - (int)rk[home];
+                pb[k] = j - (int)rk[j];
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < SB; ++k)
+            if (pa[k] != pb[k]) unite_rel(rel + (int64_t)k * N, list.home_orig, home, j);  // same parent: one set
+    }
+    unsigned int nedge_all = 0;
+#pragma unroll
+    for (int k = 0; k < SB; ++k) {
+        double lpd = lp[k];
+        for (int o = 16; o > 0; o >>= 1) lpd += __shfl_xor_sync(kAll, lpd, o);
+        if (h0 == 0) lpd += list.head->logp0;  // log p(y) = log p(all absent) + sum over the sampled edges of t
+        if (lane == 0 && lpd != 0.0) atomicAdd(logp + k, lpd);
+        nedge_all += nedge[k];
+    }
+    for (int o = 16; o > 0; o >>= 1) nedge_all += __shfl_xor_sync(kAll, nedge_all, o);
+    if (lane == 0 && nedge_all) atomicAdd(&ctrl->edges, (unsigned long long)nedge_all);  // sampled edges, all samples
+    if (h0 == 0 && lane == 0 && keys.count_potential) ctrl->pair_tests = list.head->potential;
+}
+
 static inline unsigned int blocks_for(int64_t n, int per_block) { return (unsigned int)((n + per_block - 1) / per_block); }
 
 static unsigned int stoch_key(unsigned long long seed, unsigned int sample)
@@ -636,6 +961,83 @@ cudaError_t launch_link_stochastic_batch(const float4 *sorted, int64_t N, Grid g
         int *lab = labels + (size_t)k * (size_t)N;
         iota_kernel<<<grid, kBlock, 0, s>>>(lab, N);
         if ((e = launch_write_labels(rel_s + (size_t)k * (size_t)N, idx_s, lab, N, nullptr, nullptr, nullptr, 0, nullptr, s)) != cudaSuccess) return e;
+    }
+    return cudaGetLastError();
+}
+
+static StochParams stoch_params(float b_link, float alpha)
+{
+    StochParams sp;
+    sp.b2 = b_link * b_link;
+    sp.c = alpha / sp.b2;
+    sp.gscale = -2.0f * sp.c;
+    sp.key = 0u;
+    return sp;
+}
+
+// counts[slot] = records of the home particle in `slot` (the neighbour search without the per-pair work)
+cudaError_t launch_stoch_list_count(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
+                                    const int *idx_s, unsigned int *counts, cudaStream_t s)
+{
+    if (N <= 0) return cudaSuccess;
+    StochList none = {};
+    stoch_list_kernel<false><<<blocks_for(N, kBlock), kBlock, 0, s>>>(sorted, N, g, cell_start, idx_s,
+                                                                      stoch_params(1.0f, 0.0f), none, counts);
+    return cudaGetLastError();
+}
+
+// counts -> list.roff (exclusive scan, roff[N] = total) and list.head->records
+cudaError_t launch_stoch_list_offsets(const unsigned int *counts, int64_t N, StochList list, cudaStream_t s)
+{
+    const int nb = (int)((N + kListScanTile) / kListScanTile);  // tiles over N + 1 entries
+    cudaError_t e;
+    if (N > 0 && (e = cudaMemcpyAsync(list.roff, counts, (size_t)N * sizeof(unsigned int), cudaMemcpyDeviceToDevice, s)) != cudaSuccess)
+        return e;
+    list_scan_sums_kernel<<<nb, kListScanThreads, 0, s>>>(list.roff, N, list.bsum);
+    list_scan_top_kernel<<<1, 1024, 0, s>>>(list.bsum, nb, list.head);
+    list_scan_apply_kernel<<<nb, kListScanThreads, 0, s>>>(list.roff, N, list.bsum, list.head);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_stoch_list_fill(const float4 *sorted, int64_t N, Grid g, const unsigned int *cell_start,
+                                   const int *idx_s, float b_link, float alpha, StochList list, cudaStream_t s)
+{
+    if (N <= 0) return cudaSuccess;
+    stoch_list_kernel<true><<<blocks_for(N, kBlock), kBlock, 0, s>>>(sorted, N, g, cell_start, idx_s,
+                                                                     stoch_params(b_link, alpha), list, nullptr);
+    return cudaGetLastError();
+}
+
+// S samples sample0 .. sample0 + S - 1 over the list, four per pass (then one by one).
+cudaError_t launch_link_stochastic_list(StochList list, int64_t N, float b_link, float alpha, unsigned long long seed,
+                                        unsigned int sample0, int S, unsigned int *rel_s, int *labels, double *logp,
+                                        float *grad, Ctrl *ctrl, cudaStream_t s)
+{
+    cudaError_t e;
+    if ((e = cudaMemsetAsync(logp, 0, (size_t)S * sizeof(double), s)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(&ctrl->edges, 0, 2 * sizeof(unsigned long long), s)) != cudaSuccess) return e;
+    if (N <= 0) return cudaSuccess;
+    if ((e = cudaMemsetAsync(rel_s, 0, (size_t)S * (size_t)N * sizeof(unsigned int), s)) != cudaSuccess) return e;
+    // a particle without potential edges has no record: its score function is the zero written here
+    if (grad && (e = cudaMemsetAsync(grad, 0, (size_t)S * (size_t)N * 3 * sizeof(float), s)) != cudaSuccess) return e;
+    const StochParams sp = stoch_params(b_link, alpha);
+    const unsigned int grid = blocks_for(N, kBlock);
+    for (int k0 = 0; k0 < S;) {
+        StochKeys keys = {{0u, 0u, 0u, 0u}, k0 == 0 ? 1 : 0};
+        const int sb = S - k0 >= 4 ? 4 : 1;
+        for (int k = 0; k < sb; ++k) keys.k[k] = stoch_key(seed, sample0 + (unsigned int)(k0 + k));
+        unsigned int *rel = rel_s + (size_t)k0 * (size_t)N;
+        float *gk = grad ? grad + (size_t)k0 * 3 * (size_t)N : nullptr;
+        const unsigned int sgrid = blocks_for(N, kStreamBlock);
+        if (sb == 4) stoch_stream_kernel<4><<<sgrid, kStreamBlock, 0, s>>>(list, N, keys, sp.gscale, rel, logp + k0, gk, ctrl);
+        else stoch_stream_kernel<1><<<sgrid, kStreamBlock, 0, s>>>(list, N, keys, sp.gscale, rel, logp + k0, gk, ctrl);
+        k0 += sb;
+    }
+    for (int k = 0; k < S; ++k) {
+        int *lab = labels + (size_t)k * (size_t)N;
+        iota_kernel<<<grid, kBlock, 0, s>>>(lab, N);
+        if ((e = launch_write_labels(rel_s + (size_t)k * (size_t)N, list.home_orig, lab, N, nullptr, nullptr, nullptr, 0,
+                                     nullptr, s)) != cudaSuccess) return e;
     }
     return cudaGetLastError();
 }

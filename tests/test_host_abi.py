@@ -89,6 +89,34 @@ def test_stochastic_batch_argument_and_state_errors(B):
     B.fof_destroy(h)
 
 
+def test_stochastic_list_argument_and_state_errors(B):
+    """The potential-edge list calls reject bad arguments and a missing fof_link / build before touching memory."""
+    import ctypes
+
+    L = B.lib()
+    h = B.fof_create(1000, 10.0, 1.0, 5)
+    fixed = L.fof_stochastic_list_bytes(h, 0)
+    assert fixed >= 256 + 1001 * 4 + 1000 * 4 and fixed % 256 == 0
+    assert L.fof_stochastic_list_bytes(h, 10) == fixed + 320 and L.fof_stochastic_list_bytes(None, 10) == 0
+    raw = np.zeros(4096, dtype=np.uint8)
+    p = ctypes.c_void_p((raw.ctypes.data + 255) & ~255)        # 256-B aligned host address: never dereferenced here
+    odd = ctypes.c_void_p(p.value + 4)
+    R = ctypes.c_uint64()
+    build = lambda b_link, alpha, lst=p, nbytes=fixed, ws=p: L.fof_stochastic_list_build(
+        h, ctypes.c_float(b_link), ctypes.c_float(alpha), lst, nbytes, ctypes.byref(R), ws, None)
+    assert build(1.5, 2.0) == B.FOF_ERR_INVALID_ARG            # b_link above the plan's candidate radius
+    assert build(1.0, float("inf")) == B.FOF_ERR_INVALID_ARG
+    assert build(1.0, 2.0, lst=odd) == B.FOF_ERR_INVALID_ARG   # list not 256-B aligned
+    assert build(1.0, 2.0, ws=odd) == B.FOF_ERR_INVALID_ARG
+    assert build(1.0, 2.0, nbytes=fixed - 1) == B.FOF_ERR_INVALID_ARG   # not even room for the offsets
+    assert build(1.0, 2.0) == B.FOF_ERR_STATE                  # no fof_link on this (handle, workspace) yet
+    run = lambda S, lst=p: L.fof_link_stochastic_list(h, lst, 1, 0, S, p, p, None, p, p, None)
+    assert run(0) == B.FOF_ERR_INVALID_ARG and run(2000) == B.FOF_ERR_INVALID_ARG
+    assert run(2, lst=None) == B.FOF_ERR_INVALID_ARG
+    assert run(2) == B.FOF_ERR_STATE                           # no list was built
+    B.fof_destroy(h)
+
+
 def test_grid_choice_keeps_cell_side_above_b(B):
     """H0: cell side L/n >= 1.001 b for every plan (R3), n >= 3."""
     rng = np.random.default_rng(1)

@@ -747,6 +747,71 @@ def test_stochastic_batch_equals_single_samples_and_oracle(B, S, drop):
     f.close()
 
 
+@pytest.mark.parametrize("alpha,kappa,S,drop", [(5.0, 1.5, 7, 0), (0.5, 1.25, 4, 1), (50.0, 1.0, 1, 2), (4.0, 1.5, 5, 3)])
+def test_stochastic_list_against_oracle(B, alpha, kappa, S, drop):
+    """fof_stochastic_list_build + fof_link_stochastic_list: the potential edges written down once, every sample a
+    stream over them.  Sample k = the oracle's sample (labels, potential and sampled edge counts bit-exact, log p
+    to float64 summation order, score function to float32 order) = fof_link_stochastic(sample0 + k); records =
+    2 x potential edges; a buffer that is too small reports the size it needs."""
+    w = inputs.scaled(inputs.CONFIGS["cfg1"], 40)
+    p = inputs.make_positions(w)
+    p = np.ascontiguousarray(p[:len(p) - drop]) if drop else p
+    b_link = w.b
+    b_cand = float(np.float32(kappa * w.b))
+    f = B.FoF(len(p), w.L, b_cand, w.N_min, path="cells")
+    f.link(torch.from_numpy(p).cuda())
+    small = torch.empty(B.fof_stochastic_list_bytes(f.h, 0), dtype=torch.uint8, device="cuda")
+    records, filled = B.fof_stochastic_list_build(f.h, b_link, alpha, small, f.ws)
+    o0 = oracle.stochastic(p, w.L, b_cand, b_link, alpha, 99, 3)
+    assert not filled and records == 2 * o0["n_cand"]
+    with pytest.raises(B.FofError) as e:      # a failed build leaves no valid list
+        f.link_stochastic_list(small, 99, 3, 1)
+    assert e.value.code == B.FOF_ERR_STATE
+    slist, records2 = f.stochastic_list(b_link, alpha)
+    assert records2 == records
+    for want_grad in (True, False):
+        labels, logp, grad = f.link_stochastic_list(slist, 99, 3, S, want_grad=want_grad)
+        E_all, ncand, _ = f.link_stats()
+        E_sum = 0
+        for k in range(S):
+            o = oracle.stochastic(p, w.L, b_cand, b_link, alpha, 99, 3 + k)
+            assert ncand == o["n_cand"]
+            E_sum += o["n_edge"]
+            assert np.array_equal(labels[k].cpu().numpy(), o["labels"]), f"sample {k}: components differ"
+            assert abs(float(logp[k].item()) - o["logp"]) <= 2e-6 * abs(o["logp"]) + 1e-6
+            if want_grad:
+                gk = grad[k].cpu().numpy().astype(np.float64)
+                assert np.abs(gk - o["grad"]).max() <= 2e-5 * np.abs(o["grad"]).max()
+        assert E_all == E_sum and (want_grad or grad is None)
+    l1, lp1, g1 = f.link_stochastic(b_link, alpha, 99, 3)      # the list survives the calls that recompute
+    la, lpa, ga = f.link_stochastic_list(slist, 99, 3, 1)
+    assert torch.equal(l1, la[0])
+    assert torch.allclose(g1, ga[0], rtol=0, atol=2e-5 * float(g1.abs().max()))
+    f.link(torch.from_numpy(p).cuda())                         # ... but not a new link
+    with pytest.raises(B.FofError) as e:
+        f.link_stochastic_list(slist, 99, 3, 1)
+    assert e.value.code == B.FOF_ERR_STATE
+    f.close()
+
+
+def test_stochastic_list_wraps(B):
+    """n = 5 cells per axis: every candidate run wraps; brute-force oracle."""
+    rng = np.random.default_rng(17)
+    L, b = 8.0, 1.0
+    p = (rng.random((3000, 3)) * L).astype(np.float32)
+    f = B.FoF(len(p), L, 1.5, 5, path="cells")
+    f.link(torch.from_numpy(p).cuda())
+    slist, records = f.stochastic_list(b, 3.0)
+    labels, logp, grad = f.link_stochastic_list(slist, 1, 0, 2)
+    for k in range(2):
+        o = oracle.stochastic(p, L, 1.5, b, 3.0, 1, k, brute=True)
+        assert records == 2 * o["n_cand"]
+        assert np.array_equal(labels[k].cpu().numpy(), o["labels"])
+        assert abs(float(logp[k].item()) - o["logp"]) <= 2e-6 * abs(o["logp"])
+        assert np.abs(grad[k].cpu().numpy() - o["grad"]).max() <= 2e-5 * np.abs(o["grad"]).max()
+    f.close()
+
+
 def test_groups_recounts_after_the_labels_buffer_was_reused(B):
     """fof_groups re-uses the sizes fof_link counted only for the labels fof_link wrote: once a stochastic sample has
     been written into the same buffer, the groups are those of the sample (counted afresh)."""
