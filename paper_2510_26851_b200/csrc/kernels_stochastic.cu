@@ -514,7 +514,7 @@ __global__ void __launch_bounds__(kBlock, FOF_STOCH_MINB) link_stochastic_kernel
 // SB samples of the same binning in one pass (fof_link_stochastic_batch).  keys: one generator key per
 // sample; rel: SB union-find arrays of N; logp: SB doubles; grad: SB arrays of [N][3] or nullptr.
 struct StochKeys {
-    unsigned int k[4];
+    unsigned int k[8];
     int count_potential;  // the pass that reports the potential edges (they are the same in every pass)
 };
 
@@ -807,13 +807,20 @@ __global__ void __launch_bounds__(kStreamBlock, FOF_STREAM_MINB) stoch_stream_ke
     for (int k = 0; k < SB; ++k) { lp[k] = 0.0; nedge[k] = 0u; carry[k][0] = carry[k][1] = carry[k][2] = 0.0f; }
     const unsigned int tile_orig = (unsigned int)__ldg(list.home_orig + min(h0 + lane, N - 1));  // lane l: original index of home h0 + l
     int prev_home = -1;  // home of the record before this batch
+    // the next batch is loaded while this one is worked on
+    uint4 an = make_uint4(0u, 0u, 0u, 0u), bn = make_uint4(0u, 0u, 0u, 0u);
+    if (rb + lane < re) {
+        an = __ldcs(recA + rb + lane);
+        bn = __ldcs(recB + rb + lane);
+    }
     for (unsigned int r0 = rb; r0 < re; r0 += 32) {
         const unsigned int r = r0 + lane;
         const bool has = r < re;
-        uint4 a = make_uint4(0u, 0u, 0u, 0u), b = make_uint4(0u, 0u, 0u, 0u);
-        if (has) {
-            a = __ldcs(recA + r);
-            b = __ldcs(recB + r);
+        const uint4 a = an, b = bn;
+        an = make_uint4(0u, 0u, 0u, 0u);
+        if (r + 32 < re) {
+            an = __ldcs(recA + r + 32);
+            bn = __ldcs(recB + r + 32);
         }
         const int home = has ? (int)a.w : -2 - lane;
         const bool owned = (a.x >> 31) != 0u;
@@ -829,7 +836,8 @@ __global__ void __launch_bounds__(kStreamBlock, FOF_STREAM_MINB) stoch_stream_ke
         const unsigned int heads = __ballot_sync(kAll, lane == 0 || left != home);
         const int first = 31 - __clz((int)(heads & (0xffffffffu >> (31 - lane))));
         int right = __shfl_down_sync(kAll, home, 1);
-        if (lane == 31) right = (r + 1 < re) ? (int)__ldg(&recA[r + 1].w) : -1;
+        const int next0 = __shfl_sync(kAll, (int)an.w, 0);  // home of the next batch's first record
+        if (lane == 31) right = (r + 1 < re) ? next0 : -1;
         const bool tail = has && right != home;
         const bool cont = lane == first && first == 0 && home == prev_home;  // lane 0 continues the previous batch's run
         prev_home = __shfl_sync(kAll, home, 31);
@@ -944,7 +952,7 @@ cudaError_t launch_link_stochastic_batch(const float4 *sorted, int64_t N, Grid g
     sp.key = 0u;
     const unsigned int grid = blocks_for(N, kBlock);
     for (int k0 = 0; k0 < S;) {
-        StochKeys keys = {{0u, 0u, 0u, 0u}, k0 == 0 ? 1 : 0};
+        StochKeys keys = {{0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u}, k0 == 0 ? 1 : 0};
         const int sb = S - k0 >= 4 ? 4 : 1;
         for (int k = 0; k < sb; ++k) keys.k[k] = stoch_key(seed, sample0 + (unsigned int)(k0 + k));
         unsigned int *rel = rel_s + (size_t)k0 * (size_t)N;
@@ -1023,13 +1031,18 @@ cudaError_t launch_link_stochastic_list(StochList list, int64_t N, float b_link,
     const StochParams sp = stoch_params(b_link, alpha);
     const unsigned int grid = blocks_for(N, kBlock);
     for (int k0 = 0; k0 < S;) {
-        StochKeys keys = {{0u, 0u, 0u, 0u}, k0 == 0 ? 1 : 0};
+        StochKeys keys = {{0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u}, k0 == 0 ? 1 : 0};
+#ifdef FOF_STREAM_SB8
+        const int sb = S - k0 >= 8 ? 8 : (S - k0 >= 4 ? 4 : 1);
+#else
         const int sb = S - k0 >= 4 ? 4 : 1;
+#endif
         for (int k = 0; k < sb; ++k) keys.k[k] = stoch_key(seed, sample0 + (unsigned int)(k0 + k));
         unsigned int *rel = rel_s + (size_t)k0 * (size_t)N;
         float *gk = grad ? grad + (size_t)k0 * 3 * (size_t)N : nullptr;
         const unsigned int sgrid = blocks_for(N, kStreamBlock);
-        if (sb == 4) stoch_stream_kernel<4><<<sgrid, kStreamBlock, 0, s>>>(list, N, keys, sp.gscale, rel, logp + k0, gk, ctrl);
+        if (sb == 8) stoch_stream_kernel<8><<<sgrid, kStreamBlock, 0, s>>>(list, N, keys, sp.gscale, rel, logp + k0, gk, ctrl);
+        else if (sb == 4) stoch_stream_kernel<4><<<sgrid, kStreamBlock, 0, s>>>(list, N, keys, sp.gscale, rel, logp + k0, gk, ctrl);
         else stoch_stream_kernel<1><<<sgrid, kStreamBlock, 0, s>>>(list, N, keys, sp.gscale, rel, logp + k0, gk, ctrl);
         k0 += sb;
     }
