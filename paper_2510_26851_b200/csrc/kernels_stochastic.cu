@@ -514,7 +514,7 @@ __global__ void __launch_bounds__(kBlock, FOF_STOCH_MINB) link_stochastic_kernel
 // SB samples of the same binning in one pass (fof_link_stochastic_batch).  keys: one generator key per
 // sample; rel: SB union-find arrays of N; logp: SB doubles; grad: SB arrays of [N][3] or nullptr.
 struct StochKeys {
-    unsigned int k[8];
+    unsigned int k[4];
     int count_potential;  // the pass that reports the potential edges (they are the same in every pass)
 };
 
@@ -952,7 +952,7 @@ cudaError_t launch_link_stochastic_batch(const float4 *sorted, int64_t N, Grid g
     sp.key = 0u;
     const unsigned int grid = blocks_for(N, kBlock);
     for (int k0 = 0; k0 < S;) {
-        StochKeys keys = {{0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u}, k0 == 0 ? 1 : 0};
+        StochKeys keys = {{0u, 0u, 0u, 0u}, k0 == 0 ? 1 : 0};
         const int sb = S - k0 >= 4 ? 4 : 1;
         for (int k = 0; k < sb; ++k) keys.k[k] = stoch_key(seed, sample0 + (unsigned int)(k0 + k));
         unsigned int *rel = rel_s + (size_t)k0 * (size_t)N;
@@ -1031,18 +1031,13 @@ cudaError_t launch_link_stochastic_list(StochList list, int64_t N, float b_link,
     const StochParams sp = stoch_params(b_link, alpha);
     const unsigned int grid = blocks_for(N, kBlock);
     for (int k0 = 0; k0 < S;) {
-        StochKeys keys = {{0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u}, k0 == 0 ? 1 : 0};
-#ifdef FOF_STREAM_SB8
-        const int sb = S - k0 >= 8 ? 8 : (S - k0 >= 4 ? 4 : 1);
-#else
-        const int sb = S - k0 >= 4 ? 4 : 1;
-#endif
+        StochKeys keys = {{0u, 0u, 0u, 0u}, k0 == 0 ? 1 : 0};
+        const int sb = S - k0 >= 4 ? 4 : 1;  // eight per pass: 96+ registers, 2.6 ms per sample instead of 1.8 at cfg2
         for (int k = 0; k < sb; ++k) keys.k[k] = stoch_key(seed, sample0 + (unsigned int)(k0 + k));
         unsigned int *rel = rel_s + (size_t)k0 * (size_t)N;
         float *gk = grad ? grad + (size_t)k0 * 3 * (size_t)N : nullptr;
         const unsigned int sgrid = blocks_for(N, kStreamBlock);
-        if (sb == 8) stoch_stream_kernel<8><<<sgrid, kStreamBlock, 0, s>>>(list, N, keys, sp.gscale, rel, logp + k0, gk, ctrl);
-        else if (sb == 4) stoch_stream_kernel<4><<<sgrid, kStreamBlock, 0, s>>>(list, N, keys, sp.gscale, rel, logp + k0, gk, ctrl);
+        if (sb == 4) stoch_stream_kernel<4><<<sgrid, kStreamBlock, 0, s>>>(list, N, keys, sp.gscale, rel, logp + k0, gk, ctrl);
         else stoch_stream_kernel<1><<<sgrid, kStreamBlock, 0, s>>>(list, N, keys, sp.gscale, rel, logp + k0, gk, ctrl);
         k0 += sb;
     }
