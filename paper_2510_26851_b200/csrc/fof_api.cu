@@ -205,6 +205,8 @@ int fof_create(int64_t N, float L, float b, int32_t N_min, fof_handle **out)
     return FOF_OK;
 }
 
+static void host_streams_free(fof_handle *h);
+
 void fof_destroy(fof_handle *h)
 {
     if (!h) return;
@@ -215,16 +217,7 @@ void fof_destroy(fof_handle *h)
     }
     if (h->in_stream) {
         (void)cudaDeviceSynchronize();  // a submitted input may still be in flight
-        for (auto &sl : h->slot) {
-            (void)cudaStreamDestroy(sl.out);
-            (void)cudaEventDestroy(sl.ev_in);
-            (void)cudaEventDestroy(sl.ev_linked);
-            (void)cudaEventDestroy(sl.ev_groups);
-            (void)cudaEventDestroy(sl.ev_ctrl);
-            (void)cudaFreeHost(sl.ctrl_pin);
-        }
-        (void)cudaStreamDestroy(h->in_stream);
-        (void)cudaStreamDestroy(h->run_stream);
+        host_streams_free(h);
     }
     delete h;
 }
@@ -595,7 +588,7 @@ int fof_link_stochastic_list(fof_handle *h, const void *list, uint64_t seed, uin
     h->launches += h->N > 0 ? (unsigned long long)(S / 4 + S % 4 + 2 * S) : 0;
     CK(launch_link_stochastic_list(stoch_list_views(const_cast<void *>(list), h->N), h->N, h->slist_b_link,
                                    h->slist_alpha, seed, sample0, S, static_cast<unsigned int *>(scratch), labels, logp,
-                                   grad_pos, at<Ctrl>(ws, h->off_ctrl), s),
+                                   grad_pos, at<Ctrl>(ws, h->off_ctrl), h->num_sms, s),  // num_sms: set by the fof_link before the build
        "stochastic link kernels (list)");
     return FOF_OK;
 }
@@ -785,23 +778,41 @@ int fof_run_host(fof_handle *h, const float *pos_host, const float *mass_host, i
 #undef CKD
 }
 
+// The streams, events and pinned control blocks of fof_host_submit / fof_host_wait: created on first use, all or
+// nothing (host_streams_free also serves fof_destroy; every member is null until it exists).
+static void host_streams_free(fof_handle *h)
+{
+    for (auto &sl : h->slot) {
+        if (sl.out) (void)cudaStreamDestroy(sl.out);
+        if (sl.ev_in) (void)cudaEventDestroy(sl.ev_in);
+        if (sl.ev_linked) (void)cudaEventDestroy(sl.ev_linked);
+        if (sl.ev_groups) (void)cudaEventDestroy(sl.ev_groups);
+        if (sl.ev_ctrl) (void)cudaEventDestroy(sl.ev_ctrl);
+        if (sl.ctrl_pin) (void)cudaFreeHost(sl.ctrl_pin);
+        sl = fof_handle::HostSlot{};
+    }
+    if (h->in_stream) (void)cudaStreamDestroy(h->in_stream);
+    if (h->run_stream) (void)cudaStreamDestroy(h->run_stream);
+    h->in_stream = h->run_stream = nullptr;
+}
+
 static int host_streams(fof_handle *h)
 {
     if (h->in_stream) return FOF_OK;
-    cudaStream_t in = nullptr, run = nullptr;
-    CK(cudaStreamCreateWithFlags(&in, cudaStreamNonBlocking), "cudaStreamCreate");
-    CK(cudaStreamCreateWithFlags(&run, cudaStreamNonBlocking), "cudaStreamCreate");
+    cudaError_t e = cudaStreamCreateWithFlags(&h->run_stream, cudaStreamNonBlocking);
     for (auto &sl : h->slot) {
-        CK(cudaStreamCreateWithFlags(&sl.out, cudaStreamNonBlocking), "cudaStreamCreate");
-        CK(cudaEventCreateWithFlags(&sl.ev_in, cudaEventDisableTiming), "cudaEventCreate");
-        CK(cudaEventCreateWithFlags(&sl.ev_linked, cudaEventDisableTiming), "cudaEventCreate");
-        CK(cudaEventCreateWithFlags(&sl.ev_groups, cudaEventDisableTiming), "cudaEventCreate");
-        CK(cudaEventCreateWithFlags(&sl.ev_ctrl, cudaEventDisableTiming), "cudaEventCreate");
-        CK(cudaHostAlloc((void **)&sl.ctrl_pin, sizeof(Ctrl), cudaHostAllocDefault), "cudaHostAlloc");
-        sl.busy = false;
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&sl.out, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&sl.ev_in, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&sl.ev_linked, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&sl.ev_groups, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&sl.ev_ctrl, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaHostAlloc((void **)&sl.ctrl_pin, sizeof(Ctrl), cudaHostAllocDefault);
     }
-    h->run_stream = run;
-    h->in_stream = in;  // set last: fof_destroy takes it as "all of the above exist"
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&h->in_stream, cudaStreamNonBlocking);  // last: "all exist"
+    if (e != cudaSuccess) {
+        host_streams_free(h);
+        return cuda_fail(h, e, "fof_host_submit: streams");
+    }
     return FOF_OK;
 }
 

@@ -400,7 +400,7 @@ cudaError_t launch_stoch_list_fill(const float4 *sorted, int64_t N, Grid g, cons
                                    const int *idx_s, float b_link, float alpha, StochList list, cudaStream_t s);
 cudaError_t launch_link_stochastic_list(StochList list, int64_t N, float b_link, float alpha, unsigned long long seed,
                                         unsigned int sample0, int S, unsigned int *rel_s, int *labels, double *logp,
-                                        float *grad, Ctrl *ctrl, cudaStream_t s);
+                                        float *grad, Ctrl *ctrl, int num_sms, cudaStream_t s);
 
 cudaError_t launch_subgroups(const float *pos, const float *vel, const int *particle_group, const int *group_size,
                              int64_t N, int64_t K, float L, float sigma_x, float sigma_v, float ell,

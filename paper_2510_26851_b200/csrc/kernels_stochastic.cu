@@ -786,6 +786,9 @@ __global__ void __launch_bounds__(kListScanThreads) list_scan_apply_kernel(unsig
 #ifndef FOF_STREAM_MINB
 #define FOF_STREAM_MINB 16
 #endif
+#ifndef FOF_STREAM_WAVES
+#define FOF_STREAM_WAVES 8    // CTAs launched = SMs x resident CTAs per SM x this (cfg2: 1.79 / 1.82 / 1.68 ms per sample at 1 / 2 / 8; one CTA per two tiles: 1.83)
+#endif
 constexpr int kStreamBlock = FOF_STREAM_BLOCK;
 template <int SB>
 __global__ void __launch_bounds__(kStreamBlock, FOF_STREAM_MINB) stoch_stream_kernel(StochList list, int64_t N, StochKeys keys, float gscale,
@@ -793,10 +796,6 @@ __global__ void __launch_bounds__(kStreamBlock, FOF_STREAM_MINB) stoch_stream_ke
 {
     constexpr unsigned int kAll = 0xffffffffu;
     const int lane = threadIdx.x & 31;
-    const int64_t tile = ((int64_t)blockIdx.x * kStreamBlock + threadIdx.x) >> 5;  // 32 homes
-    const int64_t h0 = tile * 32;
-    if (h0 >= N) return;  // whole warps only
-    const unsigned int rb = list.roff[h0], re = list.roff[min(h0 + 32, N)];
     const uint4 *__restrict__ recA = list.rec;
     const uint4 *__restrict__ recB = list.rec + list.roff[N];
     const bool want_grad = grad != nullptr;
@@ -805,6 +804,14 @@ __global__ void __launch_bounds__(kStreamBlock, FOF_STREAM_MINB) stoch_stream_ke
     unsigned int nedge[SB];
 #pragma unroll
     for (int k = 0; k < SB; ++k) { lp[k] = 0.0; nedge[k] = 0u; carry[k][0] = carry[k][1] = carry[k][2] = 0.0f; }
+    // Tiles of 32 homes, dealt round-robin to the warps of a grid of a few waves: a halo's tiles hold hundreds of
+    // records each, the field's a handful, and neighbouring tiles are alike: the deal evens that out without a ticket.
+    const int64_t ntiles = (N + 31) >> 5;
+    const int64_t nwarps = ((int64_t)gridDim.x * kStreamBlock) >> 5;
+    for (int64_t tile = ((int64_t)blockIdx.x * kStreamBlock + threadIdx.x) >> 5; tile < ntiles; tile += nwarps) {
+    const int64_t h0 = tile * 32;
+    const unsigned int rb = list.roff[h0], re = list.roff[min(h0 + 32, N)];
+    if (rb == re) continue;
     const unsigned int tile_orig = (unsigned int)__ldg(list.home_orig + min(h0 + lane, N - 1));  // lane l: original index of home h0 + l
     int prev_home = -1;  // home of the record before this batch
     // the next batch is loaded while this one is worked on
@@ -888,18 +895,20 @@ __global__ void __launch_bounds__(kStreamBlock, FOF_STREAM_MINB) stoch_stream_ke
         for (int k = 0; k < SB; ++k)
             if (pa[k] != pb[k]) unite_rel(rel + (int64_t)k * N, list.home_orig, home, j);  // same parent: one set
     }
+    }  // tiles
+    const bool first_warp = blockIdx.x == 0 && threadIdx.x < 32;
     unsigned int nedge_all = 0;
 #pragma unroll
     for (int k = 0; k < SB; ++k) {
         double lpd = lp[k];
         for (int o = 16; o > 0; o >>= 1) lpd += __shfl_xor_sync(kAll, lpd, o);
-        if (h0 == 0) lpd += list.head->logp0;  // log p(y) = log p(all absent) + sum over the sampled edges of t
+        if (first_warp) lpd += list.head->logp0;  // log p(y) = log p(all absent) + sum over the sampled edges of t
         if (lane == 0 && lpd != 0.0) atomicAdd(logp + k, lpd);
         nedge_all += nedge[k];
     }
     for (int o = 16; o > 0; o >>= 1) nedge_all += __shfl_xor_sync(kAll, nedge_all, o);
     if (lane == 0 && nedge_all) atomicAdd(&ctrl->edges, (unsigned long long)nedge_all);  // sampled edges, all samples
-    if (h0 == 0 && lane == 0 && keys.count_potential) ctrl->pair_tests = list.head->potential;
+    if (first_warp && lane == 0 && keys.count_potential) ctrl->pair_tests = list.head->potential;
 }
 
 static inline unsigned int blocks_for(int64_t n, int per_block) { return (unsigned int)((n + per_block - 1) / per_block); }
@@ -1019,7 +1028,7 @@ cudaError_t launch_stoch_list_fill(const float4 *sorted, int64_t N, Grid g, cons
 // S samples sample0 .. sample0 + S - 1 over the list, four per pass (then one by one).
 cudaError_t launch_link_stochastic_list(StochList list, int64_t N, float b_link, float alpha, unsigned long long seed,
                                         unsigned int sample0, int S, unsigned int *rel_s, int *labels, double *logp,
-                                        float *grad, Ctrl *ctrl, cudaStream_t s)
+                                        float *grad, Ctrl *ctrl, int num_sms, cudaStream_t s)
 {
     cudaError_t e;
     if ((e = cudaMemsetAsync(logp, 0, (size_t)S * sizeof(double), s)) != cudaSuccess) return e;
@@ -1036,7 +1045,8 @@ cudaError_t launch_link_stochastic_list(StochList list, int64_t N, float b_link,
         for (int k = 0; k < sb; ++k) keys.k[k] = stoch_key(seed, sample0 + (unsigned int)(k0 + k));
         unsigned int *rel = rel_s + (size_t)k0 * (size_t)N;
         float *gk = grad ? grad + (size_t)k0 * 3 * (size_t)N : nullptr;
-        const unsigned int sgrid = blocks_for(N, kStreamBlock);
+        const unsigned int sgrid = (unsigned int)min((int64_t)blocks_for(N, kStreamBlock),
+                                                     (int64_t)(num_sms > 0 ? num_sms : 148) * FOF_STREAM_MINB * FOF_STREAM_WAVES);
         if (sb == 4) stoch_stream_kernel<4><<<sgrid, kStreamBlock, 0, s>>>(list, N, keys, sp.gscale, rel, logp + k0, gk, ctrl);
         else stoch_stream_kernel<1><<<sgrid, kStreamBlock, 0, s>>>(list, N, keys, sp.gscale, rel, logp + k0, gk, ctrl);
         k0 += sb;
