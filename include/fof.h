@@ -242,6 +242,23 @@ int fof_group_sigma(fof_handle *h, const float *pos, const float *mass, const in
                     const float *group_mass, const float *group_com, int64_t K, void *ws, float *group_sigma,
                     void *stream);
 
+/* fof_group_sigma without a workspace, for callers that cannot allocate one (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc).  Same operation (section 3.1.1, Eq. 5), same kernels,
+ * same arguments minus `ws`: the scratch (one float64 accumulator per group) is a file-scope device array of the
+ * library, FOF_SIGMA_STATIC_MAX_GROUPS entries = 2 MiB, which every GPU that loads the library holds until the
+ * process exits.  The call allocates nothing and frees nothing (no cudaMalloc, cudaFree or allocating library
+ * routine; the first call on a device asks the runtime once for the array's device address).
+ *   K > FOF_SIGMA_STATIC_MAX_GROUPS -> FOF_ERR_CAPACITY, nothing is launched (use fof_group_sigma);
+ *   K > floor(N / N_min) or a missing pointer -> FOF_ERR_INVALID_ARG, as fof_group_sigma.
+ * Every call on a device shares that one array: it is cleared on `stream` at the start of each call, so calls one
+ * after the other on one stream (or otherwise ordered) are independent, but two calls that OVERLAP on the GPU --
+ * different streams, different handles, different host threads -- race on it and give wrong sigmas.  Serialise
+ * them, or use fof_group_sigma with a workspace per stream.  Asynchronous on `stream`. */
+#define FOF_SIGMA_STATIC_MAX_GROUPS 262144
+int fof_group_sigma_static(fof_handle *h, const float *pos, const float *mass, const int32_t *particle_group,
+                           const float *group_mass, const float *group_com, int64_t K, float *group_sigma,
+                           void *stream);
+
 /* Frozen-assignment backward (section 3.1, Eq. 4: dX^h/dtheta = (1/N) sum_i dx_i/dtheta;
  * Eq. 5 for the decoration; R24).  Membership is held fixed:
  *   grad_pos[i] = (m_i / M_k) (grad_com[k] + grad_sigma[k] delta_i / group_sigma[k]),  k = particle_group[i],

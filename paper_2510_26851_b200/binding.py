@@ -92,6 +92,8 @@ def lib():
         L.fof_combine_groups.argtypes = [vp, i64, vp, f32, vp, i64, vp, vp, vp, vp, vp, vp, vp]
         L.fof_group_sigma.restype = ctypes.c_int
         L.fof_group_sigma.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp, vp]
+        L.fof_group_sigma_static.restype = ctypes.c_int
+        L.fof_group_sigma_static.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp]
         L.fof_groups_backward.restype = ctypes.c_int
         L.fof_groups_backward.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, vp, vp]
         L.fof_host_device_bytes.restype = ctypes.c_size_t
@@ -290,6 +292,15 @@ def fof_combine_groups(want, ref, L, part_label, part_size, part_mass, part_com,
 def fof_group_sigma(h, pos, mass, particle_group, group_mass, group_com, K, ws, group_sigma, stream=None):
     _check(lib().fof_group_sigma(h, _ptr(pos), _ptr(mass), _ptr(particle_group), _ptr(group_mass), _ptr(group_com),
                                  int(K), _ptr(ws), _ptr(group_sigma), _stream_ptr(stream)), h)
+
+
+FOF_SIGMA_STATIC_MAX_GROUPS = 262144
+
+
+def fof_group_sigma_static(h, pos, mass, particle_group, group_mass, group_com, K, group_sigma, stream=None):
+    """fof_group_sigma with the library's static scratch instead of a workspace (K <= FOF_SIGMA_STATIC_MAX_GROUPS)."""
+    _check(lib().fof_group_sigma_static(h, _ptr(pos), _ptr(mass), _ptr(particle_group), _ptr(group_mass),
+                                        _ptr(group_com), int(K), _ptr(group_sigma), _stream_ptr(stream)), h)
 
 
 def fof_groups_backward(h, pos, mass, particle_group, group_mass, group_com, group_sigma, grad_com, grad_sigma, K,

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfof_b200.so")
-SOURCES = ["fof_api.cu", "kernels_sort.cu", "kernels_link.cu", "kernels_block.cu", "kernels_groups.cu", "kernels_next1.cu", "kernels_stochastic.cu", "kernels_subhalo.cu", "kernels_slab.cu", "kernels_measure.cu"]
+SOURCES = ["fof_api.cu", "kernels_sort.cu", "kernels_link.cu", "kernels_block.cu", "kernels_groups.cu", "kernels_next1.cu", "kernels_stochastic.cu", "kernels_subhalo.cu", "kernels_slab.cu", "kernels_measure.cu", "kernels_noalloc.cu"]
 HEADERS = ["fof_internal.cuh", os.path.join("..", "..", "include", "fof.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
