@@ -555,6 +555,36 @@ def test_host_pipeline_errors(B):
     torch.cuda.synchronize()
 
 
+@pytest.mark.parametrize("N", [0, 1, 5])
+def test_host_calls_on_empty_and_tiny_inputs(B, N):
+    """fof_run_host and fof_host_submit / fof_host_wait with no particle, one particle, five coincident ones."""
+    p = np.full((N, 3), 0.5, np.float32)
+    h = B.fof_create(N, 1.0, 0.1, 1)
+    cap = max(N, 1)
+    pin = lambda *s, dt=torch.int32: torch.empty(*s, dtype=dt).pin_memory()  # noqa: E731
+    hp = torch.from_numpy(p).pin_memory() if N else torch.zeros((1, 3)).pin_memory()
+    hl, gl, gs, pg = pin(cap), pin(cap), pin(cap), pin(cap)
+    gm, gc = pin(cap, dt=torch.float32), pin((cap, 3), dt=torch.float32)
+    dev = [torch.empty(B.fof_host_device_bytes(h, cap) + 256, dtype=torch.uint8, device="cuda") for _ in range(2)]
+
+    def check(K):
+        assert K == (1 if N else 0)
+        if N:
+            assert (hl.numpy()[:N] == 0).all() and gs.numpy()[0] == N and gl.numpy()[0] == 0
+            assert (pg.numpy()[:N] == 0).all() and abs(gm.numpy()[0] - N) < 1e-6
+            assert np.allclose(gc.numpy()[0], 0.5)
+
+    for t in (hl, gl, gs, pg):
+        t.fill_(-3)
+    check(B.fof_run_host(h, hp, None, hl, gl, gs, gm, gc, pg, cap, dev[0]))
+    for slot in (0, 1, 0):
+        for t in (hl, gl, gs, pg):
+            t.fill_(-3)
+        B.fof_host_submit(h, slot, hp, None, hl, gl, gs, gm, gc, pg, cap, dev[slot])
+        check(B.fof_host_wait(h, slot))
+    B.fof_destroy(h)
+
+
 @pytest.mark.parametrize("n_particles", [4099, 65537])
 def test_unaligned_caller_pointers(B, n_particles):
     """pos / labels / particle_group that are only 4-byte aligned (views one element into a buffer) and
